@@ -1,0 +1,157 @@
+/* gnn.h -- C ABI of libgnn.so: batched forward inference of a dynamic-graph EdgeConv network of the ParticleNet
+ * shape on one B200 (sm_100a), plus a host-side dynamic batcher.
+ *
+ * What is computed (citations are PAPER.md line numbers; readings R1-R27 are listed in DESIGN.md):
+ *   PAPER.md L97   "ParticleNet ... applies dynamic graph convolutional neural networks and edge convolution
+ *                   techniques to variable-dimensioned, unordered point cloud data"
+ *   PAPER.md L262  (App. B) "five input features, two coordinates, three EdgeConv Blocks using k=16 nearest
+ *                   neighbors and C=(64,64,64),(128,128,128),(256,256,256) channels, and two fully connected
+ *                   layers with 256 nodes and 0.1 dropout rate to two nodes"
+ *   PAPER.md L269  three FP32 inputs (features, coordinates, mask), FP32 output; L270 inference mode
+ *   PAPER.md L53, L268, L271  dynamic batching (preferred batch 1024) and concurrent model instances
+ * Per jet b with n particles, block l = 1..L (C_in -> C1,C2,C3), k_eff = min(k, n-1):
+ *   kNN      N_i = the k_eff particles j != i of the same jet smallest under the strict order (d_ij, j),
+ *            d_ij = sum_c (s_ic - s_jc)^2, s = coordinates for block 1, the previous block's output afterwards
+ *   EdgeConv e_ij = [x_i ; x_j - x_i];  three times h <- ReLU(scale*(W h) + shift);  a_i = mean_j h3_ij;
+ *            x'_i = ReLU(a_i + scale_s*(W_s x_i) + shift_s)
+ *   pool     g = (1/n) sum_i x^L_i (g = 0 for an empty jet);  head: hidden FC + ReLU (dropout = identity), final FC.
+ *
+ * Conventions: every function returns GNN_OK (0) or a negative gnn_status; nothing throws across the ABI.
+ * "dev" pointers are CUDA device pointers on the model's device, "host" pointers are host memory.  Only
+ * gnn_create / gnn_destroy / gnn_batcher_create / gnn_batcher_destroy / gnn_status_check allocate or synchronise;
+ * gnn_infer* and gnn_debug_* only enqueue kernels on the caller's stream and return.  There is no CPU fallback:
+ * without a CUDA device gnn_create fails with GNN_ERR_CUDA.
+ */
+#ifndef GNN_H_
+#define GNN_H_
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gnn_model   gnn_model;     /* opaque; owns device copies of the folded/packed weights + workspace */
+typedef struct gnn_batcher gnn_batcher;   /* opaque; owns threads, pinned staging buffers and CUDA streams */
+
+enum { GNN_MAX_BLOCKS = 4, GNN_MAX_FC = 3, GNN_MAX_PARTICLES = 128, GNN_MAX_K = 32, GNN_MAX_SLICES = 8 };
+
+typedef enum {
+    GNN_OK = 0,
+    GNN_ERR_NULL = -1,            /* a required pointer is NULL */
+    GNN_ERR_BAD_ARCH = -2,        /* gnn_arch field out of range (see gnn_arch) */
+    GNN_ERR_BAD_BLOB_SIZE = -3,   /* bytes != gnn_weights_bytes(arch) */
+    GNN_ERR_BATCH_TOO_LARGE = -4, /* B > max_batch_jets, N > max_batch_jets*max_particles, or bad slice */
+    GNN_ERR_CUDA = -5,            /* a CUDA runtime call failed (including: no device) */
+    GNN_ERR_BAD_OFFSETS = -6,     /* device check: offsets[0] != 0, not monotone, or offsets[B] != N (all logits NaN) */
+    GNN_ERR_JET_TOO_LARGE = -7,   /* device check: some jet has more than max_particles particles (its logits NaN) */
+    GNN_ERR_BAD_ARG = -8,         /* negative sizes, bad k / D in a debug call, bad batcher options */
+    GNN_ERR_TIMEOUT = -9,         /* gnn_batcher_wait timed out (the ticket stays valid) */
+    GNN_ERR_QUEUE_FULL = -10,     /* gnn_batcher_submit: max_pending_requests reached */
+    GNN_ERR_BAD_TICKET = -11      /* unknown or already collected ticket */
+} gnn_status;
+
+typedef enum {
+    GNN_FP32_VALIDATION = 0,  /* every contraction in fp32 FMA on CUDA cores (R18) */
+    GNN_BF16 = 1              /* edge-MLP GEMMs as bf16 x bf16 -> fp32 tcgen05 MMAs; kNN, shortcut, pool, head fp32 (R19) */
+} gnn_precision;
+
+/* Architecture.  Constraints checked by gnn_create: 1 <= n_blocks <= GNN_MAX_BLOCKS;
+ * coord_dims in [1,8]; 1 <= k <= GNN_MAX_K (BF16 mode: k a power of two); every channel count a multiple of 8
+ * (BF16 mode: one of 32, 64, 128, 256 and C1 == C2 == C3 inside a block); 0 <= n_fc_hidden <= GNN_MAX_FC;
+ * 1 <= fc widths <= 1024; 1 <= n_classes <= 64; 1 <= max_particles <= GNN_MAX_PARTICLES; max_batch_jets >= 1;
+ * 1 <= workspace_slices <= GNN_MAX_SLICES (0 is read as 1). */
+typedef struct {
+    int32_t in_features;                  /* F: per-particle input features (paper: 5; BASELINE configs: 4/7/9, R1) */
+    int32_t coord_dims;                   /* 2 (L262) */
+    int32_t k;                            /* neighbours, 16 (L262) */
+    int32_t n_blocks;                     /* EdgeConv blocks, 3 (L262) */
+    int32_t channels[GNN_MAX_BLOCKS][3];  /* (C1,C2,C3) per block */
+    int32_t n_fc_hidden;                  /* hidden FC layers before the final one: 1 (FC 256 + ReLU) */
+    int32_t fc_hidden[GNN_MAX_FC];
+    int32_t n_classes;                    /* 2 */
+    int32_t max_particles;                /* largest legal multiplicity of one jet (100 or 128 in the configs) */
+    int32_t max_batch_jets;               /* sizes the workspace: largest B of one gnn_infer call */
+    int32_t precision;                    /* gnn_precision */
+    int32_t workspace_slices;             /* independent workspaces = max concurrent gnn_infer_slice calls */
+} gnn_arch;
+
+/* Weight blob: fp32, little-endian, in this order (weights are random in the paper's benchmark).
+ * For each block l: for layer 1..3: W[out][in] row-major (layer 1: in = 2*C_in, the x_i half first, then the
+ * (x_j - x_i) half), scale[out], shift[out]; then the shortcut W[C3][C_in], scale[C3], shift[C3].  Then for each FC
+ * (hidden..., final): W[out][in], bias[out].  Block layers have no bias of their own: y = scale*(W x) + shift (R8).
+ * gnn_create folds scale into W in fp32 and (GNN_BF16) rounds the edge-MLP weights to bf16 once (RNE). */
+int gnn_weights_bytes(const gnn_arch* arch, size_t* out_bytes);
+
+/* Copies and packs the blob (host pointer, caller keeps ownership) onto CUDA device `device`, allocates
+ * `workspace_slices` workspaces sized for max_batch_jets * max_particles particles.  Synchronous. */
+int gnn_create(const void* weights_host, size_t bytes, const gnn_arch* arch, int device, gnn_model** out);
+void gnn_destroy(gnn_model* m);
+
+/* Ragged forward (BASELINE.json north_star (4): padding-free).  feats_dev [N, F] and coords_dev [N, coord_dims]
+ * row-major fp32, particles of one jet contiguous; offsets_dev int32 [B+1] CSR (offsets[0] = 0, offsets[B] = N);
+ * logits_dev fp32 [B, n_classes] (written).  Asynchronous on `cuda_stream` (a cudaStream_t; NULL = default
+ * stream).  Uses workspace slice 0 / `slice`: two calls may overlap only on different slices.  B = 0 is legal.
+ * Host-checkable errors return at once; device-checkable ones (GNN_ERR_BAD_OFFSETS, GNN_ERR_JET_TOO_LARGE) set a
+ * sticky per-slice status word read by gnn_status_check and put NaN into the offending logits.  n_b = 0 is legal
+ * (logits = head(0), R12).  NaN / Inf inputs are not checked. */
+int gnn_infer(gnn_model* m, const float* feats_dev, const float* coords_dev, const int32_t* offsets_dev,
+              int32_t B, int32_t N, float* logits_dev, void* cuda_stream);
+int gnn_infer_slice(gnn_model* m, int32_t slice, const float* feats_dev, const float* coords_dev,
+                    const int32_t* offsets_dev, int32_t B, int32_t N, float* logits_dev, void* cuda_stream);
+
+/* Padded forward (features, coordinates, mask).  feats_dev [B, P, F], coords_dev [B, P, coord_dims],
+ * mask_dev [B, P] fp32, nonzero = real particle.  Masked slots are never read beyond the mask itself (they may hold
+ * NaN); real particles may sit at any slots and keep their relative order (stable compaction, R7).  A jet with
+ * more than max_particles real particles raises GNN_ERR_JET_TOO_LARGE.  B*P <= max_batch_jets * GNN_MAX_PARTICLES. */
+int gnn_infer_padded(gnn_model* m, const float* feats_dev, const float* coords_dev, const float* mask_dev,
+                     int32_t B, int32_t P, float* logits_dev, void* cuda_stream);
+
+/* Synchronises `cuda_stream`, returns and clears the sticky device status of `slice` (GNN_OK, GNN_ERR_BAD_OFFSETS,
+ * GNN_ERR_JET_TOO_LARGE, or GNN_ERR_CUDA if the stream reports an error). */
+int gnn_status_check(gnn_model* m, int32_t slice, void* cuda_stream);
+
+const char* gnn_strerror(int status);
+/* number of kernels the library has launched on this model since gnn_create (bench.py's gpu_launches) */
+int64_t gnn_launch_count(const gnn_model* m);
+
+/* ---- per-stage entry points: the same kernels the forward uses, exposed for stage-wise parity tests --------- */
+/* kNN on an arbitrary space [N, D] (1 <= D <= 1024): idx_dev int32 [N, k], jet-local indices in (d, j) order,
+ * -1 = none (k_eff < k). */
+int gnn_debug_knn(gnn_model* m, const float* space_dev, int32_t D, const int32_t* offsets_dev, int32_t B, int32_t N,
+                  int32_t k, int32_t* idx_dev, void* cuda_stream);
+/* EdgeConv block `block` (0-based) given jet-local neighbour indices [N, arch.k]: x_dev [N, C_in] -> y_dev [N, C3],
+ * in the model's precision mode. */
+int gnn_debug_edgeconv(gnn_model* m, int32_t block, const float* x_dev, const int32_t* idx_dev,
+                       const int32_t* offsets_dev, int32_t B, int32_t N, float* y_dev, void* cuda_stream);
+/* masked global average pool + FC head: x_dev [N, C_last] -> logits_dev [B, n_classes] */
+int gnn_debug_pool_head(gnn_model* m, const float* x_dev, const int32_t* offsets_dev, int32_t B, int32_t N,
+                        float* logits_dev, void* cuda_stream);
+
+/* ---- host dynamic batcher ("dynamic batching", L268 preferred batch 1024, L271 instance group) -- */
+typedef struct {
+    int32_t max_batch_jets;        /* coalesce up to this many jets per launch (<= arch.max_batch_jets); 1024 (L268) */
+    int32_t max_queue_delay_us;    /* launch when the oldest queued request is this old; 1000 (BASELINE configs[3]) */
+    int32_t n_instances;           /* concurrent launches = CUDA streams = workspace slices used (<= arch.workspace_slices) */
+    int32_t max_pending_requests;  /* submit fails with GNN_ERR_QUEUE_FULL beyond this; 0 = 65536 */
+} gnn_batcher_opts;
+typedef struct { uint64_t id; } gnn_ticket;
+
+int gnn_batcher_create(gnn_model* m, const gnn_batcher_opts* opts, gnn_batcher** out);
+/* Thread-safe, non-blocking.  Inputs are HOST pointers laid out as in gnn_infer (offsets_host[0] = 0); they are
+ * copied before the call returns.  logits_host_out [n_jets, n_classes] must stay valid until gnn_batcher_wait
+ * returns for the ticket.  Offsets are validated on the host; a bad request fails alone (GNN_ERR_BAD_OFFSETS /
+ * GNN_ERR_JET_TOO_LARGE) without touching its batch mates. */
+int gnn_batcher_submit(gnn_batcher* b, const float* feats_host, const float* coords_host, const int32_t* offsets_host,
+                       int32_t n_jets, float* logits_host_out, gnn_ticket* out);
+/* Blocks until the ticket completes or timeout_us elapses (< 0: forever).  Returns the ticket's status.  queue_us =
+ * submit -> launch, compute_us = launch -> logits in host memory (PAPER.md L279 splits request time this way). */
+int gnn_batcher_wait(gnn_batcher* b, gnn_ticket t, int64_t timeout_us, double* queue_us, double* compute_us);
+int gnn_batcher_stats(gnn_batcher* b, uint64_t* n_requests, uint64_t* n_jets, uint64_t* n_launches,
+                      double* mean_batch_jets);
+void gnn_batcher_destroy(gnn_batcher* b);   /* drains pending tickets first */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GNN_H_ */

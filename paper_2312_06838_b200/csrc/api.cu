@@ -1,0 +1,366 @@
+// api.cu -- the C ABI of include/gnn.h: model creation (BN fold, transposition, packing), workspace slices, and the
+// launch plan of one forward pass.  Host code only enqueues kernels; every step of the path runs on the GPU.
+#include "gnn_internal.h"
+#include <cmath>
+#include <cstring>
+#include <new>
+
+int edgeconv_bf16_prepare(gnn_model& m, const float* blob_host);       // edgeconv_bf16.cu
+int launch_edgeconv_bf16(gnn_model& m, int block, const float* x, const int32_t* idx, int N, float* y, Workspace& w,
+                         cudaStream_t s);
+
+namespace {
+
+size_t blob_count(const gnn_arch& a) {
+    size_t n = 0;
+    for (int l = 0; l < a.n_blocks; ++l) {
+        size_t cin = block_in(a, l), c1 = a.channels[l][0], c2 = a.channels[l][1], c3 = a.channels[l][2];
+        n += c1 * 2 * cin + 2 * c1 + c2 * c1 + 2 * c2 + c3 * c2 + 2 * c3 + c3 * cin + 2 * c3;
+    }
+    size_t in = a.channels[a.n_blocks - 1][2];
+    for (int i = 0; i <= a.n_fc_hidden; ++i) {
+        size_t out = (i < a.n_fc_hidden) ? a.fc_hidden[i] : a.n_classes;
+        n += out * in + out;
+        in = out;
+    }
+    return n;
+}
+
+bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
+
+int check_arch(const gnn_arch& a) {
+    if (a.n_blocks < 1 || a.n_blocks > GNN_MAX_BLOCKS) return GNN_ERR_BAD_ARCH;
+    if (a.in_features < 1 || a.in_features > 1024) return GNN_ERR_BAD_ARCH;
+    if (a.coord_dims < 1 || a.coord_dims > 8) return GNN_ERR_BAD_ARCH;
+    if (a.k < 1 || a.k > GNN_MAX_K) return GNN_ERR_BAD_ARCH;
+    if (a.n_fc_hidden < 0 || a.n_fc_hidden > GNN_MAX_FC) return GNN_ERR_BAD_ARCH;
+    if (a.n_classes < 1 || a.n_classes > 64) return GNN_ERR_BAD_ARCH;
+    if (a.max_particles < 1 || a.max_particles > GNN_MAX_PARTICLES) return GNN_ERR_BAD_ARCH;
+    if (a.max_batch_jets < 1) return GNN_ERR_BAD_ARCH;
+    if (a.workspace_slices < 0 || a.workspace_slices > GNN_MAX_SLICES) return GNN_ERR_BAD_ARCH;
+    if (a.precision != GNN_FP32_VALIDATION && a.precision != GNN_BF16) return GNN_ERR_BAD_ARCH;
+    for (int l = 0; l < a.n_blocks; ++l)
+        for (int i = 0; i < 3; ++i) {
+            int c = a.channels[l][i];
+            if (c < 8 || c > 1024 || (c % 8) != 0) return GNN_ERR_BAD_ARCH;
+        }
+    for (int i = 0; i < a.n_fc_hidden; ++i)
+        if (a.fc_hidden[i] < 1 || a.fc_hidden[i] > 1024) return GNN_ERR_BAD_ARCH;
+    if (a.channels[a.n_blocks - 1][2] > 1024) return GNN_ERR_BAD_ARCH;
+    if (a.precision == GNN_BF16) {
+        if (!is_pow2(a.k)) return GNN_ERR_BAD_ARCH;
+        for (int l = 0; l < a.n_blocks; ++l) {
+            int c = a.channels[l][0];
+            if (a.channels[l][1] != c || a.channels[l][2] != c) return GNN_ERR_BAD_ARCH;
+            if (c != 32 && c != 64 && c != 128 && c != 256) return GNN_ERR_BAD_ARCH;
+        }
+    }
+    return GNN_OK;
+}
+
+template <typename T>
+int dev_alloc(gnn_model* m, T** p, size_t count) {
+    void* q = nullptr;
+    if (count == 0) count = 1;
+    GNN_CUDA_TRY(cudaMalloc(&q, count * sizeof(T)));
+    m->allocs.push_back(q);
+    *p = static_cast<T*>(q);
+    return GNN_OK;
+}
+
+// fold scale into W (fp32), transpose to Wt[Kp][N] with zero rows up to Kp, upload
+int upload_linear(gnn_model* m, const float* W, const float* scale, const float* shift_or_bias, int K, int N, LinF32* out) {
+    int Kp = (K + 3) & ~3;
+    int Np = (N + 3) & ~3;              // column padding keeps float4 loads of the SIMT kernels in bounds
+    std::vector<float> wt((size_t)Kp * Np, 0.0f), sh((size_t)Np, 0.0f);
+    for (int o = 0; o < N; ++o) {
+        float sc = scale ? scale[o] : 1.0f;
+        for (int c = 0; c < K; ++c) wt[(size_t)c * Np + o] = sc * W[(size_t)o * K + c];
+        sh[o] = shift_or_bias[o];
+    }
+    float *dW = nullptr, *dS = nullptr;
+    int rc;
+    if ((rc = dev_alloc(m, &dW, wt.size())) != GNN_OK) return rc;
+    if ((rc = dev_alloc(m, &dS, sh.size())) != GNN_OK) return rc;
+    GNN_CUDA_TRY(cudaMemcpy(dW, wt.data(), wt.size() * sizeof(float), cudaMemcpyHostToDevice));
+    GNN_CUDA_TRY(cudaMemcpy(dS, sh.data(), sh.size() * sizeof(float), cudaMemcpyHostToDevice));
+    out->Wt = dW; out->shift = dS; out->K = K; out->Kp = Kp; out->N = N; out->ld = Np;
+    return GNN_OK;
+}
+
+int build_model(gnn_model* m, const float* blob) {
+    const gnn_arch& a = m->arch;
+    const float* p = blob;
+    int rc;
+    for (int l = 0; l < a.n_blocks; ++l) {
+        BlockDev& b = m->blocks[l];
+        b.cin = block_in(a, l); b.c1 = a.channels[l][0]; b.c2 = a.channels[l][1]; b.c3 = a.channels[l][2];
+        const int ins[3] = {2 * b.cin, b.c1, b.c2}, outs[3] = {b.c1, b.c2, b.c3};
+        LinF32* dst[3] = {&b.l1, &b.l2, &b.l3};
+        for (int i = 0; i < 3; ++i) {
+            const float* W = p; p += (size_t)outs[i] * ins[i];
+            const float* sc = p; p += outs[i];
+            const float* sh = p; p += outs[i];
+            if ((rc = upload_linear(m, W, sc, sh, ins[i], outs[i], dst[i])) != GNN_OK) return rc;
+        }
+        const float* W = p; p += (size_t)b.c3 * b.cin;
+        const float* sc = p; p += b.c3;
+        const float* sh = p; p += b.c3;
+        if ((rc = upload_linear(m, W, sc, sh, b.cin, b.c3, &b.sc)) != GNN_OK) return rc;
+    }
+    int in = a.channels[a.n_blocks - 1][2];
+    m->n_fc = 0;
+    for (int i = 0; i <= a.n_fc_hidden; ++i) {
+        int out = (i < a.n_fc_hidden) ? a.fc_hidden[i] : a.n_classes;
+        const float* W = p; p += (size_t)out * in;
+        const float* bias = p; p += out;
+        if ((rc = upload_linear(m, W, nullptr, bias, in, out, &m->fc[m->n_fc])) != GNN_OK) return rc;
+        ++m->n_fc;
+        in = out;
+    }
+    return GNN_OK;
+}
+
+int alloc_workspace(gnn_model* m, Workspace& w) {
+    const gnn_arch& a = m->arch;
+    int rc;
+    size_t Nmax = (size_t)m->Nmax, Bmax = (size_t)a.max_batch_jets;
+    if ((rc = dev_alloc(m, &w.xa, Nmax * m->Cmax)) != GNN_OK) return rc;
+    if ((rc = dev_alloc(m, &w.xb, Nmax * m->Cmax)) != GNN_OK) return rc;
+    if ((rc = dev_alloc(m, &w.idx, Nmax * a.k)) != GNN_OK) return rc;
+    if ((rc = dev_alloc(m, &w.jet_start, Bmax)) != GNN_OK) return rc;
+    if ((rc = dev_alloc(m, &w.jet_n, Bmax)) != GNN_OK) return rc;
+    if ((rc = dev_alloc(m, &w.status, 1)) != GNN_OK) return rc;
+    if ((rc = dev_alloc(m, &w.meta, 2)) != GNN_OK) return rc;
+    if ((rc = dev_alloc(m, &w.pfeats, Nmax * a.in_features)) != GNN_OK) return rc;
+    if ((rc = dev_alloc(m, &w.pcoords, Nmax * a.coord_dims)) != GNN_OK) return rc;
+    if ((rc = dev_alloc(m, &w.poffsets, Bmax + 1)) != GNN_OK) return rc;
+    if ((rc = dev_alloc(m, &w.pcounts, Bmax)) != GNN_OK) return rc;
+    GNN_CUDA_TRY(cudaMemset(w.status, 0, sizeof(unsigned)));
+    GNN_CUDA_TRY(cudaMemset(w.meta, 0, 2 * sizeof(int32_t)));
+    return GNN_OK;
+}
+
+// the launch plan of one forward (SURVEY.md call stack (4)): ingest -> per block [kNN, EdgeConv] -> pool + head
+int forward(gnn_model* m, Workspace& w, const float* feats, const float* coords, const int32_t* offsets,
+            const int32_t* counts, int B, int N_exact, int N_upper, float* logits, cudaStream_t s) {
+    const gnn_arch& a = m->arch;
+    int n = 0, rc;
+    if ((rc = launch_ingest(offsets, counts, B, N_exact, (int)m->Nmax, a.max_particles, w, s)) < 0) return rc;
+    n += rc;
+    const float* x = feats;
+    float* bufs[2] = {w.xa, w.xb};
+    for (int l = 0; l < a.n_blocks; ++l) {
+        const float* space = (l == 0) ? coords : x;
+        int D = (l == 0) ? a.coord_dims : block_in(a, l);
+        if ((rc = launch_knn(space, D, a.k, B, a.max_particles, w, w.idx, 0, s)) < 0) return rc;
+        n += rc;
+        float* y = bufs[l & 1];
+        if (a.precision == GNN_BF16) rc = launch_edgeconv_bf16(*m, l, x, w.idx, N_upper, y, w, s);
+        else rc = launch_edgeconv_f32(m->blocks[l], a.k, x, w.idx, N_upper, y, w, s);
+        if (rc < 0) return rc;
+        n += rc;
+        x = y;
+    }
+    if ((rc = launch_pool_head(*m, x, B, w, logits, s)) < 0) return rc;
+    n += rc;
+    m->launches.fetch_add(n, std::memory_order_relaxed);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) {
+        std::fprintf(stderr, "libgnn: launch failed: %s\n", cudaGetErrorString(e));
+        return GNN_ERR_CUDA;
+    }
+    return GNN_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int gnn_weights_bytes(const gnn_arch* arch, size_t* out_bytes) {
+    if (!arch || !out_bytes) return GNN_ERR_NULL;
+    int rc = check_arch(*arch);
+    if (rc != GNN_OK) return rc;
+    *out_bytes = blob_count(*arch) * sizeof(float);
+    return GNN_OK;
+}
+
+int gnn_create(const void* weights_host, size_t bytes, const gnn_arch* arch, int device, gnn_model** out) {
+    if (!weights_host || !arch || !out) return GNN_ERR_NULL;
+    *out = nullptr;
+    int rc = check_arch(*arch);
+    if (rc != GNN_OK) return rc;
+    if (bytes != blob_count(*arch) * sizeof(float)) return GNN_ERR_BAD_BLOB_SIZE;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) {
+        std::fprintf(stderr, "libgnn: no usable CUDA device %d (found %d); there is no CPU fallback\n", device, ndev);
+        return GNN_ERR_CUDA;
+    }
+    GNN_CUDA_TRY(cudaSetDevice(device));
+    gnn_model* m = new (std::nothrow) gnn_model();
+    if (!m) return GNN_ERR_CUDA;
+    m->arch = *arch;
+    if (m->arch.workspace_slices == 0) m->arch.workspace_slices = 1;
+    m->device = device;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) == cudaSuccess) m->n_sms = prop.multiProcessorCount;
+    m->Nmax = (int64_t)arch->max_batch_jets * arch->max_particles;
+    m->Cmax = 8;
+    for (int l = 0; l < arch->n_blocks; ++l) m->Cmax = std::max(m->Cmax, arch->channels[l][2]);
+    if ((rc = knn_configure()) != GNN_OK || (rc = edgeconv_f32_configure()) != GNN_OK ||
+        (rc = build_model(m, static_cast<const float*>(weights_host))) != GNN_OK) {
+        gnn_destroy(m);
+        return rc;
+    }
+    m->ws.resize(m->arch.workspace_slices);
+    for (auto& w : m->ws)
+        if ((rc = alloc_workspace(m, w)) != GNN_OK) { gnn_destroy(m); return rc; }
+    if (m->arch.precision == GNN_BF16 &&
+        (rc = edgeconv_bf16_prepare(*m, static_cast<const float*>(weights_host))) != GNN_OK) {
+        gnn_destroy(m);
+        return rc;
+    }
+    GNN_CUDA_TRY(cudaDeviceSynchronize());
+    *out = m;
+    return GNN_OK;
+}
+
+void gnn_destroy(gnn_model* m) {
+    if (!m) return;
+    cudaSetDevice(m->device);
+    cudaDeviceSynchronize();
+    for (void* p : m->allocs) cudaFree(p);
+    delete m;
+}
+
+int gnn_infer_slice(gnn_model* m, int32_t slice, const float* feats_dev, const float* coords_dev,
+                    const int32_t* offsets_dev, int32_t B, int32_t N, float* logits_dev, void* cuda_stream) {
+    if (!m) return GNN_ERR_NULL;
+    if (B < 0 || N < 0) return GNN_ERR_BAD_ARG;
+    if (slice < 0 || slice >= (int)m->ws.size()) return GNN_ERR_BATCH_TOO_LARGE;
+    if (B > m->arch.max_batch_jets || (int64_t)N > m->Nmax) return GNN_ERR_BATCH_TOO_LARGE;
+    if (B == 0) return GNN_OK;
+    if (!offsets_dev || !logits_dev || (N > 0 && (!feats_dev || !coords_dev))) return GNN_ERR_NULL;
+    return forward(m, m->ws[slice], feats_dev, coords_dev, offsets_dev, nullptr, B, N, N, logits_dev,
+                   static_cast<cudaStream_t>(cuda_stream));
+}
+
+int gnn_infer(gnn_model* m, const float* feats_dev, const float* coords_dev, const int32_t* offsets_dev, int32_t B,
+              int32_t N, float* logits_dev, void* cuda_stream) {
+    return gnn_infer_slice(m, 0, feats_dev, coords_dev, offsets_dev, B, N, logits_dev, cuda_stream);
+}
+
+int gnn_infer_padded(gnn_model* m, const float* feats_dev, const float* coords_dev, const float* mask_dev, int32_t B,
+                     int32_t P, float* logits_dev, void* cuda_stream) {
+    if (!m) return GNN_ERR_NULL;
+    if (B < 0 || P < 0) return GNN_ERR_BAD_ARG;
+    if (B > m->arch.max_batch_jets || (int64_t)B * P > (int64_t)m->arch.max_batch_jets * GNN_MAX_PARTICLES)
+        return GNN_ERR_BATCH_TOO_LARGE;
+    if (B == 0) return GNN_OK;
+    if (!logits_dev || (P > 0 && (!feats_dev || !coords_dev || !mask_dev))) return GNN_ERR_NULL;
+    Workspace& w = m->ws[0];
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    int rc = launch_compact_padded(feats_dev, coords_dev, mask_dev, B, P, m->arch.in_features, m->arch.coord_dims,
+                                   m->arch.max_particles, w, s);
+    if (rc < 0) return rc;
+    m->launches.fetch_add(rc, std::memory_order_relaxed);
+    int64_t upper = std::min<int64_t>((int64_t)B * std::min<int>(P, m->arch.max_particles), m->Nmax);
+    return forward(m, w, w.pfeats, w.pcoords, w.poffsets, w.pcounts, B, -1, (int)upper, logits_dev, s);
+}
+
+int gnn_status_check(gnn_model* m, int32_t slice, void* cuda_stream) {
+    if (!m) return GNN_ERR_NULL;
+    if (slice < 0 || slice >= (int)m->ws.size()) return GNN_ERR_BATCH_TOO_LARGE;
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    unsigned st = 0;
+    GNN_CUDA_TRY(cudaMemcpyAsync(&st, m->ws[slice].status, sizeof(unsigned), cudaMemcpyDeviceToHost, s));
+    GNN_CUDA_TRY(cudaStreamSynchronize(s));
+    if (st) {
+        GNN_CUDA_TRY(cudaMemsetAsync(m->ws[slice].status, 0, sizeof(unsigned), s));
+        GNN_CUDA_TRY(cudaStreamSynchronize(s));
+    }
+    if (st & GNN_DEV_BAD_OFFSETS) return GNN_ERR_BAD_OFFSETS;
+    if (st & GNN_DEV_JET_TOO_LARGE) return GNN_ERR_JET_TOO_LARGE;
+    return GNN_OK;
+}
+
+const char* gnn_strerror(int status) {
+    switch (status) {
+        case GNN_OK: return "ok";
+        case GNN_ERR_NULL: return "null pointer";
+        case GNN_ERR_BAD_ARCH: return "architecture field out of range";
+        case GNN_ERR_BAD_BLOB_SIZE: return "weight blob size does not match the architecture";
+        case GNN_ERR_BATCH_TOO_LARGE: return "batch exceeds the workspace (max_batch_jets / max_particles / slice)";
+        case GNN_ERR_CUDA: return "CUDA runtime error (or no CUDA device: there is no CPU fallback)";
+        case GNN_ERR_BAD_OFFSETS: return "offsets are not a valid CSR (offsets[0] != 0, not monotone, or offsets[B] != N)";
+        case GNN_ERR_JET_TOO_LARGE: return "a jet has more than max_particles particles";
+        case GNN_ERR_BAD_ARG: return "bad argument";
+        case GNN_ERR_TIMEOUT: return "timed out";
+        case GNN_ERR_QUEUE_FULL: return "batcher queue full";
+        case GNN_ERR_BAD_TICKET: return "unknown or already collected ticket";
+        default: return "unknown status";
+    }
+}
+
+int64_t gnn_launch_count(const gnn_model* m) { return m ? m->launches.load(std::memory_order_relaxed) : 0; }
+
+// ---- per-stage entry points ------------------------------------------------------------------------------------
+int gnn_debug_knn(gnn_model* m, const float* space_dev, int32_t D, const int32_t* offsets_dev, int32_t B, int32_t N,
+                  int32_t k, int32_t* idx_dev, void* cuda_stream) {
+    if (!m) return GNN_ERR_NULL;
+    if (B < 0 || N < 0 || D < 1 || D > 1024 || k < 1 || k > GNN_MAX_K) return GNN_ERR_BAD_ARG;
+    if (B > m->arch.max_batch_jets || (int64_t)N > m->Nmax) return GNN_ERR_BATCH_TOO_LARGE;
+    if (B == 0) return GNN_OK;
+    if (!offsets_dev || !idx_dev || (N > 0 && !space_dev)) return GNN_ERR_NULL;
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    Workspace& w = m->ws[0];
+    int n = 0, rc;
+    if ((rc = launch_ingest(offsets_dev, nullptr, B, N, (int)m->Nmax, m->arch.max_particles, w, s)) < 0) return rc;
+    n += rc;
+    if ((rc = launch_knn(space_dev, D, k, B, m->arch.max_particles, w, idx_dev, 1, s)) < 0) return rc;
+    n += rc;
+    m->launches.fetch_add(n, std::memory_order_relaxed);
+    return cudaGetLastError() == cudaSuccess ? GNN_OK : GNN_ERR_CUDA;
+}
+
+int gnn_debug_edgeconv(gnn_model* m, int32_t block, const float* x_dev, const int32_t* idx_dev,
+                       const int32_t* offsets_dev, int32_t B, int32_t N, float* y_dev, void* cuda_stream) {
+    if (!m) return GNN_ERR_NULL;
+    if (block < 0 || block >= m->arch.n_blocks || B < 0 || N < 0) return GNN_ERR_BAD_ARG;
+    if (B > m->arch.max_batch_jets || (int64_t)N > m->Nmax) return GNN_ERR_BATCH_TOO_LARGE;
+    if (B == 0 || N == 0) return GNN_OK;
+    if (!offsets_dev || !idx_dev || !x_dev || !y_dev) return GNN_ERR_NULL;
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    Workspace& w = m->ws[0];
+    int n = 0, rc;
+    if ((rc = launch_ingest(offsets_dev, nullptr, B, N, (int)m->Nmax, m->arch.max_particles, w, s)) < 0) return rc;
+    n += rc;
+    if ((rc = launch_globalize_idx(idx_dev, m->arch.k, B, w, w.idx, s)) < 0) return rc;
+    n += rc;
+    if (m->arch.precision == GNN_BF16) rc = launch_edgeconv_bf16(*m, block, x_dev, w.idx, N, y_dev, w, s);
+    else rc = launch_edgeconv_f32(m->blocks[block], m->arch.k, x_dev, w.idx, N, y_dev, w, s);
+    if (rc < 0) return rc;
+    n += rc;
+    m->launches.fetch_add(n, std::memory_order_relaxed);
+    return cudaGetLastError() == cudaSuccess ? GNN_OK : GNN_ERR_CUDA;
+}
+
+int gnn_debug_pool_head(gnn_model* m, const float* x_dev, const int32_t* offsets_dev, int32_t B, int32_t N,
+                        float* logits_dev, void* cuda_stream) {
+    if (!m) return GNN_ERR_NULL;
+    if (B < 0 || N < 0) return GNN_ERR_BAD_ARG;
+    if (B > m->arch.max_batch_jets || (int64_t)N > m->Nmax) return GNN_ERR_BATCH_TOO_LARGE;
+    if (B == 0) return GNN_OK;
+    if (!offsets_dev || !logits_dev || (N > 0 && !x_dev)) return GNN_ERR_NULL;
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    Workspace& w = m->ws[0];
+    int n = 0, rc;
+    if ((rc = launch_ingest(offsets_dev, nullptr, B, N, (int)m->Nmax, m->arch.max_particles, w, s)) < 0) return rc;
+    n += rc;
+    if ((rc = launch_pool_head(*m, x_dev, B, w, logits_dev, s)) < 0) return rc;
+    n += rc;
+    m->launches.fetch_add(n, std::memory_order_relaxed);
+    return cudaGetLastError() == cudaSuccess ? GNN_OK : GNN_ERR_CUDA;
+}
+
+}  // extern "C"

@@ -1,0 +1,83 @@
+// gnn_internal.h -- host runtime structures and kernel launch prototypes of libgnn.so (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <atomic>
+#include <cstdint>
+#include <cstdio>
+#include <vector>
+#include "../../include/gnn.h"
+
+// device status bits (sticky word per workspace slice)
+enum : unsigned { GNN_DEV_BAD_OFFSETS = 1u, GNN_DEV_JET_TOO_LARGE = 2u };
+
+// One folded linear layer as the fp32 SIMT kernels read it: Wt [Kp][Nout] (transposed, K padded to a multiple of
+// 4 with zero rows), shift [Nout].  scale is already folded into Wt (include/gnn.h "Weight blob").
+struct LinF32 {
+    const float* Wt = nullptr;
+    const float* shift = nullptr;
+    int K = 0, Kp = 0, N = 0, ld = 0;   // ld = N rounded up to a multiple of 4 (row stride of Wt)
+};
+
+struct BlockDev {
+    int cin = 0, c1 = 0, c2 = 0, c3 = 0;
+    LinF32 l1, l2, l3, sc;   // fp32 path (and the shortcut / shifts in every mode)
+    // bf16 tcgen05 path (edgeconv_bf16.cu): per-particle pre-GEMM weights and packed edge-MLP weights
+    const void* bf16_pack = nullptr;
+};
+
+struct Workspace {
+    float* xa = nullptr;        // [Nmax, Cmax] ping
+    float* xb = nullptr;        // [Nmax, Cmax] pong
+    int32_t* idx = nullptr;     // [Nmax, k] global particle indices, -1 = none
+    int32_t* jet_start = nullptr;  // [Bmax] sanitised CSR
+    int32_t* jet_n = nullptr;      // [Bmax] sanitised multiplicities (< 0 = offending jet; -n if it owns n packed rows)
+    unsigned* status = nullptr;    // [1] sticky device status word
+    int32_t* meta = nullptr;       // [2] per call: meta[0] = batch poisoned, meta[1] = particles in the batch
+    // padded entry
+    float* pfeats = nullptr;    // [Nmax, F]
+    float* pcoords = nullptr;   // [Nmax, CD]
+    int32_t* poffsets = nullptr;  // [Bmax + 1]
+    int32_t* pcounts = nullptr;   // [Bmax]
+    void* bf16_scratch = nullptr;  // per-slice scratch of the bf16 path
+};
+
+struct gnn_model {
+    gnn_arch arch{};
+    int device = 0;
+    int n_sms = 148;
+    int64_t Nmax = 0;
+    int Cmax = 0;
+    std::vector<void*> allocs;          // everything cudaMalloc'ed, freed in gnn_destroy
+    BlockDev blocks[GNN_MAX_BLOCKS];
+    LinF32 fc[GNN_MAX_FC + 1];
+    int n_fc = 0;
+    std::vector<Workspace> ws;
+    std::atomic<int64_t> launches{0};
+};
+
+#define GNN_CUDA_TRY(expr)                                                              \
+    do {                                                                                \
+        cudaError_t _e = (expr);                                                        \
+        if (_e != cudaSuccess) {                                                        \
+            std::fprintf(stderr, "libgnn: %s failed: %s (%s:%d)\n", #expr, cudaGetErrorString(_e), __FILE__, __LINE__); \
+            return GNN_ERR_CUDA;                                                        \
+        }                                                                               \
+    } while (0)
+
+static inline int block_in(const gnn_arch& a, int l) { return l == 0 ? a.in_features : a.channels[l - 1][2]; }
+
+// ---- kernel launchers (each returns the number of kernels it enqueued, or a negative gnn_status) ----------------
+int launch_ingest(const int32_t* offsets, const int32_t* counts, int B, int N_exact, int N_cap, int max_particles,
+                  Workspace& w, cudaStream_t s);
+int launch_compact_padded(const float* feats, const float* coords, const float* mask, int B, int P, int F, int CD,
+                          int max_particles, Workspace& w, cudaStream_t s);
+// kNN: space [N, D]; out [N, k] global indices (local_out = 0) or jet-local (local_out = 1)
+int launch_knn(const float* space, int D, int k, int B, int max_particles, const Workspace& w, int32_t* idx_out,
+               int local_out, cudaStream_t s);
+int launch_edgeconv_f32(const BlockDev& b, int k, const float* x, const int32_t* idx, int N, float* y,
+                        const Workspace& w, cudaStream_t s);
+int launch_globalize_idx(const int32_t* idx_local, int k, int B, const Workspace& w, int32_t* idx_global, cudaStream_t s);
+int launch_pool_head(const gnn_model& m, const float* x, int B, const Workspace& w, float* logits, cudaStream_t s);
+int knn_configure();
+int edgeconv_f32_configure();
+

@@ -1,0 +1,123 @@
+// ingest.cu -- step a0 of the hot path: ragged descriptors (BASELINE.json north_star subsystem (4), padding-free
+// handling of the ragged batch) and the stable compaction behind the padded entry point (features,
+// coordinates, mask; R7: masked particles do not exist).
+#include "gnn_internal.h"
+
+// One CTA walks all jets: sanitised (start, n) so that no later kernel can index out of bounds whatever the caller's
+// offsets hold.  Globally inconsistent offsets poison the whole batch (meta[0] = 1, GNN_DEV_BAD_OFFSETS); a jet
+// larger than max_particles poisons only itself (jet_n < 0, GNN_DEV_JET_TOO_LARGE).  meta[1] = number of particles
+// later kernels may touch.  `counts` (padded entry only) carries -1 for jets whose mask selected too many slots.
+__global__ void __launch_bounds__(1024) ingest_kernel(const int32_t* __restrict__ offsets,
+                                                      const int32_t* __restrict__ counts, int B, int N_exact, int N_cap,
+                                                      int max_particles, int32_t* __restrict__ jet_start,
+                                                      int32_t* __restrict__ jet_n, int32_t* __restrict__ meta,
+                                                      unsigned* status) {
+    int any_bad = 0, any_big = 0;
+    for (int b = threadIdx.x; b < B; b += blockDim.x) {
+        int s = offsets[b], e = offsets[b + 1];
+        bool bad = (s < 0) || (e < s) || (e > N_cap) || (b == 0 && s != 0) || (N_exact >= 0 && b == B - 1 && e != N_exact);
+        int n = e - s;
+        if (bad) { any_bad = 1; s = 0; n = -1; }
+        else if (counts != nullptr && counts[b] < 0) { any_big = 1; n = -1; }       // padded: owns no packed rows
+        else if (n > max_particles) { any_big = 1; n = -n; }                        // ragged: jet_n = -multiplicity
+        jet_start[b] = s;
+        jet_n[b] = n;
+    }
+    any_bad = __syncthreads_or(any_bad);
+    any_big = __syncthreads_or(any_big);
+    if (threadIdx.x == 0) {
+        meta[0] = any_bad;
+        meta[1] = any_bad ? 0 : offsets[B];
+        if (any_bad) atomicOr(status, GNN_DEV_BAD_OFFSETS);
+        if (any_big) atomicOr(status, GNN_DEV_JET_TOO_LARGE);
+    }
+}
+
+int launch_ingest(const int32_t* offsets, const int32_t* counts, int B, int N_exact, int N_cap, int max_particles,
+                  Workspace& w, cudaStream_t s) {
+    ingest_kernel<<<1, 1024, 0, s>>>(offsets, counts, B, N_exact, N_cap, max_particles, w.jet_start, w.jet_n, w.meta, w.status);
+    return 1;
+}
+
+// ---- padded entry: count -> exclusive scan -> stable scatter ----------------------------------------------------
+__global__ void count_mask_kernel(const float* __restrict__ mask, int B, int P, int max_particles,
+                                  int32_t* __restrict__ counts) {
+    int b = blockIdx.x;
+    int c = 0;
+    for (int p = threadIdx.x; p < P; p += blockDim.x) c += (mask[(size_t)b * P + p] != 0.0f) ? 1 : 0;
+    __shared__ int red[32];
+    for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = c;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int t = 0;
+        for (int i = 0; i < (int)(blockDim.x + 31) / 32; ++i) t += red[i];
+        counts[b] = (t > max_particles) ? -1 : t;     // -1: offending jet, contributes no rows
+    }
+}
+
+// single CTA, B <= a few 10^4: chunked Hillis-Steele scan in shared memory
+__global__ void scan_counts_kernel(const int32_t* __restrict__ counts, int B, int32_t* __restrict__ offsets) {
+    __shared__ int buf[1024];
+    __shared__ int carry;
+    if (threadIdx.x == 0) { carry = 0; offsets[0] = 0; }
+    __syncthreads();
+    for (int base = 0; base < B; base += 1024) {
+        int i = base + threadIdx.x;
+        int v = (i < B) ? max(counts[i], 0) : 0;
+        buf[threadIdx.x] = v;
+        __syncthreads();
+        for (int o = 1; o < 1024; o <<= 1) {
+            int t = (threadIdx.x >= (unsigned)o) ? buf[threadIdx.x - o] : 0;
+            __syncthreads();
+            buf[threadIdx.x] += t;
+            __syncthreads();
+        }
+        if (i < B) offsets[i + 1] = carry + buf[threadIdx.x];
+        __syncthreads();
+        if (threadIdx.x == 1023) carry += buf[1023];
+        __syncthreads();
+    }
+}
+
+// one CTA (128 threads = 4 warps) per jet; slots are walked in order in chunks of 128 so the compaction is stable
+__global__ void scatter_padded_kernel(const float* __restrict__ feats, const float* __restrict__ coords,
+                                      const float* __restrict__ mask, int P, int F, int CD, int max_particles,
+                                      const int32_t* __restrict__ offsets, const int32_t* __restrict__ counts,
+                                      float* __restrict__ pfeats, float* __restrict__ pcoords) {
+    int b = blockIdx.x;
+    int base_out = offsets[b];
+    if (counts[b] < 0) return;             // offending jet: ingest flags it, it owns no packed rows
+    __shared__ int wsum[4];
+    __shared__ int running;
+    if (threadIdx.x == 0) running = 0;
+    __syncthreads();
+    for (int p0 = 0; p0 < P; p0 += 128) {
+        int p = p0 + threadIdx.x;
+        bool keep = (p < P) && (mask[(size_t)b * P + p] != 0.0f);
+        unsigned bal = __ballot_sync(0xffffffffu, keep);
+        int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+        if (lane == 0) wsum[wid] = __popc(bal);
+        __syncthreads();
+        int pre = running;
+        for (int i = 0; i < wid; ++i) pre += wsum[i];
+        pre += __popc(bal & ((1u << lane) - 1u));
+        if (keep) {
+            size_t src = (size_t)b * P + p, dst = (size_t)base_out + pre;
+            for (int c = 0; c < F; ++c) pfeats[dst * F + c] = feats[src * F + c];
+            for (int c = 0; c < CD; ++c) pcoords[dst * CD + c] = coords[src * CD + c];
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) running += wsum[0] + wsum[1] + wsum[2] + wsum[3];
+        __syncthreads();
+    }
+}
+
+int launch_compact_padded(const float* feats, const float* coords, const float* mask, int B, int P, int F, int CD,
+                          int max_particles, Workspace& w, cudaStream_t s) {
+    if (B == 0) return 0;
+    count_mask_kernel<<<B, 128, 0, s>>>(mask, B, P, max_particles, w.pcounts);
+    scan_counts_kernel<<<1, 1024, 0, s>>>(w.pcounts, B, w.poffsets);
+    scatter_padded_kernel<<<B, 128, 0, s>>>(feats, coords, mask, P, F, CD, max_particles, w.poffsets, w.pcounts, w.pfeats, w.pcoords);
+    return 3;
+}

@@ -1,0 +1,81 @@
+"""Host-side checks that need no GPU: libgnn.so builds, loads and exports every symbol include/gnn.h declares;
+argument validation that happens before any CUDA call."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+import synth
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2312_06838_b200 import build
+    build.build()
+    import paper_2312_06838_b200 as gnn
+    return gnn.lib()
+
+
+def test_exports_every_declared_symbol(lib):
+    hdr = open(os.path.join(ROOT, "include", "gnn.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    names = sorted(set(re.findall(r"\b(gnn_[a-z_0-9]+)\s*\(", hdr)))
+    assert len(names) == 17
+    for n in names:
+        assert hasattr(lib, n), "libgnn.so does not export %s" % n
+
+
+def test_weights_bytes_and_arch_validation(lib):
+    import paper_2312_06838_b200 as gnn
+    for name, cnt in (("particlenet", 366146), ("wide", 1453186), ("tiny", 2754)):
+        a = gnn.arch_struct(synth.ARCHS[name])
+        assert gnn.weights_bytes(a) == 4 * cnt == 4 * synth.weight_count(synth.ARCHS[name])
+    bad = gnn.arch_struct(synth.ARCHS["particlenet"])
+    bad.k = 0
+    n = C.c_size_t(0)
+    assert lib.gnn_weights_bytes(C.byref(bad), C.byref(n)) == -2
+    bad = gnn.arch_struct(synth.ARCHS["particlenet"])
+    bad.channels[1][1] = 100                       # not a multiple of 8
+    assert lib.gnn_weights_bytes(C.byref(bad), C.byref(n)) == -2
+    assert lib.gnn_weights_bytes(None, C.byref(n)) == -1
+    assert b"no CPU fallback" in lib.gnn_strerror(-5)
+
+
+def test_create_rejects_wrong_blob_size_before_touching_cuda(lib):
+    import paper_2312_06838_b200 as gnn
+    a = gnn.arch_struct(synth.ARCHS["tiny"])
+    w = np.zeros(10, np.float32)
+    h = C.c_void_p()
+    assert lib.gnn_create(w.ctypes.data_as(C.c_void_p), w.nbytes, C.byref(a), 0, C.byref(h)) == -3
+    assert lib.gnn_create(None, 0, C.byref(a), 0, C.byref(h)) == -1
+
+
+def test_no_cpu_fallback_without_a_gpu(lib):
+    """On a box without a CUDA device gnn_create must fail loudly (GNN_ERR_CUDA), never compute on the CPU."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    import paper_2312_06838_b200 as gnn
+    a = synth.ARCHS["tiny"]
+    with pytest.raises(gnn.GnnError) as e:
+        gnn.Model(gnn.arch_struct(a), synth.make_weights(a))
+    assert e.value.code == -5
+
+
+def test_product_does_not_import_the_oracle():
+    pkg = os.path.join(ROOT, "paper_2312_06838_b200")
+    for dp, _, fs in os.walk(pkg):
+        if os.path.basename(dp) == "build":
+            continue
+        for f in fs:
+            if f.endswith((".py", ".cu", ".h", ".cpp", ".cuh")):
+                src = open(os.path.join(dp, f)).read()
+                assert not re.search(r"^\s*(import|from)\s+oracle", src, flags=re.M), f
+                assert "oracle/" not in src and "liboracle" not in src, f
+    osrc = open(os.path.join(ROOT, "oracle", "__init__.py")).read() + open(os.path.join(ROOT, "oracle", "oracle.c")).read()
+    assert not re.search(r"^\s*(import|from)\s+paper_2312_06838_b200", osrc, flags=re.M)
+    assert "gnn.h\"" not in osrc
