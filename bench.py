@@ -1,0 +1,337 @@
+#!/usr/bin/env python
+"""bench.py -- jets/s of the EdgeConv-GNN forward (BASELINE.json metric) on N B200s of one node.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--precision bf16|fp32]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 --master-port P \
+        bench.py --gpus N --steps K --warmup W
+
+A step = one pass of the whole hot path (ingest, 3 x [kNN, EdgeConv], pool + head) over one batch of
+BASELINE.json configs[1]: 1024 seeded synthetic jets, multiplicity ~ clip(Poisson(40), 5, 100), 7 features, k = 16,
+delivered ragged (padding-free) through gnn_infer.  Prints ONE JSON line (rank 0).  Keys beyond the base contract:
+  roofline      dominant kernel (EdgeConv block 3): algorithmic FLOPs / CUDA-event duration vs the measured bf16 peak
+  forward       whole-forward algorithmic FLOPs / ms_per_step vs the same peak (the north_star's 50 % target)
+  stages_ms     mean CUDA-event time of every stage over the timed steps (gnn_profile_*)
+  e2e           same metric through gnn_infer_host: pinned host buffers in, logits in host memory out, per step
+  latency_b16   p50 / p99 of one gnn_infer on a device-resident 16-jet batch (the metric's second half)
+  cpu_baseline  the fp64 oracle as it stands, on the box's host cores, on a bounded sample of the same batch
+Multi-GPU: jets are independent and the weights are < 3 MB, so the path shards by jets with no collective ("replicas
+only"): every rank runs its own batches; value = all ranks' jets / max-over-ranks time.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "jets/s (EdgeConv GNN, P=100, k=16, bf16) on 1 B200"
+UNIT = "jets/s"
+WORKLOAD = "configs[1] ParticleNet-shaped: B=1024 ragged jets, n~clip(Poisson(40),5,100), F=7, k=16, (64,128,256)"
+N_BATCHES = 4                      # distinct pre-generated batches the steps rotate over (seeds 1002 + 10000 r)
+FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+
+
+def parse_args():
+    p = argparse.ArgumentParser()
+    p.add_argument("--gpus", type=int, default=1)
+    p.add_argument("--steps", type=int, default=200)
+    p.add_argument("--warmup", type=int, default=20)
+    p.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    p.add_argument("--precision", default="bf16", choices=["bf16", "fp32"])
+    p.add_argument("--batch", type=int, default=1024)
+    p.add_argument("--no-cpu-baseline", action="store_true")
+    p.add_argument("--no-extras", action="store_true", help="skip the e2e / latency / cpu_baseline legs (profiling runs)")
+    return p.parse_args()
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        d = json.load(open(path))
+        d["_source"] = "measured (MEASURED_PEAKS.json)"
+        return d
+    d = dict(FALLBACK_PEAKS)
+    d["_source"] = "fallback (B200_PROFILING.md)"
+    return d
+
+
+# ---- algorithmic work -- counting only, no arithmetic of the method ----
+def work(arch, counts):
+    """FLOPs of one forward over jets with multiplicities `counts`.  'min' is the factorised form (layer 1 is linear
+    in [x_i ; x_j - x_i], so it needs two per-particle GEMMs, not one per edge) and is the roofline numerator whatever
+    the kernel does; 'stated' forms every edge feature.  Returns per-block and total FLOPs (2 per MAC)."""
+    counts = np.asarray(counts, np.int64)
+    keff = np.minimum(arch.k, np.maximum(counts - 1, 0))
+    n_pts, n_edges = int(counts.sum()), int((counts * keff).sum())
+    blocks_min, blocks_stated = [], []
+    for l, (c1, c2, c3) in enumerate(arch.channels):
+        cin = arch.block_in(l)
+        blocks_min.append(2 * (n_pts * (2 * cin * c1 + cin * c3) + n_edges * (c1 * c2 + c2 * c3)))
+        blocks_stated.append(2 * (n_pts * cin * c3 + n_edges * (2 * cin * c1 + c1 * c2 + c2 * c3)))
+    head, i = 0, arch.channels[-1][2]
+    for d in tuple(arch.fc_hidden) + (arch.n_classes,):
+        head += 2 * d * i * len(counts)
+        i = d
+    return {"blocks_min": blocks_min, "blocks_stated": blocks_stated, "head": head,
+            "min": sum(blocks_min) + head, "stated": sum(blocks_stated) + head}
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock, power and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.stop_flag, self.samples, self.reasons, self.err = index, False, [], 0, None
+        self.sm_max = None
+
+    def run(self):
+        try:
+            import pynvml as nv
+            nv.nvmlInit()
+            h = nv.nvmlDeviceGetHandleByIndex(self.index)
+            self.sm_max = int(nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM))
+            while not self.stop_flag:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM)))
+                self.reasons |= int(nv.nvmlDeviceGetCurrentClocksEventReasons(h))
+                time.sleep(0.004)
+        except Exception as e:                     # noqa: BLE001 -- clocks are a side record, never fatal
+            self.err = repr(e)
+
+    def summary(self):
+        names = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap",
+                 0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x100: "display_clock_setting"}
+        out = {"sm_mhz": float(np.median(self.samples)) if self.samples else None, "sm_max_mhz": self.sm_max,
+               "reasons": [n for b, n in names.items() if self.reasons & b], "samples": len(self.samples)}
+        if self.err:
+            out["error"] = self.err
+        return out
+
+
+def dist_env():
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return rank, world, local
+
+
+def make_batches(synth, rank, n_jets):
+    return [synth.make_particlenet_batch(seed=1002 + 10000 * r + 1000003 * rank, n_jets=n_jets) for r in range(N_BATCHES)]
+
+
+def time_oracle(arch, weights, batch, n_jets):
+    import oracle
+    sub = batch.head(min(n_jets, batch.n_jets))
+    t0 = time.perf_counter()
+    oracle.forward(arch, weights, sub.feats, sub.coords, sub.offsets)
+    return sub.n_jets, time.perf_counter() - t0
+
+
+def cpu_baseline(arch, weights, batch, target_s=12.0):
+    """The oracle as it stands, all host cores (OpenMP over jets), on the first jets of the timed batch."""
+    import oracle
+    n0, t0 = time_oracle(arch, weights, batch, 32)
+    n = int(max(32, min(batch.n_jets, n0 / t0 * target_s)))
+    n, t = time_oracle(arch, weights, batch, n)
+    return {"value": n / t, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle",
+            "sample": "first %d jets of batch 0 (%d particles), one oracle.forward call, %.1f s" %
+                      (n, int(batch.offsets[n]), t)}
+
+
+def run_reference(args):
+    """--impl reference: the fp64 oracle timed on the host cores; each step is a bounded sample of the workload."""
+    rank, world, _ = dist_env()
+    if rank != 0:
+        return
+    import oracle
+    import synth
+    arch = synth.ARCHS["particlenet"]
+    weights = synth.make_weights(arch)
+    batch = synth.make_particlenet_batch(seed=1002, n_jets=args.batch)
+    n0, t0 = time_oracle(arch, weights, batch, 16)
+    total = max(1, args.steps + args.warmup)
+    per_step = int(max(4, min(batch.n_jets, (n0 / t0) * 100.0 / total)))
+    starts = [(i * per_step) % max(1, batch.n_jets - per_step + 1) for i in range(total)]
+    subs = {s: batch.select(range(s, s + per_step)) for s in set(starts)}
+    for i in range(args.warmup):
+        s = subs[starts[i]]
+        oracle.forward(arch, weights, s.feats, s.coords, s.offsets)
+    t = time.perf_counter()
+    for i in range(args.warmup, total):
+        s = subs[starts[i]]
+        oracle.forward(arch, weights, s.feats, s.coords, s.offsets)
+    dt = time.perf_counter() - t
+    val = per_step * args.steps / dt
+    sample = "%d-jet slices of the B=%d batch, one oracle.forward per step" % (per_step, batch.n_jets)
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "sample": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import synth
+    import paper_2312_06838_b200 as gnn
+
+    rank, world, local = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    pk = peaks()
+    arch = synth.ARCHS["particlenet"]
+    weights = synth.make_weights(arch)
+    prec = gnn.BF16 if args.precision == "bf16" else gnn.FP32_VALIDATION
+    B = args.batch
+    model = gnn.Model(gnn.arch_struct(arch, max_batch_jets=B, precision=prec, max_particles=128), weights, device=local)
+    batches = make_batches(synth, rank, B)
+    dev = torch.device("cuda", local)
+    dbat = [(torch.from_numpy(b.feats).to(dev), torch.from_numpy(b.coords).to(dev), torch.from_numpy(b.offsets).to(dev))
+            for b in batches]
+    logits = torch.empty((B, arch.n_classes), dtype=torch.float32, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)        # 2 x L2 (126 MB)
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident leg: K steps, each bracketed by its own CUDA events, L2 flushed between steps ------------
+    for i in range(args.warmup):
+        f, c, o = dbat[i % N_BATCHES]
+        model.infer(f, c, o, logits=logits)
+    barrier()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    sampler = ClockSampler(local)
+    sampler.start()
+    launches0 = model.launch_count()
+    model.profile_enable(True)
+    barrier()
+    wall0 = time.perf_counter()
+    for i in range(args.steps):
+        f, c, o = dbat[i % N_BATCHES]
+        flush.zero_()                               # outside the timed events: evicts the previous step from L2
+        ev[i][0].record(stream)
+        model.infer(f, c, o, logits=logits)
+        ev[i][1].record(stream)
+    barrier()
+    wall = time.perf_counter() - wall0
+    sampler.stop_flag = True
+    model.profile_enable(False)
+    launches = model.launch_count() - launches0
+    assert model.status_check() == 0
+    step_ms = np.array([a.elapsed_time(b) for a, b in ev])
+    total_ms = float(step_ms.sum())
+    t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms_max = float(t.item())
+    jets_total = B * args.steps * world
+    value = jets_total / (total_ms_max * 1e-3)
+    stages, n_fw = model.profile_read()
+    sampler.join(1.0)
+
+    # ---- work accounting and rooflines ----------------------------------------------------------------------------
+    wk = [work(arch, b.counts()) for b in batches]
+    steps_of = [len(range(r, args.steps, N_BATCHES)) for r in range(N_BATCHES)]
+    mean_of = lambda key, idx=None: sum((w[key] if idx is None else w[key][idx]) * s for w, s in zip(wk, steps_of)) / max(1, args.steps)
+    peak_tf = pk["bf16_tflops"] if args.precision == "bf16" else None
+    dom = max((s for s in stages if s[0].startswith("edgeconv")), key=lambda s: s[1])
+    dom_l = int(dom[0][len("edgeconv"):])
+    dom_flops = mean_of("blocks_min", dom_l)
+    roof_peak = pk["bf16_tflops"]
+    roofline = {"bound": "tensor", "kernel": dom[0], "achieved": dom_flops / (dom[1] * 1e-3) / 1e12, "peak": roof_peak,
+                "unit": "TFLOP/s", "frac": dom_flops / (dom[1] * 1e-3) / 1e12 / roof_peak, "traffic": None,
+                "peak_source": pk["_source"] + ", burst cuBLAS bf16", "flops_per_launch_min": dom_flops,
+                "flops_per_launch_stated": mean_of("blocks_stated", dom_l), "ms_per_launch": dom[1],
+                "forwards_averaged": n_fw}
+    ms_per_step = total_ms_max / args.steps
+    fwd = {"flops_min": mean_of("min"), "flops_stated": mean_of("stated"),
+           "achieved_tflops": mean_of("min") / (ms_per_step * 1e-3) / 1e12,
+           "frac_of_bf16_peak": mean_of("min") / (ms_per_step * 1e-3) / 1e12 / roof_peak,
+           "t_roof_us": mean_of("min") / (roof_peak * 1e12) * 1e6}
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "bf16" if args.precision == "bf16" else "f32", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "batch_jets": B, "particles_per_batch": [int(b.n_particles) for b in batches],
+                   "entry": "gnn_infer (ragged, device-resident)", "precision": args.precision,
+                   "parallelism": "replicas only (jets sharded, no collective)" if world > 1 else "1 GPU",
+                   "l2": "flushed between steps (256 MiB memset outside the per-step CUDA events); %d batches rotate" % N_BATCHES},
+        "roofline": roofline, "forward": fwd, "stages_ms": {k: v for k, v in stages},
+        "gpu_launches": int(launches), "wall_s_timed_region": wall,
+    }
+
+    if not args.no_extras:
+        # ---- e2e: the same step through gnn_infer_host, pinned host buffers, logits back in host memory ------------
+        hbat = [(torch.from_numpy(b.feats).pin_memory(), torch.from_numpy(b.coords).pin_memory(),
+                 torch.from_numpy(b.offsets).pin_memory()) for b in batches]
+        hlog = torch.empty((B, arch.n_classes), dtype=torch.float32).pin_memory()
+        for i in range(max(3, args.warmup // 4)):
+            model.infer_host(*hbat[i % N_BATCHES], hlog)
+        barrier()
+        t0 = time.perf_counter()
+        for i in range(args.steps):
+            model.infer_host(*hbat[i % N_BATCHES], hlog)
+        torch.cuda.synchronize()
+        dt = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(dt, op=dist.ReduceOp.MAX)
+        h2d = int(np.mean([b.feats.nbytes + b.coords.nbytes + b.offsets.nbytes for b in batches]))
+        out["e2e"] = {"value": jets_total / float(dt.item()), "unit": UNIT, "h2d_bytes_per_step": h2d,
+                      "d2h_bytes_per_step": int(B * arch.n_classes * 4), "entry": "gnn_infer_host (blocking, pinned host buffers)",
+                      "ms_per_step": float(dt.item()) / args.steps * 1e3}
+        # ---- p50 / p99 latency of a device-resident 16-jet batch -------------------------------------------------
+        if rank == 0:
+            b16 = batches[0].head(16)
+            f, c, o = (torch.from_numpy(x).to(dev) for x in (b16.feats, b16.coords, b16.offsets))
+            l16 = torch.empty((16, arch.n_classes), dtype=torch.float32, device=dev)
+            for _ in range(50):
+                model.infer(f, c, o, logits=l16)
+            n_it = 1000
+            e16 = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n_it)]
+            torch.cuda.synchronize()
+            for a, b in e16:
+                a.record(stream)
+                model.infer(f, c, o, logits=l16)
+                b.record(stream)
+            torch.cuda.synchronize()
+            lat = np.array([a.elapsed_time(b) for a, b in e16]) * 1e3
+            out["latency_b16"] = {"p50_us": float(np.percentile(lat, 50)), "p99_us": float(np.percentile(lat, 99)),
+                                  "iterations": n_it, "entry": "gnn_infer, 16 jets device-resident, CUDA events"}
+    out["clocks"] = sampler.summary()
+    if rank == 0 and world == 1 and not args.no_cpu_baseline and not args.no_extras:
+        out["cpu_baseline"] = cpu_baseline(arch, weights, batches[0])
+    model.close()
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(out))
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        from paper_2312_06838_b200 import build
+        build.build()
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -111,9 +111,27 @@ int gnn_infer_padded(gnn_model* m, const float* feats_dev, const float* coords_d
  * GNN_ERR_JET_TOO_LARGE, or GNN_ERR_CUDA if the stream reports an error). */
 int gnn_status_check(gnn_model* m, int32_t slice, void* cuda_stream);
 
+/* The same forward from HOST buffers (layouts as gnn_infer; pinned memory makes the copies asynchronous): copies the
+ * inputs to device staging owned by `slice`, runs the forward, copies logits_host [B, n_classes] back and
+ * synchronises `cuda_stream` before returning.  This is the one blocking inference call.  Device-side errors are
+ * returned directly (the sticky word is read and cleared). */
+int gnn_infer_host(gnn_model* m, int32_t slice, const float* feats_host, const float* coords_host,
+                   const int32_t* offsets_host, int32_t B, int32_t N, float* logits_host, void* cuda_stream);
+
 const char* gnn_strerror(int status);
 /* number of kernels the library has launched on this model since gnn_create (bench.py's gpu_launches) */
 int64_t gnn_launch_count(const gnn_model* m);
+
+/* ---- stage timing (bench.py's roofline leg) ---------------------------------------------------------------------
+ * While enabled for a slice, every gnn_infer* on it records one CUDA event before the first and after each stage
+ * (ingest, kNN l, EdgeConv l, ..., pool+head) on the caller's stream; up to 512 forwards are kept.  gnn_profile_read
+ * synchronises on the recorded events and writes the mean milliseconds per stage over the recorded forwards;
+ * *n_stages_out = stages of one forward, *n_forwards_out = forwards averaged.  Enabling clears earlier records. */
+int gnn_profile_enable(gnn_model* m, int32_t slice, int32_t on);
+int gnn_profile_read(gnn_model* m, int32_t slice, int32_t max_stages, float* ms_mean_out, int32_t* n_stages_out,
+                     int32_t* n_forwards_out);
+/* name of stage `stage` of the last recorded forward ("ingest", "knn0", "edgeconv0", ..., "pool_head"), or NULL */
+const char* gnn_profile_stage_name(gnn_model* m, int32_t slice, int32_t stage);
 
 /* ---- per-stage entry points: the same kernels the forward uses, exposed for stage-wise parity tests --------- */
 /* kNN on an arbitrary space [N, D] (1 <= D <= 1024): idx_dev int32 [N, k], jet-local indices in (d, j) order,

@@ -49,6 +49,10 @@ def lib():
         L.gnn_infer_slice.argtypes = [vp, i32, f32p, f32p, i32p, i32, i32, f32p, vp]
         L.gnn_infer_padded.argtypes = [vp, f32p, f32p, f32p, i32, i32, f32p, vp]
         L.gnn_status_check.argtypes = [vp, i32, vp]
+        L.gnn_infer_host.argtypes = [vp, i32, vp, vp, vp, i32, i32, vp, vp]
+        L.gnn_profile_enable.argtypes = [vp, i32, i32]
+        L.gnn_profile_read.argtypes = [vp, i32, i32, C.POINTER(C.c_float), C.POINTER(i32), C.POINTER(i32)]
+        L.gnn_profile_stage_name.argtypes = [vp, i32, i32]; L.gnn_profile_stage_name.restype = C.c_char_p
         L.gnn_strerror.argtypes = [C.c_int]; L.gnn_strerror.restype = C.c_char_p
         L.gnn_launch_count.argtypes = [vp]; L.gnn_launch_count.restype = C.c_int64
         L.gnn_debug_knn.argtypes = [vp, f32p, i32, i32p, i32, i32, i32, i32p, vp]
@@ -94,6 +98,14 @@ def weights_bytes(arch: GnnArch) -> int:
 
 def _ptr(t):
     return None if t is None else C.c_void_p(t.data_ptr())
+
+
+def _hptr(t):
+    if t is None:
+        return None
+    if isinstance(t, np.ndarray):
+        return t.ctypes.data_as(C.c_void_p)
+    return C.c_void_p(t.data_ptr())
 
 
 def _stream(stream):
@@ -145,6 +157,25 @@ class Model:
         self._check(lib().gnn_infer_padded(self.h, _ptr(feats), _ptr(coords), _ptr(mask), B, P, _ptr(logits),
                                            _stream(stream)), "gnn_infer_padded")
         return logits
+
+    def infer_host(self, feats, coords, offsets, logits, stream=None, slice=0):
+        """gnn_infer_host: host tensors / arrays in (torch CPU tensors, ideally pinned, or numpy), logits written into
+        `logits` (host).  Blocks until the logits are in host memory."""
+        B, N = int(offsets.shape[0]) - 1, int(feats.shape[0])
+        self._check(lib().gnn_infer_host(self.h, slice, _hptr(feats), _hptr(coords), _hptr(offsets), B, N,
+                                         _hptr(logits), _stream(stream)), "gnn_infer_host")
+        return logits
+
+    def profile_enable(self, on=True, slice=0):
+        self._check(lib().gnn_profile_enable(self.h, slice, 1 if on else 0), "gnn_profile_enable")
+
+    def profile_read(self, slice=0):
+        """-> (list of (stage name, mean ms), forwards averaged)"""
+        ms = (C.c_float * 64)()
+        ns, nf = C.c_int32(0), C.c_int32(0)
+        self._check(lib().gnn_profile_read(self.h, slice, 64, ms, C.byref(ns), C.byref(nf)), "gnn_profile_read")
+        names = [(lib().gnn_profile_stage_name(self.h, slice, i) or b"?").decode() for i in range(ns.value)]
+        return list(zip(names, [float(ms[i]) for i in range(ns.value)])), int(nf.value)
 
     def status_check(self, slice=0, stream=None) -> int:
         return int(lib().gnn_status_check(self.h, slice, _stream(stream)))

@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstring>
 #include <new>
+#include <string>
 
 int edgeconv_bf16_prepare(gnn_model& m, const float* blob_host);       // edgeconv_bf16.cu
 int launch_edgeconv_bf16(gnn_model& m, int block, const float* x, const int32_t* idx, int N, float* y, Workspace& w,
@@ -136,18 +137,45 @@ int alloc_workspace(gnn_model* m, Workspace& w) {
     if ((rc = dev_alloc(m, &w.pcoords, Nmax * a.coord_dims)) != GNN_OK) return rc;
     if ((rc = dev_alloc(m, &w.poffsets, Bmax + 1)) != GNN_OK) return rc;
     if ((rc = dev_alloc(m, &w.pcounts, Bmax)) != GNN_OK) return rc;
+    if ((rc = dev_alloc(m, &w.hlogits, Bmax * a.n_classes)) != GNN_OK) return rc;
     GNN_CUDA_TRY(cudaMemset(w.status, 0, sizeof(unsigned)));
     GNN_CUDA_TRY(cudaMemset(w.meta, 0, 2 * sizeof(int32_t)));
     return GNN_OK;
 }
+
+// stage timing: one event before the first stage and one after each stage, on the caller's stream
+struct StageTimer {
+    Workspace& w; cudaStream_t s; bool on; int stage = 0; size_t base = 0;
+    StageTimer(Workspace& w_, cudaStream_t s_, int n_stages) : w(w_), s(s_) {
+        on = w.prof_on && w.prof_forwards < PROF_MAX_FORWARDS;
+        if (!on) return;
+        if (w.prof_stages != n_stages) { w.prof_stages = n_stages; w.prof_names.assign(n_stages, ""); w.prof_forwards = 0; }
+        base = (size_t)w.prof_forwards * (n_stages + 1);
+        while (w.prof_events.size() < base + n_stages + 1) {
+            cudaEvent_t e = nullptr;
+            if (cudaEventCreate(&e) != cudaSuccess) { on = false; return; }
+            w.prof_events.push_back(e);
+        }
+        cudaEventRecord(w.prof_events[base], s);
+    }
+    void mark(const char* name, int l = -1) {
+        if (!on) return;
+        if (w.prof_names[stage].empty()) w.prof_names[stage] = l < 0 ? std::string(name) : std::string(name) + std::to_string(l);
+        cudaEventRecord(w.prof_events[base + stage + 1], s);
+        ++stage;
+    }
+    ~StageTimer() { if (on) ++w.prof_forwards; }
+};
 
 // the launch plan of one forward (SURVEY.md call stack (4)): ingest -> per block [kNN, EdgeConv] -> pool + head
 int forward(gnn_model* m, Workspace& w, const float* feats, const float* coords, const int32_t* offsets,
             const int32_t* counts, int B, int N_exact, int N_upper, float* logits, cudaStream_t s) {
     const gnn_arch& a = m->arch;
     int n = 0, rc;
+    StageTimer tm(w, s, 2 + 2 * a.n_blocks);
     if ((rc = launch_ingest(offsets, counts, B, N_exact, (int)m->Nmax, a.max_particles, w, s)) < 0) return rc;
     n += rc;
+    tm.mark("ingest");
     const float* x = feats;
     float* bufs[2] = {w.xa, w.xb};
     for (int l = 0; l < a.n_blocks; ++l) {
@@ -155,15 +183,18 @@ int forward(gnn_model* m, Workspace& w, const float* feats, const float* coords,
         int D = (l == 0) ? a.coord_dims : block_in(a, l);
         if ((rc = launch_knn(space, D, a.k, B, a.max_particles, w, w.idx, 0, s)) < 0) return rc;
         n += rc;
+        tm.mark("knn", l);
         float* y = bufs[l & 1];
         if (a.precision == GNN_BF16) rc = launch_edgeconv_bf16(*m, l, x, w.idx, N_upper, y, w, s);
         else rc = launch_edgeconv_f32(m->blocks[l], a.k, x, w.idx, N_upper, y, w, s);
         if (rc < 0) return rc;
         n += rc;
+        tm.mark("edgeconv", l);
         x = y;
     }
     if ((rc = launch_pool_head(*m, x, B, w, logits, s)) < 0) return rc;
     n += rc;
+    tm.mark("pool_head");
     m->launches.fetch_add(n, std::memory_order_relaxed);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) {
@@ -230,6 +261,8 @@ void gnn_destroy(gnn_model* m) {
     cudaSetDevice(m->device);
     cudaDeviceSynchronize();
     for (void* p : m->allocs) cudaFree(p);
+    for (auto& w : m->ws)
+        for (cudaEvent_t e : w.prof_events) cudaEventDestroy(e);
     delete m;
 }
 
@@ -266,6 +299,66 @@ int gnn_infer_padded(gnn_model* m, const float* feats_dev, const float* coords_d
     m->launches.fetch_add(rc, std::memory_order_relaxed);
     int64_t upper = std::min<int64_t>((int64_t)B * std::min<int>(P, m->arch.max_particles), m->Nmax);
     return forward(m, w, w.pfeats, w.pcoords, w.poffsets, w.pcounts, B, -1, (int)upper, logits_dev, s);
+}
+
+int gnn_infer_host(gnn_model* m, int32_t slice, const float* feats_host, const float* coords_host,
+                   const int32_t* offsets_host, int32_t B, int32_t N, float* logits_host, void* cuda_stream) {
+    if (!m) return GNN_ERR_NULL;
+    if (B < 0 || N < 0) return GNN_ERR_BAD_ARG;
+    if (slice < 0 || slice >= (int)m->ws.size()) return GNN_ERR_BATCH_TOO_LARGE;
+    if (B > m->arch.max_batch_jets || (int64_t)N > m->Nmax) return GNN_ERR_BATCH_TOO_LARGE;
+    if (B == 0) return GNN_OK;
+    if (!offsets_host || !logits_host || (N > 0 && (!feats_host || !coords_host))) return GNN_ERR_NULL;
+    const gnn_arch& a = m->arch;
+    Workspace& w = m->ws[slice];
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    if (N > 0) {
+        GNN_CUDA_TRY(cudaMemcpyAsync(w.pfeats, feats_host, (size_t)N * a.in_features * sizeof(float), cudaMemcpyHostToDevice, s));
+        GNN_CUDA_TRY(cudaMemcpyAsync(w.pcoords, coords_host, (size_t)N * a.coord_dims * sizeof(float), cudaMemcpyHostToDevice, s));
+    }
+    GNN_CUDA_TRY(cudaMemcpyAsync(w.poffsets, offsets_host, (size_t)(B + 1) * sizeof(int32_t), cudaMemcpyHostToDevice, s));
+    int rc = forward(m, w, w.pfeats, w.pcoords, w.poffsets, nullptr, B, N, N, w.hlogits, s);
+    if (rc != GNN_OK) return rc;
+    GNN_CUDA_TRY(cudaMemcpyAsync(logits_host, w.hlogits, (size_t)B * a.n_classes * sizeof(float), cudaMemcpyDeviceToHost, s));
+    return gnn_status_check(m, slice, cuda_stream);
+}
+
+int gnn_profile_enable(gnn_model* m, int32_t slice, int32_t on) {
+    if (!m) return GNN_ERR_NULL;
+    if (slice < 0 || slice >= (int)m->ws.size()) return GNN_ERR_BAD_ARG;
+    m->ws[slice].prof_on = on != 0;
+    if (on) m->ws[slice].prof_forwards = 0;
+    return GNN_OK;
+}
+
+int gnn_profile_read(gnn_model* m, int32_t slice, int32_t max_stages, float* ms_mean_out, int32_t* n_stages_out,
+                     int32_t* n_forwards_out) {
+    if (!m || !ms_mean_out || !n_stages_out || !n_forwards_out) return GNN_ERR_NULL;
+    if (slice < 0 || slice >= (int)m->ws.size()) return GNN_ERR_BAD_ARG;
+    Workspace& w = m->ws[slice];
+    const int S = w.prof_stages, R = w.prof_forwards;
+    *n_stages_out = S; *n_forwards_out = R;
+    if (S > max_stages) return GNN_ERR_BAD_ARG;
+    for (int i = 0; i < S; ++i) ms_mean_out[i] = 0.0f;
+    if (R == 0) return GNN_OK;
+    for (int r = 0; r < R; ++r) {
+        size_t base = (size_t)r * (S + 1);
+        GNN_CUDA_TRY(cudaEventSynchronize(w.prof_events[base + S]));
+        for (int i = 0; i < S; ++i) {
+            float ms = 0.0f;
+            GNN_CUDA_TRY(cudaEventElapsedTime(&ms, w.prof_events[base + i], w.prof_events[base + i + 1]));
+            ms_mean_out[i] += ms;
+        }
+    }
+    for (int i = 0; i < S; ++i) ms_mean_out[i] /= (float)R;
+    return GNN_OK;
+}
+
+const char* gnn_profile_stage_name(gnn_model* m, int32_t slice, int32_t stage) {
+    if (!m || slice < 0 || slice >= (int)m->ws.size()) return nullptr;
+    Workspace& w = m->ws[slice];
+    if (stage < 0 || stage >= (int)w.prof_names.size()) return nullptr;
+    return w.prof_names[stage].c_str();
 }
 
 int gnn_status_check(gnn_model* m, int32_t slice, void* cuda_stream) {

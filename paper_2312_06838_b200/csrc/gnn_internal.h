@@ -4,6 +4,7 @@
 #include <atomic>
 #include <cstdint>
 #include <cstdio>
+#include <string>
 #include <vector>
 #include "../../include/gnn.h"
 
@@ -39,7 +40,15 @@ struct Workspace {
     int32_t* poffsets = nullptr;  // [Bmax + 1]
     int32_t* pcounts = nullptr;   // [Bmax]
     void* bf16_scratch = nullptr;  // per-slice scratch of the bf16 path
+    float* hlogits = nullptr;      // [Bmax, n_classes] device staging of gnn_infer_host (inputs stage in pfeats/pcoords/poffsets)
+    // stage timing (gnn_profile_*): events of up to PROF_MAX_FORWARDS forwards, (n_stages + 1) per forward
+    bool prof_on = false;
+    int prof_stages = 0;                       // stages per forward (fixed for a model)
+    int prof_forwards = 0;                     // forwards recorded since enable
+    std::vector<cudaEvent_t> prof_events;
+    std::vector<std::string> prof_names;
 };
+enum { PROF_MAX_FORWARDS = 512 };
 
 struct gnn_model {
     gnn_arch arch{};
