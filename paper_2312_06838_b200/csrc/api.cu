@@ -7,6 +7,7 @@
 #include <string>
 
 int edgeconv_bf16_prepare(gnn_model& m, const float* blob_host);       // edgeconv_bf16.cu
+void edgeconv_bf16_release(gnn_model& m);
 int launch_edgeconv_bf16(gnn_model& m, int block, const float* x, const int32_t* idx, int N, float* y, Workspace& w,
                          cudaStream_t s);
 
@@ -261,6 +262,7 @@ void gnn_destroy(gnn_model* m) {
     cudaSetDevice(m->device);
     cudaDeviceSynchronize();
     for (void* p : m->allocs) cudaFree(p);
+    edgeconv_bf16_release(*m);
     for (auto& w : m->ws)
         for (cudaEvent_t e : w.prof_events) cudaEventDestroy(e);
     delete m;

@@ -22,8 +22,6 @@ struct LinF32 {
 struct BlockDev {
     int cin = 0, c1 = 0, c2 = 0, c3 = 0;
     LinF32 l1, l2, l3, sc;   // fp32 path (and the shortcut / shifts in every mode)
-    // bf16 tcgen05 path (edgeconv_bf16.cu): per-particle pre-GEMM weights and packed edge-MLP weights
-    const void* bf16_pack = nullptr;
 };
 
 struct Workspace {
@@ -62,6 +60,7 @@ struct gnn_model {
     int n_fc = 0;
     std::vector<Workspace> ws;
     std::atomic<int64_t> launches{0};
+    void* bf16_blocks = nullptr;        // edgeconv_bf16.cu: per-block packed weights of the tcgen05 path
 };
 
 #define GNN_CUDA_TRY(expr)                                                              \
