@@ -6,19 +6,25 @@
 // Factorisation: layer 1 is linear in e_ij = [x_i ; x_j - x_i], so
 //     s1 * (W1 e_ij) + t1 = u_i + v_j,   u_i = s1*(W1a - W1b) x_i + t1,   v_j = s1*W1b x_j
 // needs two per-PARTICLE products instead of one per edge.  Two kernels per block:
-//   pre_kernel   per particle: u_i, v_i (stored bf16) and the shortcut r_i = ss*(Ws x_i) + ts (fp32), fp32 FMA.
-//   edge_kernel  per tile of 128 edge rows (128/k particles x k neighbours), all on chip:
-//     build   H1[r] = bf16(relu(u_i + v_j))  written straight into the 128B-swizzled K-major operand tile in smem
-//     MMA     D  = H1 * W2'^T   (tcgen05.mma kind::f16, M = 128, N = C, bf16 x bf16 -> fp32 in TMEM; W2' = s2*W2)
-//     E2      H2 = bf16(relu(D + t2))  TMEM -> registers -> the same operand tile (H1 is dead by then)
-//     MMA     D  = H2 * W3'^T
-//     E3      relu(D + t3), mean over the k_eff valid neighbour rows of each particle by a halving butterfly of
+//   pre kernel   per particle: u_i, v_i (stored bf16) and the shortcut r_i = ss*(Ws x_i) + ts (fp32).
+//   edge_kernel  persistent; per tile of 128 edge rows (128/k particles x k neighbours), all on chip:
+//     build   H1[r] = bf16(relu(u_i + v_j))  gathered straight into the 128B-swizzled K-major operand tile in smem
+//     MMA2    D0 = H1 * W2'^T   (tcgen05.mma kind::f16, N = C, bf16 x bf16 -> fp32 in TMEM; W2' = s2*W2)
+//     E2      H2 = bf16(relu(D0 + t2))  TMEM -> registers -> the same operand tile (H1 is dead by then)
+//     MMA3    D1 = H2 * W3'^T
+//     E3      relu(D1 + t3), mean over the k_eff valid neighbour rows of each particle by a halving butterfly of
 //             warp shuffles (rows = TMEM lanes = threads), + r_i, ReLU, coalesced fp32 store.
-// Weights reach shared memory as pre-swizzled [rows][64] chunk images by 1-D bulk (TMA) copies into a ring of
-// slots guarded by full/empty mbarriers; when both layers fit (C <= 128) every chunk is loaded once per CTA and stays
-// resident, otherwise (C = 256) the ring streams them per tile from L2.
-// Warp roles: warps 0-7 build / epilogue (two warpgroups = two column halves of the TMEM lanes quadrants), warp 8
-// allocates TMEM and its lane 0 issues every tcgen05.mma, warp 9 lane 0 is the weight-chunk producer.
+// Both layers' weights are RESIDENT in shared memory as pre-swizzled [rows][64] chunk images (one bulk/TMA copy per
+// chunk at kernel start).  For C = 256 the 256 KB of W2', W3' do not fit one SM, so the kernel runs as CTA PAIRS
+// (cluster of 2, tcgen05 cta_group::2, M = 256): each CTA owns its own 128-row tile (A operand) and half of the output
+// channels of the weights (B operand, 128 KB), the leader CTA issues every MMA for the pair, and each CTA's TMEM
+// receives its 128 rows x all 256 columns.  Nothing is streamed from L2 per tile.
+// Pipelining inside a CTA (pair): two accumulators (D0 for layer 2, D1 for layer 3), one operand tile H handed over
+// per 64-column K block: warps (q, kb) own lane quadrant q and K block kb; the MMA issuer starts a layer's K block as
+// soon as that block is written (h_ready[kb]) and releases it (h_free[kb], tcgen05.commit) as soon as layer 3 has read
+// it, so E3 of tile t and the gather of tile t+1 run under MMA3(t) / MMA2(t+1).  No block-wide barrier in the loop.
+// Warp roles: warps 0..NW-1 build / epilogue, warp NW allocates TMEM and its lane 0 issues every tcgen05.mma (leader
+// CTA only in pair mode), warp NW+1 lane 0 loads the weights.
 #include "gnn_internal.h"
 #include "tc05.cuh"
 #include <cuda_bf16.h>
@@ -28,26 +34,27 @@ namespace {
 
 using namespace tc05;
 
-constexpr int EDGE_ALU_THREADS = 256;
-constexpr int EDGE_THREADS = 320;
 constexpr int TILE_ROWS = 128;
 
 template <int C>
 struct EdgeCfg {
-    static constexpr int NR = C > 256 ? 256 : C;              // weight rows (= MMA N) per chunk
-    static constexpr int NH = C / NR;                         // N halves per layer
-    static constexpr int KB = (C + 63) / 64;                  // 64-wide K blocks per layer
+    static constexpr bool PAIR = C >= 256;                    // CTA pair: the weights, split over two SMs, stay resident
+    static constexpr int KB = (C + 63) / 64;                  // 64-wide K blocks per layer = column groups of the ALU warps
+    static constexpr int CW = C < 64 ? C : 64;                // columns per ALU warp
+    static constexpr int NW = 4 * KB;                         // ALU warps (lane quadrant q = w & 3, K block kb = w >> 2)
+    static constexpr int THREADS = 32 * (NW + 2);
     static constexpr int KSTEPS_LAST = ((C - (KB - 1) * 64) + 15) / 16;
-    static constexpr int CHUNK_BYTES = NR * 128;              // [NR][64] bf16, 128B-swizzled
-    static constexpr int NCHUNK = 2 * NH * KB;                // both layers
-    static constexpr bool RESIDENT = (size_t)NCHUNK * CHUNK_BYTES <= 96 * 1024;
-    static constexpr int NSLOT = RESIDENT ? NCHUNK : (CHUNK_BYTES <= 32 * 1024 ? 4 : 2);
-    static constexpr int H_BYTES = KB * TILE_ROWS * 128;      // KB K-blocks of [128][64] bf16
-    static constexpr int TMEM_COLS = C < 32 ? 32 : C;
-    static constexpr int RING_BYTES = NSLOT * CHUNK_BYTES;
-    // dynamic shared memory: [ring][H][t2,t3 fp32][idx int32 x128][barriers][tmem ptr] (+1024 alignment slack)
-    static constexpr int SMALL_BYTES = 2 * C * 4 + TILE_ROWS * 4 + (2 * NSLOT + 2) * 8 + 16;
-    static constexpr int SMEM_BYTES = RING_BYTES + H_BYTES + SMALL_BYTES + 1024;
+    static constexpr int NRB = PAIR ? C / 2 : C;              // weight rows (output channels) one CTA holds
+    static constexpr int CHUNK_BYTES = NRB * 128;             // [NRB][64] bf16, 128B-swizzled
+    static constexpr int W_BYTES = 2 * KB * CHUNK_BYTES;      // both layers
+    static constexpr int HK_BYTES = TILE_ROWS * 128;          // one K block of the operand tile: [128][64] bf16
+    static constexpr int H_BYTES = KB * HK_BYTES;
+    static constexpr int TMEM_COLS = 2 * C < 32 ? 32 : 2 * C; // D0 | D1
+    static constexpr int NBAR = 2 * KB + 6;
+    static constexpr int SMALL_BYTES = 2 * C * 4 + NBAR * 8 + 16;
+    static constexpr int SMEM_BYTES = W_BYTES + H_BYTES + SMALL_BYTES + 1024;
+    static constexpr int MIN_CTAS = C >= 256 ? 1 : (C >= 128 ? 2 : 3);
+    static constexpr int NRANKS = PAIR ? 2 : 1;
 };
 
 struct EdgeParams {
@@ -57,185 +64,218 @@ struct EdgeParams {
     const int32_t* idx;          // [N, k] global neighbour rows, -1 = none
     float* y;                    // [N, C]
     const int32_t* meta;         // meta[0] poisoned batch, meta[1] = N
-    const uint8_t* wimg;         // NCHUNK chunk images in consumption order
+    const uint8_t* wimg;         // per CTA rank: 2*KB chunk images in consumption order
     const float* shifts;         // [t2 | t3]
     int k, logk, TP, n_tiles;
 };
 
 template <int C>
-__global__ void __launch_bounds__(EDGE_THREADS, (C <= 128 ? 2 : 1)) edge_kernel(EdgeParams p) {
+__global__ void __launch_bounds__(EdgeCfg<C>::THREADS, EdgeCfg<C>::MIN_CTAS) edge_kernel(EdgeParams p) {
     using Cfg = EdgeCfg<C>;
+    constexpr bool PAIR = Cfg::PAIR;
+    constexpr int KB = Cfg::KB, NW = Cfg::NW, CW = Cfg::CW;
     extern __shared__ uint8_t smem_raw[];
-    if (p.meta[0]) return;
+    if (p.meta[0]) return;                                       // grid-uniform
     const int N = p.meta[1];
     const int n_tiles = min(p.n_tiles, (N + p.TP - 1) / p.TP);
-    if ((int)blockIdx.x >= n_tiles) return;
+    const uint32_t rank = PAIR ? cluster_ctarank() : 0u;
+    const int unit = PAIR ? (int)cluster_id_x() : (int)blockIdx.x;     // scheduling unit: a CTA or a CTA pair
+    const int n_units = PAIR ? (int)gridDim.x / 2 : (int)gridDim.x;
+    const int n_work = PAIR ? (n_tiles + 1) / 2 : n_tiles;              // (pair) tiles
+    if (unit >= n_work) return;                                  // uniform over the pair
+    const int T = (n_work - unit + n_units - 1) / n_units;       // (pair) tiles of this unit: unit, unit + n_units, ...
+
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
-    uint8_t* ring = smem;
-    uint8_t* H = ring + Cfg::RING_BYTES;
+    uint8_t* Wsm = smem;
+    uint8_t* H = Wsm + Cfg::W_BYTES;
     float* shifts_s = reinterpret_cast<float*>(H + Cfg::H_BYTES);
-    int32_t* idx_s = reinterpret_cast<int32_t*>(shifts_s + 2 * C);
-    uint64_t* bars = reinterpret_cast<uint64_t*>(idx_s + TILE_ROWS);
-    uint64_t* full = bars;                        // [NSLOT] weight chunk landed
-    uint64_t* empty = bars + Cfg::NSLOT;          // [NSLOT] weight chunk consumed (streaming only)
-    uint64_t* h_ready = bars + 2 * Cfg::NSLOT;    // operand tile written by the 256 ALU threads
-    uint64_t* d_full = h_ready + 1;               // accumulator complete
-    uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(d_full + 1);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(shifts_s + 2 * C);
+    uint64_t* h_ready = bars;                 // [KB] K block of H written (H1 and H2 fills alternate)   ALU -> MMA (leader)
+    uint64_t* h_free = bars + KB;             // [KB] layer 3 has read K block of H2                      MMA -> ALU (both)
+    uint64_t* d_full = bars + 2 * KB;         // [2]  accumulator of layer 2 / 3 complete                 MMA -> ALU (both)
+    uint64_t* d_free = d_full + 2;            // [2]  accumulator drained by the epilogue                 ALU -> MMA (leader)
+    uint64_t* w_full = d_free + 2;            // weights of this CTA landed
+    uint64_t* w_peer = w_full + 1;            // pair mode: the peer's weights landed (leader's copy is used)
+    uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(w_peer + 1);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     if (tid == 0) {
-        for (int i = 0; i < Cfg::NSLOT; ++i) { mbar_init(&full[i], 1); mbar_init(&empty[i], 1); }
-        mbar_init(h_ready, EDGE_ALU_THREADS);
-        mbar_init(d_full, 1);
+        for (int i = 0; i < KB; ++i) { mbar_init(&h_ready[i], 4 * Cfg::NRANKS); mbar_init(&h_free[i], 1); }
+        for (int i = 0; i < 2; ++i) { mbar_init(&d_full[i], 1); mbar_init(&d_free[i], NW * Cfg::NRANKS); }
+        mbar_init(w_full, 1);
+        mbar_init(w_peer, 1);
         fence_mbar_init();
     }
-    for (int i = tid; i < 2 * C; i += EDGE_THREADS) shifts_s[i] = p.shifts[i];
-    if (warp == 8) tmem_alloc(tmem_ptr, Cfg::TMEM_COLS);
+    for (int i = tid; i < 2 * C; i += Cfg::THREADS) shifts_s[i] = p.shifts[i];
+    if (warp == NW) tmem_alloc_g<PAIR>(tmem_ptr, Cfg::TMEM_COLS);
     tc_fence_before();
-    __syncthreads();
+    if constexpr (PAIR) cluster_sync_all(); else __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tmem_ptr;
-    const int my_tiles = (n_tiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
 
-    if (warp == 9) {
-        // ===== weight-chunk producer ======================================================================
+    if (warp == NW + 1) {
+        // ===== weight loader: every chunk once, resident for the life of the CTA ==================================
         if (lane == 0) {
-            const int total = Cfg::RESIDENT ? Cfg::NCHUNK : Cfg::NCHUNK * my_tiles;
-            for (int n = 0; n < total; ++n) {
-                const int slot = n % Cfg::NSLOT;
-                if (n >= Cfg::NSLOT) mbar_wait(&empty[slot], ((n / Cfg::NSLOT) - 1) & 1);
-                mbar_arrive_expect_tx(&full[slot], Cfg::CHUNK_BYTES);
-                bulk_g2s(ring + (size_t)slot * Cfg::CHUNK_BYTES, p.wimg + (size_t)(n % Cfg::NCHUNK) * Cfg::CHUNK_BYTES,
-                         Cfg::CHUNK_BYTES, &full[slot]);
-            }
+            mbar_arrive_expect_tx(w_full, Cfg::W_BYTES);
+            const uint8_t* src = p.wimg + (size_t)rank * Cfg::W_BYTES;
+            for (int c = 0; c < 2 * KB; ++c)
+                bulk_g2s(Wsm + (size_t)c * Cfg::CHUNK_BYTES, src + (size_t)c * Cfg::CHUNK_BYTES, Cfg::CHUNK_BYTES, w_full);
+            if (PAIR && rank == 1) { mbar_wait(w_full, 0); mbar_arrive_cluster(w_peer, 0); }
         }
-    } else if (warp == 8) {
-        // ===== MMA issuer =================================================================================
-        if (lane == 0) {
-            constexpr uint32_t idesc = idesc_bf16_f32(128, Cfg::NR);
-            const uint32_t h_addr = smem_u32(H), ring_addr = smem_u32(ring);
-            uint32_t ph_h = 0;
-            int n = 0;                                           // chunks consumed so far
-            for (int t = 0; t < my_tiles; ++t) {
+    } else if (warp == NW) {
+        // ===== MMA issuer (leader CTA of a pair) ==================================================================
+        if (lane == 0 && rank == 0) {
+            constexpr uint32_t idesc = idesc_bf16_f32(PAIR ? 256 : 128, C);
+            const uint32_t h_addr = smem_u32(H), w_addr = smem_u32(Wsm);
+            mbar_wait(w_full, 0);
+            if (PAIR) mbar_wait(w_peer, 0);
+            for (int t = 0; t < T; ++t) {
                 for (int layer = 0; layer < 2; ++layer) {
-                    mbar_wait(h_ready, ph_h); ph_h ^= 1;
+                    mbar_wait(&d_free[layer], (t & 1) ^ 1);      // epilogue of tile t-1 has drained this accumulator
                     tc_fence_after();
-                    for (int nh = 0; nh < Cfg::NH; ++nh) {
-                        for (int kb = 0; kb < Cfg::KB; ++kb, ++n) {
-                            const int slot = Cfg::RESIDENT ? (n % Cfg::NCHUNK) : (n % Cfg::NSLOT);
-                            if (!Cfg::RESIDENT || t == 0) mbar_wait(&full[slot], Cfg::RESIDENT ? 0 : ((n / Cfg::NSLOT) & 1));
-                            tc_fence_after();
-                            const int ksteps = (kb == Cfg::KB - 1) ? Cfg::KSTEPS_LAST : 4;
-                            for (int ks = 0; ks < ksteps; ++ks) {
-                                const uint64_t ad = desc_sw128(h_addr + kb * (TILE_ROWS * 128) + ks * 32);
-                                const uint64_t bd = desc_sw128(ring_addr + slot * Cfg::CHUNK_BYTES + ks * 32);
-                                mma_bf16_ss(tmem + nh * 256, ad, bd, idesc, (kb | ks) != 0);
-                            }
-                            if (!Cfg::RESIDENT) mma_commit(&empty[slot]);
+#pragma unroll
+                    for (int kb = 0; kb < KB; ++kb) {
+                        mbar_wait(&h_ready[kb], layer);          // fill 2t (H1) has parity 0, fill 2t+1 (H2) parity 1
+                        tc_fence_after();
+                        const int ksteps = (kb == KB - 1) ? Cfg::KSTEPS_LAST : 4;
+                        for (int ks = 0; ks < ksteps; ++ks) {
+                            const uint64_t ad = desc_sw128(h_addr + kb * Cfg::HK_BYTES + ks * 32);
+                            const uint64_t bd = desc_sw128(w_addr + (layer * KB + kb) * Cfg::CHUNK_BYTES + ks * 32);
+                            mma_bf16_ss_g<PAIR>(tmem + layer * C, ad, bd, idesc, (kb | ks) != 0);
                         }
+                        if (layer == 1) mma_commit_g<PAIR>(&h_free[kb]);   // gather of the next tile may overwrite it
                     }
-                    mma_commit(d_full);
+                    mma_commit_g<PAIR>(&d_full[layer]);
                 }
             }
         }
     } else {
-        // ===== build / epilogue warps ======================================================================
-        const int q = warp & 3, half = warp >> 2;
+        // ===== build / epilogue warps ==============================================================================
+        const int q = warp & 3, kb = warp >> 2;
         const int row = 32 * q + lane;                           // TMEM lane = edge row of the tile
+        const int col0 = kb * 64;                                // first of this warp's CW columns
         const int k = p.k, logk = p.logk;
-        constexpr int CH = C / 8;                                // 16-byte chunks per operand row
-        constexpr int ITEMS = TILE_ROWS * CH / EDGE_ALU_THREADS; // (row, chunk) items per thread
-        constexpr int SLABS = (C >= 64) ? C / 64 : 1;            // 32-column slabs per warp (C = 32: warps 4-7 idle)
-        const bool epi_active = (C >= 64) || half == 0;
-        uint32_t ph_d = 0;
-        for (int t = 0; t < my_tiles; ++t) {
-            const int tile = blockIdx.x + t * gridDim.x;
-            const int p0 = tile * p.TP;
-            asm volatile("bar.sync 1, 256;" ::: "memory");       // previous tile's readers of idx_s are done
-            if (tid < TILE_ROWS) {
-                const int pt = p0 + (tid >> logk);
-                idx_s[tid] = (pt < N) ? p.idx[(size_t)pt * k + (tid & (k - 1))] : -1;
+        constexpr int CPR = CW / 8;                              // 16-byte chunks per row of this warp's K block
+        constexpr int RPI = 32 / CPR;                            // rows per gather iteration
+        constexpr int ITERS = 32 / RPI;
+        constexpr int SLABS = CW / 32;
+        const int gc = lane % CPR, grs = lane / CPR;
+        uint8_t* Hk = H + kb * Cfg::HK_BYTES;
+        const uint32_t tbase = tmem + ((uint32_t)(32 * q) << 16) + col0;
+        const float* t2 = shifts_s + col0;
+        const float* t3 = shifts_s + C + col0;
+
+        auto tile_p0 = [&](int t) { const int w = unit + t * n_units; return (PAIR ? 2 * w + (int)rank : w) * p.TP; };
+        auto load_idx = [&](int p0) {
+            const int pt = p0 + (row >> logk);
+            return (pt < N) ? __ldg(p.idx + (size_t)pt * k + (row & (k - 1))) : -1;
+        };
+        auto arrive_leader = [&](uint64_t* bar) {
+            __syncwarp();
+            if (lane == 0) { if constexpr (PAIR) mbar_arrive_cluster(bar, 0); else mbar_arrive(bar); }
+        };
+        // gather H1 = bf16(relu(u_i + v_j)) for rows 32q..32q+31, K block kb; wait_parity >= 0: the K block is still being
+        // read by layer 3 of the previous tile, loads are issued first and the stores wait for h_free
+        auto build = [&](int idx_reg, int p0, int wait_parity) {
+            uint4 h[ITERS];
+#pragma unroll
+            for (int it = 0; it < ITERS; ++it) {
+                const int rl = it * RPI + grs;
+                const int j = __shfl_sync(0xffffffffu, idx_reg, rl);
+                uint4 vv = make_uint4(0, 0, 0, 0), uu = make_uint4(0, 0, 0, 0);
+                if (j >= 0) {
+                    const int pt = p0 + ((32 * q + rl) >> logk);
+                    vv = __ldg(reinterpret_cast<const uint4*>(p.V + (size_t)j * C + col0) + gc);
+                    uu = __ldg(reinterpret_cast<const uint4*>(p.U + (size_t)pt * C + col0) + gc);
+                }
+                h[it].x = add_relu_bf16x2(vv.x, uu.x); h[it].y = add_relu_bf16x2(vv.y, uu.y);
+                h[it].z = add_relu_bf16x2(vv.z, uu.z); h[it].w = add_relu_bf16x2(vv.w, uu.w);
             }
-            asm volatile("bar.sync 1, 256;" ::: "memory");
-            // ---- build H1 = bf16(relu(u_i + v_j)) ------------------------------------------------------
+            if (wait_parity >= 0) mbar_wait(&h_free[kb], (uint32_t)wait_parity);
 #pragma unroll
-            for (int i0 = 0; i0 < ITEMS; i0 += 8) {
-                uint4 vv[8], uu[8];
-#pragma unroll
-                for (int i = 0; i < 8; ++i) {
-                    if (i0 + i < ITEMS) {
-                        const int it = tid + (i0 + i) * EDGE_ALU_THREADS;
-                        const int r = it / CH, ch = it % CH;
-                        const int j = idx_s[r];
-                        if (j >= 0) {
-                            vv[i] = __ldg(reinterpret_cast<const uint4*>(p.V + (size_t)j * C) + ch);
-                            uu[i] = __ldg(reinterpret_cast<const uint4*>(p.U + (size_t)(p0 + (r >> logk)) * C) + ch);
-                        } else {
-                            vv[i] = make_uint4(0, 0, 0, 0); uu[i] = make_uint4(0, 0, 0, 0);
-                        }
-                    }
-                }
-#pragma unroll
-                for (int i = 0; i < 8; ++i) {
-                    if (i0 + i < ITEMS) {
-                        const int it = tid + (i0 + i) * EDGE_ALU_THREADS;
-                        const int r = it / CH, ch = it % CH;
-                        uint4 h;
-                        h.x = add_relu_bf16x2(vv[i].x, uu[i].x); h.y = add_relu_bf16x2(vv[i].y, uu[i].y);
-                        h.z = add_relu_bf16x2(vv[i].z, uu[i].z); h.w = add_relu_bf16x2(vv[i].w, uu[i].w);
-                        *reinterpret_cast<uint4*>(H + (ch >> 3) * (TILE_ROWS * 128) + r * 128 + (((ch & 7) ^ (r & 7)) << 4)) = h;
-                    }
-                }
+            for (int it = 0; it < ITERS; ++it) {
+                const int r = 32 * q + it * RPI + grs;
+                *reinterpret_cast<uint4*>(Hk + r * 128 + ((gc ^ (r & 7)) << 4)) = h[it];
             }
             fence_proxy_async();
-            mbar_arrive(h_ready);
-            // ---- E2: H2 = bf16(relu(D + t2)) -----------------------------------------------------------
-            mbar_wait(d_full, ph_d); ph_d ^= 1;
+            arrive_leader(&h_ready[kb]);
+        };
+
+        int idx_cur = load_idx(tile_p0(0));
+        build(idx_cur, tile_p0(0), -1);
+        for (int t = 0; t < T; ++t) {
+            const uint32_t ph = t & 1;
+            const int p0 = tile_p0(t);
+            const int p0_next = tile_p0(t + 1);
+            const int idx_next = (t + 1 < T) ? load_idx(p0_next) : -1;
+            // ---- E2: H2 = bf16(relu(D0 + t2)) ----------------------------------------------------------------
+            mbar_wait(&d_full[0], ph);                           // implies every layer-2 read of H1 is done
             tc_fence_after();
-            if (epi_active) {
-#pragma unroll 1
-                for (int s = 0; s < SLABS; ++s) {
-                    const int col = (C >= 64) ? half * (C / 2) + s * 32 : 0;
-                    float v[32];
-                    tmem_ld32(tmem + ((uint32_t)(32 * q) << 16) + (col >> 8) * 256 + (col & 255), v);
-                    tmem_ld_wait();
-                    uint32_t pk[16];
 #pragma unroll
-                    for (int i = 0; i < 16; ++i)
-                        pk[i] = pack_relu_bf16x2(v[2 * i] + shifts_s[col + 2 * i], v[2 * i + 1] + shifts_s[col + 2 * i + 1]);
-                    uint8_t* dst = H + (col >> 6) * (TILE_ROWS * 128) + row * 128;
-                    const int c8 = (col & 63) >> 3;
+            for (int s = 0; s < SLABS; ++s) {
+                float v[32];
+                tmem_ld32(tbase + s * 32, v);
+                tmem_ld_wait();
+                uint32_t pk[16];
 #pragma unroll
-                    for (int c = 0; c < 4; ++c)
-                        *reinterpret_cast<uint4*>(dst + (((c8 + c) ^ (row & 7)) << 4)) =
-                            make_uint4(pk[4 * c], pk[4 * c + 1], pk[4 * c + 2], pk[4 * c + 3]);
+                for (int i = 0; i < 8; ++i) {
+                    const float4 sh = *reinterpret_cast<const float4*>(t2 + s * 32 + 4 * i);
+                    pk[2 * i] = pack_relu_bf16x2(v[4 * i] + sh.x, v[4 * i + 1] + sh.y);
+                    pk[2 * i + 1] = pack_relu_bf16x2(v[4 * i + 2] + sh.z, v[4 * i + 3] + sh.w);
                 }
+                uint8_t* dst = Hk + row * 128;
+#pragma unroll
+                for (int c = 0; c < 4; ++c)
+                    *reinterpret_cast<uint4*>(dst + (((4 * s + c) ^ (row & 7)) << 4)) =
+                        make_uint4(pk[4 * c], pk[4 * c + 1], pk[4 * c + 2], pk[4 * c + 3]);
             }
             tc_fence_before();
+            arrive_leader(&d_free[0]);
             fence_proxy_async();
-            mbar_arrive(h_ready);
-            // ---- E3: mean over the valid neighbours of relu(D + t3), + shortcut, ReLU ----------------------
-            mbar_wait(d_full, ph_d); ph_d ^= 1;
-            tc_fence_after();
-            if (epi_active) {
-                const bool valid = idx_s[row] >= 0;
-                const unsigned gmask = (k >= 32) ? 0xffffffffu : (((1u << k) - 1u) << (lane & ~(k - 1)));
-                const int cnt = __popc(__ballot_sync(0xffffffffu, valid) & gmask);
-                const float inv = cnt > 0 ? 1.0f / (float)cnt : 0.0f;
-                const int pt = p0 + (row >> logk);
-                int cb = 0;                                      // first of the 32 >> logk columns this lane ends up with
-                for (int s = 0; s < logk; ++s) cb += ((lane >> s) & 1) * (16 >> s);
-                const int nout = 32 >> logk;
-                const float* t3 = shifts_s + C;
-#pragma unroll 1
-                for (int s = 0; s < SLABS; ++s) {
-                    const int col = (C >= 64) ? half * (C / 2) + s * 32 : 0;
-                    float v[32];
-                    tmem_ld32(tmem + ((uint32_t)(32 * q) << 16) + (col >> 8) * 256 + (col & 255), v);
-                    tmem_ld_wait();
+            arrive_leader(&h_ready[kb]);
+            // ---- shortcut values of this tile's outputs (k >= 16: two per lane and slab), fetched ahead of E3 ----------
+            const int pt = p0 + (row >> logk);
+            int cb = 0;                                          // first of the 32 >> logk columns this lane ends up with
+            for (int s = 0; s < logk; ++s) cb += ((lane >> s) & 1) * (16 >> s);
+            const int nout = 32 >> logk;
+            const size_t obase = (size_t)pt * C + col0 + cb;
+            float2 rr[SLABS];
 #pragma unroll
-                    for (int i = 0; i < 32; ++i) v[i] = valid ? fmaxf(v[i] + t3[col + i], 0.0f) : 0.0f;
-                    // halving butterfly: after step s a lane keeps 16 >> s partial sums over 2^(s+1) rows
+            for (int s = 0; s < SLABS; ++s) {
+                rr[s] = make_float2(0.0f, 0.0f);
+                if (pt < N) {
+                    if (nout == 2) rr[s] = __ldg(reinterpret_cast<const float2*>(p.R + obase + s * 32));
+                    else if (nout == 1) rr[s].x = __ldg(p.R + obase + s * 32);
+                }
+            }
+            // ---- gather of the next tile under MMA3(t) --------------------------------------------------------
+            if (t + 1 < T) build(idx_next, p0_next, (int)ph);
+            // ---- E3: mean over the valid neighbours of relu(D1 + t3), + shortcut, ReLU -------------------------
+            mbar_wait(&d_full[1], ph);
+            tc_fence_after();
+            {
+                const bool valid = idx_cur >= 0;
+                const unsigned vmask = __ballot_sync(0xffffffffu, valid);
+                const unsigned gmask = (k >= 32) ? 0xffffffffu : (((1u << k) - 1u) << (lane & ~(k - 1)));
+                const int cnt = __popc(vmask & gmask);
+                const float inv = cnt > 0 ? 1.0f / (float)cnt : 0.0f;
+#pragma unroll
+                for (int s = 0; s < SLABS; ++s) {
+                    float v[32];
+                    tmem_ld32(tbase + C + s * 32, v);
+                    tmem_ld_wait();
+                    if (s == SLABS - 1) { tc_fence_before(); arrive_leader(&d_free[1]); }
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const float4 sh = *reinterpret_cast<const float4*>(t3 + s * 32 + 4 * i);
+                        v[4 * i] = fmaxf(v[4 * i] + sh.x, 0.0f); v[4 * i + 1] = fmaxf(v[4 * i + 1] + sh.y, 0.0f);
+                        v[4 * i + 2] = fmaxf(v[4 * i + 2] + sh.z, 0.0f); v[4 * i + 3] = fmaxf(v[4 * i + 3] + sh.w, 0.0f);
+                    }
+                    if (vmask != 0xffffffffu) {
+#pragma unroll
+                        for (int i = 0; i < 32; ++i) v[i] = valid ? v[i] : 0.0f;
+                    }
+                    // halving butterfly: after step s2 a lane keeps 16 >> s2 partial sums over 2^(s2+1) rows
 #pragma unroll
                     for (int s2 = 0; s2 < 5; ++s2) {
                         if (s2 < logk) {
@@ -252,18 +292,31 @@ __global__ void __launch_bounds__(EDGE_THREADS, (C <= 128 ? 2 : 1)) edge_kernel(
                         }
                     }
                     if (pt < N) {
-                        const size_t o = (size_t)pt * C + col + cb;
+                        const size_t o = obase + s * 32;
+                        if (nout == 2) {
+                            *reinterpret_cast<float2*>(p.y + o) =
+                                make_float2(fmaxf(fmaf(v[0], inv, rr[s].x), 0.0f), fmaxf(fmaf(v[1], inv, rr[s].y), 0.0f));
+                        } else if (nout == 1) {
+                            p.y[o] = fmaxf(fmaf(v[0], inv, rr[s].x), 0.0f);
+                        } else {
 #pragma unroll
-                        for (int i = 0; i < 32; ++i)
-                            if (i < nout) p.y[o + i] = fmaxf(fmaf(v[i], inv, __ldg(p.R + o + i)), 0.0f);
+                            for (int i = 0; i < 32; i += 4)
+                                if (i < nout) {
+                                    const float4 r4 = __ldg(reinterpret_cast<const float4*>(p.R + o + i));
+                                    *reinterpret_cast<float4*>(p.y + o + i) =
+                                        make_float4(fmaxf(fmaf(v[i], inv, r4.x), 0.0f), fmaxf(fmaf(v[i + 1], inv, r4.y), 0.0f),
+                                                    fmaxf(fmaf(v[i + 2], inv, r4.z), 0.0f), fmaxf(fmaf(v[i + 3], inv, r4.w), 0.0f));
+                                }
+                        }
                     }
                 }
             }
-            tc_fence_before();
+            idx_cur = idx_next;
         }
     }
-    __syncthreads();
-    if (warp == 8) tmem_dealloc(tmem, Cfg::TMEM_COLS);
+    tc_fence_before();
+    if constexpr (PAIR) cluster_sync_all(); else __syncthreads();
+    if (warp == NW) tmem_dealloc_g<PAIR>(tmem, Cfg::TMEM_COLS);
 }
 
 // ---- pre kernel: per-particle u (bf16), v (bf16), shortcut r (fp32) in fp32 FMA ------------------------------------------
@@ -371,37 +424,66 @@ int upload(gnn_model& m, const std::vector<T>& h, const T** out) {
     return GNN_OK;
 }
 
-// [C][C] folded fp32 weights of one layer -> chunk images (nh, kb), appended to img
-void pack_layer(const std::vector<float>& W, int C, std::vector<uint8_t>& img) {
-    const int NR = C > 256 ? 256 : C, NH = C / NR, KB = (C + 63) / 64;
-    for (int nh = 0; nh < NH; ++nh)
-        for (int kb = 0; kb < KB; ++kb) {
-            const size_t base = img.size();
-            img.resize(base + (size_t)NR * 128, 0);
-            for (int nl = 0; nl < NR; ++nl)
-                for (int kk = 0; kk < 64; ++kk) {
-                    const int kcol = kb * 64 + kk, n = nh * NR + nl;
-                    const uint16_t v = kcol < C ? f32_to_bf16_rne(W[(size_t)n * C + kcol]) : 0;
-                    const size_t off = base + (size_t)nl * 128 + (size_t)(((kk >> 3) ^ (nl & 7)) << 4) + (kk & 7) * 2;
-                    std::memcpy(&img[off], &v, 2);
-                }
-        }
+// [C][C] folded fp32 weights of one layer -> the KB chunk images [NRB][64] of output rows [row0, row0 + NRB), appended
+void pack_layer(const std::vector<float>& W, int C, int NRB, int row0, std::vector<uint8_t>& img) {
+    const int KB = (C + 63) / 64;
+    for (int kb = 0; kb < KB; ++kb) {
+        const size_t base = img.size();
+        img.resize(base + (size_t)NRB * 128, 0);
+        for (int nl = 0; nl < NRB; ++nl)
+            for (int kk = 0; kk < 64; ++kk) {
+                const int kcol = kb * 64 + kk, n = row0 + nl;
+                const uint16_t v = kcol < C ? f32_to_bf16_rne(W[(size_t)n * C + kcol]) : 0;
+                const size_t off = base + (size_t)nl * 128 + (size_t)(((kk >> 3) ^ (nl & 7)) << 4) + (kk & 7) * 2;
+                std::memcpy(&img[off], &v, 2);
+            }
+    }
 }
 
 template <int C>
 int configure_edge(Bf16BlockDev& b, int n_sms) {
-    GNN_CUDA_TRY(cudaFuncSetAttribute(edge_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, EdgeCfg<C>::SMEM_BYTES));
-    int occ = 0;
-    GNN_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, edge_kernel<C>, EDGE_THREADS, EdgeCfg<C>::SMEM_BYTES));
-    if (occ < 1) return GNN_ERR_BAD_ARCH;
-    const int tmem_cap = 512 / EdgeCfg<C>::TMEM_COLS;           // co-resident CTAs must all fit their TMEM columns
-    b.grid_cap = n_sms * std::min(occ, tmem_cap);
+    using Cfg = EdgeCfg<C>;
+    GNN_CUDA_TRY(cudaFuncSetAttribute(edge_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES));
+    GNN_CUDA_TRY(cudaFuncSetAttribute(edge_kernel<C>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+    if (Cfg::PAIR) {
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3(n_sms & ~1); cfg.blockDim = dim3(Cfg::THREADS); cfg.dynamicSmemBytes = Cfg::SMEM_BYTES;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        int ncl = 0;
+        GNN_CUDA_TRY(cudaOccupancyMaxActiveClusters(&ncl, edge_kernel<C>, &cfg));
+        if (ncl < 1) return GNN_ERR_BAD_ARCH;
+        b.grid_cap = 2 * std::min(ncl, n_sms / 2);
+    } else {
+        int occ = 0;
+        GNN_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, edge_kernel<C>, Cfg::THREADS, Cfg::SMEM_BYTES));
+        if (occ < 1) return GNN_ERR_BAD_ARCH;
+        occ = std::max(occ, Cfg::MIN_CTAS);                    // the kernel is compiled for MIN_CTAS resident CTAs per SM
+        const int tmem_cap = 512 / Cfg::TMEM_COLS;              // co-resident CTAs must all fit their TMEM columns
+        b.grid_cap = n_sms * std::min(occ, tmem_cap);
+    }
     return GNN_OK;
 }
 
 template <int C>
-void launch_edge_t(const EdgeParams& p, int grid, cudaStream_t s) {
-    edge_kernel<C><<<grid, EDGE_THREADS, EdgeCfg<C>::SMEM_BYTES, s>>>(p);
+int launch_edge_t(const EdgeParams& p, int grid_cap, cudaStream_t s) {
+    using Cfg = EdgeCfg<C>;
+    if (Cfg::PAIR) {
+        const int n_work = (p.n_tiles + 1) / 2;
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3(2 * std::min(n_work, grid_cap / 2)); cfg.blockDim = dim3(Cfg::THREADS);
+        cfg.dynamicSmemBytes = Cfg::SMEM_BYTES; cfg.stream = s;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        GNN_CUDA_TRY(cudaLaunchKernelEx(&cfg, edge_kernel<C>, p));
+    } else {
+        edge_kernel<C><<<std::min(p.n_tiles, grid_cap), Cfg::THREADS, Cfg::SMEM_BYTES, s>>>(p);
+    }
+    return GNN_OK;
 }
 
 }  // namespace
@@ -446,9 +528,12 @@ int edgeconv_bf16_prepare(gnn_model& m, const float* blob) {
             }
             sh[o] = t2[o]; sh[C + o] = t3[o];
         }
-        std::vector<uint8_t> img;
-        pack_layer(W2f, C, img);
-        pack_layer(W3f, C, img);
+        std::vector<uint8_t> img;                              // per CTA rank: [W2' chunks | W3' chunks] of its output rows
+        const int nranks = C >= 256 ? 2 : 1, NRB = C / nranks;
+        for (int r = 0; r < nranks; ++r) {
+            pack_layer(W2f, C, NRB, r * NRB, img);
+            pack_layer(W3f, C, NRB, r * NRB, img);
+        }
         int rc;
         if ((rc = upload(m, Wt, &b.pre_Wt)) != GNN_OK || (rc = upload(m, bias, &b.pre_bias)) != GNN_OK ||
             (rc = upload(m, img, &b.wimg)) != GNN_OK || (rc = upload(m, sh, &b.shifts)) != GNN_OK)
@@ -497,13 +582,14 @@ int launch_edgeconv_bf16(gnn_model& m, int block, const float* x, const int32_t*
     while ((1 << ep.logk) < k) ++ep.logk;
     ep.TP = TILE_ROWS / k;
     ep.n_tiles = (N + ep.TP - 1) / ep.TP;
-    const int grid = std::min(ep.n_tiles, b.grid_cap);
+    int rc;
     switch (b.C) {
-        case 32: launch_edge_t<32>(ep, grid, s); break;
-        case 64: launch_edge_t<64>(ep, grid, s); break;
-        case 128: launch_edge_t<128>(ep, grid, s); break;
-        case 256: launch_edge_t<256>(ep, grid, s); break;
+        case 32: rc = launch_edge_t<32>(ep, b.grid_cap, s); break;
+        case 64: rc = launch_edge_t<64>(ep, b.grid_cap, s); break;
+        case 128: rc = launch_edge_t<128>(ep, b.grid_cap, s); break;
+        case 256: rc = launch_edge_t<256>(ep, b.grid_cap, s); break;
         default: return GNN_ERR_BAD_ARCH;
     }
+    if (rc != GNN_OK) return rc;
     return 2;
 }
