@@ -391,12 +391,191 @@ __global__ void __launch_bounds__(PRE_THREADS) pre_kernel(PreParams p) {
     }
 }
 
+// ---- pre kernel on the tensor cores (blocks whose input width is a multiple of 32): [u | v | r] = x * Wpre^T + bias --------
+// One GEMM [N, CIN] x [CIN, 3C] in tf32 (kind::tf32, fp32 accumulate in TMEM): x is rounded to tf32 (RNA) on its way
+// into shared memory, Wpre is rounded once on the host.  The 3C output columns are three slices of C columns (u, v,
+// r); a CTA keeps ONE slice of the weights resident ([C][CIN] tf32 as 128B-swizzled K blocks of 32 floats) and walks
+// the 128-row tiles of its slice group, so per tile only the x rows move (L2 -> smem).  A is single-buffered and handed
+// over per K block (a_ready / a_free), the accumulator is double-buffered (2 x C TMEM columns): epilogue(t) and the
+// loads of tile t+1 run under MMA(t+1) / MMA(t).
+// Warps: 0-3 epilogue (thread = row = TMEM lane), 4-7 x loaders, 8 MMA issuer + TMEM owner + weight load.
+constexpr int PTC_THREADS = 288;
+
+template <int CIN, int C>
+struct PreTcCfg {
+    static constexpr int KBA = CIN / 32;                      // K blocks of 32 tf32 (128 bytes per row)
+    static constexpr int AK_BYTES = TILE_ROWS * 128;
+    static constexpr int A_BYTES = KBA * AK_BYTES;
+    static constexpr int WK_BYTES = C * 128;                  // [C][32] tf32 chunk
+    static constexpr int W_BYTES = KBA * WK_BYTES;            // one slice
+    static constexpr int TMEM_COLS = 2 * C;
+    static constexpr int NBAR = 2 * KBA + 5;
+    static constexpr int SMEM_BYTES = W_BYTES + A_BYTES + C * 4 + NBAR * 8 + 16 + 1024;
+};
+
+struct PreTcParams {
+    const float* x;              // [N, CIN]
+    const uint8_t* wimg;         // 3 slices x KBA chunk images
+    const float* bias;           // [3C] = [t1 | 0 | ts]
+    __nv_bfloat16* U;            // [N, C]
+    __nv_bfloat16* V;            // [N, C]
+    float* R;                    // [N, C]
+    const int32_t* meta;
+    int n_tiles;
+};
+
+__device__ __forceinline__ uint32_t f32_to_tf32_rna(float f) {
+    uint32_t r;
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(f));
+    return r;
+}
+
+template <int CIN, int C>
+__global__ void __launch_bounds__(PTC_THREADS, 1) pre_tc_kernel(PreTcParams p) {
+    using Cfg = PreTcCfg<CIN, C>;
+    constexpr int KBA = Cfg::KBA;
+    extern __shared__ uint8_t smem_raw[];
+    if (p.meta[0]) return;
+    const int N = p.meta[1];
+    const int n_tiles = min(p.n_tiles, (N + TILE_ROWS - 1) / TILE_ROWS);
+    const int slice = blockIdx.x % 3, gi = blockIdx.x / 3, ng = gridDim.x / 3;
+    if (gi >= n_tiles) return;
+    const int T = (n_tiles - gi + ng - 1) / ng;
+
+    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+    uint8_t* Wsm = smem;
+    uint8_t* A = Wsm + Cfg::W_BYTES;
+    float* bias_s = reinterpret_cast<float*>(A + Cfg::A_BYTES);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(bias_s + C);
+    uint64_t* a_ready = bars;                 // [KBA] loaders -> MMA
+    uint64_t* a_free = bars + KBA;            // [KBA] MMA -> loaders
+    uint64_t* d_full = bars + 2 * KBA;        // [2]
+    uint64_t* d_free = d_full + 2;            // [2]
+    uint64_t* w_full = d_free + 2;
+    uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(w_full + 1);
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    if (tid == 0) {
+        for (int i = 0; i < KBA; ++i) { mbar_init(&a_ready[i], 4); mbar_init(&a_free[i], 1); }
+        for (int i = 0; i < 2; ++i) { mbar_init(&d_full[i], 1); mbar_init(&d_free[i], 4); }
+        mbar_init(w_full, 1);
+        fence_mbar_init();
+    }
+    for (int i = tid; i < C; i += PTC_THREADS) bias_s[i] = p.bias[slice * C + i];
+    if (warp == 8) tmem_alloc(tmem_ptr, Cfg::TMEM_COLS);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = *tmem_ptr;
+
+    if (warp == 8) {
+        // ===== weight load + MMA issuer =================================================================================
+        if (lane == 0) {
+            mbar_arrive_expect_tx(w_full, Cfg::W_BYTES);
+            const uint8_t* src = p.wimg + (size_t)slice * Cfg::W_BYTES;
+            for (int c = 0; c < KBA; ++c)
+                bulk_g2s(Wsm + (size_t)c * Cfg::WK_BYTES, src + (size_t)c * Cfg::WK_BYTES, Cfg::WK_BYTES, w_full);
+            constexpr uint32_t idesc = idesc_tf32_f32(128, C);
+            const uint32_t a_addr = smem_u32(A), w_addr = smem_u32(Wsm);
+            mbar_wait(w_full, 0);
+            for (int t = 0; t < T; ++t) {
+                const int acc = t & 1;
+                mbar_wait(&d_free[acc], ((t >> 1) & 1) ^ 1);
+                tc_fence_after();
+#pragma unroll
+                for (int kb = 0; kb < KBA; ++kb) {
+                    mbar_wait(&a_ready[kb], t & 1);
+                    tc_fence_after();
+#pragma unroll
+                    for (int ks = 0; ks < 4; ++ks) {             // K = 8 tf32 = 32 bytes per step
+                        const uint64_t ad = desc_sw128(a_addr + kb * Cfg::AK_BYTES + ks * 32);
+                        const uint64_t bd = desc_sw128(w_addr + kb * Cfg::WK_BYTES + ks * 32);
+                        mma_tf32_ss(tmem + acc * C, ad, bd, idesc, (kb | ks) != 0);
+                    }
+                    mma_commit(&a_free[kb]);
+                }
+                mma_commit(&d_full[acc]);
+            }
+        }
+    } else if (warp >= 4) {
+        // ===== x loaders: rows 32*lw .. +31 of every K block, 8 lanes per row (one 128-byte line) ==========================
+        const int lw = warp - 4;
+        const int gc = lane & 7, grs = lane >> 3;
+        for (int t = 0; t < T; ++t) {
+            const int r0 = (gi + t * ng) * TILE_ROWS;
+#pragma unroll 1
+            for (int kb = 0; kb < KBA; ++kb) {
+                float4 v[8];
+#pragma unroll
+                for (int it = 0; it < 8; ++it) {
+                    const int r = 32 * lw + it * 4 + grs;
+                    v[it] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+                    if (r0 + r < N) v[it] = __ldg(reinterpret_cast<const float4*>(p.x + (size_t)(r0 + r) * CIN + kb * 32) + gc);
+                }
+                mbar_wait(&a_free[kb], (t & 1) ^ 1);
+#pragma unroll
+                for (int it = 0; it < 8; ++it) {
+                    const int r = 32 * lw + it * 4 + grs;
+                    const uint4 w = make_uint4(f32_to_tf32_rna(v[it].x), f32_to_tf32_rna(v[it].y), f32_to_tf32_rna(v[it].z),
+                                               f32_to_tf32_rna(v[it].w));
+                    *reinterpret_cast<uint4*>(A + kb * Cfg::AK_BYTES + r * 128 + ((gc ^ (r & 7)) << 4)) = w;
+                }
+                fence_proxy_async();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&a_ready[kb]);
+            }
+        }
+    } else {
+        // ===== epilogue: thread = row = TMEM lane; slice 0 -> U (bf16), 1 -> V (bf16), 2 -> R (fp32) ======================
+        const int row = 32 * warp + lane;
+        for (int t = 0; t < T; ++t) {
+            const int acc = t & 1;
+            const int gr = (gi + t * ng) * TILE_ROWS + row;
+            mbar_wait(&d_full[acc], (t >> 1) & 1);
+            tc_fence_after();
+#pragma unroll 1
+            for (int s = 0; s < C / 32; ++s) {
+                float v[32];
+                tmem_ld32(tmem + ((uint32_t)(32 * warp) << 16) + acc * C + s * 32, v);
+                tmem_ld_wait();
+                if (s == C / 32 - 1) {
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&d_free[acc]);
+                }
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    const float4 b = *reinterpret_cast<const float4*>(bias_s + s * 32 + 4 * i);
+                    v[4 * i] += b.x; v[4 * i + 1] += b.y; v[4 * i + 2] += b.z; v[4 * i + 3] += b.w;
+                }
+                if (gr < N) {
+                    if (slice == 2) {
+                        float4* dst = reinterpret_cast<float4*>(p.R + (size_t)gr * C + s * 32);
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) dst[i] = make_float4(v[4 * i], v[4 * i + 1], v[4 * i + 2], v[4 * i + 3]);
+                    } else {
+                        uint4* dst = reinterpret_cast<uint4*>((slice == 0 ? p.U : p.V) + (size_t)gr * C + s * 32);
+#pragma unroll
+                        for (int i = 0; i < 4; ++i)
+                            dst[i] = make_uint4(pack_bf16x2(v[8 * i], v[8 * i + 1]), pack_bf16x2(v[8 * i + 2], v[8 * i + 3]),
+                                                pack_bf16x2(v[8 * i + 4], v[8 * i + 5]), pack_bf16x2(v[8 * i + 6], v[8 * i + 7]));
+                    }
+                }
+            }
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 8) tmem_dealloc(tmem, Cfg::TMEM_COLS);
+}
+
 // ---- host side: weight packing and launch -----------------------------------------------------------------------------
 struct Bf16BlockDev {
     const uint8_t* wimg = nullptr;
     const float* shifts = nullptr;
     const float* pre_Wt = nullptr;
     const float* pre_bias = nullptr;
+    const uint8_t* pre_wimg = nullptr;   // tf32 chunk images of the tensor-core pre kernel (null: SIMT pre kernel)
     int cin = 0, Kp = 0, C = 0, NC = 0;
     int grid_cap = 148;
 };
@@ -538,6 +717,25 @@ int edgeconv_bf16_prepare(gnn_model& m, const float* blob) {
         if ((rc = upload(m, Wt, &b.pre_Wt)) != GNN_OK || (rc = upload(m, bias, &b.pre_bias)) != GNN_OK ||
             (rc = upload(m, img, &b.wimg)) != GNN_OK || (rc = upload(m, sh, &b.shifts)) != GNN_OK)
             return rc;
+        if ((cin == 64 && C == 128) || (cin == 128 && C == 256)) {
+            // tensor-core pre kernel: per slice (u, v, r) and K block of 32: [C][32] tf32 (RNA), 128B-swizzled
+            std::vector<uint8_t> pimg((size_t)3 * C * cin * 4, 0);
+            size_t base = 0;
+            for (int sl = 0; sl < 3; ++sl)
+                for (int kb = 0; kb < cin / 32; ++kb, base += (size_t)C * 128)
+                    for (int nl = 0; nl < C; ++nl)
+                        for (int kk = 0; kk < 32; ++kk) {
+                            const float f = Wt[(size_t)(kb * 32 + kk) * b.NC + sl * C + nl];
+                            uint32_t u;
+                            std::memcpy(&u, &f, 4);
+                            u = (u + 0x1000u) & ~0x1fffu;
+                            const size_t off = base + (size_t)nl * 128 + (size_t)(((kk >> 2) ^ (nl & 7)) << 4) + (kk & 3) * 4;
+                            std::memcpy(&pimg[off], &u, 4);
+                        }
+            if ((rc = upload(m, pimg, &b.pre_wimg)) != GNN_OK) return rc;
+            if (C == 128) GNN_CUDA_TRY(cudaFuncSetAttribute(pre_tc_kernel<64, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize, PreTcCfg<64, 128>::SMEM_BYTES));
+            else GNN_CUDA_TRY(cudaFuncSetAttribute(pre_tc_kernel<128, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, PreTcCfg<128, 256>::SMEM_BYTES));
+        }
         switch (C) {
             case 32: rc = configure_edge<32>(b, m.n_sms); break;
             case 64: rc = configure_edge<64>(b, m.n_sms); break;
@@ -571,11 +769,20 @@ int launch_edgeconv_bf16(gnn_model& m, int block, const float* x, const int32_t*
     const Bf16BlockDev& b = static_cast<const Bf16BlockDev*>(m.bf16_blocks)[block];
     const Bf16Scratch& sc = *static_cast<const Bf16Scratch*>(w.bf16_scratch);
     const int k = m.arch.k;
-    PreParams pp;
-    pp.x = x; pp.Wt = b.pre_Wt; pp.bias = b.pre_bias; pp.U = sc.U; pp.V = sc.V; pp.R = sc.R; pp.meta = w.meta;
-    pp.cin = b.cin; pp.Kp = b.Kp; pp.C1 = b.C; pp.C3 = b.C; pp.NC = b.NC;
-    const size_t pre_smem = (size_t)PRE_ROWS * (b.Kp + 4) * sizeof(float);
-    pre_kernel<<<(N + PRE_ROWS - 1) / PRE_ROWS, PRE_THREADS, pre_smem, s>>>(pp);
+    if (b.pre_wimg) {
+        PreTcParams tp;
+        tp.x = x; tp.wimg = b.pre_wimg; tp.bias = b.pre_bias; tp.U = sc.U; tp.V = sc.V; tp.R = sc.R; tp.meta = w.meta;
+        tp.n_tiles = (N + TILE_ROWS - 1) / TILE_ROWS;
+        const int grid = 3 * std::min(tp.n_tiles, std::max(1, m.n_sms / 3));
+        if (b.C == 128) pre_tc_kernel<64, 128><<<grid, PTC_THREADS, PreTcCfg<64, 128>::SMEM_BYTES, s>>>(tp);
+        else pre_tc_kernel<128, 256><<<grid, PTC_THREADS, PreTcCfg<128, 256>::SMEM_BYTES, s>>>(tp);
+    } else {
+        PreParams pp;
+        pp.x = x; pp.Wt = b.pre_Wt; pp.bias = b.pre_bias; pp.U = sc.U; pp.V = sc.V; pp.R = sc.R; pp.meta = w.meta;
+        pp.cin = b.cin; pp.Kp = b.Kp; pp.C1 = b.C; pp.C3 = b.C; pp.NC = b.NC;
+        const size_t pre_smem = (size_t)PRE_ROWS * (b.Kp + 4) * sizeof(float);
+        pre_kernel<<<(N + PRE_ROWS - 1) / PRE_ROWS, PRE_THREADS, pre_smem, s>>>(pp);
+    }
     EdgeParams ep;
     ep.U = sc.U; ep.V = sc.V; ep.R = sc.R; ep.idx = idx; ep.y = y; ep.meta = w.meta; ep.wimg = b.wimg; ep.shifts = b.shifts;
     ep.k = k; ep.logk = 0;
