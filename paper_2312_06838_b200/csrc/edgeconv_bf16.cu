@@ -36,6 +36,13 @@ using namespace tc05;
 
 constexpr int TILE_ROWS = 128;
 
+#ifdef GNN_EDGE_TIMING   // developer instrumentation (never defined in the product build): clock64 stamps of cluster 0
+__device__ long long g_edge_ts[4][64][16];
+#define TS(who, t, ev) do { if ((who) >= 0 && (t) < 64 && lane == 0) g_edge_ts[who][t][ev] = clock64(); } while (0)
+#else
+#define TS(who, t, ev) do { } while (0)
+#endif
+
 template <int C>
 struct EdgeCfg {
     static constexpr bool PAIR = C >= 256;                    // CTA pair: the weights, split over two SMs, stay resident
@@ -74,7 +81,7 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS, EdgeCfg<C>::MIN_CTAS) edg
     using Cfg = EdgeCfg<C>;
     constexpr bool PAIR = Cfg::PAIR;
     constexpr int KB = Cfg::KB, NW = Cfg::NW, CW = Cfg::CW;
-    extern __shared__ uint8_t smem_raw[];
+    extern __shared__ __align__(1024) uint8_t smem_raw[];
     if (p.meta[0]) return;                                       // grid-uniform
     const int N = p.meta[1];
     const int n_tiles = min(p.n_tiles, (N + p.TP - 1) / p.TP);
@@ -85,7 +92,10 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS, EdgeCfg<C>::MIN_CTAS) edg
     if (unit >= n_work) return;                                  // uniform over the pair
     const int T = (n_work - unit + n_units - 1) / n_units;       // (pair) tiles of this unit: unit, unit + n_units, ...
 
-    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+    // no pointer arithmetic through integers here: the compiler must keep the shared address space (STS/LDS, not generic
+    // ST/LD); these kernels have no static shared memory, so the dynamic window starts 1024-byte aligned (checked)
+    uint8_t* smem = smem_raw;
+    if ((smem_u32(smem) & 1023u) != 0u) __trap();
     uint8_t* Wsm = smem;
     uint8_t* H = Wsm + Cfg::W_BYTES;
     float* shifts_s = reinterpret_cast<float*>(H + Cfg::H_BYTES);
@@ -121,6 +131,15 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS, EdgeCfg<C>::MIN_CTAS) edg
             for (int c = 0; c < 2 * KB; ++c)
                 bulk_g2s(Wsm + (size_t)c * Cfg::CHUNK_BYTES, src + (size_t)c * Cfg::CHUNK_BYTES, Cfg::CHUNK_BYTES, w_full);
             if (PAIR && rank == 1) { mbar_wait(w_full, 0); mbar_arrive_cluster(w_peer, 0); }
+#ifdef GNN_EDGE_TIMING
+            if (unit == 0 && C == 256 && rank == 0)
+                for (int t = 0; t < T && t < 64; ++t) {                   // monitor: true completion times of the commits
+                    mbar_wait(&d_full[0], t & 1); g_edge_ts[1][t][8] = clock64();
+                    mbar_wait(&h_free[0], t & 1); g_edge_ts[1][t][9] = clock64();
+                    mbar_wait(&h_free[KB - 1], t & 1); g_edge_ts[1][t][10] = clock64();
+                    mbar_wait(&d_full[1], t & 1); g_edge_ts[1][t][11] = clock64();
+                }
+#endif
         }
     } else if (warp == NW) {
         // ===== MMA issuer (leader CTA of a pair) ==================================================================
@@ -133,10 +152,12 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS, EdgeCfg<C>::MIN_CTAS) edg
                 for (int layer = 0; layer < 2; ++layer) {
                     mbar_wait(&d_free[layer], (t & 1) ^ 1);      // epilogue of tile t-1 has drained this accumulator
                     tc_fence_after();
+                    TS((unit == 0 && C == 256) ? 2 : -1, t, layer * 6);
 #pragma unroll
                     for (int kb = 0; kb < KB; ++kb) {
                         mbar_wait(&h_ready[kb], layer);          // fill 2t (H1) has parity 0, fill 2t+1 (H2) parity 1
                         tc_fence_after();
+                        TS((unit == 0 && C == 256) ? 2 : -1, t, layer * 6 + 1 + kb);
                         const int ksteps = (kb == KB - 1) ? Cfg::KSTEPS_LAST : 4;
                         for (int ks = 0; ks < ksteps; ++ks) {
                             const uint64_t ad = desc_sw128(h_addr + kb * Cfg::HK_BYTES + ks * 32);
@@ -146,12 +167,16 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS, EdgeCfg<C>::MIN_CTAS) edg
                         if (layer == 1) mma_commit_g<PAIR>(&h_free[kb]);   // gather of the next tile may overwrite it
                     }
                     mma_commit_g<PAIR>(&d_full[layer]);
+                    TS((unit == 0 && C == 256) ? 2 : -1, t, layer * 6 + 5);
                 }
             }
         }
     } else {
         // ===== build / epilogue warps ==============================================================================
         const int q = warp & 3, kb = warp >> 2;
+#ifdef GNN_EDGE_TIMING
+        const int who = (unit == 0 && C == 256) ? ((rank == 0 && warp == 0) ? 0 : (rank == 0 && warp == NW - 4) ? 1 : (rank == 1 && warp == 0) ? 3 : -1) : -1;
+#endif
         const int row = 32 * q + lane;                           // TMEM lane = edge row of the tile
         const int col0 = kb * 64;                                // first of this warp's CW columns
         const int k = p.k, logk = p.logk;
@@ -176,6 +201,7 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS, EdgeCfg<C>::MIN_CTAS) edg
         };
         // gather H1 = bf16(relu(u_i + v_j)) for rows 32q..32q+31, K block kb; wait_parity >= 0: the K block is still being
         // read by layer 3 of the previous tile, loads are issued first and the stores wait for h_free
+        int tcur = 0;
         auto build = [&](int idx_reg, int p0, int wait_parity) {
             uint4 h[ITERS];
 #pragma unroll
@@ -192,6 +218,7 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS, EdgeCfg<C>::MIN_CTAS) edg
                 h[it].z = add_relu_bf16x2(vv.z, uu.z); h[it].w = add_relu_bf16x2(vv.w, uu.w);
             }
             if (wait_parity >= 0) mbar_wait(&h_free[kb], (uint32_t)wait_parity);
+            TS(who, tcur, 6);
 #pragma unroll
             for (int it = 0; it < ITERS; ++it) {
                 const int r = 32 * q + it * RPI + grs;
@@ -205,12 +232,15 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS, EdgeCfg<C>::MIN_CTAS) edg
         build(idx_cur, tile_p0(0), -1);
         for (int t = 0; t < T; ++t) {
             const uint32_t ph = t & 1;
+            tcur = t;
             const int p0 = tile_p0(t);
             const int p0_next = tile_p0(t + 1);
             const int idx_next = (t + 1 < T) ? load_idx(p0_next) : -1;
             // ---- E2: H2 = bf16(relu(D0 + t2)) ----------------------------------------------------------------
+            TS(who, t, 0);
             mbar_wait(&d_full[0], ph);                           // implies every layer-2 read of H1 is done
             tc_fence_after();
+            TS(who, t, 1);
 #pragma unroll
             for (int s = 0; s < SLABS; ++s) {
                 float v[32];
@@ -233,6 +263,7 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS, EdgeCfg<C>::MIN_CTAS) edg
             arrive_leader(&d_free[0]);
             fence_proxy_async();
             arrive_leader(&h_ready[kb]);
+            TS(who, t, 2);
             // ---- shortcut values of this tile's outputs (k >= 16: two per lane and slab), fetched ahead of E3 ----------
             const int pt = p0 + (row >> logk);
             int cb = 0;                                          // first of the 32 >> logk columns this lane ends up with
@@ -250,9 +281,11 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS, EdgeCfg<C>::MIN_CTAS) edg
             }
             // ---- gather of the next tile under MMA3(t) --------------------------------------------------------
             if (t + 1 < T) build(idx_next, p0_next, (int)ph);
+            TS(who, t, 3);
             // ---- E3: mean over the valid neighbours of relu(D1 + t3), + shortcut, ReLU -------------------------
             mbar_wait(&d_full[1], ph);
             tc_fence_after();
+            TS(who, t, 4);
             {
                 const bool valid = idx_cur >= 0;
                 const unsigned vmask = __ballot_sync(0xffffffffu, valid);
@@ -311,6 +344,7 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS, EdgeCfg<C>::MIN_CTAS) edg
                     }
                 }
             }
+            TS(who, t, 5);
             idx_cur = idx_next;
         }
     }
@@ -398,8 +432,10 @@ __global__ void __launch_bounds__(PRE_THREADS) pre_kernel(PreParams p) {
 // the 128-row tiles of its slice group, so per tile only the x rows move (L2 -> smem).  A is single-buffered and handed
 // over per K block (a_ready / a_free), the accumulator is double-buffered (2 x C TMEM columns): epilogue(t) and the
 // loads of tile t+1 run under MMA(t+1) / MMA(t).
-// Warps: 0-3 epilogue (thread = row = TMEM lane), 4-7 x loaders, 8 MMA issuer + TMEM owner + weight load.
-constexpr int PTC_THREADS = 288;
+// Warps: 0-3 epilogue (thread = row = TMEM lane), 4-11 x loaders (a whole tile in flight in registers), 12 MMA issuer +
+// TMEM owner + weight load.
+constexpr int PTC_THREADS = 416;
+constexpr int PTC_MMA_WARP = 12;
 
 template <int CIN, int C>
 struct PreTcCfg {
@@ -410,7 +446,8 @@ struct PreTcCfg {
     static constexpr int W_BYTES = KBA * WK_BYTES;            // one slice
     static constexpr int TMEM_COLS = 2 * C;
     static constexpr int NBAR = 2 * KBA + 5;
-    static constexpr int SMEM_BYTES = W_BYTES + A_BYTES + C * 4 + NBAR * 8 + 16 + 1024;
+    static constexpr int STAGE_BYTES = 4 * 4096;              // per epilogue warp: [32 rows][32 cols] fp32, swizzled
+    static constexpr int SMEM_BYTES = W_BYTES + A_BYTES + STAGE_BYTES + C * 4 + NBAR * 8 + 16 + 1024;
 };
 
 struct PreTcParams {
@@ -434,7 +471,7 @@ template <int CIN, int C>
 __global__ void __launch_bounds__(PTC_THREADS, 1) pre_tc_kernel(PreTcParams p) {
     using Cfg = PreTcCfg<CIN, C>;
     constexpr int KBA = Cfg::KBA;
-    extern __shared__ uint8_t smem_raw[];
+    extern __shared__ __align__(1024) uint8_t smem_raw[];
     if (p.meta[0]) return;
     const int N = p.meta[1];
     const int n_tiles = min(p.n_tiles, (N + TILE_ROWS - 1) / TILE_ROWS);
@@ -442,10 +479,14 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) pre_tc_kernel(PreTcParams p) {
     if (gi >= n_tiles) return;
     const int T = (n_tiles - gi + ng - 1) / ng;
 
-    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+    // no pointer arithmetic through integers here: the compiler must keep the shared address space (STS/LDS, not generic
+    // ST/LD); these kernels have no static shared memory, so the dynamic window starts 1024-byte aligned (checked)
+    uint8_t* smem = smem_raw;
+    if ((smem_u32(smem) & 1023u) != 0u) __trap();
     uint8_t* Wsm = smem;
     uint8_t* A = Wsm + Cfg::W_BYTES;
-    float* bias_s = reinterpret_cast<float*>(A + Cfg::A_BYTES);
+    uint8_t* stage = A + Cfg::A_BYTES;
+    float* bias_s = reinterpret_cast<float*>(stage + Cfg::STAGE_BYTES);
     uint64_t* bars = reinterpret_cast<uint64_t*>(bias_s + C);
     uint64_t* a_ready = bars;                 // [KBA] loaders -> MMA
     uint64_t* a_free = bars + KBA;            // [KBA] MMA -> loaders
@@ -456,19 +497,19 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) pre_tc_kernel(PreTcParams p) {
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     if (tid == 0) {
-        for (int i = 0; i < KBA; ++i) { mbar_init(&a_ready[i], 4); mbar_init(&a_free[i], 1); }
+        for (int i = 0; i < KBA; ++i) { mbar_init(&a_ready[i], 8); mbar_init(&a_free[i], 1); }
         for (int i = 0; i < 2; ++i) { mbar_init(&d_full[i], 1); mbar_init(&d_free[i], 4); }
         mbar_init(w_full, 1);
         fence_mbar_init();
     }
     for (int i = tid; i < C; i += PTC_THREADS) bias_s[i] = p.bias[slice * C + i];
-    if (warp == 8) tmem_alloc(tmem_ptr, Cfg::TMEM_COLS);
+    if (warp == PTC_MMA_WARP) tmem_alloc(tmem_ptr, Cfg::TMEM_COLS);
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tmem_ptr;
 
-    if (warp == 8) {
+    if (warp == PTC_MMA_WARP) {
         // ===== weight load + MMA issuer =================================================================================
         if (lane == 0) {
             mbar_arrive_expect_tx(w_full, Cfg::W_BYTES);
@@ -498,26 +539,29 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) pre_tc_kernel(PreTcParams p) {
             }
         }
     } else if (warp >= 4) {
-        // ===== x loaders: rows 32*lw .. +31 of every K block, 8 lanes per row (one 128-byte line) ==========================
+        // ===== x loaders: rows 16*lw .. +15 of every K block, 8 lanes per row (one 128-byte line); all K blocks of a tile
+        // are requested before the first store, so a whole tile per CTA is in flight while the previous one is multiplied
         const int lw = warp - 4;
         const int gc = lane & 7, grs = lane >> 3;
         for (int t = 0; t < T; ++t) {
             const int r0 = (gi + t * ng) * TILE_ROWS;
-#pragma unroll 1
-            for (int kb = 0; kb < KBA; ++kb) {
-                float4 v[8];
+            float4 v[KBA][4];
 #pragma unroll
-                for (int it = 0; it < 8; ++it) {
-                    const int r = 32 * lw + it * 4 + grs;
-                    v[it] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-                    if (r0 + r < N) v[it] = __ldg(reinterpret_cast<const float4*>(p.x + (size_t)(r0 + r) * CIN + kb * 32) + gc);
+            for (int kb = 0; kb < KBA; ++kb)
+#pragma unroll
+                for (int it = 0; it < 4; ++it) {
+                    const int r = 16 * lw + it * 4 + grs;
+                    v[kb][it] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+                    if (r0 + r < N) v[kb][it] = __ldg(reinterpret_cast<const float4*>(p.x + (size_t)(r0 + r) * CIN + kb * 32) + gc);
                 }
+#pragma unroll
+            for (int kb = 0; kb < KBA; ++kb) {
                 mbar_wait(&a_free[kb], (t & 1) ^ 1);
 #pragma unroll
-                for (int it = 0; it < 8; ++it) {
-                    const int r = 32 * lw + it * 4 + grs;
-                    const uint4 w = make_uint4(f32_to_tf32_rna(v[it].x), f32_to_tf32_rna(v[it].y), f32_to_tf32_rna(v[it].z),
-                                               f32_to_tf32_rna(v[it].w));
+                for (int it = 0; it < 4; ++it) {
+                    const int r = 16 * lw + it * 4 + grs;
+                    const uint4 w = make_uint4(f32_to_tf32_rna(v[kb][it].x), f32_to_tf32_rna(v[kb][it].y),
+                                               f32_to_tf32_rna(v[kb][it].z), f32_to_tf32_rna(v[kb][it].w));
                     *reinterpret_cast<uint4*>(A + kb * Cfg::AK_BYTES + r * 128 + ((gc ^ (r & 7)) << 4)) = w;
                 }
                 fence_proxy_async();
@@ -548,25 +592,44 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) pre_tc_kernel(PreTcParams p) {
                     const float4 b = *reinterpret_cast<const float4*>(bias_s + s * 32 + 4 * i);
                     v[4 * i] += b.x; v[4 * i + 1] += b.y; v[4 * i + 2] += b.z; v[4 * i + 3] += b.w;
                 }
-                if (gr < N) {
-                    if (slice == 2) {
-                        float4* dst = reinterpret_cast<float4*>(p.R + (size_t)gr * C + s * 32);
+                // transpose through this warp's staging tile so that global stores are whole 128-byte (fp32) / 64-byte
+                // (bf16) row segments: thread = row writes swizzled 16-byte chunks, then 8 (4) lanes read one row back
+                uint8_t* st = stage + warp * 4096;
+                const int tr0 = (gi + t * ng) * TILE_ROWS + 32 * warp;
+                if (slice == 2) {
 #pragma unroll
-                        for (int i = 0; i < 8; ++i) dst[i] = make_float4(v[4 * i], v[4 * i + 1], v[4 * i + 2], v[4 * i + 3]);
-                    } else {
-                        uint4* dst = reinterpret_cast<uint4*>((slice == 0 ? p.U : p.V) + (size_t)gr * C + s * 32);
+                    for (int i = 0; i < 8; ++i)
+                        *reinterpret_cast<float4*>(st + lane * 128 + ((i ^ (lane & 7)) << 4)) =
+                            make_float4(v[4 * i], v[4 * i + 1], v[4 * i + 2], v[4 * i + 3]);
+                    __syncwarp();
 #pragma unroll
-                        for (int i = 0; i < 4; ++i)
-                            dst[i] = make_uint4(pack_bf16x2(v[8 * i], v[8 * i + 1]), pack_bf16x2(v[8 * i + 2], v[8 * i + 3]),
-                                                pack_bf16x2(v[8 * i + 4], v[8 * i + 5]), pack_bf16x2(v[8 * i + 6], v[8 * i + 7]));
+                    for (int it = 0; it < 8; ++it) {
+                        const int r = it * 4 + (lane >> 3), c = lane & 7;
+                        const float4 o = *reinterpret_cast<const float4*>(st + r * 128 + ((c ^ (r & 7)) << 4));
+                        if (tr0 + r < N) *(reinterpret_cast<float4*>(p.R + (size_t)(tr0 + r) * C + s * 32) + c) = o;
+                    }
+                } else {
+#pragma unroll
+                    for (int i = 0; i < 4; ++i)
+                        *reinterpret_cast<uint4*>(st + lane * 64 + ((i ^ ((lane >> 1) & 3)) << 4)) =
+                            make_uint4(pack_bf16x2(v[8 * i], v[8 * i + 1]), pack_bf16x2(v[8 * i + 2], v[8 * i + 3]),
+                                       pack_bf16x2(v[8 * i + 4], v[8 * i + 5]), pack_bf16x2(v[8 * i + 6], v[8 * i + 7]));
+                    __syncwarp();
+                    __nv_bfloat16* outp = slice == 0 ? p.U : p.V;
+#pragma unroll
+                    for (int it = 0; it < 4; ++it) {
+                        const int r = it * 8 + (lane >> 2), c = lane & 3;
+                        const uint4 o = *reinterpret_cast<const uint4*>(st + r * 64 + ((c ^ ((r >> 1) & 3)) << 4));
+                        if (tr0 + r < N) *(reinterpret_cast<uint4*>(outp + (size_t)(tr0 + r) * C + s * 32) + c) = o;
                     }
                 }
+                __syncwarp();
             }
         }
     }
     tc_fence_before();
     __syncthreads();
-    if (warp == 8) tmem_dealloc(tmem, Cfg::TMEM_COLS);
+    if (warp == PTC_MMA_WARP) tmem_dealloc(tmem, Cfg::TMEM_COLS);
 }
 
 // ---- host side: weight packing and launch -----------------------------------------------------------------------------
@@ -800,3 +863,9 @@ int launch_edgeconv_bf16(gnn_model& m, int block, const float* x, const int32_t*
     if (rc != GNN_OK) return rc;
     return 2;
 }
+
+#ifdef GNN_EDGE_TIMING
+extern "C" int gnn_debug_edge_timing(long long* out_host) {
+    return cudaMemcpyFromSymbol(out_host, g_edge_ts, sizeof(long long) * 4 * 64 * 16) == cudaSuccess ? 0 : -1;
+}
+#endif
