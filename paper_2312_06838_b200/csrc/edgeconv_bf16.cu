@@ -36,20 +36,16 @@ using namespace tc05;
 
 constexpr int TILE_ROWS = 128;
 
-#ifdef GNN_EDGE_TIMING   // developer instrumentation (never defined in the product build): clock64 stamps of cluster 0
-__device__ long long g_edge_ts[4][64][16];
-#define TS(who, t, ev) do { if ((who) >= 0 && (t) < 64 && lane == 0) g_edge_ts[who][t][ev] = clock64(); } while (0)
-#else
-#define TS(who, t, ev) do { } while (0)
-#endif
-
 template <int C>
 struct EdgeCfg {
     static constexpr bool PAIR = C >= 256;                    // CTA pair: the weights, split over two SMs, stay resident
-    static constexpr int KB = (C + 63) / 64;                  // 64-wide K blocks per layer = column groups of the ALU warps
-    static constexpr int CW = C < 64 ? C : 64;                // columns per ALU warp
-    static constexpr int NW = 4 * KB;                         // ALU warps (lane quadrant q = w & 3, K block kb = w >> 2)
-    static constexpr int THREADS = 32 * (NW + 2);
+    static constexpr int KB = (C + 63) / 64;                  // 64-wide K blocks per layer
+    static constexpr int KW = C < 64 ? C : 64;                // columns of one K block that are in use
+    static constexpr int NE = C >= 256 ? 8 : 4;               // epilogue warps: lane quadrant q = w & 3, column group w >> 2
+    static constexpr int CWE = C / (NE / 4);                  // columns per epilogue warp
+    static constexpr int NG = 2 * KB;                         // gather warps: K block g % KB, row half g / KB
+    static constexpr int MMA_WARP = NE + NG;
+    static constexpr int THREADS = 32 * (NE + NG + 2);
     static constexpr int KSTEPS_LAST = ((C - (KB - 1) * 64) + 15) / 16;
     static constexpr int NRB = PAIR ? C / 2 : C;              // weight rows (output channels) one CTA holds
     static constexpr int CHUNK_BYTES = NRB * 128;             // [NRB][64] bf16, 128B-swizzled
@@ -57,7 +53,7 @@ struct EdgeCfg {
     static constexpr int HK_BYTES = TILE_ROWS * 128;          // one K block of the operand tile: [128][64] bf16
     static constexpr int H_BYTES = KB * HK_BYTES;
     static constexpr int TMEM_COLS = 2 * C < 32 ? 32 : 2 * C; // D0 | D1
-    static constexpr int NBAR = 2 * KB + 6;
+    static constexpr int NBAR = 3 * KB + 6;
     static constexpr int SMALL_BYTES = 2 * C * 4 + NBAR * 8 + 16;
     static constexpr int SMEM_BYTES = W_BYTES + H_BYTES + SMALL_BYTES + 1024;
     static constexpr int MIN_CTAS = C >= 256 ? 1 : (C >= 128 ? 2 : 3);
@@ -76,11 +72,12 @@ struct EdgeParams {
     int k, logk, TP, n_tiles;
 };
 
-template <int C>
+// LOGK >= 0: k = 2^LOGK known at compile time (lets the gather keep one u chunk per particle in registers); -1: runtime
+template <int C, int LOGK>
 __global__ void __launch_bounds__(EdgeCfg<C>::THREADS, EdgeCfg<C>::MIN_CTAS) edge_kernel(EdgeParams p) {
     using Cfg = EdgeCfg<C>;
     constexpr bool PAIR = Cfg::PAIR;
-    constexpr int KB = Cfg::KB, NW = Cfg::NW, CW = Cfg::CW;
+    constexpr int KB = Cfg::KB, NE = Cfg::NE, NG = Cfg::NG, CWE = Cfg::CWE;
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     if (p.meta[0]) return;                                       // grid-uniform
     const int N = p.meta[1];
@@ -91,39 +88,51 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS, EdgeCfg<C>::MIN_CTAS) edg
     const int n_work = PAIR ? (n_tiles + 1) / 2 : n_tiles;              // (pair) tiles
     if (unit >= n_work) return;                                  // uniform over the pair
     const int T = (n_work - unit + n_units - 1) / n_units;       // (pair) tiles of this unit: unit, unit + n_units, ...
+    const int k = LOGK >= 0 ? (1 << LOGK) : p.k, logk = LOGK >= 0 ? LOGK : p.logk;
 
     // no pointer arithmetic through integers here: the compiler must keep the shared address space (STS/LDS, not generic
-    // ST/LD); these kernels have no static shared memory, so the dynamic window starts 1024-byte aligned (checked)
+    // ST/LD); this kernel has no static shared memory, so the dynamic window starts 1024-byte aligned (checked)
     uint8_t* smem = smem_raw;
     if ((smem_u32(smem) & 1023u) != 0u) __trap();
     uint8_t* Wsm = smem;
     uint8_t* H = Wsm + Cfg::W_BYTES;
     float* shifts_s = reinterpret_cast<float*>(H + Cfg::H_BYTES);
     uint64_t* bars = reinterpret_cast<uint64_t*>(shifts_s + 2 * C);
-    uint64_t* h_ready = bars;                 // [KB] K block of H written (H1 and H2 fills alternate)   ALU -> MMA (leader)
-    uint64_t* h_free = bars + KB;             // [KB] layer 3 has read K block of H2                      MMA -> ALU (both)
-    uint64_t* d_full = bars + 2 * KB;         // [2]  accumulator of layer 2 / 3 complete                 MMA -> ALU (both)
-    uint64_t* d_free = d_full + 2;            // [2]  accumulator drained by the epilogue                 ALU -> MMA (leader)
+    uint64_t* h1_ready = bars;                // [KB] K block of H1 gathered                              gather -> MMA (leader)
+    uint64_t* h2_ready = bars + KB;           // [KB] K block of H2 written by E2                         epilogue -> MMA (leader)
+    uint64_t* h_free = bars + 2 * KB;         // [KB] layer 3 has read K block of H2                      MMA -> gather (both)
+    uint64_t* d_full = bars + 3 * KB;         // [2]  accumulator of layer 2 / 3 complete                 MMA -> epilogue (both)
+    uint64_t* d_free = d_full + 2;            // [2]  accumulator drained by the epilogue                 epilogue -> MMA (leader)
     uint64_t* w_full = d_free + 2;            // weights of this CTA landed
     uint64_t* w_peer = w_full + 1;            // pair mode: the peer's weights landed (leader's copy is used)
     uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(w_peer + 1);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     if (tid == 0) {
-        for (int i = 0; i < KB; ++i) { mbar_init(&h_ready[i], 4 * Cfg::NRANKS); mbar_init(&h_free[i], 1); }
-        for (int i = 0; i < 2; ++i) { mbar_init(&d_full[i], 1); mbar_init(&d_free[i], NW * Cfg::NRANKS); }
+        for (int i = 0; i < KB; ++i) {
+            mbar_init(&h1_ready[i], 2 * Cfg::NRANKS);
+            mbar_init(&h2_ready[i], 4 * Cfg::NRANKS);
+            mbar_init(&h_free[i], 1);
+        }
+        for (int i = 0; i < 2; ++i) { mbar_init(&d_full[i], 1); mbar_init(&d_free[i], NE * Cfg::NRANKS); }
         mbar_init(w_full, 1);
         mbar_init(w_peer, 1);
         fence_mbar_init();
     }
     for (int i = tid; i < 2 * C; i += Cfg::THREADS) shifts_s[i] = p.shifts[i];
-    if (warp == NW) tmem_alloc_g<PAIR>(tmem_ptr, Cfg::TMEM_COLS);
+    if (warp == Cfg::MMA_WARP) tmem_alloc_g<PAIR>(tmem_ptr, Cfg::TMEM_COLS);
     tc_fence_before();
     if constexpr (PAIR) cluster_sync_all(); else __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tmem_ptr;
 
-    if (warp == NW + 1) {
+    auto tile_p0 = [&](int t) { const int w = unit + t * n_units; return (PAIR ? 2 * w + (int)rank : w) * p.TP; };
+    auto arrive_leader = [&](uint64_t* bar) {
+        __syncwarp();
+        if (lane == 0) { if constexpr (PAIR) mbar_arrive_cluster(bar, 0); else mbar_arrive(bar); }
+    };
+
+    if (warp == Cfg::MMA_WARP + 1) {
         // ===== weight loader: every chunk once, resident for the life of the CTA ==================================
         if (lane == 0) {
             mbar_arrive_expect_tx(w_full, Cfg::W_BYTES);
@@ -131,17 +140,8 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS, EdgeCfg<C>::MIN_CTAS) edg
             for (int c = 0; c < 2 * KB; ++c)
                 bulk_g2s(Wsm + (size_t)c * Cfg::CHUNK_BYTES, src + (size_t)c * Cfg::CHUNK_BYTES, Cfg::CHUNK_BYTES, w_full);
             if (PAIR && rank == 1) { mbar_wait(w_full, 0); mbar_arrive_cluster(w_peer, 0); }
-#ifdef GNN_EDGE_TIMING
-            if (unit == 0 && C == 256 && rank == 0)
-                for (int t = 0; t < T && t < 64; ++t) {                   // monitor: true completion times of the commits
-                    mbar_wait(&d_full[0], t & 1); g_edge_ts[1][t][8] = clock64();
-                    mbar_wait(&h_free[0], t & 1); g_edge_ts[1][t][9] = clock64();
-                    mbar_wait(&h_free[KB - 1], t & 1); g_edge_ts[1][t][10] = clock64();
-                    mbar_wait(&d_full[1], t & 1); g_edge_ts[1][t][11] = clock64();
-                }
-#endif
         }
-    } else if (warp == NW) {
+    } else if (warp == Cfg::MMA_WARP) {
         // ===== MMA issuer (leader CTA of a pair) ==================================================================
         if (lane == 0 && rank == 0) {
             constexpr uint32_t idesc = idesc_bf16_f32(PAIR ? 256 : 128, C);
@@ -152,12 +152,10 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS, EdgeCfg<C>::MIN_CTAS) edg
                 for (int layer = 0; layer < 2; ++layer) {
                     mbar_wait(&d_free[layer], (t & 1) ^ 1);      // epilogue of tile t-1 has drained this accumulator
                     tc_fence_after();
-                    TS((unit == 0 && C == 256) ? 2 : -1, t, layer * 6);
 #pragma unroll
                     for (int kb = 0; kb < KB; ++kb) {
-                        mbar_wait(&h_ready[kb], layer);          // fill 2t (H1) has parity 0, fill 2t+1 (H2) parity 1
+                        mbar_wait(layer == 0 ? &h1_ready[kb] : &h2_ready[kb], t & 1);
                         tc_fence_after();
-                        TS((unit == 0 && C == 256) ? 2 : -1, t, layer * 6 + 1 + kb);
                         const int ksteps = (kb == KB - 1) ? Cfg::KSTEPS_LAST : 4;
                         for (int ks = 0; ks < ksteps; ++ks) {
                             const uint64_t ad = desc_sw128(h_addr + kb * Cfg::HK_BYTES + ks * 32);
@@ -167,108 +165,97 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS, EdgeCfg<C>::MIN_CTAS) edg
                         if (layer == 1) mma_commit_g<PAIR>(&h_free[kb]);   // gather of the next tile may overwrite it
                     }
                     mma_commit_g<PAIR>(&d_full[layer]);
-                    TS((unit == 0 && C == 256) ? 2 : -1, t, layer * 6 + 5);
                 }
             }
         }
-    } else {
-        // ===== build / epilogue warps ==============================================================================
-        const int q = warp & 3, kb = warp >> 2;
-#ifdef GNN_EDGE_TIMING
-        const int who = (unit == 0 && C == 256) ? ((rank == 0 && warp == 0) ? 0 : (rank == 0 && warp == NW - 4) ? 1 : (rank == 1 && warp == 0) ? 3 : -1) : -1;
-#endif
-        const int row = 32 * q + lane;                           // TMEM lane = edge row of the tile
-        const int col0 = kb * 64;                                // first of this warp's CW columns
-        const int k = p.k, logk = p.logk;
-        constexpr int CPR = CW / 8;                              // 16-byte chunks per row of this warp's K block
-        constexpr int RPI = 32 / CPR;                            // rows per gather iteration
-        constexpr int ITERS = 32 / RPI;
-        constexpr int SLABS = CW / 32;
+    } else if (warp >= NE) {
+        // ===== gather warps: H1 = bf16(relu(u_i + v_j)) for K block gk, rows 64*half .. +63; they run one tile ahead of the
+        // epilogue (their only dependency is h_free of the previous tile), so the L2 latency of the gather is off the
+        // MMA <-> epilogue critical path ===============================================================================
+        const int g = warp - NE, gk = g % KB, half = g / KB;
+        constexpr int CPR = Cfg::KW / 8;                         // 16-byte chunks per row of a K block
+        constexpr int RPI = 32 / CPR;                            // rows per warp iteration
+        constexpr int ITERS = 64 / RPI;
+        constexpr int BATCH = ITERS < 8 ? ITERS : 8;
+        constexpr int NB = ITERS / BATCH;
+        constexpr bool HOIST = LOGK >= 0 && (1 << (LOGK >= 0 ? LOGK : 0)) >= RPI;   // rows of an iteration share a particle
+        constexpr int NPB = HOIST ? ((BATCH * RPI) >> (LOGK >= 0 ? LOGK : 0)) : 1;  // particles per batch
+        constexpr int NPBc = NPB < 1 ? 1 : NPB;
         const int gc = lane % CPR, grs = lane / CPR;
-        uint8_t* Hk = H + kb * Cfg::HK_BYTES;
+        uint8_t* Hk = H + gk * Cfg::HK_BYTES;
+        const int col0 = gk * 64;
+        for (int t = 0; t < T; ++t) {
+            const int p0 = tile_p0(t);
+            int idx_r[2];
+#pragma unroll
+            for (int a = 0; a < 2; ++a) {
+                const int r = 64 * half + 32 * a + lane;
+                const int pt = p0 + (r >> logk);
+                idx_r[a] = (pt < N) ? __ldg(p.idx + (size_t)pt * k + (r & (k - 1))) : -1;
+            }
+            uint4 h[NB][BATCH];
+#pragma unroll
+            for (int b = 0; b < NB; ++b) {
+                uint4 uh[NPBc];
+                if constexpr (HOIST) {
+#pragma unroll
+                    for (int i = 0; i < NPBc; ++i) {
+                        const int pt = p0 + ((64 * half + b * BATCH * RPI) >> logk) + i;
+                        uh[i] = make_uint4(0, 0, 0, 0);
+                        if (pt < N) uh[i] = __ldg(reinterpret_cast<const uint4*>(p.U + (size_t)pt * C + col0) + gc);
+                    }
+                }
+#pragma unroll
+                for (int it = 0; it < BATCH; ++it) {
+                    const int rl0 = (b * BATCH + it) * RPI;      // compile-time; this lane's row is rl0 + grs
+                    const int j = __shfl_sync(0xffffffffu, idx_r[rl0 >> 5], (rl0 & 31) + grs);
+                    uint4 vv = make_uint4(0, 0, 0, 0), uu = make_uint4(0, 0, 0, 0);
+                    if (j >= 0) vv = __ldg(reinterpret_cast<const uint4*>(p.V + (size_t)j * C + col0) + gc);
+                    if constexpr (HOIST) {
+                        uu = uh[NPBc == 1 ? 0 : ((it * RPI) >> (LOGK >= 0 ? LOGK : 0))];
+                    } else {
+                        const int pt = p0 + ((64 * half + rl0 + grs) >> logk);
+                        if (j >= 0) uu = __ldg(reinterpret_cast<const uint4*>(p.U + (size_t)pt * C + col0) + gc);
+                    }
+                    h[b][it].x = add_relu_bf16x2(vv.x, uu.x); h[b][it].y = add_relu_bf16x2(vv.y, uu.y);
+                    h[b][it].z = add_relu_bf16x2(vv.z, uu.z); h[b][it].w = add_relu_bf16x2(vv.w, uu.w);
+                }
+            }
+            if (t > 0) mbar_wait(&h_free[gk], (uint32_t)((t - 1) & 1));   // layer 3 of the previous tile has read this K block
+#pragma unroll
+            for (int b = 0; b < NB; ++b)
+#pragma unroll
+                for (int it = 0; it < BATCH; ++it) {
+                    const int r = 64 * half + (b * BATCH + it) * RPI + grs;
+                    *reinterpret_cast<uint4*>(Hk + r * 128 + ((gc ^ (r & 7)) << 4)) = h[b][it];
+                }
+            fence_proxy_async();
+            arrive_leader(&h1_ready[gk]);
+        }
+    } else {
+        // ===== epilogue warps: E2 (D0 -> H2) and E3 (D1 -> mean -> y) for lane quadrant q, columns [cg*CWE, +CWE) ==========
+        const int q = warp & 3, cg = warp >> 2;
+        const int row = 32 * q + lane;                           // TMEM lane = edge row of the tile
+        const int col0 = cg * CWE;
+        constexpr int SLABS = CWE / 32;
         const uint32_t tbase = tmem + ((uint32_t)(32 * q) << 16) + col0;
         const float* t2 = shifts_s + col0;
         const float* t3 = shifts_s + C + col0;
-
-        auto tile_p0 = [&](int t) { const int w = unit + t * n_units; return (PAIR ? 2 * w + (int)rank : w) * p.TP; };
+        int cb = 0;                                              // first of the 32 >> logk columns this lane ends up with
+        for (int s = 0; s < logk; ++s) cb += ((lane >> s) & 1) * (16 >> s);
+        const int nout = 32 >> logk;
+        const unsigned gmask = (k >= 32) ? 0xffffffffu : (((1u << k) - 1u) << (lane & ~(k - 1)));
         auto load_idx = [&](int p0) {
             const int pt = p0 + (row >> logk);
             return (pt < N) ? __ldg(p.idx + (size_t)pt * k + (row & (k - 1))) : -1;
         };
-        auto arrive_leader = [&](uint64_t* bar) {
-            __syncwarp();
-            if (lane == 0) { if constexpr (PAIR) mbar_arrive_cluster(bar, 0); else mbar_arrive(bar); }
-        };
-        // gather H1 = bf16(relu(u_i + v_j)) for rows 32q..32q+31, K block kb; wait_parity >= 0: the K block is still being
-        // read by layer 3 of the previous tile, loads are issued first and the stores wait for h_free
-        int tcur = 0;
-        auto build = [&](int idx_reg, int p0, int wait_parity) {
-            uint4 h[ITERS];
-#pragma unroll
-            for (int it = 0; it < ITERS; ++it) {
-                const int rl = it * RPI + grs;
-                const int j = __shfl_sync(0xffffffffu, idx_reg, rl);
-                uint4 vv = make_uint4(0, 0, 0, 0), uu = make_uint4(0, 0, 0, 0);
-                if (j >= 0) {
-                    const int pt = p0 + ((32 * q + rl) >> logk);
-                    vv = __ldg(reinterpret_cast<const uint4*>(p.V + (size_t)j * C + col0) + gc);
-                    uu = __ldg(reinterpret_cast<const uint4*>(p.U + (size_t)pt * C + col0) + gc);
-                }
-                h[it].x = add_relu_bf16x2(vv.x, uu.x); h[it].y = add_relu_bf16x2(vv.y, uu.y);
-                h[it].z = add_relu_bf16x2(vv.z, uu.z); h[it].w = add_relu_bf16x2(vv.w, uu.w);
-            }
-            if (wait_parity >= 0) mbar_wait(&h_free[kb], (uint32_t)wait_parity);
-            TS(who, tcur, 6);
-#pragma unroll
-            for (int it = 0; it < ITERS; ++it) {
-                const int r = 32 * q + it * RPI + grs;
-                *reinterpret_cast<uint4*>(Hk + r * 128 + ((gc ^ (r & 7)) << 4)) = h[it];
-            }
-            fence_proxy_async();
-            arrive_leader(&h_ready[kb]);
-        };
-
         int idx_cur = load_idx(tile_p0(0));
-        build(idx_cur, tile_p0(0), -1);
         for (int t = 0; t < T; ++t) {
             const uint32_t ph = t & 1;
-            tcur = t;
             const int p0 = tile_p0(t);
-            const int p0_next = tile_p0(t + 1);
-            const int idx_next = (t + 1 < T) ? load_idx(p0_next) : -1;
-            // ---- E2: H2 = bf16(relu(D0 + t2)) ----------------------------------------------------------------
-            TS(who, t, 0);
-            mbar_wait(&d_full[0], ph);                           // implies every layer-2 read of H1 is done
-            tc_fence_after();
-            TS(who, t, 1);
-#pragma unroll
-            for (int s = 0; s < SLABS; ++s) {
-                float v[32];
-                tmem_ld32(tbase + s * 32, v);
-                tmem_ld_wait();
-                uint32_t pk[16];
-#pragma unroll
-                for (int i = 0; i < 8; ++i) {
-                    const float4 sh = *reinterpret_cast<const float4*>(t2 + s * 32 + 4 * i);
-                    pk[2 * i] = pack_relu_bf16x2(v[4 * i] + sh.x, v[4 * i + 1] + sh.y);
-                    pk[2 * i + 1] = pack_relu_bf16x2(v[4 * i + 2] + sh.z, v[4 * i + 3] + sh.w);
-                }
-                uint8_t* dst = Hk + row * 128;
-#pragma unroll
-                for (int c = 0; c < 4; ++c)
-                    *reinterpret_cast<uint4*>(dst + (((4 * s + c) ^ (row & 7)) << 4)) =
-                        make_uint4(pk[4 * c], pk[4 * c + 1], pk[4 * c + 2], pk[4 * c + 3]);
-            }
-            tc_fence_before();
-            arrive_leader(&d_free[0]);
-            fence_proxy_async();
-            arrive_leader(&h_ready[kb]);
-            TS(who, t, 2);
-            // ---- shortcut values of this tile's outputs (k >= 16: two per lane and slab), fetched ahead of E3 ----------
+            const int idx_next = (t + 1 < T) ? load_idx(tile_p0(t + 1)) : -1;
+            // shortcut values of this tile's outputs (k >= 16: at most two per lane and slab), fetched ahead of E3
             const int pt = p0 + (row >> logk);
-            int cb = 0;                                          // first of the 32 >> logk columns this lane ends up with
-            for (int s = 0; s < logk; ++s) cb += ((lane >> s) & 1) * (16 >> s);
-            const int nout = 32 >> logk;
             const size_t obase = (size_t)pt * C + col0 + cb;
             float2 rr[SLABS];
 #pragma unroll
@@ -279,34 +266,62 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS, EdgeCfg<C>::MIN_CTAS) edg
                     else if (nout == 1) rr[s].x = __ldg(p.R + obase + s * 32);
                 }
             }
-            // ---- gather of the next tile under MMA3(t) --------------------------------------------------------
-            if (t + 1 < T) build(idx_next, p0_next, (int)ph);
-            TS(who, t, 3);
-            // ---- E3: mean over the valid neighbours of relu(D1 + t3), + shortcut, ReLU -------------------------
+            // ---- E2: H2 = bf16(relu(D0 + t2)); the TMEM load of slab s+1 is in flight while slab s is converted ----------
+            mbar_wait(&d_full[0], ph);                           // implies every layer-2 read of H1 is done
+            tc_fence_after();
+            {
+                float v[2][32];
+                tmem_ld32(tbase, v[0]);
+#pragma unroll
+                for (int s = 0; s < SLABS; ++s) {
+                    tmem_ld_wait();
+                    if (s + 1 < SLABS) tmem_ld32(tbase + (s + 1) * 32, v[(s + 1) & 1]);
+                    else { tc_fence_before(); arrive_leader(&d_free[0]); }
+                    const int col = col0 + s * 32;
+                    uint32_t pk[16];
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const float4 sh = *reinterpret_cast<const float4*>(t2 + s * 32 + 4 * i);
+                        pk[2 * i] = pack_relu_bf16x2(v[s & 1][4 * i] + sh.x, v[s & 1][4 * i + 1] + sh.y);
+                        pk[2 * i + 1] = pack_relu_bf16x2(v[s & 1][4 * i + 2] + sh.z, v[s & 1][4 * i + 3] + sh.w);
+                    }
+                    uint8_t* dst = H + (col >> 6) * Cfg::HK_BYTES + row * 128;
+                    const int c8 = (col & 63) >> 3;
+#pragma unroll
+                    for (int c = 0; c < 4; ++c)
+                        *reinterpret_cast<uint4*>(dst + (((c8 + c) ^ (row & 7)) << 4)) =
+                            make_uint4(pk[4 * c], pk[4 * c + 1], pk[4 * c + 2], pk[4 * c + 3]);
+                    if (((col + 32) & 63) == 0 || s == SLABS - 1) {      // this warp's part of a K block is complete
+                        fence_proxy_async();
+                        arrive_leader(&h2_ready[col >> 6]);
+                    }
+                }
+            }
+            // ---- E3: mean over the valid neighbours of relu(D1 + t3), + shortcut, ReLU ---------------------------------
             mbar_wait(&d_full[1], ph);
             tc_fence_after();
-            TS(who, t, 4);
             {
                 const bool valid = idx_cur >= 0;
                 const unsigned vmask = __ballot_sync(0xffffffffu, valid);
-                const unsigned gmask = (k >= 32) ? 0xffffffffu : (((1u << k) - 1u) << (lane & ~(k - 1)));
                 const int cnt = __popc(vmask & gmask);
                 const float inv = cnt > 0 ? 1.0f / (float)cnt : 0.0f;
+                float v[2][32];
+                tmem_ld32(tbase + C, v[0]);
 #pragma unroll
                 for (int s = 0; s < SLABS; ++s) {
-                    float v[32];
-                    tmem_ld32(tbase + C + s * 32, v);
                     tmem_ld_wait();
-                    if (s == SLABS - 1) { tc_fence_before(); arrive_leader(&d_free[1]); }
+                    if (s + 1 < SLABS) tmem_ld32(tbase + C + (s + 1) * 32, v[(s + 1) & 1]);
+                    else { tc_fence_before(); arrive_leader(&d_free[1]); }
+                    float (&w)[32] = v[s & 1];
 #pragma unroll
                     for (int i = 0; i < 8; ++i) {
                         const float4 sh = *reinterpret_cast<const float4*>(t3 + s * 32 + 4 * i);
-                        v[4 * i] = fmaxf(v[4 * i] + sh.x, 0.0f); v[4 * i + 1] = fmaxf(v[4 * i + 1] + sh.y, 0.0f);
-                        v[4 * i + 2] = fmaxf(v[4 * i + 2] + sh.z, 0.0f); v[4 * i + 3] = fmaxf(v[4 * i + 3] + sh.w, 0.0f);
+                        w[4 * i] = fmaxf(w[4 * i] + sh.x, 0.0f); w[4 * i + 1] = fmaxf(w[4 * i + 1] + sh.y, 0.0f);
+                        w[4 * i + 2] = fmaxf(w[4 * i + 2] + sh.z, 0.0f); w[4 * i + 3] = fmaxf(w[4 * i + 3] + sh.w, 0.0f);
                     }
                     if (vmask != 0xffffffffu) {
 #pragma unroll
-                        for (int i = 0; i < 32; ++i) v[i] = valid ? v[i] : 0.0f;
+                        for (int i = 0; i < 32; ++i) w[i] = valid ? w[i] : 0.0f;
                     }
                     // halving butterfly: after step s2 a lane keeps 16 >> s2 partial sums over 2^(s2+1) rows
 #pragma unroll
@@ -317,9 +332,9 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS, EdgeCfg<C>::MIN_CTAS) edg
 #pragma unroll
                             for (int i = 0; i < 16; ++i) {
                                 if (i < cntv) {
-                                    const float keep = up ? v[i + cntv] : v[i];
-                                    const float send = up ? v[i] : v[i + cntv];
-                                    v[i] = keep + __shfl_xor_sync(0xffffffffu, send, 1 << s2);
+                                    const float keep = up ? w[i + cntv] : w[i];
+                                    const float send = up ? w[i] : w[i + cntv];
+                                    w[i] = keep + __shfl_xor_sync(0xffffffffu, send, 1 << s2);
                                 }
                             }
                         }
@@ -328,29 +343,28 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS, EdgeCfg<C>::MIN_CTAS) edg
                         const size_t o = obase + s * 32;
                         if (nout == 2) {
                             *reinterpret_cast<float2*>(p.y + o) =
-                                make_float2(fmaxf(fmaf(v[0], inv, rr[s].x), 0.0f), fmaxf(fmaf(v[1], inv, rr[s].y), 0.0f));
+                                make_float2(fmaxf(fmaf(w[0], inv, rr[s].x), 0.0f), fmaxf(fmaf(w[1], inv, rr[s].y), 0.0f));
                         } else if (nout == 1) {
-                            p.y[o] = fmaxf(fmaf(v[0], inv, rr[s].x), 0.0f);
+                            p.y[o] = fmaxf(fmaf(w[0], inv, rr[s].x), 0.0f);
                         } else {
 #pragma unroll
                             for (int i = 0; i < 32; i += 4)
                                 if (i < nout) {
                                     const float4 r4 = __ldg(reinterpret_cast<const float4*>(p.R + o + i));
                                     *reinterpret_cast<float4*>(p.y + o + i) =
-                                        make_float4(fmaxf(fmaf(v[i], inv, r4.x), 0.0f), fmaxf(fmaf(v[i + 1], inv, r4.y), 0.0f),
-                                                    fmaxf(fmaf(v[i + 2], inv, r4.z), 0.0f), fmaxf(fmaf(v[i + 3], inv, r4.w), 0.0f));
+                                        make_float4(fmaxf(fmaf(w[i], inv, r4.x), 0.0f), fmaxf(fmaf(w[i + 1], inv, r4.y), 0.0f),
+                                                    fmaxf(fmaf(w[i + 2], inv, r4.z), 0.0f), fmaxf(fmaf(w[i + 3], inv, r4.w), 0.0f));
                                 }
                         }
                     }
                 }
             }
-            TS(who, t, 5);
             idx_cur = idx_next;
         }
     }
     tc_fence_before();
     if constexpr (PAIR) cluster_sync_all(); else __syncthreads();
-    if (warp == NW) tmem_dealloc_g<PAIR>(tmem, Cfg::TMEM_COLS);
+    if (warp == Cfg::MMA_WARP) tmem_dealloc_g<PAIR>(tmem, Cfg::TMEM_COLS);
 }
 
 // ---- pre kernel: per-particle u (bf16), v (bf16), shortcut r (fp32) in fp32 FMA ------------------------------------------
@@ -682,11 +696,12 @@ void pack_layer(const std::vector<float>& W, int C, int NRB, int row0, std::vect
     }
 }
 
-template <int C>
+template <int C, int LOGK>
 int configure_edge(Bf16BlockDev& b, int n_sms) {
     using Cfg = EdgeCfg<C>;
-    GNN_CUDA_TRY(cudaFuncSetAttribute(edge_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES));
-    GNN_CUDA_TRY(cudaFuncSetAttribute(edge_kernel<C>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+    auto* kern = edge_kernel<C, LOGK>;
+    GNN_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES));
+    GNN_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
     if (Cfg::PAIR) {
         cudaLaunchConfig_t cfg{};
         cfg.gridDim = dim3(n_sms & ~1); cfg.blockDim = dim3(Cfg::THREADS); cfg.dynamicSmemBytes = Cfg::SMEM_BYTES;
@@ -695,12 +710,12 @@ int configure_edge(Bf16BlockDev& b, int n_sms) {
         at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
         cfg.attrs = at; cfg.numAttrs = 1;
         int ncl = 0;
-        GNN_CUDA_TRY(cudaOccupancyMaxActiveClusters(&ncl, edge_kernel<C>, &cfg));
+        GNN_CUDA_TRY(cudaOccupancyMaxActiveClusters(&ncl, kern, &cfg));
         if (ncl < 1) return GNN_ERR_BAD_ARCH;
         b.grid_cap = 2 * std::min(ncl, n_sms / 2);
     } else {
         int occ = 0;
-        GNN_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, edge_kernel<C>, Cfg::THREADS, Cfg::SMEM_BYTES));
+        GNN_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, Cfg::THREADS, Cfg::SMEM_BYTES));
         if (occ < 1) return GNN_ERR_BAD_ARCH;
         occ = std::max(occ, Cfg::MIN_CTAS);                    // the kernel is compiled for MIN_CTAS resident CTAs per SM
         const int tmem_cap = 512 / Cfg::TMEM_COLS;              // co-resident CTAs must all fit their TMEM columns
@@ -709,7 +724,7 @@ int configure_edge(Bf16BlockDev& b, int n_sms) {
     return GNN_OK;
 }
 
-template <int C>
+template <int C, int LOGK>
 int launch_edge_t(const EdgeParams& p, int grid_cap, cudaStream_t s) {
     using Cfg = EdgeCfg<C>;
     if (Cfg::PAIR) {
@@ -721,9 +736,9 @@ int launch_edge_t(const EdgeParams& p, int grid_cap, cudaStream_t s) {
         at[0].id = cudaLaunchAttributeClusterDimension;
         at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
         cfg.attrs = at; cfg.numAttrs = 1;
-        GNN_CUDA_TRY(cudaLaunchKernelEx(&cfg, edge_kernel<C>, p));
+        GNN_CUDA_TRY(cudaLaunchKernelEx(&cfg, edge_kernel<C, LOGK>, p));
     } else {
-        edge_kernel<C><<<std::min(p.n_tiles, grid_cap), Cfg::THREADS, Cfg::SMEM_BYTES, s>>>(p);
+        edge_kernel<C, LOGK><<<std::min(p.n_tiles, grid_cap), Cfg::THREADS, Cfg::SMEM_BYTES, s>>>(p);
     }
     return GNN_OK;
 }
@@ -800,10 +815,10 @@ int edgeconv_bf16_prepare(gnn_model& m, const float* blob) {
             else GNN_CUDA_TRY(cudaFuncSetAttribute(pre_tc_kernel<128, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, PreTcCfg<128, 256>::SMEM_BYTES));
         }
         switch (C) {
-            case 32: rc = configure_edge<32>(b, m.n_sms); break;
-            case 64: rc = configure_edge<64>(b, m.n_sms); break;
-            case 128: rc = configure_edge<128>(b, m.n_sms); break;
-            case 256: rc = configure_edge<256>(b, m.n_sms); break;
+            case 32: rc = a.k == 16 ? configure_edge<32, 4>(b, m.n_sms) : configure_edge<32, -1>(b, m.n_sms); break;
+            case 64: rc = a.k == 16 ? configure_edge<64, 4>(b, m.n_sms) : configure_edge<64, -1>(b, m.n_sms); break;
+            case 128: rc = a.k == 16 ? configure_edge<128, 4>(b, m.n_sms) : configure_edge<128, -1>(b, m.n_sms); break;
+            case 256: rc = a.k == 16 ? configure_edge<256, 4>(b, m.n_sms) : configure_edge<256, -1>(b, m.n_sms); break;
             default: rc = GNN_ERR_BAD_ARCH;
         }
         if (rc != GNN_OK) return rc;
@@ -854,18 +869,13 @@ int launch_edgeconv_bf16(gnn_model& m, int block, const float* x, const int32_t*
     ep.n_tiles = (N + ep.TP - 1) / ep.TP;
     int rc;
     switch (b.C) {
-        case 32: rc = launch_edge_t<32>(ep, b.grid_cap, s); break;
-        case 64: rc = launch_edge_t<64>(ep, b.grid_cap, s); break;
-        case 128: rc = launch_edge_t<128>(ep, b.grid_cap, s); break;
-        case 256: rc = launch_edge_t<256>(ep, b.grid_cap, s); break;
+        case 32: rc = k == 16 ? launch_edge_t<32, 4>(ep, b.grid_cap, s) : launch_edge_t<32, -1>(ep, b.grid_cap, s); break;
+        case 64: rc = k == 16 ? launch_edge_t<64, 4>(ep, b.grid_cap, s) : launch_edge_t<64, -1>(ep, b.grid_cap, s); break;
+        case 128: rc = k == 16 ? launch_edge_t<128, 4>(ep, b.grid_cap, s) : launch_edge_t<128, -1>(ep, b.grid_cap, s); break;
+        case 256: rc = k == 16 ? launch_edge_t<256, 4>(ep, b.grid_cap, s) : launch_edge_t<256, -1>(ep, b.grid_cap, s); break;
         default: return GNN_ERR_BAD_ARCH;
     }
     if (rc != GNN_OK) return rc;
     return 2;
 }
 
-#ifdef GNN_EDGE_TIMING
-extern "C" int gnn_debug_edge_timing(long long* out_host) {
-    return cudaMemcpyFromSymbol(out_host, g_edge_ts, sizeof(long long) * 4 * 64 * 16) == cudaSuccess ? 0 : -1;
-}
-#endif
