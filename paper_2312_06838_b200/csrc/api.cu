@@ -130,6 +130,7 @@ int alloc_workspace(gnn_model* m, Workspace& w) {
     if ((rc = dev_alloc(m, &w.xa, Nmax * m->Cmax)) != GNN_OK) return rc;
     if ((rc = dev_alloc(m, &w.xb, Nmax * m->Cmax)) != GNN_OK) return rc;
     if ((rc = dev_alloc(m, &w.idx, Nmax * a.k)) != GNN_OK) return rc;
+    if ((rc = dev_alloc(m, &w.dm, Nmax * (size_t)((a.max_particles + 3) & ~3))) != GNN_OK) return rc;
     if ((rc = dev_alloc(m, &w.jet_start, Bmax)) != GNN_OK) return rc;
     if ((rc = dev_alloc(m, &w.jet_n, Bmax)) != GNN_OK) return rc;
     if ((rc = dev_alloc(m, &w.status, 1)) != GNN_OK) return rc;
@@ -239,7 +240,7 @@ int gnn_create(const void* weights_host, size_t bytes, const gnn_arch* arch, int
     m->Nmax = (int64_t)arch->max_batch_jets * arch->max_particles;
     m->Cmax = 8;
     for (int l = 0; l < arch->n_blocks; ++l) m->Cmax = std::max(m->Cmax, arch->channels[l][2]);
-    if ((rc = knn_configure()) != GNN_OK || (rc = edgeconv_f32_configure()) != GNN_OK ||
+    if ((rc = knn_configure()) != GNN_OK || (rc = pool_head_configure()) != GNN_OK || (rc = edgeconv_f32_configure()) != GNN_OK ||
         (rc = build_model(m, static_cast<const float*>(weights_host))) != GNN_OK) {
         gnn_destroy(m);
         return rc;

@@ -28,6 +28,7 @@ struct Workspace {
     float* xa = nullptr;        // [Nmax, Cmax] ping
     float* xb = nullptr;        // [Nmax, Cmax] pong
     int32_t* idx = nullptr;     // [Nmax, k] global particle indices, -1 = none
+    float* dm = nullptr;        // [Nmax, max_particles rounded to 4] per-jet pairwise squared distances (kNN)
     int32_t* jet_start = nullptr;  // [Bmax] sanitised CSR
     int32_t* jet_n = nullptr;      // [Bmax] sanitised multiplicities (< 0 = offending jet; -n if it owns n packed rows)
     unsigned* status = nullptr;    // [1] sticky device status word
@@ -87,5 +88,6 @@ int launch_edgeconv_f32(const BlockDev& b, int k, const float* x, const int32_t*
 int launch_globalize_idx(const int32_t* idx_local, int k, int B, const Workspace& w, int32_t* idx_global, cudaStream_t s);
 int launch_pool_head(const gnn_model& m, const float* x, int B, const Workspace& w, float* logits, cudaStream_t s);
 int knn_configure();
+int pool_head_configure();
 int edgeconv_f32_configure();
 

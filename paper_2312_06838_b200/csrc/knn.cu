@@ -2,14 +2,17 @@
 // "dynamic graph"; BASELINE.json north_star (1): pairwise distances in shared memory, top-k with ties broken by the
 // lower index; on (eta, phi) for block 1 and on the features for later blocks).
 //
-// One CTA per jet.  Readings: R3 squared Euclidean, direct differences (R18: no Gram form -- its
-// cancellation error exceeds the 1e-5 near-tie band); R4 self excluded by index; R5 strict order on (d, j); R6
-// k_eff = min(k, n-1).  fp32 arithmetic, d = fma(t, t, d) with t = s_i - s_j, dimensions summed in index order.
+// One CTA per (jet, tile of 32 queries): a jet of n particles occupies ceil(n/32) small CTAs, so an SM holds many
+// (the selection phase is a serial insertion per query; its latency is hidden by CTAs, not by threads of one CTA).
+// Readings: R3 squared Euclidean, direct differences (R18: no Gram form -- its cancellation error
+// exceeds the 1e-5 near-tie band); R4 self excluded by index; R5 strict order on (d, j); R6 k_eff = min(k, n-1).
+// fp32 arithmetic, d = fma(t, t, d) with t = s_i - s_j, dimensions summed in index order.
 //
-// Phase 1 (ALU-bound): each thread owns 4x4 (query x candidate) register tiles; rows of the space are staged in
-//   shared memory with a row stride of D+4 floats so that the eight lanes of a quarter-warp reading eight
-//   consecutive rows with LDS.128 hit eight different 16-byte bank groups.  Distances go to a [n][n+1] matrix in
-//   shared memory with d_ii = +inf.
+// Phase 1 (ALU-bound): the jet's rows are staged 32 dimensions at a time ([n4][36] floats: with this row stride the
+//   eight lanes of a quarter-warp reading eight consecutive rows with LDS.128 hit eight different bank groups); each
+//   thread owns up to two 4x4 (query x candidate) register tiles that accumulate over the chunks; chunks are
+//   double-buffered and staged with cp.async so that the next one lands while this one is used.  Distances of the 32
+//   queries go to a [32][n|1] matrix in shared memory with d_ii = +inf.
 // Phase 2: one thread per query walks its row and keeps the k smallest 64-bit keys (float bits of d << 32 | j) in a
 //   sorted register list -- d >= 0, so unsigned order on the bits is numeric order and equal distances fall back
 //   to the lower index for free.  (The paper-era "warp-level top-k" is replaced by this: see DESIGN.md.)
@@ -18,7 +21,10 @@
 
 namespace {
 
-constexpr int KNN_THREADS = 256;
+constexpr int KNN_THREADS = 128;
+constexpr int KNN_QT = 32;      // queries per CTA
+constexpr int KNN_DC = 32;      // dimensions staged per chunk
+constexpr int KNN_LD = KNN_DC + 4;
 
 template <int K>
 __device__ __forceinline__ void topk_insert(unsigned long long (&best)[K], unsigned long long key) {
@@ -33,107 +39,182 @@ __device__ __forceinline__ void topk_insert(unsigned long long (&best)[K], unsig
     }
 }
 
-template <int K>
 __global__ void __launch_bounds__(KNN_THREADS)
-knn_kernel(const float* __restrict__ space, int D, int k, const int32_t* __restrict__ jet_start,
-           const int32_t* __restrict__ jet_n, const int32_t* __restrict__ meta, int32_t* __restrict__ idx_out,
-           int local_out) {
+knn_dist_kernel(const float* __restrict__ space, int D, const int32_t* __restrict__ jet_start,
+                const int32_t* __restrict__ jet_n, const int32_t* __restrict__ meta, float* __restrict__ dm, int pld,
+                int tiles_per_jet) {
     extern __shared__ __align__(16) float smem[];
     if (meta[0]) return;
-    const int b = blockIdx.x;
+    const int b = blockIdx.x / tiles_per_jet, qt = blockIdx.x - b * tiles_per_jet;
     const int n = jet_n[b];
     const int start = jet_start[b];
-    if (n < -1) {                             // offending ragged jet (jet_n = -multiplicity): its packed rows exist and
-        for (int e = threadIdx.x; e < -n * k; e += KNN_THREADS)   // the point-tiled EdgeConv walks them: no neighbours
-            idx_out[(size_t)start * k + e] = -1;
-        return;
-    }
-    if (n <= 0) return;                       // empty jet (or offending padded jet, which owns no rows)
-    const int Dp = (D + 3) & ~3;
-    const int ld = Dp + 4;                    // row stride in floats
+    const int q0 = qt * KNN_QT;
+    if (n <= 0 || q0 >= n) return;            // empty jet (or offending padded jet, which owns no rows) / tile past the jet
     const int n4 = (n + 3) & ~3;
-    float* S = smem;                          // [n4][ld]
-    float* Dm = smem + (size_t)n4 * ld;       // [n][n+1]
-    const int ldd = n + 1;
-
-    // stage rows (coalesced over the contiguous [n, D] span of the jet), zero the padding
-    const float* src = space + (size_t)start * D;
-    for (int e = threadIdx.x; e < n4 * Dp; e += KNN_THREADS) {
-        int r = e / Dp, c = e - r * Dp;
-        S[r * ld + c] = (r < n && c < D) ? src[(size_t)r * D + c] : 0.0f;
-    }
-    __syncthreads();
-
-    // phase 1: 4x4 register tiles.  Thread-tile (ig, jg) covers query rows ig + nG*r and candidate rows jg + nG*r.
     const int nG = n4 >> 2;
-    for (int t = threadIdx.x; t < nG * nG; t += KNN_THREADS) {
-        const int ig = t / nG, jg = t - ig * nG;
-        float acc[4][4];
+    float* S0 = smem;                         // [2][n4][KNN_LD] double-buffered chunk of dimensions of every row of the jet
+    float* Dm = dm + (size_t)(start + q0) * pld;  // rows of this tile's queries in the global distance matrix
+    const float* src = space + (size_t)start * D;
+
+    // staging of dimensions [c0, c0 + 32): 16-byte cp.async when the rows are 16-byte aligned (D % 4 == 0), so a whole
+    // chunk is in flight without register staging; rows >= n and the tail of the last chunk are zero
+    auto stage = [&](int c0, float* Sb) {
+        const int dc = min(KNN_DC, D - c0), dc4 = (dc + 3) & ~3;
+        if ((D & 3) == 0) {
+            const int nq = dc4 >> 2;
+            for (int e = threadIdx.x; e < n4 * nq; e += KNN_THREADS) {
+                const int r = (nq == 8) ? (e >> 3) : e / nq, c = e - r * nq;
+                float* dst = Sb + r * KNN_LD + 4 * c;
+                if (r < n) {
+                    const unsigned sa = (unsigned)__cvta_generic_to_shared(dst);
+                    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(src + (size_t)r * D + c0 + 4 * c) : "memory");
+                } else {
+                    *reinterpret_cast<float4*>(dst) = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+                }
+            }
+        } else {
+            for (int e = threadIdx.x; e < n4 * dc4; e += KNN_THREADS) {
+                const int r = e / dc4, c = e - r * dc4;
+                Sb[r * KNN_LD + c] = (r < n && c < dc) ? __ldg(src + (size_t)r * D + c0 + c) : 0.0f;
+            }
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+
+    // phase 1: thread-tile (ig, jg) covers queries q0 + ig + 8a and candidates jg + nG*c (a, c = 0..3)
+    const int n_tt = 8 * nG;                  // <= 256: at most two tiles per thread
+    float acc[2][4][4];
+#pragma unroll
+    for (int u = 0; u < 2; ++u)
 #pragma unroll
         for (int a = 0; a < 4; ++a)
 #pragma unroll
-            for (int c = 0; c < 4; ++c) acc[a][c] = 0.0f;
-        const float* pi = S + ig * ld;
-        const float* pj = S + jg * ld;
-        for (int c0 = 0; c0 < Dp; c0 += 4) {
-            float4 qi[4], qj[4];
+            for (int c = 0; c < 4; ++c) acc[u][a][c] = 0.0f;
+    stage(0, S0);
+    for (int c0 = 0, ci = 0; c0 < D; c0 += KNN_DC, ++ci) {
+        const int dc = min(KNN_DC, D - c0), dc4 = (dc + 3) & ~3;
+        const float* S = S0 + (size_t)(ci & 1) * n4 * KNN_LD;
+        if (c0 + KNN_DC < D) {
+            stage(c0 + KNN_DC, S0 + (size_t)((ci + 1) & 1) * n4 * KNN_LD);
+            asm volatile("cp.async.wait_group 1;" ::: "memory");
+        } else {
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
+        }
+        __syncthreads();
 #pragma unroll
-            for (int r = 0; r < 4; ++r) {
-                qi[r] = *reinterpret_cast<const float4*>(pi + (size_t)r * nG * ld + c0);
-                qj[r] = *reinterpret_cast<const float4*>(pj + (size_t)r * nG * ld + c0);
+        for (int u = 0; u < 2; ++u) {
+            const int tt = threadIdx.x + u * KNN_THREADS;
+            if (tt < n_tt) {
+                const int ig = tt / nG, jg = tt - ig * nG;
+                const float* pi = S + (q0 + ig) * KNN_LD;
+                const float* pj = S + jg * KNN_LD;
+                for (int cc = 0; cc < dc4; cc += 4) {
+                    float4 qi[4], qj[4];
+#pragma unroll
+                    for (int r = 0; r < 4; ++r) {
+                        const int qr = min(q0 + ig + 8 * r, n4 - 1) - (q0 + ig);     // tail tile: clamp (result unused)
+                        qi[r] = *reinterpret_cast<const float4*>(pi + qr * KNN_LD + cc);
+                        qj[r] = *reinterpret_cast<const float4*>(pj + r * nG * KNN_LD + cc);
+                    }
+#pragma unroll
+                    for (int a = 0; a < 4; ++a)
+#pragma unroll
+                        for (int c = 0; c < 4; ++c) {
+                            float t0 = qi[a].x - qj[c].x; acc[u][a][c] = fmaf(t0, t0, acc[u][a][c]);
+                            float t1 = qi[a].y - qj[c].y; acc[u][a][c] = fmaf(t1, t1, acc[u][a][c]);
+                            float t2 = qi[a].z - qj[c].z; acc[u][a][c] = fmaf(t2, t2, acc[u][a][c]);
+                            float t3 = qi[a].w - qj[c].w; acc[u][a][c] = fmaf(t3, t3, acc[u][a][c]);
+                        }
+                }
             }
+        }
+        __syncthreads();                      // this buffer is restaged two chunks from now
+    }
 #pragma unroll
-            for (int a = 0; a < 4; ++a)
+    for (int u = 0; u < 2; ++u) {
+        const int tt = threadIdx.x + u * KNN_THREADS;
+        if (tt < n_tt) {
+            const int ig = tt / nG, jg = tt - ig * nG;
+#pragma unroll
+            for (int a = 0; a < 4; ++a) {
+                const int qi = ig + 8 * a;                        // query within the tile
+                if (q0 + qi >= n) continue;
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
-                    float t0 = qi[a].x - qj[c].x; acc[a][c] = fmaf(t0, t0, acc[a][c]);
-                    float t1 = qi[a].y - qj[c].y; acc[a][c] = fmaf(t1, t1, acc[a][c]);
-                    float t2 = qi[a].z - qj[c].z; acc[a][c] = fmaf(t2, t2, acc[a][c]);
-                    float t3 = qi[a].w - qj[c].w; acc[a][c] = fmaf(t3, t3, acc[a][c]);
+                    const int j = jg + nG * c;
+                    if (j < n) Dm[(size_t)qi * pld + j] = acc[u][a][c];
                 }
-        }
-#pragma unroll
-        for (int a = 0; a < 4; ++a) {
-            int i = ig + nG * a;
-            if (i >= n) continue;
-#pragma unroll
-            for (int c = 0; c < 4; ++c) {
-                int j = jg + nG * c;
-                if (j < n) Dm[i * ldd + j] = (i == j) ? INFINITY : acc[a][c];
             }
         }
-    }
-    __syncthreads();
-
-    // phase 2: thread i selects for query i
-    for (int i = threadIdx.x; i < n; i += KNN_THREADS) {
-        unsigned long long best[K];
-#pragma unroll
-        for (int m = 0; m < K; ++m) best[m] = ~0ull;
-        const float* row = Dm + i * ldd;
-        for (int j = 0; j < n; ++j) {
-            if (j == i) continue;                                       // R4: by index
-            unsigned long long key = ((unsigned long long)__float_as_uint(row[j]) << 32) | (unsigned)j;
-            if (key < best[K - 1]) topk_insert<K>(best, key);
-        }
-        int32_t* out = idx_out + (size_t)(start + i) * k;
-        const int base = local_out ? 0 : start;
-#pragma unroll
-        for (int m = 0; m < K; ++m)
-            if (m < k) out[m] = (best[m] == ~0ull) ? -1 : (int32_t)(best[m] & 0xffffffffull) + base;
     }
 }
 
-size_t knn_smem_bytes(int D, int P) {
-    int Dp = (D + 3) & ~3, ld = Dp + 4, n4 = (P + 3) & ~3;
-    return ((size_t)n4 * ld + (size_t)P * (P + 1)) * sizeof(float);
+// Phase 2, its own kernel so that every lane of every warp owns a query: thread q = particle q of the packed batch.
+// d(i, j) is read as d(j, i) (the matrix is exactly symmetric: (a-b)^2 and (b-a)^2 round identically), which makes the
+// loads of a warp's consecutive queries consecutive addresses.
+constexpr int KSEL_THREADS = 128;
+template <int K>
+__global__ void __launch_bounds__(KSEL_THREADS)
+knn_select_kernel(const float* __restrict__ dm, int pld, int k, int B, const int32_t* __restrict__ jet_start,
+                  const int32_t* __restrict__ jet_n, const int32_t* __restrict__ meta, int32_t* __restrict__ idx_out,
+                  int local_out) {
+    if (meta[0]) return;
+    const int q = blockIdx.x * KSEL_THREADS + threadIdx.x;
+    if (q >= meta[1]) return;
+    int lo = 0, hi = B - 1;                                     // the jet that owns row q: last b with jet_start[b] <= q
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (__ldg(jet_start + mid) <= q) lo = mid; else hi = mid - 1;
+    }
+    const int n = jet_n[lo], start = jet_start[lo];
+    int32_t* out = idx_out + (size_t)q * k;
+    if (n < 0) {                              // offending ragged jet (jet_n = -multiplicity): its packed rows exist and the
+        for (int m = 0; m < k; ++m) out[m] = -1;                  // point-tiled EdgeConv walks them: no neighbours
+        return;
+    }
+    const int i = q - start;
+    unsigned long long best[K];
+#pragma unroll
+    for (int m = 0; m < K; ++m) best[m] = ~0ull;
+    const float* col = dm + (size_t)start * pld + i;
+    int j = 0;
+    for (; j + 3 < n; j += 4) {
+        float d[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) d[u] = __ldg(col + (size_t)(j + u) * pld);
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            if (j + u == i) continue;                                   // R4: by index
+            const unsigned long long key = ((unsigned long long)__float_as_uint(d[u]) << 32) | (unsigned)(j + u);
+            if (key < best[K - 1]) topk_insert<K>(best, key);
+        }
+    }
+    for (; j < n; ++j) {
+        if (j == i) continue;
+        const unsigned long long key = ((unsigned long long)__float_as_uint(__ldg(col + (size_t)j * pld)) << 32) | (unsigned)j;
+        if (key < best[K - 1]) topk_insert<K>(best, key);
+    }
+    const int base = local_out ? 0 : start;
+#pragma unroll
+    for (int m = 0; m < K; ++m)
+        if (m < k) out[m] = (best[m] == ~0ull) ? -1 : (int32_t)(best[m] & 0xffffffffull) + base;
+}
+
+size_t knn_smem_bytes(int P) {
+    const int n4 = (P + 3) & ~3;
+    return (size_t)2 * n4 * KNN_LD * sizeof(float);
 }
 
 template <int K>
 int launch_knn_t(const float* space, int D, int k, int B, int P, const Workspace& w, int32_t* idx_out, int local_out,
                  cudaStream_t s) {
-    knn_kernel<K><<<B, KNN_THREADS, knn_smem_bytes(D, P), s>>>(space, D, k, w.jet_start, w.jet_n, w.meta, idx_out, local_out);
-    return 1;
+    const int tiles = (P + KNN_QT - 1) / KNN_QT;
+    const int pld = (P + 3) & ~3;
+    knn_dist_kernel<<<B * tiles, KNN_THREADS, knn_smem_bytes(P), s>>>(space, D, w.jet_start, w.jet_n, w.meta, w.dm, pld, tiles);
+    const long long n_upper = (long long)B * P;
+    knn_select_kernel<K><<<(unsigned)((n_upper + KSEL_THREADS - 1) / KSEL_THREADS), KSEL_THREADS, 0, s>>>(
+        w.dm, pld, k, B, w.jet_start, w.jet_n, w.meta, idx_out, local_out);
+    return 2;
 }
 
 }  // namespace
@@ -141,7 +222,7 @@ int launch_knn_t(const float* space, int D, int k, int B, int P, const Workspace
 int launch_knn(const float* space, int D, int k, int B, int max_particles, const Workspace& w, int32_t* idx_out,
                int local_out, cudaStream_t s) {
     if (B == 0) return 0;
-    if (knn_smem_bytes(D, max_particles) > 227 * 1024) return GNN_ERR_BAD_ARG;
+    if (knn_smem_bytes(max_particles) > 227 * 1024) return GNN_ERR_BAD_ARG;
     if (k <= 4) return launch_knn_t<4>(space, D, k, B, max_particles, w, idx_out, local_out, s);
     if (k <= 8) return launch_knn_t<8>(space, D, k, B, max_particles, w, idx_out, local_out, s);
     if (k <= 16) return launch_knn_t<16>(space, D, k, B, max_particles, w, idx_out, local_out, s);
@@ -169,12 +250,7 @@ int launch_globalize_idx(const int32_t* idx_local, int k, int B, const Workspace
     return 1;
 }
 
-// opt every instantiation into the full 227 KB of dynamic shared memory (called once from gnn_create)
 int knn_configure() {
-    const int lim = 227 * 1024;
-    if (cudaFuncSetAttribute(knn_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim) != cudaSuccess) return GNN_ERR_CUDA;
-    if (cudaFuncSetAttribute(knn_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim) != cudaSuccess) return GNN_ERR_CUDA;
-    if (cudaFuncSetAttribute(knn_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim) != cudaSuccess) return GNN_ERR_CUDA;
-    if (cudaFuncSetAttribute(knn_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim) != cudaSuccess) return GNN_ERR_CUDA;
-    return GNN_OK;
+    return cudaFuncSetAttribute(knn_dist_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024) == cudaSuccess
+               ? GNN_OK : GNN_ERR_CUDA;
 }

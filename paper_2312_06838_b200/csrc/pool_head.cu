@@ -3,50 +3,168 @@
 // => dropout is the identity; BASELINE.json north_star (3)).  fp32 in every precision mode (R19).
 // Ragged input makes the "mask" implicit: only the n_b real particles of jet b are ever stored (R7, R12).
 //
-// One CTA per jet: thread c sums channel c over the jet's rows (coalesced: consecutive threads read consecutive
-// channels of one row), then the FC layers run as coalesced mat-vecs on the transposed weights Wt[in][out].
+// One CTA per PH_JETS consecutive jets: (1) pooling, float4 loads, the CTA's threads split into row groups x channel
+// quads and the group partials are reduced through shared memory in a fixed order (deterministic); (2) the FC layers as
+// mat-vecs on the transposed weights Wt[in][out] with PH_JETS accumulators per thread, so a weight is read once per
+// CTA instead of once per jet (the 256 KB of FC-1 weights were 268 MB of L2 traffic per forward at one jet per CTA).
 #include "gnn_internal.h"
 
 namespace {
 
 constexpr int PH_THREADS = 256;
-constexpr int PH_MAXW = 1024;
+constexpr int PH_JETS = 8;
 
 struct HeadParams {
     LinF32 fc[GNN_MAX_FC + 1];
     int n_fc;
     int C;
     int n_classes;
+    int wmax;        // widest activation vector (row stride of the staging arrays)
 };
 
 __global__ void __launch_bounds__(PH_THREADS)
 pool_head_kernel(const float* __restrict__ x, const int32_t* __restrict__ jet_start, const int32_t* __restrict__ jet_n,
-                 const int32_t* __restrict__ meta, HeadParams hp, float* __restrict__ logits) {
-    __shared__ float z0[PH_MAXW], z1[PH_MAXW];
-    const int b = blockIdx.x;
-    const int n = jet_n[b];
-    if (meta[0] || n < 0) {                       // poisoned batch or offending jet: NaN logits (include/gnn.h)
-        for (int o = threadIdx.x; o < hp.n_classes; o += PH_THREADS) logits[(size_t)b * hp.n_classes + o] = __int_as_float(0x7fc00000);
-        return;
-    }
-    const int C = hp.C;
-    const float* xb = x + (size_t)jet_start[b] * C;
-    for (int c = threadIdx.x; c < C; c += PH_THREADS) {
-        float s = 0.0f;
-        for (int i = 0; i < n; ++i) s += xb[(size_t)i * C + c];
-        z0[c] = (n > 0) ? s / (float)n : 0.0f;    // R12: empty jet pools to 0
+                 const int32_t* __restrict__ meta, HeadParams hp, int B, float* __restrict__ logits) {
+    extern __shared__ __align__(16) float zs[];      // z0 [PH_JETS][wmax] | z1 [PH_JETS][wmax] | partials
+    __shared__ int s_end[PH_JETS], s_n[PH_JETS];     // row range ends (relative to the CTA's first row) and multiplicities
+    const int b0 = blockIdx.x * PH_JETS;
+    const int nj = min(PH_JETS, B - b0);
+    const int C = hp.C, W = hp.wmax;
+    float* z0 = zs;
+    float* z1 = zs + PH_JETS * W;
+    float* part = z1 + PH_JETS * W;                  // pooling: [G][PH_JETS][C]; FC: [KS][PH_JETS][ld]
+    const bool poisoned = meta[0] != 0;
+    // ---- pooling: the jets of this CTA are one contiguous span of rows; thread (row group rg, channel quad cq) walks rows
+    // rg, rg + G, ... with eight loads in flight and flushes its partial sum when a row crosses into the next jet ---------
+    const int row0 = jet_start[b0];
+    if (threadIdx.x < PH_JETS) {
+        const int jb = threadIdx.x;
+        int n = (jb < nj && !poisoned) ? jet_n[b0 + jb] : 0;
+        if (n < 0) n = 0;                            // offending jet: pools nothing (its logits become NaN below)
+        s_n[jb] = n;
+        s_end[jb] = (jb < nj) ? jet_start[b0 + jb] - row0 + n : 0x7fffffff;
     }
     __syncthreads();
+    const int CQ = C >> 2;                           // channel quads
+    const int TQ = min(CQ, PH_THREADS);
+    const int G = max(1, PH_THREADS / CQ);           // row groups
+    // rows of jets are contiguous only for well-formed batches; offending jets own rows too, so walk jet by jet ranges
+    for (int cq0 = 0; cq0 < CQ; cq0 += PH_THREADS) {
+        const int cq = cq0 + (int)threadIdx.x % TQ, rg = (int)threadIdx.x / TQ;
+        if (cq < CQ && rg < G) {
+            for (int jb = 0; jb < PH_JETS; ++jb) {
+                const int n = s_n[jb];
+                const float4* xb = reinterpret_cast<const float4*>(x + (size_t)(jb < nj ? jet_start[b0 + jb] : 0) * C) + cq;
+                float4 s = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+                int i = rg;
+                for (; i + 7 * G < n; i += 8 * G) {
+                    float4 a[8];
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) a[u] = __ldg(xb + (size_t)(i + u * G) * CQ);
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) { s.x += a[u].x; s.y += a[u].y; s.z += a[u].z; s.w += a[u].w; }
+                }
+                float4 a[8];
+#pragma unroll
+                for (int u = 0; u < 8; ++u) {
+                    a[u] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+                    if (i + u * G < n) a[u] = __ldg(xb + (size_t)(i + u * G) * CQ);
+                }
+#pragma unroll
+                for (int u = 0; u < 8; ++u) { s.x += a[u].x; s.y += a[u].y; s.z += a[u].z; s.w += a[u].w; }
+                *reinterpret_cast<float4*>(part + ((size_t)rg * PH_JETS + jb) * C + 4 * cq) = s;
+            }
+        }
+        __syncthreads();
+        for (int it = threadIdx.x; it < PH_JETS * TQ; it += PH_THREADS) {
+            const int jb = it / TQ, c4 = cq0 + it % TQ;
+            if (c4 >= CQ) continue;
+            float4 s = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+            for (int g2 = 0; g2 < G; ++g2) {
+                const float4 o = *reinterpret_cast<const float4*>(part + ((size_t)g2 * PH_JETS + jb) * C + 4 * c4);
+                s.x += o.x; s.y += o.y; s.z += o.z; s.w += o.w;
+            }
+            const int n = s_n[jb];
+            const float inv = n > 0 ? 1.0f / (float)n : 0.0f;           // R12: empty jet pools to 0
+            *reinterpret_cast<float4*>(z0 + jb * W + 4 * c4) = make_float4(s.x * inv, s.y * inv, s.z * inv, s.w * inv);
+        }
+        __syncthreads();
+    }
+    // ---- FC head: wide layers split K over thread groups (float4 of outputs x K slice, eight weight loads in flight),
+    // narrow layers (the final one) run one thread per (jet, output) ---------------------------------------------------------
     float* zin = z0; float* zout = z1;
     for (int l = 0; l < hp.n_fc; ++l) {
         const LinF32 L = hp.fc[l];
         const bool last = (l == hp.n_fc - 1);
-        for (int o = threadIdx.x; o < L.N; o += PH_THREADS) {
-            float acc = 0.0f;
-            for (int c = 0; c < L.K; ++c) acc = fmaf(zin[c], __ldg(L.Wt + (size_t)c * L.ld + o), acc);
-            acc += __ldg(L.shift + o);
-            if (last) logits[(size_t)b * hp.n_classes + o] = acc;
-            else zout[o] = fmaxf(acc, 0.0f);
+        const int OQ = L.ld >> 2;
+        if (OQ >= 16 && OQ <= PH_THREADS) {
+            const int KS = PH_THREADS / OQ;                      // K slices
+            const int oq = (int)threadIdx.x % OQ, ks = (int)threadIdx.x / OQ;
+            if (ks < KS) {
+                const int kper = (L.K + KS - 1) / KS, k0 = ks * kper, k1 = min(L.K, k0 + kper);
+                float4 acc[PH_JETS];
+#pragma unroll
+                for (int jb = 0; jb < PH_JETS; ++jb) acc[jb] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+                const float4* wp = reinterpret_cast<const float4*>(L.Wt) + oq;
+                for (int c = k0; c < k1; c += 8) {
+                    float4 wv[8];
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) {
+                        wv[u] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+                        if (c + u < k1) wv[u] = __ldg(wp + (size_t)(c + u) * OQ);
+                    }
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) {
+                        if (c + u < k1) {
+#pragma unroll
+                            for (int jb = 0; jb < PH_JETS; ++jb) {
+                                const float zv = zin[jb * W + c + u];
+                                acc[jb].x = fmaf(zv, wv[u].x, acc[jb].x); acc[jb].y = fmaf(zv, wv[u].y, acc[jb].y);
+                                acc[jb].z = fmaf(zv, wv[u].z, acc[jb].z); acc[jb].w = fmaf(zv, wv[u].w, acc[jb].w);
+                            }
+                        }
+                    }
+                }
+#pragma unroll
+                for (int jb = 0; jb < PH_JETS; ++jb)
+                    *reinterpret_cast<float4*>(part + ((size_t)ks * PH_JETS + jb) * L.ld + 4 * oq) = acc[jb];
+            }
+            __syncthreads();
+            for (int it = threadIdx.x; it < PH_JETS * L.N; it += PH_THREADS) {
+                const int jb = it / L.N, o = it - jb * L.N;
+                float v = __ldg(L.shift + o);
+                for (int k2 = 0; k2 < KS; ++k2) v += part[((size_t)k2 * PH_JETS + jb) * L.ld + o];
+                if (jb < nj) {
+                    if (last) {
+                        const bool bad = poisoned || jet_n[b0 + jb] < 0;
+                        logits[(size_t)(b0 + jb) * hp.n_classes + o] = bad ? __int_as_float(0x7fc00000) : v;
+                    } else {
+                        zout[jb * W + o] = fmaxf(v, 0.0f);
+                    }
+                }
+            }
+        } else {
+            for (int it = threadIdx.x; it < PH_JETS * L.N; it += PH_THREADS) {
+                const int jb = it / L.N, o = it - jb * L.N;
+                float a0 = 0.0f, a1 = 0.0f, a2 = 0.0f, a3 = 0.0f;
+                int c = 0;
+                for (; c + 3 < L.K; c += 4) {
+                    a0 = fmaf(zin[jb * W + c], __ldg(L.Wt + (size_t)c * L.ld + o), a0);
+                    a1 = fmaf(zin[jb * W + c + 1], __ldg(L.Wt + (size_t)(c + 1) * L.ld + o), a1);
+                    a2 = fmaf(zin[jb * W + c + 2], __ldg(L.Wt + (size_t)(c + 2) * L.ld + o), a2);
+                    a3 = fmaf(zin[jb * W + c + 3], __ldg(L.Wt + (size_t)(c + 3) * L.ld + o), a3);
+                }
+                for (; c < L.K; ++c) a0 = fmaf(zin[jb * W + c], __ldg(L.Wt + (size_t)c * L.ld + o), a0);
+                const float v = ((a0 + a1) + (a2 + a3)) + __ldg(L.shift + o);
+                if (jb < nj) {
+                    if (last) {
+                        const bool bad = poisoned || jet_n[b0 + jb] < 0;
+                        logits[(size_t)(b0 + jb) * hp.n_classes + o] = bad ? __int_as_float(0x7fc00000) : v;
+                    } else {
+                        zout[jb * W + o] = fmaxf(v, 0.0f);
+                    }
+                }
+            }
         }
         __syncthreads();
         float* t = zin; zin = zout; zout = t;
@@ -62,6 +180,20 @@ int launch_pool_head(const gnn_model& m, const float* x, int B, const Workspace&
     for (int i = 0; i < m.n_fc; ++i) hp.fc[i] = m.fc[i];
     hp.C = m.arch.channels[m.arch.n_blocks - 1][2];
     hp.n_classes = m.arch.n_classes;
-    pool_head_kernel<<<B, PH_THREADS, 0, s>>>(x, w.jet_start, w.jet_n, w.meta, hp, logits);
+    hp.wmax = hp.C;
+    for (int i = 0; i < m.n_fc; ++i) hp.wmax = std::max(hp.wmax, (m.fc[i].N + 3) & ~3);
+    const int G = std::max(1, PH_THREADS / (hp.C / 4));
+    size_t part = (size_t)G * PH_JETS * hp.C;                    // pooling partials, reused as the split-K partials
+    for (int i = 0; i < m.n_fc; ++i) {
+        const int OQ = m.fc[i].ld / 4;
+        if (OQ >= 16 && OQ <= PH_THREADS) part = std::max(part, (size_t)(PH_THREADS / OQ) * PH_JETS * m.fc[i].ld);
+    }
+    const size_t smem = ((size_t)2 * PH_JETS * hp.wmax + part) * sizeof(float);
+    pool_head_kernel<<<(B + PH_JETS - 1) / PH_JETS, PH_THREADS, smem, s>>>(x, w.jet_start, w.jet_n, w.meta, hp, B, logits);
     return 1;
+}
+
+int pool_head_configure() {
+    return cudaFuncSetAttribute(pool_head_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024) == cudaSuccess
+               ? GNN_OK : GNN_ERR_CUDA;
 }
