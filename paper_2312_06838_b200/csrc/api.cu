@@ -130,6 +130,7 @@ int alloc_workspace(gnn_model* m, Workspace& w) {
     if ((rc = dev_alloc(m, &w.xa, Nmax * m->Cmax)) != GNN_OK) return rc;
     if ((rc = dev_alloc(m, &w.xb, Nmax * m->Cmax)) != GNN_OK) return rc;
     if ((rc = dev_alloc(m, &w.idx, Nmax * a.k)) != GNN_OK) return rc;
+    if ((rc = dev_alloc(m, &w.pjet, Nmax)) != GNN_OK) return rc;
     if ((rc = dev_alloc(m, &w.dm, Nmax * (size_t)((a.max_particles + 3) & ~3))) != GNN_OK) return rc;
     if ((rc = dev_alloc(m, &w.jet_start, Bmax)) != GNN_OK) return rc;
     if ((rc = dev_alloc(m, &w.jet_n, Bmax)) != GNN_OK) return rc;

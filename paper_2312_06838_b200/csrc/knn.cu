@@ -42,16 +42,25 @@ __device__ __forceinline__ void topk_insert(unsigned long long (&best)[K], unsig
 __global__ void __launch_bounds__(KNN_THREADS)
 knn_dist_kernel(const float* __restrict__ space, int D, const int32_t* __restrict__ jet_start,
                 const int32_t* __restrict__ jet_n, const int32_t* __restrict__ meta, float* __restrict__ dm, int pld,
-                int tiles_per_jet) {
+                int32_t* __restrict__ pjet, int tiles_per_jet) {
     extern __shared__ __align__(16) float smem[];
     if (meta[0]) return;
     const int b = blockIdx.x / tiles_per_jet, qt = blockIdx.x - b * tiles_per_jet;
     const int n = jet_n[b];
     const int start = jet_start[b];
-    const int q0 = qt * KNN_QT;
-    if (n <= 0 || q0 >= n) return;            // empty jet (or offending padded jet, which owns no rows) / tile past the jet
+    if (n < -1) {                             // offending ragged jet: owns -n rows; only the particle -> jet map is needed
+        for (int r = qt * KNN_THREADS + threadIdx.x; r < -n; r += tiles_per_jet * KNN_THREADS) pjet[start + r] = b;
+        return;
+    }
+    if (n <= 0) return;                       // empty jet (or offending padded jet, which owns no rows)
     const int n4 = (n + 3) & ~3;
-    const int nG = n4 >> 2;
+    const int nG = n4 >> 2;                   // groups of four candidates (and of four queries)
+    // query groups per CTA: as many as fill 256 thread-tiles, so that a typical jet (n ~ 40) is ONE CTA with ~100 busy
+    // threads and no padded queries; ceil(nG / gpc) <= ceil(P / 32) CTAs of a jet have work
+    const int gpc = min(nG, 256 / nG);
+    const int q0 = qt * 4 * gpc;
+    if (q0 >= n) return;
+    if ((int)threadIdx.x < 4 * gpc && q0 + (int)threadIdx.x < n) pjet[start + q0 + threadIdx.x] = b;
     float* S0 = smem;                         // [2][n4][KNN_LD] double-buffered chunk of dimensions of every row of the jet
     float* Dm = dm + (size_t)(start + q0) * pld;  // rows of this tile's queries in the global distance matrix
     const float* src = space + (size_t)start * D;
@@ -81,8 +90,8 @@ knn_dist_kernel(const float* __restrict__ space, int D, const int32_t* __restric
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
 
-    // phase 1: thread-tile (ig, jg) covers queries q0 + ig + 8a and candidates jg + nG*c (a, c = 0..3)
-    const int n_tt = 8 * nG;                  // <= 256: at most two tiles per thread
+    // phase 1: thread-tile (ig, jg) covers queries q0 + ig + gpc*a and candidates jg + nG*c (a, c = 0..3)
+    const int n_tt = gpc * nG;                // <= 256: at most two tiles per thread
     float acc[2][4][4];
 #pragma unroll
     for (int u = 0; u < 2; ++u)
@@ -112,7 +121,7 @@ knn_dist_kernel(const float* __restrict__ space, int D, const int32_t* __restric
                     float4 qi[4], qj[4];
 #pragma unroll
                     for (int r = 0; r < 4; ++r) {
-                        const int qr = min(q0 + ig + 8 * r, n4 - 1) - (q0 + ig);     // tail tile: clamp (result unused)
+                        const int qr = min(q0 + ig + gpc * r, n4 - 1) - (q0 + ig);   // tail tile: clamp (result unused)
                         qi[r] = *reinterpret_cast<const float4*>(pi + qr * KNN_LD + cc);
                         qj[r] = *reinterpret_cast<const float4*>(pj + r * nG * KNN_LD + cc);
                     }
@@ -137,7 +146,7 @@ knn_dist_kernel(const float* __restrict__ space, int D, const int32_t* __restric
             const int ig = tt / nG, jg = tt - ig * nG;
 #pragma unroll
             for (int a = 0; a < 4; ++a) {
-                const int qi = ig + 8 * a;                        // query within the tile
+                const int qi = ig + gpc * a;                      // query within the tile
                 if (q0 + qi >= n) continue;
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
@@ -149,27 +158,25 @@ knn_dist_kernel(const float* __restrict__ space, int D, const int32_t* __restric
     }
 }
 
-// Phase 2, its own kernel so that every lane of every warp owns a query: thread q = particle q of the packed batch.
-// d(i, j) is read as d(j, i) (the matrix is exactly symmetric: (a-b)^2 and (b-a)^2 round identically), which makes the
-// loads of a warp's consecutive queries consecutive addresses.
+// Phase 2, its own kernel so that every lane of every warp has work: TWO threads per particle of the packed batch
+// (even / odd candidates), each keeping the k smallest of its half as a sorted register list; the k smallest of the
+// union are then { min(A[m], B[K-1-m]) }, a bitonic sequence that log2(K) half-cleaner stages sort in registers.  d(i, j) is read as d(j, i) (the matrix is exactly
+// symmetric: (a-b)^2 and (b-a)^2 round identically), so a warp's consecutive queries read consecutive addresses.
 constexpr int KSEL_THREADS = 128;
 template <int K>
 __global__ void __launch_bounds__(KSEL_THREADS)
-knn_select_kernel(const float* __restrict__ dm, int pld, int k, int B, const int32_t* __restrict__ jet_start,
+knn_select_kernel(const float* __restrict__ dm, int pld, int k, const int32_t* __restrict__ pjet, const int32_t* __restrict__ jet_start,
                   const int32_t* __restrict__ jet_n, const int32_t* __restrict__ meta, int32_t* __restrict__ idx_out,
                   int local_out) {
     if (meta[0]) return;
-    const int q = blockIdx.x * KSEL_THREADS + threadIdx.x;
-    if (q >= meta[1]) return;
-    int lo = 0, hi = B - 1;                                     // the jet that owns row q: last b with jet_start[b] <= q
-    while (lo < hi) {
-        const int mid = (lo + hi + 1) >> 1;
-        if (__ldg(jet_start + mid) <= q) lo = mid; else hi = mid - 1;
-    }
+    const int t = blockIdx.x * KSEL_THREADS + threadIdx.x;
+    const int q = t >> 1, half = t & 1;
+    if (q >= meta[1]) return;                                   // both lanes of a pair leave together
+    const int lo = __ldg(pjet + q);                             // the jet that owns row q (written by knn_dist_kernel)
     const int n = jet_n[lo], start = jet_start[lo];
     int32_t* out = idx_out + (size_t)q * k;
     if (n < 0) {                              // offending ragged jet (jet_n = -multiplicity): its packed rows exist and the
-        for (int m = 0; m < k; ++m) out[m] = -1;                  // point-tiled EdgeConv walks them: no neighbours
+        for (int m = half; m < k; m += 2) out[m] = -1;            // point-tiled EdgeConv walks them: no neighbours
         return;
     }
     const int i = q - start;
@@ -177,27 +184,59 @@ knn_select_kernel(const float* __restrict__ dm, int pld, int k, int B, const int
 #pragma unroll
     for (int m = 0; m < K; ++m) best[m] = ~0ull;
     const float* col = dm + (size_t)start * pld + i;
-    int j = 0;
-    for (; j + 3 < n; j += 4) {
-        float d[4];
+    int j = half;
+    for (; j + 14 < n; j += 16) {             // eight loads in flight per thread
+        float d[8];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) d[u] = __ldg(col + (size_t)(j + u) * pld);
+        for (int u = 0; u < 8; ++u) d[u] = __ldg(col + (size_t)(j + 2 * u) * pld);
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            if (j + u == i) continue;                                   // R4: by index
-            const unsigned long long key = ((unsigned long long)__float_as_uint(d[u]) << 32) | (unsigned)(j + u);
+        for (int u = 0; u < 8; ++u) {
+            if (j + 2 * u == i) continue;                               // R4: by index
+            const unsigned long long key = ((unsigned long long)__float_as_uint(d[u]) << 32) | (unsigned)(j + 2 * u);
             if (key < best[K - 1]) topk_insert<K>(best, key);
         }
     }
-    for (; j < n; ++j) {
+    {                                         // tail: up to eight more, predicated
+        float d[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) d[u] = (j + 2 * u < n) ? __ldg(col + (size_t)(j + 2 * u) * pld) : 0.0f;
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            if (j + 2 * u >= n || j + 2 * u == i) continue;
+            const unsigned long long key = ((unsigned long long)__float_as_uint(d[u]) << 32) | (unsigned)(j + 2 * u);
+            if (key < best[K - 1]) topk_insert<K>(best, key);
+        }
+        j = n;
+    }
+    for (; j < n; j += 2) {
         if (j == i) continue;
         const unsigned long long key = ((unsigned long long)__float_as_uint(__ldg(col + (size_t)j * pld)) << 32) | (unsigned)j;
         if (key < best[K - 1]) topk_insert<K>(best, key);
     }
+    // merge with the partner lane: slot m of the merge is min(A[m], B[K-1-m]); both lanes end up with the same set
+    const unsigned pm = __activemask();
     const int base = local_out ? 0 : start;
+    unsigned long long r[K];
+#pragma unroll
+    for (int m = 0; m < K; ++m) {
+        const unsigned long long mine = half ? best[K - 1 - m] : best[m];
+        const unsigned long long other = __shfl_xor_sync(pm, mine, 1);
+        r[m] = mine < other ? mine : other;
+    }
+    // r[] is bitonic: log2(K) half-cleaner stages sort it ascending (same order as a single sorted list would give)
+#pragma unroll
+    for (int st = K / 2; st >= 1; st >>= 1)
+#pragma unroll
+        for (int m = 0; m < K; ++m)
+            if ((m & st) == 0) {
+                const unsigned long long a = r[m], c = r[m + st];
+                const bool sw = c < a;
+                r[m] = sw ? c : a;
+                r[m + st] = sw ? a : c;
+            }
 #pragma unroll
     for (int m = 0; m < K; ++m)
-        if (m < k) out[m] = (best[m] == ~0ull) ? -1 : (int32_t)(best[m] & 0xffffffffull) + base;
+        if (m < k && (m & 1) == half) out[m] = (r[m] == ~0ull) ? -1 : (int32_t)(r[m] & 0xffffffffull) + base;
 }
 
 size_t knn_smem_bytes(int P) {
@@ -210,10 +249,10 @@ int launch_knn_t(const float* space, int D, int k, int B, int P, const Workspace
                  cudaStream_t s) {
     const int tiles = (P + KNN_QT - 1) / KNN_QT;
     const int pld = (P + 3) & ~3;
-    knn_dist_kernel<<<B * tiles, KNN_THREADS, knn_smem_bytes(P), s>>>(space, D, w.jet_start, w.jet_n, w.meta, w.dm, pld, tiles);
-    const long long n_upper = (long long)B * P;
+    knn_dist_kernel<<<B * tiles, KNN_THREADS, knn_smem_bytes(P), s>>>(space, D, w.jet_start, w.jet_n, w.meta, w.dm, pld, w.pjet, tiles);
+    const long long n_upper = 2ll * B * P;                     // two threads per particle slot
     knn_select_kernel<K><<<(unsigned)((n_upper + KSEL_THREADS - 1) / KSEL_THREADS), KSEL_THREADS, 0, s>>>(
-        w.dm, pld, k, B, w.jet_start, w.jet_n, w.meta, idx_out, local_out);
+        w.dm, pld, k, w.pjet, w.jet_start, w.jet_n, w.meta, idx_out, local_out);
     return 2;
 }
 
