@@ -24,7 +24,7 @@
 // soon as that block is written (h_ready[kb]) and releases it (h_free[kb], tcgen05.commit) as soon as layer 3 has read
 // it, so E3 of tile t and the gather of tile t+1 run under MMA3(t) / MMA2(t+1).  No block-wide barrier in the loop.
 // Warp roles: warps 0..NW-1 build / epilogue, warp NW allocates TMEM and its lane 0 issues every tcgen05.mma (leader
-// CTA only in pair mode), warp NW+1 lane 0 loads the weights.
+// CTA only in pair mode) after loading the weights.
 #include "gnn_internal.h"
 #include "tc05.cuh"
 #include <cuda_bf16.h>
@@ -41,11 +41,14 @@ struct EdgeCfg {
     static constexpr bool PAIR = C >= 256;                    // CTA pair: the weights, split over two SMs, stay resident
     static constexpr int KB = (C + 63) / 64;                  // 64-wide K blocks per layer
     static constexpr int KW = C < 64 ? C : 64;                // columns of one K block that are in use
-    static constexpr int NE = C >= 256 ? 8 : 4;               // epilogue warps: lane quadrant q = w & 3, column group w >> 2
-    static constexpr int CWE = C / (NE / 4);                  // columns per epilogue warp
-    static constexpr int NG = 2 * KB;                         // gather warps: K block g % KB, row half g / KB
+    static constexpr int CWE = C >= 128 ? 128 : C;            // columns per epilogue warp (measured best: more, narrower epilogue
+    static constexpr int NE = 4 * (C / CWE);                  // warps cost registers); lane quadrant q = w & 3, column group w >> 2
+    static constexpr int GH = 2;                              // row parts of the gather
+    static constexpr int NG = GH * KB;                        // gather warps: K block g % KB, row part g / KB
+    static constexpr int RW = TILE_ROWS / GH;                 // rows per gather warp
     static constexpr int MMA_WARP = NE + NG;
-    static constexpr int THREADS = 32 * (NE + NG + 2);
+    static constexpr int THREADS = 32 * (NE + NG + 1);
+    static constexpr int MAXREG = C >= 256 ? 96 : 80;   // registers are per SM quarter: ceil(warps / 4) * 32 * MAXREG * MIN_CTAS <= 16384
     static constexpr int KSTEPS_LAST = ((C - (KB - 1) * 64) + 15) / 16;
     static constexpr int NRB = PAIR ? C / 2 : C;              // weight rows (output channels) one CTA holds
     static constexpr int CHUNK_BYTES = NRB * 128;             // [NRB][64] bf16, 128B-swizzled
@@ -74,7 +77,7 @@ struct EdgeParams {
 
 // LOGK >= 0: k = 2^LOGK known at compile time (lets the gather keep one u chunk per particle in registers); -1: runtime
 template <int C, int LOGK>
-__global__ void __launch_bounds__(EdgeCfg<C>::THREADS, EdgeCfg<C>::MIN_CTAS) edge_kernel(EdgeParams p) {
+__global__ void __launch_bounds__(EdgeCfg<C>::THREADS) __maxnreg__(EdgeCfg<C>::MAXREG) edge_kernel(EdgeParams p) {
     using Cfg = EdgeCfg<C>;
     constexpr bool PAIR = Cfg::PAIR;
     constexpr int KB = Cfg::KB, NE = Cfg::NE, NG = Cfg::NG, CWE = Cfg::CWE;
@@ -110,8 +113,8 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS, EdgeCfg<C>::MIN_CTAS) edg
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     if (tid == 0) {
         for (int i = 0; i < KB; ++i) {
-            mbar_init(&h1_ready[i], 2 * Cfg::NRANKS);
-            mbar_init(&h2_ready[i], 4 * Cfg::NRANKS);
+            mbar_init(&h1_ready[i], Cfg::GH * Cfg::NRANKS);
+            mbar_init(&h2_ready[i], 4 * (Cfg::KW > CWE ? Cfg::KW / CWE : 1) * Cfg::NRANKS);   // epilogue warps per K block
             mbar_init(&h_free[i], 1);
         }
         for (int i = 0; i < 2; ++i) { mbar_init(&d_full[i], 1); mbar_init(&d_free[i], NE * Cfg::NRANKS); }
@@ -132,8 +135,8 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS, EdgeCfg<C>::MIN_CTAS) edg
         if (lane == 0) { if constexpr (PAIR) mbar_arrive_cluster(bar, 0); else mbar_arrive(bar); }
     };
 
-    if (warp == Cfg::MMA_WARP + 1) {
-        // ===== weight loader: every chunk once, resident for the life of the CTA ==================================
+    if (warp == Cfg::MMA_WARP) {
+        // ===== weight load (every chunk once, resident for the life of the CTA), then MMA issuer (leader CTA of a pair) ====
         if (lane == 0) {
             mbar_arrive_expect_tx(w_full, Cfg::W_BYTES);
             const uint8_t* src = p.wimg + (size_t)rank * Cfg::W_BYTES;
@@ -141,8 +144,6 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS, EdgeCfg<C>::MIN_CTAS) edg
                 bulk_g2s(Wsm + (size_t)c * Cfg::CHUNK_BYTES, src + (size_t)c * Cfg::CHUNK_BYTES, Cfg::CHUNK_BYTES, w_full);
             if (PAIR && rank == 1) { mbar_wait(w_full, 0); mbar_arrive_cluster(w_peer, 0); }
         }
-    } else if (warp == Cfg::MMA_WARP) {
-        // ===== MMA issuer (leader CTA of a pair) ==================================================================
         if (lane == 0 && rank == 0) {
             constexpr uint32_t idesc = idesc_bf16_f32(PAIR ? 256 : 128, C);
             const uint32_t h_addr = smem_u32(H), w_addr = smem_u32(Wsm);
@@ -150,7 +151,7 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS, EdgeCfg<C>::MIN_CTAS) edg
             if (PAIR) mbar_wait(w_peer, 0);
             for (int t = 0; t < T; ++t) {
                 for (int layer = 0; layer < 2; ++layer) {
-                    mbar_wait(&d_free[layer], (t & 1) ^ 1);      // epilogue of tile t-1 has drained this accumulator
+                    mbar_wait(&d_free[layer], t & 1);            // the epilogue has drained this accumulator and reset it to the shift
                     tc_fence_after();
 #pragma unroll
                     for (int kb = 0; kb < KB; ++kb) {
@@ -160,7 +161,7 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS, EdgeCfg<C>::MIN_CTAS) edg
                         for (int ks = 0; ks < ksteps; ++ks) {
                             const uint64_t ad = desc_sw128(h_addr + kb * Cfg::HK_BYTES + ks * 32);
                             const uint64_t bd = desc_sw128(w_addr + (layer * KB + kb) * Cfg::CHUNK_BYTES + ks * 32);
-                            mma_bf16_ss_g<PAIR>(tmem + layer * C, ad, bd, idesc, (kb | ks) != 0);
+                            mma_bf16_ss_g<PAIR>(tmem + layer * C, ad, bd, idesc, 1u);
                         }
                         if (layer == 1) mma_commit_g<PAIR>(&h_free[kb]);   // gather of the next tile may overwrite it
                     }
@@ -175,7 +176,8 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS, EdgeCfg<C>::MIN_CTAS) edg
         const int g = warp - NE, gk = g % KB, half = g / KB;
         constexpr int CPR = Cfg::KW / 8;                         // 16-byte chunks per row of a K block
         constexpr int RPI = 32 / CPR;                            // rows per warp iteration
-        constexpr int ITERS = 64 / RPI;
+        constexpr int RW = Cfg::RW, NI = RW / 32;
+        constexpr int ITERS = RW / RPI;
         constexpr int BATCH = ITERS < 8 ? ITERS : 8;
         constexpr int NB = ITERS / BATCH;
         constexpr bool HOIST = LOGK >= 0 && (1 << (LOGK >= 0 ? LOGK : 0)) >= RPI;   // rows of an iteration share a particle
@@ -184,23 +186,45 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS, EdgeCfg<C>::MIN_CTAS) edg
         const int gc = lane % CPR, grs = lane / CPR;
         uint8_t* Hk = H + gk * Cfg::HK_BYTES;
         const int col0 = gk * 64;
+        auto load_idx2 = [&](int p0, int (&dst)[NI]) {
+#pragma unroll
+            for (int a = 0; a < NI; ++a) {
+                const int r = RW * half + 32 * a + lane;
+                const int pt = p0 + (r >> logk);
+                dst[a] = (pt < N) ? __ldg(p.idx + (size_t)pt * k + (r & (k - 1))) : -1;
+            }
+        };
+        int idx_r[NI], idx_n[NI];
+        load_idx2(tile_p0(0), idx_r);
         for (int t = 0; t < T; ++t) {
             const int p0 = tile_p0(t);
-            int idx_r[2];
+            // The U/V/R/x working set of a large batch exceeds L2, so the gathered rows come from HBM (~2300 cycles per
+            // dependent batch, measured).  Pull the NEXT tile's rows into L2 now (no registers held): its loads then hit.
 #pragma unroll
-            for (int a = 0; a < 2; ++a) {
-                const int r = 64 * half + 32 * a + lane;
-                const int pt = p0 + (r >> logk);
-                idx_r[a] = (pt < N) ? __ldg(p.idx + (size_t)pt * k + (r & (k - 1))) : -1;
+            for (int a = 0; a < NI; ++a) idx_n[a] = -1;
+            if (t + 1 < T) {
+                const int p0n = tile_p0(t + 1);
+                load_idx2(p0n, idx_n);
+#pragma unroll
+                for (int it = 0; it < ITERS; ++it) {
+                    const int rl0 = it * RPI;
+                    const int j = __shfl_sync(0xffffffffu, idx_n[rl0 >> 5], (rl0 & 31) + grs);
+                    if (j >= 0 && gc == 0)
+                        asm volatile("prefetch.global.L2 [%0];" ::"l"(p.V + (size_t)j * C + col0));
+                }
+                if (lane < (RW >> logk) + 1) {
+                    const int pt = p0n + ((RW * half) >> logk) + lane;
+                    if (pt < N) asm volatile("prefetch.global.L2 [%0];" ::"l"(p.U + (size_t)pt * C + col0));
+                }
             }
-            uint4 h[NB][BATCH];
 #pragma unroll
             for (int b = 0; b < NB; ++b) {
+                uint4 h[BATCH];
                 uint4 uh[NPBc];
                 if constexpr (HOIST) {
 #pragma unroll
                     for (int i = 0; i < NPBc; ++i) {
-                        const int pt = p0 + ((64 * half + b * BATCH * RPI) >> logk) + i;
+                        const int pt = p0 + ((RW * half + b * BATCH * RPI) >> logk) + i;
                         uh[i] = make_uint4(0, 0, 0, 0);
                         if (pt < N) uh[i] = __ldg(reinterpret_cast<const uint4*>(p.U + (size_t)pt * C + col0) + gc);
                     }
@@ -214,23 +238,24 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS, EdgeCfg<C>::MIN_CTAS) edg
                     if constexpr (HOIST) {
                         uu = uh[NPBc == 1 ? 0 : ((it * RPI) >> (LOGK >= 0 ? LOGK : 0))];
                     } else {
-                        const int pt = p0 + ((64 * half + rl0 + grs) >> logk);
+                        const int pt = p0 + ((RW * half + rl0 + grs) >> logk);
                         if (j >= 0) uu = __ldg(reinterpret_cast<const uint4*>(p.U + (size_t)pt * C + col0) + gc);
                     }
-                    h[b][it].x = add_relu_bf16x2(vv.x, uu.x); h[b][it].y = add_relu_bf16x2(vv.y, uu.y);
-                    h[b][it].z = add_relu_bf16x2(vv.z, uu.z); h[b][it].w = add_relu_bf16x2(vv.w, uu.w);
+                    h[it].x = add_relu_bf16x2(vv.x, uu.x); h[it].y = add_relu_bf16x2(vv.y, uu.y);
+                    h[it].z = add_relu_bf16x2(vv.z, uu.z); h[it].w = add_relu_bf16x2(vv.w, uu.w);
                 }
-            }
-            if (t > 0) mbar_wait(&h_free[gk], (uint32_t)((t - 1) & 1));   // layer 3 of the previous tile has read this K block
-#pragma unroll
-            for (int b = 0; b < NB; ++b)
+                // layer 3 of the previous tile must have read this K block before the first store
+                if (b == 0 && t > 0) mbar_wait(&h_free[gk], (uint32_t)((t - 1) & 1));
 #pragma unroll
                 for (int it = 0; it < BATCH; ++it) {
-                    const int r = 64 * half + (b * BATCH + it) * RPI + grs;
-                    *reinterpret_cast<uint4*>(Hk + r * 128 + ((gc ^ (r & 7)) << 4)) = h[b][it];
+                    const int r = RW * half + (b * BATCH + it) * RPI + grs;
+                    *reinterpret_cast<uint4*>(Hk + r * 128 + ((gc ^ (r & 7)) << 4)) = h[it];
                 }
+            }
             fence_proxy_async();
             arrive_leader(&h1_ready[gk]);
+#pragma unroll
+            for (int a = 0; a < NI; ++a) idx_r[a] = idx_n[a];
         }
     } else {
         // ===== epilogue warps: E2 (D0 -> H2) and E3 (D1 -> mean -> y) for lane quadrant q, columns [cg*CWE, +CWE) ==========
@@ -249,42 +274,52 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS, EdgeCfg<C>::MIN_CTAS) edg
             const int pt = p0 + (row >> logk);
             return (pt < N) ? __ldg(p.idx + (size_t)pt * k + (row & (k - 1))) : -1;
         };
+        // The accumulators are never zeroed: the epilogue that drains one writes the layer's shift back into it (tcgen05.st,
+        // one instruction per 32 columns), so every MMA accumulates and the epilogues need no bias add.
+        auto reset_acc = [&](int layer) {
+            const float* sh = layer ? t3 : t2;
+#pragma unroll
+            for (int s = 0; s < SLABS; ++s) {
+                float w[32];
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    const float4 f = *reinterpret_cast<const float4*>(sh + s * 32 + 4 * i);
+                    w[4 * i] = f.x; w[4 * i + 1] = f.y; w[4 * i + 2] = f.z; w[4 * i + 3] = f.w;
+                }
+                tmem_st32(tbase + layer * C + s * 32, w);
+            }
+            tmem_st_wait();
+            tc_fence_before();
+            arrive_leader(&d_free[layer]);
+        };
+        reset_acc(0);
+        reset_acc(1);
         int idx_cur = load_idx(tile_p0(0));
         for (int t = 0; t < T; ++t) {
             const uint32_t ph = t & 1;
             const int p0 = tile_p0(t);
-            const int idx_next = (t + 1 < T) ? load_idx(tile_p0(t + 1)) : -1;
-            // shortcut values of this tile's outputs (k >= 16: at most two per lane and slab), fetched ahead of E3
+            // shortcut values of this tile's outputs (k >= 16: at most two per lane and slab): pulled into L2 now, loaded at
+            // the start of E3 (a value held in registers across E2 is spilled, and the spill store waits for the load)
             const int pt = p0 + (row >> logk);
             const size_t obase = (size_t)pt * C + col0 + cb;
-            float2 rr[SLABS];
+            if (pt < N && nout <= 2) {
 #pragma unroll
-            for (int s = 0; s < SLABS; ++s) {
-                rr[s] = make_float2(0.0f, 0.0f);
-                if (pt < N) {
-                    if (nout == 2) rr[s] = __ldg(reinterpret_cast<const float2*>(p.R + obase + s * 32));
-                    else if (nout == 1) rr[s].x = __ldg(p.R + obase + s * 32);
-                }
+                for (int s = 0; s < SLABS; ++s) asm volatile("prefetch.global.L2 [%0];" ::"l"(p.R + obase + s * 32));
             }
-            // ---- E2: H2 = bf16(relu(D0 + t2)); the TMEM load of slab s+1 is in flight while slab s is converted ----------
+            // ---- E2: H2 = bf16(relu(D0)); the TMEM load of slab s+1 is in flight while slab s is converted ---------------
             mbar_wait(&d_full[0], ph);                           // implies every layer-2 read of H1 is done
             tc_fence_after();
             {
-                float v[2][32];
-                tmem_ld32(tbase, v[0]);
+                float v[32];
+                tmem_ld32(tbase, v);
 #pragma unroll
                 for (int s = 0; s < SLABS; ++s) {
                     tmem_ld_wait();
-                    if (s + 1 < SLABS) tmem_ld32(tbase + (s + 1) * 32, v[(s + 1) & 1]);
-                    else { tc_fence_before(); arrive_leader(&d_free[0]); }
                     const int col = col0 + s * 32;
                     uint32_t pk[16];
 #pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        const float4 sh = *reinterpret_cast<const float4*>(t2 + s * 32 + 4 * i);
-                        pk[2 * i] = pack_relu_bf16x2(v[s & 1][4 * i] + sh.x, v[s & 1][4 * i + 1] + sh.y);
-                        pk[2 * i + 1] = pack_relu_bf16x2(v[s & 1][4 * i + 2] + sh.z, v[s & 1][4 * i + 3] + sh.w);
-                    }
+                    for (int i = 0; i < 16; ++i) pk[i] = pack_relu_bf16x2(v[2 * i], v[2 * i + 1]);
+                    if (s + 1 < SLABS) tmem_ld32(tbase + (s + 1) * 32, v);     // in flight while this slab is stored
                     uint8_t* dst = H + (col >> 6) * Cfg::HK_BYTES + row * 128;
                     const int c8 = (col & 63) >> 3;
 #pragma unroll
@@ -297,7 +332,19 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS, EdgeCfg<C>::MIN_CTAS) edg
                     }
                 }
             }
-            // ---- E3: mean over the valid neighbours of relu(D1 + t3), + shortcut, ReLU ---------------------------------
+            if (t + 1 < T) reset_acc(0);
+            // ---- E3: mean over the valid neighbours of relu(D1), + shortcut, ReLU.  The row reduction runs on packed f16x2
+            // (two columns per register): a halving butterfly over the k rows of a particle, fp32 again for the mean ------------
+            const int idx_next = (t + 1 < T) ? load_idx(tile_p0(t + 1)) : -1;
+            float2 rr[SLABS];
+#pragma unroll
+            for (int s = 0; s < SLABS; ++s) {
+                rr[s] = make_float2(0.0f, 0.0f);
+                if (pt < N) {
+                    if (nout == 2) rr[s] = __ldg(reinterpret_cast<const float2*>(p.R + obase + s * 32));
+                    else if (nout == 1) rr[s].x = __ldg(p.R + obase + s * 32);
+                }
+            }
             mbar_wait(&d_full[1], ph);
             tc_fence_after();
             {
@@ -305,60 +352,61 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS, EdgeCfg<C>::MIN_CTAS) edg
                 const unsigned vmask = __ballot_sync(0xffffffffu, valid);
                 const int cnt = __popc(vmask & gmask);
                 const float inv = cnt > 0 ? 1.0f / (float)cnt : 0.0f;
-                float v[2][32];
-                tmem_ld32(tbase + C, v[0]);
+                float v[32];
+                tmem_ld32(tbase + C, v);
 #pragma unroll
                 for (int s = 0; s < SLABS; ++s) {
                     tmem_ld_wait();
-                    if (s + 1 < SLABS) tmem_ld32(tbase + C + (s + 1) * 32, v[(s + 1) & 1]);
-                    else { tc_fence_before(); arrive_leader(&d_free[1]); }
-                    float (&w)[32] = v[s & 1];
+                    uint32_t w[16];
 #pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        const float4 sh = *reinterpret_cast<const float4*>(t3 + s * 32 + 4 * i);
-                        w[4 * i] = fmaxf(w[4 * i] + sh.x, 0.0f); w[4 * i + 1] = fmaxf(w[4 * i + 1] + sh.y, 0.0f);
-                        w[4 * i + 2] = fmaxf(w[4 * i + 2] + sh.z, 0.0f); w[4 * i + 3] = fmaxf(w[4 * i + 3] + sh.w, 0.0f);
-                    }
+                    for (int i = 0; i < 16; ++i) w[i] = pack_relu_f16x2(v[2 * i], v[2 * i + 1]);
+                    if (s + 1 < SLABS) tmem_ld32(tbase + C + (s + 1) * 32, v);  // in flight during this slab's butterfly
                     if (vmask != 0xffffffffu) {
 #pragma unroll
-                        for (int i = 0; i < 32; ++i) w[i] = valid ? w[i] : 0.0f;
+                        for (int i = 0; i < 16; ++i) w[i] = valid ? w[i] : 0u;
                     }
-                    // halving butterfly: after step s2 a lane keeps 16 >> s2 partial sums over 2^(s2+1) rows
+                    // after step s2 a lane keeps 8 >> s2 registers = partial sums over 2^(s2+1) rows of 16 >> s2 columns
 #pragma unroll
-                    for (int s2 = 0; s2 < 5; ++s2) {
+                    for (int s2 = 0; s2 < 4; ++s2) {
                         if (s2 < logk) {
                             const bool up = (lane >> s2) & 1;
-                            const int cntv = 16 >> s2;
+                            const int cntv = 8 >> s2;
 #pragma unroll
-                            for (int i = 0; i < 16; ++i) {
+                            for (int i = 0; i < 8; ++i) {
                                 if (i < cntv) {
-                                    const float keep = up ? w[i + cntv] : w[i];
-                                    const float send = up ? w[i] : w[i + cntv];
-                                    w[i] = keep + __shfl_xor_sync(0xffffffffu, send, 1 << s2);
+                                    const uint32_t keep = up ? w[i + cntv] : w[i];
+                                    const uint32_t send = up ? w[i] : w[i + cntv];
+                                    w[i] = add_f16x2(keep, __shfl_xor_sync(0xffffffffu, send, 1 << s2));
                                 }
                             }
                         }
                     }
-                    if (pt < N) {
-                        const size_t o = obase + s * 32;
+                    const size_t o = obase + s * 32;
+                    if (logk == 5) {                              // k = 32: one more step splits the last register's two columns
+                        const float2 f = unpack_f16x2(w[0]);
+                        const bool up = (lane >> 4) & 1;
+                        const float sum = (up ? f.y : f.x) + __shfl_xor_sync(0xffffffffu, up ? f.x : f.y, 16);
+                        if (pt < N) p.y[o] = fmaxf(fmaf(sum, inv, rr[s].x), 0.0f);
+                    } else if (pt < N) {
                         if (nout == 2) {
+                            const float2 f = unpack_f16x2(w[0]);
                             *reinterpret_cast<float2*>(p.y + o) =
-                                make_float2(fmaxf(fmaf(w[0], inv, rr[s].x), 0.0f), fmaxf(fmaf(w[1], inv, rr[s].y), 0.0f));
-                        } else if (nout == 1) {
-                            p.y[o] = fmaxf(fmaf(w[0], inv, rr[s].x), 0.0f);
+                                make_float2(fmaxf(fmaf(f.x, inv, rr[s].x), 0.0f), fmaxf(fmaf(f.y, inv, rr[s].y), 0.0f));
                         } else {
 #pragma unroll
-                            for (int i = 0; i < 32; i += 4)
-                                if (i < nout) {
-                                    const float4 r4 = __ldg(reinterpret_cast<const float4*>(p.R + o + i));
-                                    *reinterpret_cast<float4*>(p.y + o + i) =
-                                        make_float4(fmaxf(fmaf(w[i], inv, r4.x), 0.0f), fmaxf(fmaf(w[i + 1], inv, r4.y), 0.0f),
-                                                    fmaxf(fmaf(w[i + 2], inv, r4.z), 0.0f), fmaxf(fmaf(w[i + 3], inv, r4.w), 0.0f));
+                            for (int i = 0; i < 16; i += 2)
+                                if (2 * i < nout) {
+                                    const float2 f0 = unpack_f16x2(w[i]), f1 = unpack_f16x2(w[i + 1]);
+                                    const float4 r4 = __ldg(reinterpret_cast<const float4*>(p.R + o + 2 * i));
+                                    *reinterpret_cast<float4*>(p.y + o + 2 * i) =
+                                        make_float4(fmaxf(fmaf(f0.x, inv, r4.x), 0.0f), fmaxf(fmaf(f0.y, inv, r4.y), 0.0f),
+                                                    fmaxf(fmaf(f1.x, inv, r4.z), 0.0f), fmaxf(fmaf(f1.y, inv, r4.w), 0.0f));
                                 }
                         }
                     }
                 }
             }
+            if (t + 1 < T) reset_acc(1);
             idx_cur = idx_next;
         }
     }
@@ -711,12 +759,12 @@ int configure_edge(Bf16BlockDev& b, int n_sms) {
         cfg.attrs = at; cfg.numAttrs = 1;
         int ncl = 0;
         GNN_CUDA_TRY(cudaOccupancyMaxActiveClusters(&ncl, kern, &cfg));
-        if (ncl < 1) return GNN_ERR_BAD_ARCH;
+        if (ncl < 1) { std::fprintf(stderr, "libgnn: edge_kernel<%d>: no resident cluster (threads %d, smem %d)\n", C, Cfg::THREADS, Cfg::SMEM_BYTES); return GNN_ERR_BAD_ARCH; }
         b.grid_cap = 2 * std::min(ncl, n_sms / 2);
     } else {
         int occ = 0;
         GNN_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, Cfg::THREADS, Cfg::SMEM_BYTES));
-        if (occ < 1) return GNN_ERR_BAD_ARCH;
+        if (occ < 1) { std::fprintf(stderr, "libgnn: edge_kernel<%d>: occupancy 0 (threads %d, smem %d)\n", C, Cfg::THREADS, Cfg::SMEM_BYTES); return GNN_ERR_BAD_ARCH; }
         occ = std::max(occ, Cfg::MIN_CTAS);                    // the kernel is compiled for MIN_CTAS resident CTAs per SM
         const int tmem_cap = 512 / Cfg::TMEM_COLS;              // co-resident CTAs must all fit their TMEM columns
         b.grid_cap = n_sms * std::min(occ, tmem_cap);
