@@ -10,6 +10,8 @@ int edgeconv_bf16_prepare(gnn_model& m, const float* blob_host);       // edgeco
 void edgeconv_bf16_release(gnn_model& m);
 int launch_edgeconv_bf16(gnn_model& m, int block, const float* x, const int32_t* idx, int N, float* y, Workspace& w,
                          cudaStream_t s);
+int launch_pre_bf16(gnn_model& m, int block, const float* x, int N, Workspace& w, cudaStream_t s);
+int launch_edge_bf16(gnn_model& m, int block, const int32_t* idx, int N, float* y, Workspace& w, cudaStream_t s);
 
 namespace {
 
@@ -141,6 +143,9 @@ int alloc_workspace(gnn_model* m, Workspace& w) {
     if ((rc = dev_alloc(m, &w.poffsets, Bmax + 1)) != GNN_OK) return rc;
     if ((rc = dev_alloc(m, &w.pcounts, Bmax)) != GNN_OK) return rc;
     if ((rc = dev_alloc(m, &w.hlogits, Bmax * a.n_classes)) != GNN_OK) return rc;
+    GNN_CUDA_TRY(cudaStreamCreateWithFlags(&w.aux, cudaStreamNonBlocking));
+    GNN_CUDA_TRY(cudaEventCreateWithFlags(&w.ev_x, cudaEventDisableTiming));
+    GNN_CUDA_TRY(cudaEventCreateWithFlags(&w.ev_pre, cudaEventDisableTiming));
     GNN_CUDA_TRY(cudaMemset(w.status, 0, sizeof(unsigned)));
     GNN_CUDA_TRY(cudaMemset(w.meta, 0, 2 * sizeof(int32_t)));
     return GNN_OK;
@@ -184,11 +189,21 @@ int forward(gnn_model* m, Workspace& w, const float* feats, const float* coords,
     for (int l = 0; l < a.n_blocks; ++l) {
         const float* space = (l == 0) ? coords : x;
         int D = (l == 0) ? a.coord_dims : block_in(a, l);
+        float* y = bufs[l & 1];
+        const bool fork = a.precision == GNN_BF16 && w.aux != nullptr;
+        if (fork) {                         // u, v, shortcut of this block depend on x only: beside the kNN, on the aux stream
+            if (cudaEventRecord(w.ev_x, s) != cudaSuccess || cudaStreamWaitEvent(w.aux, w.ev_x, 0) != cudaSuccess) return GNN_ERR_CUDA;
+            if ((rc = launch_pre_bf16(*m, l, x, N_upper, w, w.aux)) < 0) return rc;
+            n += rc;
+            if (cudaEventRecord(w.ev_pre, w.aux) != cudaSuccess) return GNN_ERR_CUDA;
+        }
         if ((rc = launch_knn(space, D, a.k, B, a.max_particles, w, w.idx, 0, s)) < 0) return rc;
         n += rc;
         tm.mark("knn", l);
-        float* y = bufs[l & 1];
-        if (a.precision == GNN_BF16) rc = launch_edgeconv_bf16(*m, l, x, w.idx, N_upper, y, w, s);
+        if (fork) {
+            if (cudaStreamWaitEvent(s, w.ev_pre, 0) != cudaSuccess) return GNN_ERR_CUDA;
+            rc = launch_edge_bf16(*m, l, w.idx, N_upper, y, w, s);
+        } else if (a.precision == GNN_BF16) rc = launch_edgeconv_bf16(*m, l, x, w.idx, N_upper, y, w, s);
         else rc = launch_edgeconv_f32(m->blocks[l], a.k, x, w.idx, N_upper, y, w, s);
         if (rc < 0) return rc;
         n += rc;
@@ -265,8 +280,12 @@ void gnn_destroy(gnn_model* m) {
     cudaDeviceSynchronize();
     for (void* p : m->allocs) cudaFree(p);
     edgeconv_bf16_release(*m);
-    for (auto& w : m->ws)
+    for (auto& w : m->ws) {
         for (cudaEvent_t e : w.prof_events) cudaEventDestroy(e);
+        if (w.ev_x) cudaEventDestroy(w.ev_x);
+        if (w.ev_pre) cudaEventDestroy(w.ev_pre);
+        if (w.aux) cudaStreamDestroy(w.aux);
+    }
     delete m;
 }
 

@@ -889,12 +889,12 @@ void edgeconv_bf16_release(gnn_model& m) {
     for (auto& w : m.ws) { delete static_cast<Bf16Scratch*>(w.bf16_scratch); w.bf16_scratch = nullptr; }
 }
 
-int launch_edgeconv_bf16(gnn_model& m, int block, const float* x, const int32_t* idx, int N, float* y, Workspace& w,
-                         cudaStream_t s) {
+// per-particle part of a block (u, v, shortcut): depends on x only, so the forward runs it on the workspace's auxiliary
+// stream next to the kNN of the same block
+int launch_pre_bf16(gnn_model& m, int block, const float* x, int N, Workspace& w, cudaStream_t s) {
     if (N == 0) return 0;
     const Bf16BlockDev& b = static_cast<const Bf16BlockDev*>(m.bf16_blocks)[block];
     const Bf16Scratch& sc = *static_cast<const Bf16Scratch*>(w.bf16_scratch);
-    const int k = m.arch.k;
     if (b.pre_wimg) {
         PreTcParams tp;
         tp.x = x; tp.wimg = b.pre_wimg; tp.bias = b.pre_bias; tp.U = sc.U; tp.V = sc.V; tp.R = sc.R; tp.meta = w.meta;
@@ -909,6 +909,15 @@ int launch_edgeconv_bf16(gnn_model& m, int block, const float* x, const int32_t*
         const size_t pre_smem = (size_t)PRE_ROWS * (b.Kp + 4) * sizeof(float);
         pre_kernel<<<(N + PRE_ROWS - 1) / PRE_ROWS, PRE_THREADS, pre_smem, s>>>(pp);
     }
+    return 1;
+}
+
+// per-edge part: gather, layers 2-3 on the tensor cores, mean, shortcut (needs idx and the pre kernel's U, V, R)
+int launch_edge_bf16(gnn_model& m, int block, const int32_t* idx, int N, float* y, Workspace& w, cudaStream_t s) {
+    if (N == 0) return 0;
+    const Bf16BlockDev& b = static_cast<const Bf16BlockDev*>(m.bf16_blocks)[block];
+    const Bf16Scratch& sc = *static_cast<const Bf16Scratch*>(w.bf16_scratch);
+    const int k = m.arch.k;
     EdgeParams ep;
     ep.U = sc.U; ep.V = sc.V; ep.R = sc.R; ep.idx = idx; ep.y = y; ep.meta = w.meta; ep.wimg = b.wimg; ep.shifts = b.shifts;
     ep.k = k; ep.logk = 0;
@@ -924,6 +933,14 @@ int launch_edgeconv_bf16(gnn_model& m, int block, const float* x, const int32_t*
         default: return GNN_ERR_BAD_ARCH;
     }
     if (rc != GNN_OK) return rc;
-    return 2;
+    return 1;
+}
+
+int launch_edgeconv_bf16(gnn_model& m, int block, const float* x, const int32_t* idx, int N, float* y, Workspace& w,
+                         cudaStream_t s) {
+    const int a = launch_pre_bf16(m, block, x, N, w, s);
+    if (a < 0) return a;
+    const int b = launch_edge_bf16(m, block, idx, N, y, w, s);
+    return b < 0 ? b : a + b;
 }
 

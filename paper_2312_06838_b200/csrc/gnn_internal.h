@@ -40,6 +40,8 @@ struct Workspace {
     int32_t* poffsets = nullptr;  // [Bmax + 1]
     int32_t* pcounts = nullptr;   // [Bmax]
     void* bf16_scratch = nullptr;  // per-slice scratch of the bf16 path
+    cudaStream_t aux = nullptr;    // second stream of the forward: the pre kernel of a block runs beside its kNN
+    cudaEvent_t ev_x = nullptr, ev_pre = nullptr;
     float* hlogits = nullptr;      // [Bmax, n_classes] device staging of gnn_infer_host (inputs stage in pfeats/pcoords/poffsets)
     // stage timing (gnn_profile_*): events of up to PROF_MAX_FORWARDS forwards, (n_stages + 1) per forward
     bool prof_on = false;
