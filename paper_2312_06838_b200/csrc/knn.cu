@@ -180,11 +180,39 @@ knn_select_kernel(const float* __restrict__ dm, int pld, int k, const int32_t* _
         return;
     }
     const int i = q - start;
-    unsigned long long best[K];
-#pragma unroll
-    for (int m = 0; m < K; ++m) best[m] = ~0ull;
     const float* col = dm + (size_t)start * pld + i;
-    int j = half;
+    // the first K candidates of this half (j = half, half + 2, ...) are loaded together and ordered by a bitonic network
+    // in registers (a sorted insert costs ~100 instructions, the whole K = 16 network ~500); later ones are inserted
+    unsigned long long best[K];
+    {
+        float d[K];
+#pragma unroll
+        for (int u = 0; u < K; ++u) {
+            const int j = half + 2 * u;
+            d[u] = (j < n) ? __ldg(col + (size_t)j * pld) : 0.0f;
+        }
+#pragma unroll
+        for (int u = 0; u < K; ++u) {
+            const int j = half + 2 * u;
+            best[u] = (j < n && j != i) ? (((unsigned long long)__float_as_uint(d[u]) << 32) | (unsigned)j) : ~0ull;   // R4
+        }
+    }
+#pragma unroll
+    for (int size = 2; size <= K; size <<= 1)
+#pragma unroll
+        for (int st = size >> 1; st > 0; st >>= 1)
+#pragma unroll
+            for (int m = 0; m < K; ++m) {
+                const int o = m ^ st;
+                if (o > m) {
+                    const bool asc = (m & size) == 0 || size == K;
+                    const unsigned long long a = best[m], c = best[o];
+                    const bool sw = asc ? (c < a) : (a < c);
+                    best[m] = sw ? c : a;
+                    best[o] = sw ? a : c;
+                }
+            }
+    int j = half + 2 * K;
     for (; j + 14 < n; j += 16) {             // eight loads in flight per thread
         float d[8];
 #pragma unroll
@@ -196,7 +224,7 @@ knn_select_kernel(const float* __restrict__ dm, int pld, int k, const int32_t* _
             if (key < best[K - 1]) topk_insert<K>(best, key);
         }
     }
-    {                                         // tail: up to eight more, predicated
+    if (j < n) {                              // tail: up to eight more, predicated
         float d[8];
 #pragma unroll
         for (int u = 0; u < 8; ++u) d[u] = (j + 2 * u < n) ? __ldg(col + (size_t)(j + 2 * u) * pld) : 0.0f;
@@ -206,12 +234,6 @@ knn_select_kernel(const float* __restrict__ dm, int pld, int k, const int32_t* _
             const unsigned long long key = ((unsigned long long)__float_as_uint(d[u]) << 32) | (unsigned)(j + 2 * u);
             if (key < best[K - 1]) topk_insert<K>(best, key);
         }
-        j = n;
-    }
-    for (; j < n; j += 2) {
-        if (j == i) continue;
-        const unsigned long long key = ((unsigned long long)__float_as_uint(__ldg(col + (size_t)j * pld)) << 32) | (unsigned)j;
-        if (key < best[K - 1]) topk_insert<K>(best, key);
     }
     // merge with the partner lane: slot m of the merge is min(A[m], B[K-1-m]); both lanes end up with the same set
     const unsigned pm = __activemask();

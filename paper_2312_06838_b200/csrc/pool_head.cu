@@ -12,7 +12,7 @@
 namespace {
 
 constexpr int PH_THREADS = 256;
-constexpr int PH_JETS = 8;
+constexpr int PH_JETS = 4;
 
 struct HeadParams {
     LinF32 fc[GNN_MAX_FC + 1];
