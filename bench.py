@@ -8,7 +8,7 @@
 A step = one pass of the whole hot path (ingest, 3 x [kNN, EdgeConv], pool + head) over one batch of
 BASELINE.json configs[1]: 1024 seeded synthetic jets, multiplicity ~ clip(Poisson(40), 5, 100), 7 features, k = 16,
 delivered ragged (padding-free) through gnn_infer.  Prints ONE JSON line (rank 0).  Keys beyond the base contract:
-  roofline      dominant kernel (EdgeConv block 3): algorithmic FLOPs / CUDA-event duration vs the measured bf16 peak
+  roofline      dominant kernel (edge_kernel of EdgeConv block 3): algorithmic FLOPs / CUDA-event duration vs the measured bf16 peak
   forward       whole-forward algorithmic FLOPs / ms_per_step vs the same peak (the north_star's 50 % target)
   stages_ms     mean CUDA-event time of every stage over the timed steps (gnn_profile_*)
   e2e           same metric through gnn_infer_host: pinned host buffers in, logits in host memory out, per step
@@ -69,16 +69,17 @@ def work(arch, counts):
     counts = np.asarray(counts, np.int64)
     keff = np.minimum(arch.k, np.maximum(counts - 1, 0))
     n_pts, n_edges = int(counts.sum()), int((counts * keff).sum())
-    blocks_min, blocks_stated = [], []
+    blocks_min, blocks_stated, blocks_edge = [], [], []
     for l, (c1, c2, c3) in enumerate(arch.channels):
         cin = arch.block_in(l)
         blocks_min.append(2 * (n_pts * (2 * cin * c1 + cin * c3) + n_edges * (c1 * c2 + c2 * c3)))
         blocks_stated.append(2 * (n_pts * cin * c3 + n_edges * (2 * cin * c1 + c1 * c2 + c2 * c3)))
+        blocks_edge.append(2 * n_edges * (c1 * c2 + c2 * c3))        # per-edge layers 2-3: what edge_kernel computes
     head, i = 0, arch.channels[-1][2]
     for d in tuple(arch.fc_hidden) + (arch.n_classes,):
         head += 2 * d * i * len(counts)
         i = d
-    return {"blocks_min": blocks_min, "blocks_stated": blocks_stated, "head": head,
+    return {"blocks_min": blocks_min, "blocks_stated": blocks_stated, "blocks_edge": blocks_edge, "head": head,
             "min": sum(blocks_min) + head, "stated": sum(blocks_stated) + head}
 
 
@@ -251,12 +252,20 @@ def run_ours(args):
     peak_tf = pk["bf16_tflops"] if args.precision == "bf16" else None
     dom = max((s for s in stages if s[0].startswith("edgeconv")), key=lambda s: s[1])
     dom_l = int(dom[0][len("edgeconv"):])
-    dom_flops = mean_of("blocks_min", dom_l)
+    # the stage "edgeconv<l>" is the edge kernel alone: the per-particle pre kernel runs on the auxiliary stream beside the
+    # kNN of the block (its time is inside "knn<l>"), so the kernel's algorithmic FLOPs are the per-edge layers 2-3
+    dom_flops = mean_of("blocks_edge", dom_l)
     roof_peak = pk["bf16_tflops"]
-    roofline = {"bound": "tensor", "kernel": dom[0], "achieved": dom_flops / (dom[1] * 1e-3) / 1e12, "peak": roof_peak,
-                "unit": "TFLOP/s", "frac": dom_flops / (dom[1] * 1e-3) / 1e12 / roof_peak, "traffic": None,
-                "peak_source": pk["_source"] + ", burst cuBLAS bf16", "flops_per_launch_min": dom_flops,
-                "flops_per_launch_stated": mean_of("blocks_stated", dom_l), "ms_per_launch": dom[1],
+    traffic = None                                   # dram bytes per launch of that kernel, from the committed ncu capture
+    tpath = os.path.join(ROOT, "profiles", "r01_traffic.txt")
+    if os.path.exists(tpath):
+        traffic = json.load(open(tpath)).get("edge_kernel_c%d_dram_bytes_per_launch" % arch.channels[dom_l][0])
+    roofline = {"bound": "tensor", "kernel": "edge_kernel<%d> (stage %s: EdgeConv block %d, per-edge layers 2-3)" % (arch.channels[dom_l][0], dom[0], dom_l + 1),
+                "achieved": dom_flops / (dom[1] * 1e-3) / 1e12, "peak": roof_peak,
+                "unit": "TFLOP/s", "frac": dom_flops / (dom[1] * 1e-3) / 1e12 / roof_peak, "traffic": traffic,
+                "peak_source": pk["_source"] + ", burst cuBLAS bf16", "flops_per_launch": dom_flops,
+                "flops_per_launch_block_min": mean_of("blocks_min", dom_l),
+                "flops_per_launch_block_stated": mean_of("blocks_stated", dom_l), "ms_per_launch": dom[1],
                 "forwards_averaged": n_fw}
     ms_per_step = total_ms_max / args.steps
     fwd = {"flops_min": mean_of("min"), "flops_stated": mean_of("stated"),
