@@ -56,7 +56,7 @@ int check_arch(const gnn_arch& a) {
         for (int l = 0; l < a.n_blocks; ++l) {
             int c = a.channels[l][0];
             if (a.channels[l][1] != c || a.channels[l][2] != c) return GNN_ERR_BAD_ARCH;
-            if (c != 32 && c != 64 && c != 128 && c != 256) return GNN_ERR_BAD_ARCH;
+            if (c != 32 && c != 64 && c != 128 && c != 256 && c != 512) return GNN_ERR_BAD_ARCH;
         }
     }
     return GNN_OK;

@@ -415,6 +415,238 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS) __maxnreg__(EdgeCfg<C>::M
     if (warp == Cfg::MMA_WARP) tmem_dealloc_g<PAIR>(tmem, Cfg::TMEM_COLS);
 }
 
+// ---- wide blocks (C = 512, configs[4] wide variant): the 1 MB of W2', W3' cannot be resident even split over a CTA pair,
+// and two 512-column accumulators exceed TMEM.  This kernel is the simple, sequential form: one CTA per SM, one tile at a
+// time, ONE accumulator of C columns (two N halves of 256), weights streamed from L2 per tile through a two-slot ring of
+// [256][64] chunk images (full / empty mbarriers), build -> MMA2 -> E2 -> MMA3 -> E3.  Correct first; the resident-weight
+// pipelined design above is what the narrower blocks use.
+constexpr int WIDE_ALU_THREADS = 256;
+constexpr int WIDE_THREADS = 320;
+
+template <int C>
+struct WideCfg {
+    static constexpr int NR = C > 256 ? 256 : C;              // weight rows (= MMA N) per chunk
+    static constexpr int NH = C / NR;                         // N halves per layer
+    static constexpr int KB = (C + 63) / 64;                  // 64-wide K blocks per layer
+    static constexpr int KSTEPS_LAST = ((C - (KB - 1) * 64) + 15) / 16;
+    static constexpr int CHUNK_BYTES = NR * 128;              // [NR][64] bf16, 128B-swizzled
+    static constexpr int NCHUNK = 2 * NH * KB;                // both layers
+    static constexpr bool RESIDENT = (size_t)NCHUNK * CHUNK_BYTES <= 96 * 1024;
+    static constexpr int NSLOT = RESIDENT ? NCHUNK : (CHUNK_BYTES < 32 * 1024 ? 4 : 2);
+    static constexpr int H_BYTES = KB * TILE_ROWS * 128;      // KB K-blocks of [128][64] bf16
+    static constexpr int TMEM_COLS = C < 32 ? 32 : C;
+    static constexpr int RING_BYTES = NSLOT * CHUNK_BYTES;
+    // dynamic shared memory: [ring][H][t2,t3 fp32][idx int32 x128][barriers][tmem ptr] (+1024 alignment slack)
+    static constexpr int SMALL_BYTES = 2 * C * 4 + TILE_ROWS * 4 + (2 * NSLOT + 2) * 8 + 16;
+    static constexpr int SMEM_BYTES = RING_BYTES + H_BYTES + SMALL_BYTES + 1024;
+};
+
+
+template <int C>
+__global__ void __launch_bounds__(WIDE_THREADS, 1) edge_wide_kernel(EdgeParams p) {
+    using Cfg = WideCfg<C>;
+    extern __shared__ __align__(1024) uint8_t smem_raw[];
+    if (p.meta[0]) return;
+    const int N = p.meta[1];
+    const int n_tiles = min(p.n_tiles, (N + p.TP - 1) / p.TP);
+    if ((int)blockIdx.x >= n_tiles) return;
+    uint8_t* smem = smem_raw;                                    // keeps the shared address space (see edge_kernel)
+    if ((smem_u32(smem) & 1023u) != 0u) __trap();
+    uint8_t* ring = smem;
+    uint8_t* H = ring + Cfg::RING_BYTES;
+    float* shifts_s = reinterpret_cast<float*>(H + Cfg::H_BYTES);
+    int32_t* idx_s = reinterpret_cast<int32_t*>(shifts_s + 2 * C);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(idx_s + TILE_ROWS);
+    uint64_t* full = bars;                        // [NSLOT] weight chunk landed
+    uint64_t* empty = bars + Cfg::NSLOT;          // [NSLOT] weight chunk consumed (streaming only)
+    uint64_t* h_ready = bars + 2 * Cfg::NSLOT;    // operand tile written by the 256 ALU threads
+    uint64_t* d_full = h_ready + 1;               // accumulator complete
+    uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(d_full + 1);
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    if (tid == 0) {
+        for (int i = 0; i < Cfg::NSLOT; ++i) { mbar_init(&full[i], 1); mbar_init(&empty[i], 1); }
+        mbar_init(h_ready, WIDE_ALU_THREADS);
+        mbar_init(d_full, 1);
+        fence_mbar_init();
+    }
+    for (int i = tid; i < 2 * C; i += WIDE_THREADS) shifts_s[i] = p.shifts[i];
+    if (warp == 8) tmem_alloc(tmem_ptr, Cfg::TMEM_COLS);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = *tmem_ptr;
+    const int my_tiles = (n_tiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+
+    if (warp == 9) {
+        // ===== weight-chunk producer ======================================================================
+        if (lane == 0) {
+            const int total = Cfg::RESIDENT ? Cfg::NCHUNK : Cfg::NCHUNK * my_tiles;
+            for (int n = 0; n < total; ++n) {
+                const int slot = n % Cfg::NSLOT;
+                if (n >= Cfg::NSLOT) mbar_wait(&empty[slot], ((n / Cfg::NSLOT) - 1) & 1);
+                mbar_arrive_expect_tx(&full[slot], Cfg::CHUNK_BYTES);
+                bulk_g2s(ring + (size_t)slot * Cfg::CHUNK_BYTES, p.wimg + (size_t)(n % Cfg::NCHUNK) * Cfg::CHUNK_BYTES,
+                         Cfg::CHUNK_BYTES, &full[slot]);
+            }
+        }
+    } else if (warp == 8) {
+        // ===== MMA issuer =================================================================================
+        if (lane == 0) {
+            constexpr uint32_t idesc = idesc_bf16_f32(128, Cfg::NR);
+            const uint32_t h_addr = smem_u32(H), ring_addr = smem_u32(ring);
+            uint32_t ph_h = 0;
+            int n = 0;                                           // chunks consumed so far
+            for (int t = 0; t < my_tiles; ++t) {
+                for (int layer = 0; layer < 2; ++layer) {
+                    mbar_wait(h_ready, ph_h); ph_h ^= 1;
+                    tc_fence_after();
+                    for (int nh = 0; nh < Cfg::NH; ++nh) {
+                        for (int kb = 0; kb < Cfg::KB; ++kb, ++n) {
+                            const int slot = Cfg::RESIDENT ? (n % Cfg::NCHUNK) : (n % Cfg::NSLOT);
+                            if (!Cfg::RESIDENT || t == 0) mbar_wait(&full[slot], Cfg::RESIDENT ? 0 : ((n / Cfg::NSLOT) & 1));
+                            tc_fence_after();
+                            const int ksteps = (kb == Cfg::KB - 1) ? Cfg::KSTEPS_LAST : 4;
+                            for (int ks = 0; ks < ksteps; ++ks) {
+                                const uint64_t ad = desc_sw128(h_addr + kb * (TILE_ROWS * 128) + ks * 32);
+                                const uint64_t bd = desc_sw128(ring_addr + slot * Cfg::CHUNK_BYTES + ks * 32);
+                                mma_bf16_ss(tmem + nh * 256, ad, bd, idesc, (kb | ks) != 0);
+                            }
+                            if (!Cfg::RESIDENT) mma_commit(&empty[slot]);
+                        }
+                    }
+                    mma_commit(d_full);
+                }
+            }
+        }
+    } else {
+        // ===== build / epilogue warps ======================================================================
+        const int q = warp & 3, half = warp >> 2;
+        const int row = 32 * q + lane;                           // TMEM lane = edge row of the tile
+        const int k = p.k, logk = p.logk;
+        constexpr int CH = C / 8;                                // 16-byte chunks per operand row
+        constexpr int ITEMS = TILE_ROWS * CH / WIDE_ALU_THREADS; // (row, chunk) items per thread
+        constexpr int SLABS = (C >= 64) ? C / 64 : 1;            // 32-column slabs per warp (C = 32: warps 4-7 idle)
+        const bool epi_active = (C >= 64) || half == 0;
+        uint32_t ph_d = 0;
+        for (int t = 0; t < my_tiles; ++t) {
+            const int tile = blockIdx.x + t * gridDim.x;
+            const int p0 = tile * p.TP;
+            asm volatile("bar.sync 1, 256;" ::: "memory");       // previous tile's readers of idx_s are done
+            if (tid < TILE_ROWS) {
+                const int pt = p0 + (tid >> logk);
+                idx_s[tid] = (pt < N) ? p.idx[(size_t)pt * k + (tid & (k - 1))] : -1;
+            }
+            asm volatile("bar.sync 1, 256;" ::: "memory");
+            // ---- build H1 = bf16(relu(u_i + v_j)) ------------------------------------------------------
+#pragma unroll
+            for (int i0 = 0; i0 < ITEMS; i0 += 8) {
+                uint4 vv[8], uu[8];
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    if (i0 + i < ITEMS) {
+                        const int it = tid + (i0 + i) * WIDE_ALU_THREADS;
+                        const int r = it / CH, ch = it % CH;
+                        const int j = idx_s[r];
+                        if (j >= 0) {
+                            vv[i] = __ldg(reinterpret_cast<const uint4*>(p.V + (size_t)j * C) + ch);
+                            uu[i] = __ldg(reinterpret_cast<const uint4*>(p.U + (size_t)(p0 + (r >> logk)) * C) + ch);
+                        } else {
+                            vv[i] = make_uint4(0, 0, 0, 0); uu[i] = make_uint4(0, 0, 0, 0);
+                        }
+                    }
+                }
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    if (i0 + i < ITEMS) {
+                        const int it = tid + (i0 + i) * WIDE_ALU_THREADS;
+                        const int r = it / CH, ch = it % CH;
+                        uint4 h;
+                        h.x = add_relu_bf16x2(vv[i].x, uu[i].x); h.y = add_relu_bf16x2(vv[i].y, uu[i].y);
+                        h.z = add_relu_bf16x2(vv[i].z, uu[i].z); h.w = add_relu_bf16x2(vv[i].w, uu[i].w);
+                        *reinterpret_cast<uint4*>(H + (ch >> 3) * (TILE_ROWS * 128) + r * 128 + (((ch & 7) ^ (r & 7)) << 4)) = h;
+                    }
+                }
+            }
+            fence_proxy_async();
+            mbar_arrive(h_ready);
+            // ---- E2: H2 = bf16(relu(D + t2)) -----------------------------------------------------------
+            mbar_wait(d_full, ph_d); ph_d ^= 1;
+            tc_fence_after();
+            if (epi_active) {
+#pragma unroll 1
+                for (int s = 0; s < SLABS; ++s) {
+                    const int col = (C >= 64) ? half * (C / 2) + s * 32 : 0;
+                    float v[32];
+                    tmem_ld32(tmem + ((uint32_t)(32 * q) << 16) + (col >> 8) * 256 + (col & 255), v);
+                    tmem_ld_wait();
+                    uint32_t pk[16];
+#pragma unroll
+                    for (int i = 0; i < 16; ++i)
+                        pk[i] = pack_relu_bf16x2(v[2 * i] + shifts_s[col + 2 * i], v[2 * i + 1] + shifts_s[col + 2 * i + 1]);
+                    uint8_t* dst = H + (col >> 6) * (TILE_ROWS * 128) + row * 128;
+                    const int c8 = (col & 63) >> 3;
+#pragma unroll
+                    for (int c = 0; c < 4; ++c)
+                        *reinterpret_cast<uint4*>(dst + (((c8 + c) ^ (row & 7)) << 4)) =
+                            make_uint4(pk[4 * c], pk[4 * c + 1], pk[4 * c + 2], pk[4 * c + 3]);
+                }
+            }
+            tc_fence_before();
+            fence_proxy_async();
+            mbar_arrive(h_ready);
+            // ---- E3: mean over the valid neighbours of relu(D + t3), + shortcut, ReLU ----------------------
+            mbar_wait(d_full, ph_d); ph_d ^= 1;
+            tc_fence_after();
+            if (epi_active) {
+                const bool valid = idx_s[row] >= 0;
+                const unsigned gmask = (k >= 32) ? 0xffffffffu : (((1u << k) - 1u) << (lane & ~(k - 1)));
+                const int cnt = __popc(__ballot_sync(0xffffffffu, valid) & gmask);
+                const float inv = cnt > 0 ? 1.0f / (float)cnt : 0.0f;
+                const int pt = p0 + (row >> logk);
+                int cb = 0;                                      // first of the 32 >> logk columns this lane ends up with
+                for (int s = 0; s < logk; ++s) cb += ((lane >> s) & 1) * (16 >> s);
+                const int nout = 32 >> logk;
+                const float* t3 = shifts_s + C;
+#pragma unroll 1
+                for (int s = 0; s < SLABS; ++s) {
+                    const int col = (C >= 64) ? half * (C / 2) + s * 32 : 0;
+                    float v[32];
+                    tmem_ld32(tmem + ((uint32_t)(32 * q) << 16) + (col >> 8) * 256 + (col & 255), v);
+                    tmem_ld_wait();
+#pragma unroll
+                    for (int i = 0; i < 32; ++i) v[i] = valid ? fmaxf(v[i] + t3[col + i], 0.0f) : 0.0f;
+                    // halving butterfly: after step s a lane keeps 16 >> s partial sums over 2^(s+1) rows
+#pragma unroll
+                    for (int s2 = 0; s2 < 5; ++s2) {
+                        if (s2 < logk) {
+                            const bool up = (lane >> s2) & 1;
+                            const int cntv = 16 >> s2;
+#pragma unroll
+                            for (int i = 0; i < 16; ++i) {
+                                if (i < cntv) {
+                                    const float keep = up ? v[i + cntv] : v[i];
+                                    const float send = up ? v[i] : v[i + cntv];
+                                    v[i] = keep + __shfl_xor_sync(0xffffffffu, send, 1 << s2);
+                                }
+                            }
+                        }
+                    }
+                    if (pt < N) {
+                        const size_t o = (size_t)pt * C + col + cb;
+#pragma unroll
+                        for (int i = 0; i < 32; ++i)
+                            if (i < nout) p.y[o + i] = fmaxf(fmaf(v[i], inv, __ldg(p.R + o + i)), 0.0f);
+                    }
+                }
+            }
+            tc_fence_before();
+        }
+    }
+    __syncthreads();
+    if (warp == 8) tmem_dealloc(tmem, Cfg::TMEM_COLS);
+}
+
 // ---- pre kernel: per-particle u (bf16), v (bf16), shortcut r (fp32) in fp32 FMA ------------------------------------------
 // One CTA per tile of PRE_ROWS particles; x rows staged in shared memory; a thread owns 8 rows x 4 output columns of
 // [u | v | r] = x * Wpre^T + bpre, Wpre^T stored [Kp][NC] (K padded to a multiple of 4 with zero rows).
@@ -834,10 +1066,15 @@ int edgeconv_bf16_prepare(gnn_model& m, const float* blob) {
             sh[o] = t2[o]; sh[C + o] = t3[o];
         }
         std::vector<uint8_t> img;                              // per CTA rank: [W2' chunks | W3' chunks] of its output rows
-        const int nranks = C >= 256 ? 2 : 1, NRB = C / nranks;
-        for (int r = 0; r < nranks; ++r) {
-            pack_layer(W2f, C, NRB, r * NRB, img);
-            pack_layer(W3f, C, NRB, r * NRB, img);
+        if (C > 256) {                                          // streamed: layer-major, N halves of 256 rows, K blocks
+            for (int h = 0; h < C / 256; ++h) pack_layer(W2f, C, 256, h * 256, img);
+            for (int h = 0; h < C / 256; ++h) pack_layer(W3f, C, 256, h * 256, img);
+        } else {
+            const int nranks = C >= 256 ? 2 : 1, NRB = C / nranks;
+            for (int r = 0; r < nranks; ++r) {
+                pack_layer(W2f, C, NRB, r * NRB, img);
+                pack_layer(W3f, C, NRB, r * NRB, img);
+            }
         }
         int rc;
         if ((rc = upload(m, Wt, &b.pre_Wt)) != GNN_OK || (rc = upload(m, bias, &b.pre_bias)) != GNN_OK ||
@@ -867,11 +1104,15 @@ int edgeconv_bf16_prepare(gnn_model& m, const float* blob) {
             case 64: rc = a.k == 16 ? configure_edge<64, 4>(b, m.n_sms) : configure_edge<64, -1>(b, m.n_sms); break;
             case 128: rc = a.k == 16 ? configure_edge<128, 4>(b, m.n_sms) : configure_edge<128, -1>(b, m.n_sms); break;
             case 256: rc = a.k == 16 ? configure_edge<256, 4>(b, m.n_sms) : configure_edge<256, -1>(b, m.n_sms); break;
+            case 512:
+                rc = cudaFuncSetAttribute(edge_wide_kernel<512>, cudaFuncAttributeMaxDynamicSharedMemorySize, WideCfg<512>::SMEM_BYTES) == cudaSuccess ? GNN_OK : GNN_ERR_CUDA;
+                b.grid_cap = m.n_sms;
+                break;
             default: rc = GNN_ERR_BAD_ARCH;
         }
         if (rc != GNN_OK) return rc;
     }
-    GNN_CUDA_TRY(cudaFuncSetAttribute(pre_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024));
+    GNN_CUDA_TRY(cudaFuncSetAttribute(pre_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
     for (auto& w : m.ws) {
         auto* sc = new Bf16Scratch();
         w.bf16_scratch = sc;
@@ -930,6 +1171,10 @@ int launch_edge_bf16(gnn_model& m, int block, const int32_t* idx, int N, float* 
         case 64: rc = k == 16 ? launch_edge_t<64, 4>(ep, b.grid_cap, s) : launch_edge_t<64, -1>(ep, b.grid_cap, s); break;
         case 128: rc = k == 16 ? launch_edge_t<128, 4>(ep, b.grid_cap, s) : launch_edge_t<128, -1>(ep, b.grid_cap, s); break;
         case 256: rc = k == 16 ? launch_edge_t<256, 4>(ep, b.grid_cap, s) : launch_edge_t<256, -1>(ep, b.grid_cap, s); break;
+        case 512:
+            edge_wide_kernel<512><<<std::min(ep.n_tiles, b.grid_cap), WIDE_THREADS, WideCfg<512>::SMEM_BYTES, s>>>(ep);
+            rc = GNN_OK;
+            break;
         default: return GNN_ERR_BAD_ARCH;
     }
     if (rc != GNN_OK) return rc;

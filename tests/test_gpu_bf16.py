@@ -56,6 +56,28 @@ def test_edgeconv_stage_given_oracle_indices(name, block):
     m.close()
 
 
+@pytest.mark.parametrize("k", [1, 2, 8, 32])
+def test_edgeconv_stage_other_k(k):
+    """Neighbour counts other than the configs' 16 and 4 take the runtime-k path of the gather and, for k = 32, the
+    extra fp32 step of the E3 row reduction; blocks with C = 64 (SIMT pre kernel) and C = 128 (tcgen05 tf32 pre kernel)."""
+    a = synth.Arch(in_features=6, k=k, channels=((64, 64, 64), (128, 128, 128)), fc_hidden=(32,), max_particles=64)
+    w = synth.make_weights(a)
+    m = make_model(a, w, precision=gnn.BF16, max_batch_jets=32)
+    rng = np.random.default_rng(100 + k)
+    counts = [1, 2, 3, 9, 33, 40, 64, 17, 5, 40, 64, 31]
+    off = np.zeros(len(counts) + 1, np.int32); off[1:] = np.cumsum(counts)
+    for block in (0, 1):
+        x = rng.normal(0, 1, (off[-1], a.block_in(block))).astype(np.float32)
+        if block > 0:
+            x = np.maximum(x, 0)
+        idx, _, _ = oracle.knn(x, off, a.k)
+        y = m.debug_edgeconv(block, dev(x), dev(idx), dev(off)).cpu().numpy()
+        ref = oracle.edgeconv(a, w, block, x, idx, off)
+        err = np.abs(y - ref)
+        assert err.max() < 6e-3 * max(1.0, np.abs(ref).max()), (k, block, err.max())
+    m.close()
+
+
 # ---- whole network -----------------------------------------------------------------------------------------------------
 def test_tiny_end_to_end():
     a, w, m = bf16_model("tiny", 64)
@@ -101,6 +123,27 @@ def test_sweep_base_1024_sampled(pn):
     check_logits(lg[:256], ref)
     for B in (1, 16):                                          # nested batch sizes give the same jets
         assert np.array_equal(run_ragged(m, b.head(B)), lg[:B])
+
+
+def test_sweep_wide_256_sampled():
+    """configs[4] wide variant (EdgeConv channels 128, 256, 512, FC 512) at B = 256; the oracle runs the first 64 jets.
+    Block 3 (C = 512) takes the streamed-weight kernel, its stage is also checked alone."""
+    a, w, m = bf16_model("wide", 256)
+    b = synth.make_sweep_batch(n_jets=256)
+    lg = run_ragged(m, b)
+    assert m.status_check() == 0 and np.isfinite(lg).all()
+    h = b.head(64)
+    ref = oracle.forward(a, w, h.feats, h.coords, h.offsets)
+    check_logits(lg[:64], ref)
+    rng = np.random.default_rng(7)
+    counts = [1, 2, 17, 40, 100, 5, 16, 61, 128, 3]
+    off = np.zeros(len(counts) + 1, np.int32); off[1:] = np.cumsum(counts)
+    x = np.maximum(rng.normal(0, 1, (off[-1], a.block_in(2))), 0).astype(np.float32)
+    idx, _, _ = oracle.knn(x, off, a.k)
+    y = m.debug_edgeconv(2, dev(x), dev(idx), dev(off)).cpu().numpy()
+    r2 = oracle.edgeconv(a, w, 2, x, idx, off)
+    assert np.abs(y - r2).max() < 6e-3 * max(1.0, np.abs(r2).max())
+    m.close()
 
 
 def test_edge_case_set(pn):
