@@ -191,15 +191,17 @@ int forward(gnn_model* m, Workspace& w, const float* feats, const float* coords,
         int D = (l == 0) ? a.coord_dims : block_in(a, l);
         float* y = bufs[l & 1];
         const bool fork = a.precision == GNN_BF16 && w.aux != nullptr;
+        if (fork && (cudaEventRecord(w.ev_x, s) != cudaSuccess || cudaStreamWaitEvent(w.aux, w.ev_x, 0) != cudaSuccess)) return GNN_ERR_CUDA;
+        if ((rc = launch_knn(space, D, a.k, B, a.max_particles, w, w.idx, 0, (a.precision == GNN_BF16 && l > 0) ? 1 : 0, s)) < 0) return rc;
+        n += rc;
+        tm.mark("knn", l);
         if (fork) {                         // u, v, shortcut of this block depend on x only: beside the kNN, on the aux stream
-            if (cudaEventRecord(w.ev_x, s) != cudaSuccess || cudaStreamWaitEvent(w.aux, w.ev_x, 0) != cudaSuccess) return GNN_ERR_CUDA;
+            // (enqueued after the kNN kernels so that the short distance kernel gets the SMs first and the pre kernel,
+            // which fills every SM's shared memory, runs beside the selection kernel, which uses none)
             if ((rc = launch_pre_bf16(*m, l, x, N_upper, w, w.aux)) < 0) return rc;
             n += rc;
             if (cudaEventRecord(w.ev_pre, w.aux) != cudaSuccess) return GNN_ERR_CUDA;
         }
-        if ((rc = launch_knn(space, D, a.k, B, a.max_particles, w, w.idx, 0, s)) < 0) return rc;
-        n += rc;
-        tm.mark("knn", l);
         if (fork) {
             if (cudaStreamWaitEvent(s, w.ev_pre, 0) != cudaSuccess) return GNN_ERR_CUDA;
             rc = launch_edge_bf16(*m, l, w.idx, N_upper, y, w, s);
@@ -256,7 +258,7 @@ int gnn_create(const void* weights_host, size_t bytes, const gnn_arch* arch, int
     m->Nmax = (int64_t)arch->max_batch_jets * arch->max_particles;
     m->Cmax = 8;
     for (int l = 0; l < arch->n_blocks; ++l) m->Cmax = std::max(m->Cmax, arch->channels[l][2]);
-    if ((rc = knn_configure()) != GNN_OK || (rc = pool_head_configure()) != GNN_OK || (rc = edgeconv_f32_configure()) != GNN_OK ||
+    if ((rc = knn_configure()) != GNN_OK || (rc = pool_head_configure()) != GNN_OK || (rc = knn_tc_configure()) != GNN_OK || (rc = edgeconv_f32_configure()) != GNN_OK ||
         (rc = build_model(m, static_cast<const float*>(weights_host))) != GNN_OK) {
         gnn_destroy(m);
         return rc;
@@ -433,7 +435,7 @@ int gnn_debug_knn(gnn_model* m, const float* space_dev, int32_t D, const int32_t
     int n = 0, rc;
     if ((rc = launch_ingest(offsets_dev, nullptr, B, N, (int)m->Nmax, m->arch.max_particles, w, s)) < 0) return rc;
     n += rc;
-    if ((rc = launch_knn(space_dev, D, k, B, m->arch.max_particles, w, idx_dev, 1, s)) < 0) return rc;
+    if ((rc = launch_knn(space_dev, D, k, B, m->arch.max_particles, w, idx_dev, 1, 0, s)) < 0) return rc;
     n += rc;
     m->launches.fetch_add(n, std::memory_order_relaxed);
     return cudaGetLastError() == cudaSuccess ? GNN_OK : GNN_ERR_CUDA;

@@ -19,6 +19,8 @@
 #include "gnn_internal.h"
 #include <cfloat>
 
+int launch_knn_gram(const float* space, int D, int B, int max_particles, const Workspace& w, cudaStream_t s);   // knn_tc.cu
+
 namespace {
 
 constexpr int KNN_THREADS = 128;
@@ -268,10 +270,13 @@ size_t knn_smem_bytes(int P) {
 
 template <int K>
 int launch_knn_t(const float* space, int D, int k, int B, int P, const Workspace& w, int32_t* idx_out, int local_out,
-                 cudaStream_t s) {
+                 int gram, cudaStream_t s) {
     const int tiles = (P + KNN_QT - 1) / KNN_QT;
     const int pld = (P + 3) & ~3;
-    knn_dist_kernel<<<B * tiles, KNN_THREADS, knn_smem_bytes(P), s>>>(space, D, w.jet_start, w.jet_n, w.meta, w.dm, pld, w.pjet, tiles);
+    // distances: the Gram form on the tensor cores where the caller allows it (bf16 mode, feature spaces) and D has one,
+    // else the exact direct-difference kernel
+    if (!(gram && launch_knn_gram(space, D, B, P, w, s) == 1))
+        knn_dist_kernel<<<B * tiles, KNN_THREADS, knn_smem_bytes(P), s>>>(space, D, w.jet_start, w.jet_n, w.meta, w.dm, pld, w.pjet, tiles);
     const long long n_upper = 2ll * B * P;                     // two threads per particle slot
     knn_select_kernel<K><<<(unsigned)((n_upper + KSEL_THREADS - 1) / KSEL_THREADS), KSEL_THREADS, 0, s>>>(
         w.dm, pld, k, w.pjet, w.jet_start, w.jet_n, w.meta, idx_out, local_out);
@@ -281,13 +286,13 @@ int launch_knn_t(const float* space, int D, int k, int B, int P, const Workspace
 }  // namespace
 
 int launch_knn(const float* space, int D, int k, int B, int max_particles, const Workspace& w, int32_t* idx_out,
-               int local_out, cudaStream_t s) {
+               int local_out, int gram, cudaStream_t s) {
     if (B == 0) return 0;
     if (knn_smem_bytes(max_particles) > 227 * 1024) return GNN_ERR_BAD_ARG;
-    if (k <= 4) return launch_knn_t<4>(space, D, k, B, max_particles, w, idx_out, local_out, s);
-    if (k <= 8) return launch_knn_t<8>(space, D, k, B, max_particles, w, idx_out, local_out, s);
-    if (k <= 16) return launch_knn_t<16>(space, D, k, B, max_particles, w, idx_out, local_out, s);
-    return launch_knn_t<32>(space, D, k, B, max_particles, w, idx_out, local_out, s);
+    if (k <= 4) return launch_knn_t<4>(space, D, k, B, max_particles, w, idx_out, local_out, gram, s);
+    if (k <= 8) return launch_knn_t<8>(space, D, k, B, max_particles, w, idx_out, local_out, gram, s);
+    if (k <= 16) return launch_knn_t<16>(space, D, k, B, max_particles, w, idx_out, local_out, gram, s);
+    return launch_knn_t<32>(space, D, k, B, max_particles, w, idx_out, local_out, gram, s);
 }
 
 // debug entry: jet-local neighbour indices -> the global ones the EdgeConv kernels read (out-of-jet values -> -1)
