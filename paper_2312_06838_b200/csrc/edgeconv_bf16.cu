@@ -46,9 +46,11 @@ struct EdgeCfg {
     static constexpr int GH = 2;                              // row parts of the gather
     static constexpr int NG = GH * KB;                        // gather warps: K block g % KB, row part g / KB
     static constexpr int RW = TILE_ROWS / GH;                 // rows per gather warp
-    static constexpr int MMA_WARP = NE + NG;
-    static constexpr int THREADS = 32 * (NE + NG + 1);
-    static constexpr int MAXREG = C >= 256 ? 96 : 80;   // registers are per SM quarter: ceil(warps / 4) * 32 * MAXREG * MIN_CTAS <= 16384
+    static constexpr bool SPLIT = C >= 256;                     // E2 and E3 on separate warp sets: E2(t+1) need not wait for E3(t)
+    static constexpr int NEP = SPLIT ? 2 * NE : NE;           // epilogue warps in total: [0, NE) run E2, [NE, 2 NE) run E3
+    static constexpr int MMA_WARP = NEP + NG;
+    static constexpr int THREADS = 32 * (NEP + NG + 1);
+    static constexpr int MAXREG = C >= 256 ? 72 : 80;   // registers are per SM quarter: ceil(warps / 4) * 32 * MAXREG * MIN_CTAS <= 16384
     static constexpr int KSTEPS_LAST = ((C - (KB - 1) * 64) + 15) / 16;
     static constexpr int NRB = PAIR ? C / 2 : C;              // weight rows (output channels) one CTA holds
     static constexpr int CHUNK_BYTES = NRB * 128;             // [NRB][64] bf16, 128B-swizzled
@@ -169,11 +171,11 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS) __maxnreg__(EdgeCfg<C>::M
                 }
             }
         }
-    } else if (warp >= NE) {
+    } else if (warp >= Cfg::NEP) {
         // ===== gather warps: H1 = bf16(relu(u_i + v_j)) for K block gk, rows 64*half .. +63; they run one tile ahead of the
         // epilogue (their only dependency is h_free of the previous tile), so the L2 latency of the gather is off the
         // MMA <-> epilogue critical path ===============================================================================
-        const int g = warp - NE, gk = g % KB, half = g / KB;
+        const int g = warp - Cfg::NEP, gk = g % KB, half = g / KB;
         constexpr int CPR = Cfg::KW / 8;                         // 16-byte chunks per row of a K block
         constexpr int RPI = 32 / CPR;                            // rows per warp iteration
         constexpr int RW = Cfg::RW, NI = RW / 32;
@@ -259,7 +261,8 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS) __maxnreg__(EdgeCfg<C>::M
         }
     } else {
         // ===== epilogue warps: E2 (D0 -> H2) and E3 (D1 -> mean -> y) for lane quadrant q, columns [cg*CWE, +CWE) ==========
-        const int q = warp & 3, cg = warp >> 2;
+        const int q = warp & 3, cg = (warp % NE) >> 2;
+        const bool doE2 = !Cfg::SPLIT || warp < NE, doE3 = !Cfg::SPLIT || warp >= NE;
         const int row = 32 * q + lane;                           // TMEM lane = edge row of the tile
         const int col0 = cg * CWE;
         constexpr int SLABS = CWE / 32;
@@ -292,8 +295,8 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS) __maxnreg__(EdgeCfg<C>::M
             tc_fence_before();
             arrive_leader(&d_free[layer]);
         };
-        reset_acc(0);
-        reset_acc(1);
+        if (doE2) reset_acc(0);
+        if (doE3) reset_acc(1);
         int idx_cur = load_idx(tile_p0(0));
         for (int t = 0; t < T; ++t) {
             const uint32_t ph = t & 1;
@@ -307,6 +310,7 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS) __maxnreg__(EdgeCfg<C>::M
                 for (int s = 0; s < SLABS; ++s) asm volatile("prefetch.global.L2 [%0];" ::"l"(p.R + obase + s * 32));
             }
             // ---- E2: H2 = bf16(relu(D0)); the TMEM load of slab s+1 is in flight while slab s is converted ---------------
+            if (doE2) {
             mbar_wait(&d_full[0], ph);                           // implies every layer-2 read of H1 is done
             tc_fence_after();
             {
@@ -333,8 +337,10 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS) __maxnreg__(EdgeCfg<C>::M
                 }
             }
             if (t + 1 < T) reset_acc(0);
+            }
             // ---- E3: mean over the valid neighbours of relu(D1), + shortcut, ReLU.  The row reduction runs on packed f16x2
             // (two columns per register): a halving butterfly over the k rows of a particle, fp32 again for the mean ------------
+            if (doE3) {
             const int idx_next = (t + 1 < T) ? load_idx(tile_p0(t + 1)) : -1;
             float2 rr[SLABS];
 #pragma unroll
@@ -408,6 +414,7 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS) __maxnreg__(EdgeCfg<C>::M
             }
             if (t + 1 < T) reset_acc(1);
             idx_cur = idx_next;
+            }
         }
     }
     tc_fence_before();
