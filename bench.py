@@ -121,8 +121,25 @@ def dist_env():
     return rank, world, local
 
 
+def aggregate_throughput(local_ms, jets_per_rank, world, dist=None, device="cpu"):
+    """Whole-job jets/s of a replicas-only run: every rank processed `jets_per_rank` jets in
+    `local_ms` device milliseconds; the job took the MAX over ranks (one all-reduce of a scalar is the only
+    communication of the benchmark).  Returns (jets/s, max ms)."""
+    import torch
+    t = torch.tensor([float(local_ms)], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    t_max = float(t.item())
+    return jets_per_rank * world / (t_max * 1e-3), t_max
+
+
+def batch_seed(r, rank):
+    """Seed of rotating batch r on rank `rank`: ranks draw disjoint batches of the same distribution (weak scaling)."""
+    return 1002 + 10000 * r + 1000003 * rank
+
+
 def make_batches(synth, rank, n_jets):
-    return [synth.make_particlenet_batch(seed=1002 + 10000 * r + 1000003 * rank, n_jets=n_jets) for r in range(N_BATCHES)]
+    return [synth.make_particlenet_batch(seed=batch_seed(r, rank), n_jets=n_jets) for r in range(N_BATCHES)]
 
 
 def time_oracle(arch, weights, batch, n_jets):
@@ -236,12 +253,8 @@ def run_ours(args):
     assert model.status_check() == 0
     step_ms = np.array([a.elapsed_time(b) for a, b in ev])
     total_ms = float(step_ms.sum())
-    t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms_max = float(t.item())
+    value, total_ms_max = aggregate_throughput(total_ms, B * args.steps, world, dist, dev)
     jets_total = B * args.steps * world
-    value = jets_total / (total_ms_max * 1e-3)
     stages, n_fw = model.profile_read()
     sampler.join(1.0)
 
