@@ -192,7 +192,7 @@ int forward(gnn_model* m, Workspace& w, const float* feats, const float* coords,
         float* y = bufs[l & 1];
         const bool fork = a.precision == GNN_BF16 && w.aux != nullptr;
         if (fork && (cudaEventRecord(w.ev_x, s) != cudaSuccess || cudaStreamWaitEvent(w.aux, w.ev_x, 0) != cudaSuccess)) return GNN_ERR_CUDA;
-        if ((rc = launch_knn(space, D, a.k, B, a.max_particles, w, w.idx, 0, (a.precision == GNN_BF16 && l > 0) ? 1 : 0, s)) < 0) return rc;
+        if ((rc = launch_knn(space, D, a.k, B, a.max_particles, w, w.idx, 0, a.precision == GNN_BF16 ? 1 : 0, s)) < 0) return rc;
         n += rc;
         tm.mark("knn", l);
         if (fork) {                         // u, v, shortcut of this block depend on x only: beside the kNN, on the aux stream

@@ -84,7 +84,8 @@ int launch_ingest(const int32_t* offsets, const int32_t* counts, int B, int N_ex
 int launch_compact_padded(const float* feats, const float* coords, const float* mask, int B, int P, int F, int CD,
                           int max_particles, Workspace& w, cudaStream_t s);
 // kNN: space [N, D]; out [N, k] global indices (local_out = 0) or jet-local (local_out = 1)
-// gram != 0: distances may take the tensor-core Gram form (bf16 mode, feature spaces); 0: exact direct differences
+// gram != 0 (bf16 mode, R28): distances may take the tensor-core Gram form where D has one, and the selection
+// orders 32-bit keys (d to 16 mantissa bits | j); 0: exact direct differences and exact (d, j) order
 int launch_knn(const float* space, int D, int k, int B, int max_particles, const Workspace& w, int32_t* idx_out,
                int local_out, int gram, cudaStream_t s);
 int launch_edgeconv_f32(const BlockDev& b, int k, const float* x, const int32_t* idx, int N, float* y,

@@ -28,12 +28,28 @@ constexpr int KNN_QT = 32;      // queries per CTA
 constexpr int KNN_DC = 32;      // dimensions staged per chunk
 constexpr int KNN_LD = KNN_DC + 4;
 
-template <int K>
-__device__ __forceinline__ void topk_insert(unsigned long long (&best)[K], unsigned long long key) {
+// Selection keys.  Key64 = (float bits of d) << 32 | j: exact lexicographic (d, j) order (d >= 0, so unsigned order on the
+// bits is numeric order).  Key32 (GNN_BF16 mode only, R28) = float bits with the low 7 mantissa bits replaced
+// by j (j < 128): d to 16 mantissa bits -- finer than the tf32 inputs it was computed from -- at half the instructions.
+struct Key64 {
+    typedef unsigned long long T;
+    static __device__ __forceinline__ T none() { return ~0ull; }
+    static __device__ __forceinline__ T make(float d, int j) { return ((T)__float_as_uint(d) << 32) | (unsigned)j; }
+    static __device__ __forceinline__ int index(T k) { return (int)(k & 0xffffffffull); }
+};
+struct Key32 {
+    typedef unsigned T;
+    static __device__ __forceinline__ T none() { return ~0u; }
+    static __device__ __forceinline__ T make(float d, int j) { return (__float_as_uint(d) & ~0x7fu) | (unsigned)j; }
+    static __device__ __forceinline__ int index(T k) { return (int)(k & 0x7fu); }
+};
+
+template <int K, typename KT>
+__device__ __forceinline__ void topk_insert(KT (&best)[K], KT key) {
     // best[] ascending; key < best[K-1] is known
 #pragma unroll
     for (int m = K - 1; m >= 0; --m) {
-        unsigned long long lo = (m > 0) ? best[m - 1] : 0ull;
+        KT lo = (m > 0) ? best[m - 1] : (KT)0;
         bool shift = (m > 0) && (key < lo);
         bool place = (key < best[m]) && !shift;
         if (shift) best[m] = lo;
@@ -165,7 +181,7 @@ knn_dist_kernel(const float* __restrict__ space, int D, const int32_t* __restric
 // union are then { min(A[m], B[K-1-m]) }, a bitonic sequence that log2(K) half-cleaner stages sort in registers.  d(i, j) is read as d(j, i) (the matrix is exactly
 // symmetric: (a-b)^2 and (b-a)^2 round identically), so a warp's consecutive queries read consecutive addresses.
 constexpr int KSEL_THREADS = 128;
-template <int K>
+template <int K, typename KEY>
 __global__ void __launch_bounds__(KSEL_THREADS)
 knn_select_kernel(const float* __restrict__ dm, int pld, int k, const int32_t* __restrict__ pjet, const int32_t* __restrict__ jet_start,
                   const int32_t* __restrict__ jet_n, const int32_t* __restrict__ meta, int32_t* __restrict__ idx_out,
@@ -185,7 +201,8 @@ knn_select_kernel(const float* __restrict__ dm, int pld, int k, const int32_t* _
     const float* col = dm + (size_t)start * pld + i;
     // the first K candidates of this half (j = half, half + 2, ...) are loaded together and ordered by a bitonic network
     // in registers (a sorted insert costs ~100 instructions, the whole K = 16 network ~500); later ones are inserted
-    unsigned long long best[K];
+    typedef typename KEY::T KT;
+    KT best[K];
     {
         float d[K];
 #pragma unroll
@@ -196,7 +213,7 @@ knn_select_kernel(const float* __restrict__ dm, int pld, int k, const int32_t* _
 #pragma unroll
         for (int u = 0; u < K; ++u) {
             const int j = half + 2 * u;
-            best[u] = (j < n && j != i) ? (((unsigned long long)__float_as_uint(d[u]) << 32) | (unsigned)j) : ~0ull;   // R4
+            best[u] = (j < n && j != i) ? KEY::make(d[u], j) : KEY::none();   // R4
         }
     }
 #pragma unroll
@@ -208,7 +225,7 @@ knn_select_kernel(const float* __restrict__ dm, int pld, int k, const int32_t* _
                 const int o = m ^ st;
                 if (o > m) {
                     const bool asc = (m & size) == 0 || size == K;
-                    const unsigned long long a = best[m], c = best[o];
+                    const KT a = best[m], c = best[o];
                     const bool sw = asc ? (c < a) : (a < c);
                     best[m] = sw ? c : a;
                     best[o] = sw ? a : c;
@@ -222,8 +239,8 @@ knn_select_kernel(const float* __restrict__ dm, int pld, int k, const int32_t* _
 #pragma unroll
         for (int u = 0; u < 8; ++u) {
             if (j + 2 * u == i) continue;                               // R4: by index
-            const unsigned long long key = ((unsigned long long)__float_as_uint(d[u]) << 32) | (unsigned)(j + 2 * u);
-            if (key < best[K - 1]) topk_insert<K>(best, key);
+            const KT key = KEY::make(d[u], j + 2 * u);
+            if (key < best[K - 1]) topk_insert<K, KT>(best, key);
         }
     }
     if (j < n) {                              // tail: up to eight more, predicated
@@ -233,18 +250,18 @@ knn_select_kernel(const float* __restrict__ dm, int pld, int k, const int32_t* _
 #pragma unroll
         for (int u = 0; u < 8; ++u) {
             if (j + 2 * u >= n || j + 2 * u == i) continue;
-            const unsigned long long key = ((unsigned long long)__float_as_uint(d[u]) << 32) | (unsigned)(j + 2 * u);
-            if (key < best[K - 1]) topk_insert<K>(best, key);
+            const KT key = KEY::make(d[u], j + 2 * u);
+            if (key < best[K - 1]) topk_insert<K, KT>(best, key);
         }
     }
     // merge with the partner lane: slot m of the merge is min(A[m], B[K-1-m]); both lanes end up with the same set
     const unsigned pm = __activemask();
     const int base = local_out ? 0 : start;
-    unsigned long long r[K];
+    KT r[K];
 #pragma unroll
     for (int m = 0; m < K; ++m) {
-        const unsigned long long mine = half ? best[K - 1 - m] : best[m];
-        const unsigned long long other = __shfl_xor_sync(pm, mine, 1);
+        const KT mine = half ? best[K - 1 - m] : best[m];
+        const KT other = __shfl_xor_sync(pm, mine, 1);
         r[m] = mine < other ? mine : other;
     }
     // r[] is bitonic: log2(K) half-cleaner stages sort it ascending (same order as a single sorted list would give)
@@ -253,14 +270,14 @@ knn_select_kernel(const float* __restrict__ dm, int pld, int k, const int32_t* _
 #pragma unroll
         for (int m = 0; m < K; ++m)
             if ((m & st) == 0) {
-                const unsigned long long a = r[m], c = r[m + st];
+                const KT a = r[m], c = r[m + st];
                 const bool sw = c < a;
                 r[m] = sw ? c : a;
                 r[m + st] = sw ? a : c;
             }
 #pragma unroll
     for (int m = 0; m < K; ++m)
-        if (m < k && (m & 1) == half) out[m] = (r[m] == ~0ull) ? -1 : (int32_t)(r[m] & 0xffffffffull) + base;
+        if (m < k && (m & 1) == half) out[m] = (r[m] == KEY::none()) ? -1 : KEY::index(r[m]) + base;
 }
 
 size_t knn_smem_bytes(int P) {
@@ -278,8 +295,11 @@ int launch_knn_t(const float* space, int D, int k, int B, int P, const Workspace
     if (!(gram && launch_knn_gram(space, D, B, P, w, s) == 1))
         knn_dist_kernel<<<B * tiles, KNN_THREADS, knn_smem_bytes(P), s>>>(space, D, w.jet_start, w.jet_n, w.meta, w.dm, pld, w.pjet, tiles);
     const long long n_upper = 2ll * B * P;                     // two threads per particle slot
-    knn_select_kernel<K><<<(unsigned)((n_upper + KSEL_THREADS - 1) / KSEL_THREADS), KSEL_THREADS, 0, s>>>(
-        w.dm, pld, k, w.pjet, w.jet_start, w.jet_n, w.meta, idx_out, local_out);
+    const unsigned grid = (unsigned)((n_upper + KSEL_THREADS - 1) / KSEL_THREADS);
+    if (gram && P <= 128)                    // bf16 mode: 32-bit keys (R28)
+        knn_select_kernel<K, Key32><<<grid, KSEL_THREADS, 0, s>>>(w.dm, pld, k, w.pjet, w.jet_start, w.jet_n, w.meta, idx_out, local_out);
+    else
+        knn_select_kernel<K, Key64><<<grid, KSEL_THREADS, 0, s>>>(w.dm, pld, k, w.pjet, w.jet_start, w.jet_n, w.meta, idx_out, local_out);
     return 2;
 }
 
