@@ -733,10 +733,11 @@ __global__ void __launch_bounds__(PRE_THREADS) pre_kernel(PreParams p) {
 // the 128-row tiles of its slice group, so per tile only the x rows move (L2 -> smem).  A is single-buffered and handed
 // over per K block (a_ready / a_free), the accumulator is double-buffered (2 x C TMEM columns): epilogue(t) and the
 // loads of tile t+1 run under MMA(t+1) / MMA(t).
-// Warps: 0-3 epilogue (thread = row = TMEM lane), 4-11 x loaders (a whole tile in flight in registers), 12 MMA issuer +
+// Warps: 0-7 epilogue (thread = row = TMEM lane), 8-15 x loaders (a whole tile in flight in registers), 16 MMA issuer +
 // TMEM owner + weight load.
-constexpr int PTC_THREADS = 416;
-constexpr int PTC_MMA_WARP = 12;
+constexpr int PTC_THREADS = 544;
+constexpr int PTC_EPI_WARPS = 8;          // lane quadrant w & 3, slabs of parity w >> 2
+constexpr int PTC_MMA_WARP = 16;
 
 template <int CIN, int C>
 struct PreTcCfg {
@@ -747,8 +748,8 @@ struct PreTcCfg {
     static constexpr int W_BYTES = KBA * WK_BYTES;            // one slice
     static constexpr int TMEM_COLS = 2 * C;
     static constexpr int NBAR = 2 * KBA + 5;
-    static constexpr int STAGE_BYTES = 4 * 4096;              // per epilogue warp: [32 rows][32 cols] fp32, swizzled
-    static constexpr int SMEM_BYTES = W_BYTES + A_BYTES + STAGE_BYTES + C * 4 + NBAR * 8 + 16 + 1024;
+    static constexpr int STAGE_BYTES = PTC_EPI_WARPS * 4096;  // per epilogue warp: [32 rows][32 cols] fp32, swizzled
+    static constexpr int SMEM_BYTES = W_BYTES + A_BYTES + STAGE_BYTES + C * 4 + NBAR * 8 + 16;
 };
 
 struct PreTcParams {
@@ -799,7 +800,7 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) pre_tc_kernel(PreTcParams p) {
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     if (tid == 0) {
         for (int i = 0; i < KBA; ++i) { mbar_init(&a_ready[i], 8); mbar_init(&a_free[i], 1); }
-        for (int i = 0; i < 2; ++i) { mbar_init(&d_full[i], 1); mbar_init(&d_free[i], 4); }
+        for (int i = 0; i < 2; ++i) { mbar_init(&d_full[i], 1); mbar_init(&d_free[i], PTC_EPI_WARPS); }
         mbar_init(w_full, 1);
         fence_mbar_init();
     }
@@ -839,10 +840,10 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) pre_tc_kernel(PreTcParams p) {
                 mma_commit(&d_full[acc]);
             }
         }
-    } else if (warp >= 4) {
+    } else if (warp >= PTC_EPI_WARPS) {
         // ===== x loaders: rows 16*lw .. +15 of every K block, 8 lanes per row (one 128-byte line); all K blocks of a tile
         // are requested before the first store, so a whole tile per CTA is in flight while the previous one is multiplied
-        const int lw = warp - 4;
+        const int lw = warp - PTC_EPI_WARPS;
         const int gc = lane & 7, grs = lane >> 3;
         for (int t = 0; t < T; ++t) {
             const int r0 = (gi + t * ng) * TILE_ROWS;
@@ -872,18 +873,17 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) pre_tc_kernel(PreTcParams p) {
         }
     } else {
         // ===== epilogue: thread = row = TMEM lane; slice 0 -> U (bf16), 1 -> V (bf16), 2 -> R (fp32) ======================
-        const int row = 32 * warp + lane;
+        const int q = warp & 3, eh = warp >> 2;
         for (int t = 0; t < T; ++t) {
             const int acc = t & 1;
-            const int gr = (gi + t * ng) * TILE_ROWS + row;
             mbar_wait(&d_full[acc], (t >> 1) & 1);
             tc_fence_after();
 #pragma unroll 1
-            for (int s = 0; s < C / 32; ++s) {
+            for (int s = eh; s < C / 32; s += 2) {
                 float v[32];
-                tmem_ld32(tmem + ((uint32_t)(32 * warp) << 16) + acc * C + s * 32, v);
+                tmem_ld32(tmem + ((uint32_t)(32 * q) << 16) + acc * C + s * 32, v);
                 tmem_ld_wait();
-                if (s == C / 32 - 1) {
+                if (s + 2 >= C / 32) {
                     tc_fence_before();
                     __syncwarp();
                     if (lane == 0) mbar_arrive(&d_free[acc]);
@@ -896,7 +896,7 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) pre_tc_kernel(PreTcParams p) {
                 // transpose through this warp's staging tile so that global stores are whole 128-byte (fp32) / 64-byte
                 // (bf16) row segments: thread = row writes swizzled 16-byte chunks, then 8 (4) lanes read one row back
                 uint8_t* st = stage + warp * 4096;
-                const int tr0 = (gi + t * ng) * TILE_ROWS + 32 * warp;
+                const int tr0 = (gi + t * ng) * TILE_ROWS + 32 * q;
                 if (slice == 2) {
 #pragma unroll
                     for (int i = 0; i < 8; ++i)
