@@ -144,19 +144,16 @@ pool_head_kernel(const float* __restrict__ x, const int32_t* __restrict__ jet_st
                 }
             }
         } else {
-            for (int it = threadIdx.x; it < PH_JETS * L.N; it += PH_THREADS) {
+            // narrow layer (the final one): one WARP per (jet, output), lanes split K, fixed-order shuffle reduction
+            const int wid = threadIdx.x >> 5, ln = threadIdx.x & 31;
+            for (int it = wid; it < PH_JETS * L.N; it += PH_THREADS / 32) {
                 const int jb = it / L.N, o = it - jb * L.N;
-                float a0 = 0.0f, a1 = 0.0f, a2 = 0.0f, a3 = 0.0f;
-                int c = 0;
-                for (; c + 3 < L.K; c += 4) {
-                    a0 = fmaf(zin[jb * W + c], __ldg(L.Wt + (size_t)c * L.ld + o), a0);
-                    a1 = fmaf(zin[jb * W + c + 1], __ldg(L.Wt + (size_t)(c + 1) * L.ld + o), a1);
-                    a2 = fmaf(zin[jb * W + c + 2], __ldg(L.Wt + (size_t)(c + 2) * L.ld + o), a2);
-                    a3 = fmaf(zin[jb * W + c + 3], __ldg(L.Wt + (size_t)(c + 3) * L.ld + o), a3);
-                }
-                for (; c < L.K; ++c) a0 = fmaf(zin[jb * W + c], __ldg(L.Wt + (size_t)c * L.ld + o), a0);
-                const float v = ((a0 + a1) + (a2 + a3)) + __ldg(L.shift + o);
-                if (jb < nj) {
+                float a0 = 0.0f;
+                for (int c = ln; c < L.K; c += 32) a0 = fmaf(zin[jb * W + c], __ldg(L.Wt + (size_t)c * L.ld + o), a0);
+#pragma unroll
+                for (int sh = 16; sh > 0; sh >>= 1) a0 += __shfl_xor_sync(0xffffffffu, a0, sh);
+                const float v = a0 + __ldg(L.shift + o);
+                if (ln == 0 && jb < nj) {
                     if (last) {
                         const bool bad = poisoned || jet_n[b0 + jb] < 0;
                         logits[(size_t)(b0 + jb) * hp.n_classes + o] = bad ? __int_as_float(0x7fc00000) : v;
