@@ -50,7 +50,7 @@ struct EdgeCfg {
     static constexpr int NEP = SPLIT ? 2 * NE : NE;           // epilogue warps in total: [0, NE) run E2, [NE, 2 NE) run E3
     static constexpr int MMA_WARP = NEP + NG;
     static constexpr int THREADS = 32 * (NEP + NG + 1);
-    static constexpr int MAXREG = C >= 256 ? 72 : 80;   // registers are per SM quarter: ceil(warps / 4) * 32 * MAXREG * MIN_CTAS <= 16384
+    static constexpr int MAXREG = C >= 256 ? 72 : (C >= 128 ? 80 : 64);   // registers are per SM quarter: ceil(warps / 4) * 32 * MAXREG * MIN_CTAS <= 16384
     static constexpr int KSTEPS_LAST = ((C - (KB - 1) * 64) + 15) / 16;
     static constexpr int NRB = PAIR ? C / 2 : C;              // weight rows (output channels) one CTA holds
     static constexpr int CHUNK_BYTES = NRB * 128;             // [NRB][64] bf16, 128B-swizzled
@@ -61,7 +61,7 @@ struct EdgeCfg {
     static constexpr int NBAR = 3 * KB + 6;
     static constexpr int SMALL_BYTES = 2 * C * 4 + NBAR * 8 + 16;
     static constexpr int SMEM_BYTES = W_BYTES + H_BYTES + SMALL_BYTES + 1024;
-    static constexpr int MIN_CTAS = C >= 256 ? 1 : (C >= 128 ? 2 : 3);
+    static constexpr int MIN_CTAS = C >= 256 ? 1 : (C >= 128 ? 2 : 4);
     static constexpr int NRANKS = PAIR ? 2 : 1;
 };
 
