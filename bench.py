@@ -13,6 +13,7 @@ delivered ragged (padding-free) through gnn_infer.  Prints ONE JSON line (rank 0
   stages_ms     mean CUDA-event time of every stage over the timed steps (gnn_profile_*)
   e2e           same metric through gnn_infer_host: pinned host buffers in, logits in host memory out, per step
   latency_b16   p50 / p99 of one gnn_infer on a device-resident 16-jet batch (the metric's second half)
+  serving       configs[3]: 64 closed-loop clients through the host dynamic batcher: jets/s, p50 / p99, queue / compute split
   cpu_baseline  the fp64 oracle as it stands, on the box's host cores, on a bounded sample of the same batch
 Multi-GPU: jets are independent and the weights are < 3 MB, so the path shards by jets with no collective ("replicas
 only"): every rank runs its own batches; value = all ranks' jets / max-over-ranks time.
@@ -159,6 +160,50 @@ def cpu_baseline(arch, weights, batch, target_s=12.0):
     return {"value": n / t, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle",
             "sample": "first %d jets of batch 0 (%d particles), one oracle.forward call, %.1f s" %
                       (n, int(batch.offsets[n]), t)}
+
+
+def serving_leg(gnn, synth, arch, weights, device, n_clients=64, warm_s=0.5, run_s=2.0):
+    """BASELINE.json configs[3]: synchronous clients (submit -> wait -> next), batcher with
+    max_batch 1024, max queue delay 1 ms, 2 instances.  Client threads are Python threads (ctypes releases the GIL in
+    submit / wait), so the Python side is part of the measured request latency."""
+    model = gnn.Model(gnn.arch_struct(arch, max_batch_jets=1024, precision=gnn.BF16, workspace_slices=2, max_particles=100),
+                      weights, device=device)
+    bt = gnn.Batcher(model, max_batch_jets=1024, max_queue_delay_us=1000, n_instances=2)
+    pools = [synth.make_client_pool(c, n_requests=16) for c in range(n_clients)]
+    lat, qs, cs, stop, t_start = [[] for _ in range(n_clients)], [[] for _ in range(n_clients)], [[] for _ in range(n_clients)], [False], [0.0]
+
+    def client(c):
+        i = 0
+        while not stop[0]:
+            r = pools[c][i % len(pools[c])]
+            t0 = time.perf_counter()
+            tk, _ = bt.submit(r.feats, r.coords, r.offsets)
+            rc, q_us, c_us = bt.wait(tk)
+            t1 = time.perf_counter()
+            if rc == 0 and t0 >= t_start[0] > 0.0:
+                lat[c].append((t1 - t0) * 1e6); qs[c].append(q_us); cs[c].append(c_us)
+            i += 1
+
+    th = [threading.Thread(target=client, args=(c,), daemon=True) for c in range(n_clients)]
+    for t in th:
+        t.start()
+    time.sleep(warm_s)
+    t_start[0] = time.perf_counter()
+    time.sleep(run_s)
+    stop[0] = True
+    t_end = time.perf_counter()
+    for t in th:
+        t.join(10.0)
+    st = bt.stats()
+    bt.close()
+    model.close()
+    allv = np.concatenate([np.asarray(v) for v in lat if v]) if any(lat) else np.zeros(1)
+    return {"workload": "configs[3]: %d closed-loop clients x 16 jets, batcher max_batch 1024, max delay 1 ms, 2 instances" % n_clients,
+            "value": 16 * allv.size / (t_end - t_start[0]), "unit": UNIT, "requests": int(allv.size),
+            "p50_us": float(np.percentile(allv, 50)), "p99_us": float(np.percentile(allv, 99)),
+            "queue_us_mean": float(np.mean(np.concatenate([np.asarray(v) for v in qs if v]))) if any(qs) else None,
+            "compute_us_mean": float(np.mean(np.concatenate([np.asarray(v) for v in cs if v]))) if any(cs) else None,
+            "mean_coalesced_batch_jets": st["mean_batch_jets"], "seconds": t_end - t_start[0]}
 
 
 def run_reference(args):
@@ -334,6 +379,9 @@ def run_ours(args):
             lat = np.array([a.elapsed_time(b) for a, b in e16]) * 1e3
             out["latency_b16"] = {"p50_us": float(np.percentile(lat, 50)), "p99_us": float(np.percentile(lat, 99)),
                                   "iterations": n_it, "entry": "gnn_infer, 16 jets device-resident, CUDA events"}
+        # ---- configs[3]: 64 closed-loop clients x 16-jet requests through the host dynamic batcher (bf16) -------------
+        if rank == 0 and args.precision == "bf16":
+            out["serving"] = serving_leg(gnn, synth, arch, weights, local)
     out["clocks"] = sampler.summary()
     if rank == 0 and world == 1 and not args.no_cpu_baseline and not args.no_extras:
         out["cpu_baseline"] = cpu_baseline(arch, weights, batches[0])

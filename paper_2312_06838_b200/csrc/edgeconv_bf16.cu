@@ -82,7 +82,7 @@ template <int C, int LOGK>
 __global__ void __launch_bounds__(EdgeCfg<C>::THREADS) __maxnreg__(EdgeCfg<C>::MAXREG) edge_kernel(EdgeParams p) {
     using Cfg = EdgeCfg<C>;
     constexpr bool PAIR = Cfg::PAIR;
-    constexpr int KB = Cfg::KB, NE = Cfg::NE, NG = Cfg::NG, CWE = Cfg::CWE;
+    constexpr int KB = Cfg::KB, NE = Cfg::NE, CWE = Cfg::CWE;
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     if (p.meta[0]) return;                                       // grid-uniform
     const int N = p.meta[1];

@@ -26,7 +26,7 @@ __global__ void __launch_bounds__(PH_THREADS)
 pool_head_kernel(const float* __restrict__ x, const int32_t* __restrict__ jet_start, const int32_t* __restrict__ jet_n,
                  const int32_t* __restrict__ meta, HeadParams hp, int B, float* __restrict__ logits) {
     extern __shared__ __align__(16) float zs[];      // z0 [PH_JETS][wmax] | z1 [PH_JETS][wmax] | partials
-    __shared__ int s_end[PH_JETS], s_n[PH_JETS];     // row range ends (relative to the CTA's first row) and multiplicities
+    __shared__ int s_n[PH_JETS];                     // multiplicities (0 for offending / absent jets)
     const int b0 = blockIdx.x * PH_JETS;
     const int nj = min(PH_JETS, B - b0);
     const int C = hp.C, W = hp.wmax;
@@ -36,13 +36,11 @@ pool_head_kernel(const float* __restrict__ x, const int32_t* __restrict__ jet_st
     const bool poisoned = meta[0] != 0;
     // ---- pooling: the jets of this CTA are one contiguous span of rows; thread (row group rg, channel quad cq) walks rows
     // rg, rg + G, ... with eight loads in flight and flushes its partial sum when a row crosses into the next jet ---------
-    const int row0 = jet_start[b0];
     if (threadIdx.x < PH_JETS) {
         const int jb = threadIdx.x;
         int n = (jb < nj && !poisoned) ? jet_n[b0 + jb] : 0;
         if (n < 0) n = 0;                            // offending jet: pools nothing (its logits become NaN below)
         s_n[jb] = n;
-        s_end[jb] = (jb < nj) ? jet_start[b0 + jb] - row0 + n : 0x7fffffff;
     }
     __syncthreads();
     const int CQ = C >> 2;                           // channel quads
