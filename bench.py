@@ -13,6 +13,7 @@ delivered ragged (padding-free) through gnn_infer.  Prints ONE JSON line (rank 0
   stages_ms     mean CUDA-event time of every stage over the timed steps (gnn_profile_*)
   e2e           same metric through gnn_infer_host: pinned host buffers in, logits in host memory out, per step
   latency_b16   p50 / p99 of one gnn_infer on a device-resident 16-jet batch (the metric's second half)
+  sweep         configs[4]: jets/s, p50 and roofline fraction vs batch size (base and wide architecture), L2 not flushed
   serving       configs[3]: 64 closed-loop clients through the host dynamic batcher: jets/s, p50 / p99, queue / compute split
   cpu_baseline  the fp64 oracle as it stands, on the box's host cores, on a bounded sample of the same batch
 Multi-GPU: jets are independent and the weights are < 3 MB, so the path shards by jets with no collective ("replicas
@@ -206,6 +207,37 @@ def serving_leg(gnn, synth, arch, weights, device, n_clients=64, warm_s=0.5, run
             "mean_coalesced_batch_jets": st["mean_batch_jets"], "seconds": t_end - t_start[0]}
 
 
+def sweep_leg(torch, gnn, synth, work_fn, peak_tf, device, reps=5):
+    """BASELINE.json configs[4]: saturation sweep, nested batches of one 16 384-jet sequence (multiplicity ~ clip(Poisson(60),
+    5, 128)), base and wide architecture, bf16; jets/s, p50 of a few launches and the fraction of the forward's bf16 roofline."""
+    dev = torch.device("cuda", device)
+    out = {}
+    full = synth.make_sweep_batch(n_jets=16384)
+    for name, sizes in (("particlenet", (1, 16, 256, 1024, 4096, 16384)), ("wide", (16, 256, 1024))):
+        arch = synth.ARCHS[name]
+        model = gnn.Model(gnn.arch_struct(arch, max_batch_jets=max(sizes), precision=gnn.BF16, max_particles=128),
+                          synth.make_weights(arch), device=device)
+        rows = []
+        for B in sizes:
+            b = full.head(B)
+            f, c, o = (torch.from_numpy(x).to(dev) for x in (b.feats, b.coords, b.offsets))
+            lg = torch.empty((B, arch.n_classes), dtype=torch.float32, device=dev)
+            for _ in range(2):
+                model.infer(f, c, o, logits=lg)
+            ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(reps)]
+            torch.cuda.synchronize()
+            for a, e in ev:
+                a.record(torch.cuda.current_stream()); model.infer(f, c, o, logits=lg); e.record(torch.cuda.current_stream())
+            torch.cuda.synchronize()
+            ms = float(np.median([a.elapsed_time(e) for a, e in ev]))
+            fl = work_fn(arch, b.counts())["min"]
+            rows.append({"batch_jets": B, "ms_p50": ms, "jets_per_s": B / (ms * 1e-3), "frac_of_bf16_peak": fl / (ms * 1e-3) / 1e12 / peak_tf})
+        assert model.status_check() == 0
+        model.close()
+        out[name] = rows
+    return out
+
+
 def run_reference(args):
     """--impl reference: the fp64 oracle timed on the host cores; each step is a bounded sample of the workload."""
     rank, world, _ = dist_env()
@@ -382,6 +414,7 @@ def run_ours(args):
         # ---- configs[3]: 64 closed-loop clients x 16-jet requests through the host dynamic batcher (bf16) -------------
         if rank == 0 and args.precision == "bf16":
             out["serving"] = serving_leg(gnn, synth, arch, weights, local)
+            out["sweep"] = sweep_leg(torch, gnn, synth, work, roof_peak, local)
     out["clocks"] = sampler.summary()
     if rank == 0 and world == 1 and not args.no_cpu_baseline and not args.no_extras:
         out["cpu_baseline"] = cpu_baseline(arch, weights, batches[0])

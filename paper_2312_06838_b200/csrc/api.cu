@@ -345,7 +345,17 @@ int gnn_infer_host(gnn_model* m, int32_t slice, const float* feats_host, const f
     int rc = forward(m, w, w.pfeats, w.pcoords, w.poffsets, nullptr, B, N, N, w.hlogits, s);
     if (rc != GNN_OK) return rc;
     GNN_CUDA_TRY(cudaMemcpyAsync(logits_host, w.hlogits, (size_t)B * a.n_classes * sizeof(float), cudaMemcpyDeviceToHost, s));
-    return gnn_status_check(m, slice, cuda_stream);
+    // the sticky status word rides the same stream: one synchronisation per call (gnn_status_check would add a second)
+    unsigned st = 0;
+    GNN_CUDA_TRY(cudaMemcpyAsync(&st, w.status, sizeof(unsigned), cudaMemcpyDeviceToHost, s));
+    GNN_CUDA_TRY(cudaStreamSynchronize(s));
+    if (st) {
+        GNN_CUDA_TRY(cudaMemsetAsync(w.status, 0, sizeof(unsigned), s));
+        GNN_CUDA_TRY(cudaStreamSynchronize(s));
+    }
+    if (st & GNN_DEV_BAD_OFFSETS) return GNN_ERR_BAD_OFFSETS;
+    if (st & GNN_DEV_JET_TOO_LARGE) return GNN_ERR_JET_TOO_LARGE;
+    return GNN_OK;
 }
 
 int gnn_profile_enable(gnn_model* m, int32_t slice, int32_t on) {
