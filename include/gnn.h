@@ -53,12 +53,14 @@ typedef enum {
 
 typedef enum {
     GNN_FP32_VALIDATION = 0,  /* every contraction in fp32 FMA on CUDA cores (R18) */
-    GNN_BF16 = 1              /* edge-MLP GEMMs as bf16 x bf16 -> fp32 tcgen05 MMAs; kNN, shortcut, pool, head fp32 (R19) */
+    GNN_BF16 = 1              /* edge-MLP GEMMs as bf16 x bf16 -> fp32 tcgen05 MMAs; per-particle GEMM of blocks >= 2 and kNN Gram
+                                 matrices of blocks >= 2 in tf32; neighbour selection on 32-bit keys; E3 row sum in f16x2;
+                                 accumulators, block outputs, pool, head fp32 (R19, R28) */
 } gnn_precision;
 
 /* Architecture.  Constraints checked by gnn_create: 1 <= n_blocks <= GNN_MAX_BLOCKS;
  * coord_dims in [1,8]; 1 <= k <= GNN_MAX_K (BF16 mode: k a power of two); every channel count a multiple of 8
- * (BF16 mode: one of 32, 64, 128, 256 and C1 == C2 == C3 inside a block); 0 <= n_fc_hidden <= GNN_MAX_FC;
+ * (BF16 mode: one of 32, 64, 128, 256, 512 and C1 == C2 == C3 inside a block); 0 <= n_fc_hidden <= GNN_MAX_FC;
  * 1 <= fc widths <= 1024; 1 <= n_classes <= 64; 1 <= max_particles <= GNN_MAX_PARTICLES; max_batch_jets >= 1;
  * 1 <= workspace_slices <= GNN_MAX_SLICES (0 is read as 1). */
 typedef struct {
@@ -92,6 +94,8 @@ void gnn_destroy(gnn_model* m);
  * row-major fp32, particles of one jet contiguous; offsets_dev int32 [B+1] CSR (offsets[0] = 0, offsets[B] = N);
  * logits_dev fp32 [B, n_classes] (written).  Asynchronous on `cuda_stream` (a cudaStream_t; NULL = default
  * stream).  Uses workspace slice 0 / `slice`: two calls may overlap only on different slices.  B = 0 is legal.
+ * (GNN_BF16: part of the work is enqueued on an auxiliary stream owned by the slice, forked from and joined back into
+ * `cuda_stream` by events, so the call is still ordered on `cuda_stream` alone; stream capture is not supported.)
  * Host-checkable errors return at once; device-checkable ones (GNN_ERR_BAD_OFFSETS, GNN_ERR_JET_TOO_LARGE) set a
  * sticky per-slice status word read by gnn_status_check and put NaN into the offending logits.  n_b = 0 is legal
  * (logits = head(0), R12).  NaN / Inf inputs are not checked. */
