@@ -125,6 +125,21 @@ def test_sweep_base_1024_sampled(pn):
         assert np.array_equal(run_ragged(m, b.head(B)), lg[:B])
 
 
+def test_sweep_base_16384_maximum_size():
+    """configs[4] at its largest batch (16 384 jets, ~983 k particles, the workspace's maximum): finite logits, no device
+    error, the first 256 jets within the parity bars of the oracle, and bitwise equal to the same jets run as a batch
+    of 256 (batch-composition invariance at the size the sweep is timed at)."""
+    a, w, m = bf16_model("particlenet", 16384)
+    b = synth.make_sweep_batch(n_jets=16384)
+    lg = run_ragged(m, b)
+    assert m.status_check() == 0 and np.isfinite(lg).all()
+    h = b.head(256)
+    ref = oracle.forward(a, w, h.feats, h.coords, h.offsets)
+    check_logits(lg[:256], ref)
+    assert np.array_equal(run_ragged(m, h), lg[:256])
+    m.close()
+
+
 def test_sweep_wide_256_sampled():
     """configs[4] wide variant (EdgeConv channels 128, 256, 512, FC 512) at B = 256; the oracle runs the first 64 jets.
     Block 3 (C = 512) takes the streamed-weight kernel, its stage is also checked alone."""
