@@ -181,9 +181,11 @@ knn_dist_kernel(const float* __restrict__ space, int D, const int32_t* __restric
 // union are then { min(A[m], B[K-1-m]) }, a bitonic sequence that log2(K) half-cleaner stages sort in registers.  d(i, j) is read as d(j, i) (the matrix is exactly
 // symmetric: (a-b)^2 and (b-a)^2 round identically), so a warp's consecutive queries read consecutive addresses.
 constexpr int KSEL_THREADS = 128;
-template <int K, typename KEY>
+// FLY (spaces of at most 4 dimensions: the coordinates of block 1): no distance matrix, d(i, j) is computed from the rows of
+// `space` with the arithmetic of knn_dist_kernel (t = s_i - s_j, d = fma(t, t, d) in index order), so both give the same bits.
+template <int K, typename KEY, bool FLY>
 __global__ void __launch_bounds__(KSEL_THREADS)
-knn_select_kernel(const float* __restrict__ dm, int pld, int k, const int32_t* __restrict__ pjet, const int32_t* __restrict__ jet_start,
+knn_select_kernel(const float* __restrict__ dm, int pld, const float* __restrict__ space, int D, int k, const int32_t* __restrict__ pjet, const int32_t* __restrict__ jet_start,
                   const int32_t* __restrict__ jet_n, const int32_t* __restrict__ meta, int32_t* __restrict__ idx_out,
                   int local_out) {
     if (meta[0]) return;
@@ -199,6 +201,21 @@ knn_select_kernel(const float* __restrict__ dm, int pld, int k, const int32_t* _
     }
     const int i = q - start;
     const float* col = dm + (size_t)start * pld + i;
+    float qx[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+    if (FLY) {
+        for (int c = 0; c < D; ++c) qx[c] = __ldg(space + (size_t)q * D + c);
+    }
+    auto dist = [&](int j) -> float {
+        if (!FLY) return __ldg(col + (size_t)j * pld);
+        const float* sj = space + (size_t)(start + j) * D;
+        float d = 0.0f;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            const float t = qx[c] - (c < D ? __ldg(sj + c) : 0.0f);
+            d = fmaf(t, t, d);
+        }
+        return d;
+    };
     // the first K candidates of this half (j = half, half + 2, ...) are loaded together and ordered by a bitonic network
     // in registers (a sorted insert costs ~100 instructions, the whole K = 16 network ~500); later ones are inserted
     typedef typename KEY::T KT;
@@ -208,7 +225,7 @@ knn_select_kernel(const float* __restrict__ dm, int pld, int k, const int32_t* _
 #pragma unroll
         for (int u = 0; u < K; ++u) {
             const int j = half + 2 * u;
-            d[u] = (j < n) ? __ldg(col + (size_t)j * pld) : 0.0f;
+            d[u] = (j < n) ? dist(j) : 0.0f;
         }
 #pragma unroll
         for (int u = 0; u < K; ++u) {
@@ -235,7 +252,7 @@ knn_select_kernel(const float* __restrict__ dm, int pld, int k, const int32_t* _
     for (; j + 14 < n; j += 16) {             // eight loads in flight per thread
         float d[8];
 #pragma unroll
-        for (int u = 0; u < 8; ++u) d[u] = __ldg(col + (size_t)(j + 2 * u) * pld);
+        for (int u = 0; u < 8; ++u) d[u] = dist(j + 2 * u);
 #pragma unroll
         for (int u = 0; u < 8; ++u) {
             if (j + 2 * u == i) continue;                               // R4: by index
@@ -246,7 +263,7 @@ knn_select_kernel(const float* __restrict__ dm, int pld, int k, const int32_t* _
     if (j < n) {                              // tail: up to eight more, predicated
         float d[8];
 #pragma unroll
-        for (int u = 0; u < 8; ++u) d[u] = (j + 2 * u < n) ? __ldg(col + (size_t)(j + 2 * u) * pld) : 0.0f;
+        for (int u = 0; u < 8; ++u) d[u] = (j + 2 * u < n) ? dist(j + 2 * u) : 0.0f;
 #pragma unroll
         for (int u = 0; u < 8; ++u) {
             if (j + 2 * u >= n || j + 2 * u == i) continue;
@@ -280,6 +297,17 @@ knn_select_kernel(const float* __restrict__ dm, int pld, int k, const int32_t* _
         if (m < k && (m & 1) == half) out[m] = (r[m] == KEY::none()) ? -1 : KEY::index(r[m]) + base;
 }
 
+// particle -> jet map for the on-the-fly selection: one thread per jet writes its rows (offending ragged jets own rows too)
+__global__ void pjet_kernel(int B, const int32_t* __restrict__ jet_start, const int32_t* __restrict__ jet_n,
+                            const int32_t* __restrict__ meta, int32_t* __restrict__ pjet) {
+    if (meta[0]) return;
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= B) return;
+    const int n = jet_n[b], start = jet_start[b];
+    const int rows = n < -1 ? -n : (n > 0 ? n : 0);
+    for (int r = 0; r < rows; ++r) pjet[start + r] = b;
+}
+
 size_t knn_smem_bytes(int P) {
     const int n4 = (P + 3) & ~3;
     return (size_t)2 * n4 * KNN_LD * sizeof(float);
@@ -290,16 +318,25 @@ int launch_knn_t(const float* space, int D, int k, int B, int P, const Workspace
                  int gram, cudaStream_t s) {
     const int tiles = (P + KNN_QT - 1) / KNN_QT;
     const int pld = (P + 3) & ~3;
+    const long long n_upper = 2ll * B * P;                     // two threads per particle slot
+    const unsigned grid = (unsigned)((n_upper + KSEL_THREADS - 1) / KSEL_THREADS);
+    if (D <= 4) {
+        // coordinates (block 1): distances on the fly inside the selection; the particle -> jet map comes from its own kernel
+        pjet_kernel<<<(B + 127) / 128, 128, 0, s>>>(B, w.jet_start, w.jet_n, w.meta, w.pjet);
+        if (gram && P <= 128)
+            knn_select_kernel<K, Key32, true><<<grid, KSEL_THREADS, 0, s>>>(w.dm, pld, space, D, k, w.pjet, w.jet_start, w.jet_n, w.meta, idx_out, local_out);
+        else
+            knn_select_kernel<K, Key64, true><<<grid, KSEL_THREADS, 0, s>>>(w.dm, pld, space, D, k, w.pjet, w.jet_start, w.jet_n, w.meta, idx_out, local_out);
+        return 2;
+    }
     // distances: the Gram form on the tensor cores where the caller allows it (bf16 mode, feature spaces) and D has one,
     // else the exact direct-difference kernel
     if (!(gram && launch_knn_gram(space, D, B, P, w, s) == 1))
         knn_dist_kernel<<<B * tiles, KNN_THREADS, knn_smem_bytes(P), s>>>(space, D, w.jet_start, w.jet_n, w.meta, w.dm, pld, w.pjet, tiles);
-    const long long n_upper = 2ll * B * P;                     // two threads per particle slot
-    const unsigned grid = (unsigned)((n_upper + KSEL_THREADS - 1) / KSEL_THREADS);
     if (gram && P <= 128)                    // bf16 mode: 32-bit keys (R28)
-        knn_select_kernel<K, Key32><<<grid, KSEL_THREADS, 0, s>>>(w.dm, pld, k, w.pjet, w.jet_start, w.jet_n, w.meta, idx_out, local_out);
+        knn_select_kernel<K, Key32, false><<<grid, KSEL_THREADS, 0, s>>>(w.dm, pld, space, D, k, w.pjet, w.jet_start, w.jet_n, w.meta, idx_out, local_out);
     else
-        knn_select_kernel<K, Key64><<<grid, KSEL_THREADS, 0, s>>>(w.dm, pld, k, w.pjet, w.jet_start, w.jet_n, w.meta, idx_out, local_out);
+        knn_select_kernel<K, Key64, false><<<grid, KSEL_THREADS, 0, s>>>(w.dm, pld, space, D, k, w.pjet, w.jet_start, w.jet_n, w.meta, idx_out, local_out);
     return 2;
 }
 
