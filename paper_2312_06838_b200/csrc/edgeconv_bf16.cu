@@ -63,6 +63,9 @@ struct EdgeCfg {
     static constexpr int SMEM_BYTES = W_BYTES + H_BYTES + SMALL_BYTES + 1024;
     static constexpr int MIN_CTAS = C >= 256 ? 1 : (C >= 128 ? 2 : 4);
     static constexpr int NRANKS = PAIR ? 2 : 1;
+    // shift pre-loaded into the accumulators (tcgen05.st by the epilogue that drains them) or added in the epilogues: the
+    // re-arm costs ~0.9 k cycles on the epilogue warps' chain, which bounds the narrow blocks (measured)
+    static constexpr bool BIAS_ACC = C >= 256;
 };
 
 struct EdgeParams {
@@ -163,7 +166,7 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS) __maxnreg__(EdgeCfg<C>::M
                         for (int ks = 0; ks < ksteps; ++ks) {
                             const uint64_t ad = desc_sw128(h_addr + kb * Cfg::HK_BYTES + ks * 32);
                             const uint64_t bd = desc_sw128(w_addr + (layer * KB + kb) * Cfg::CHUNK_BYTES + ks * 32);
-                            mma_bf16_ss_g<PAIR>(tmem + layer * C, ad, bd, idesc, 1u);
+                            mma_bf16_ss_g<PAIR>(tmem + layer * C, ad, bd, idesc, Cfg::BIAS_ACC ? 1u : (uint32_t)((kb | ks) != 0));
                         }
                         if (layer == 1) mma_commit_g<PAIR>(&h_free[kb]);   // gather of the next tile may overwrite it
                     }
@@ -281,6 +284,7 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS) __maxnreg__(EdgeCfg<C>::M
         // one instruction per 32 columns), so every MMA accumulates and the epilogues need no bias add.
         auto reset_acc = [&](int layer) {
             const float* sh = layer ? t3 : t2;
+            if constexpr (Cfg::BIAS_ACC) {
 #pragma unroll
             for (int s = 0; s < SLABS; ++s) {
                 float w[32];
@@ -292,6 +296,7 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS) __maxnreg__(EdgeCfg<C>::M
                 tmem_st32(tbase + layer * C + s * 32, w);
             }
             tmem_st_wait();
+            }
             tc_fence_before();
             arrive_leader(&d_free[layer]);
         };
@@ -322,7 +327,12 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS) __maxnreg__(EdgeCfg<C>::M
                     const int col = col0 + s * 32;
                     uint32_t pk[16];
 #pragma unroll
-                    for (int i = 0; i < 16; ++i) pk[i] = pack_relu_bf16x2(v[2 * i], v[2 * i + 1]);
+                    for (int i = 0; i < 8; ++i) {
+                        float4 sh = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+                        if constexpr (!Cfg::BIAS_ACC) sh = *reinterpret_cast<const float4*>(t2 + s * 32 + 4 * i);
+                        pk[2 * i] = pack_relu_bf16x2(v[4 * i] + sh.x, v[4 * i + 1] + sh.y);
+                        pk[2 * i + 1] = pack_relu_bf16x2(v[4 * i + 2] + sh.z, v[4 * i + 3] + sh.w);
+                    }
                     if (s + 1 < SLABS) tmem_ld32(tbase + (s + 1) * 32, v);     // in flight while this slab is stored
                     uint8_t* dst = H + (col >> 6) * Cfg::HK_BYTES + row * 128;
                     const int c8 = (col & 63) >> 3;
@@ -365,7 +375,12 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS) __maxnreg__(EdgeCfg<C>::M
                     tmem_ld_wait();
                     uint32_t w[16];
 #pragma unroll
-                    for (int i = 0; i < 16; ++i) w[i] = pack_relu_f16x2(v[2 * i], v[2 * i + 1]);
+                    for (int i = 0; i < 8; ++i) {
+                        float4 sh = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+                        if constexpr (!Cfg::BIAS_ACC) sh = *reinterpret_cast<const float4*>(t3 + s * 32 + 4 * i);
+                        w[2 * i] = pack_relu_f16x2(v[4 * i] + sh.x, v[4 * i + 1] + sh.y);
+                        w[2 * i + 1] = pack_relu_f16x2(v[4 * i + 2] + sh.z, v[4 * i + 3] + sh.w);
+                    }
                     if (s + 1 < SLABS) tmem_ld32(tbase + C + (s + 1) * 32, v);  // in flight during this slab's butterfly
                     if (vmask != 0xffffffffu) {
 #pragma unroll
