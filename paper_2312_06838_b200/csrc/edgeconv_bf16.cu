@@ -64,8 +64,8 @@ struct EdgeCfg {
     static constexpr int MIN_CTAS = C >= 256 ? 1 : (C >= 128 ? 2 : 4);
     static constexpr int NRANKS = PAIR ? 2 : 1;
     // shift pre-loaded into the accumulators (tcgen05.st by the epilogue that drains them) or added in the epilogues: the
-    // re-arm costs ~0.9 k cycles on the epilogue warps' chain, which bounds the narrow blocks (measured)
-    static constexpr bool BIAS_ACC = C >= 256;
+    // re-arm costs ~0.9 k cycles on the epilogue warps' chain and delays d_free; measured slower for every C (10 % at C <= 128)
+    static constexpr bool BIAS_ACC = false;
 };
 
 struct EdgeParams {
