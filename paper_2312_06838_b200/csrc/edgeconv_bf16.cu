@@ -46,11 +46,11 @@ struct EdgeCfg {
     static constexpr int GH = 2;                              // row parts of the gather
     static constexpr int NG = GH * KB;                        // gather warps: K block g % KB, row part g / KB
     static constexpr int RW = TILE_ROWS / GH;                 // rows per gather warp
-    static constexpr bool SPLIT = C >= 256;                     // E2 and E3 on separate warp sets: E2(t+1) need not wait for E3(t)
+    static constexpr bool SPLIT = false;                        // E2 and E3 on separate warp sets: E2(t+1) need not wait for E3(t)
     static constexpr int NEP = SPLIT ? 2 * NE : NE;           // epilogue warps in total: [0, NE) run E2, [NE, 2 NE) run E3
     static constexpr int MMA_WARP = NEP + NG;
     static constexpr int THREADS = 32 * (NEP + NG + 1);
-    static constexpr int MAXREG = C >= 256 ? 72 : (C >= 128 ? 80 : 64);   // registers are per SM quarter: ceil(warps / 4) * 32 * MAXREG * MIN_CTAS <= 16384
+    static constexpr int MAXREG = C >= 256 ? 96 : (C >= 128 ? 80 : 64);   // registers are per SM quarter: ceil(warps / 4) * 32 * MAXREG * MIN_CTAS <= 16384
     static constexpr int KSTEPS_LAST = ((C - (KB - 1) * 64) + 15) / 16;
     static constexpr int NRB = PAIR ? C / 2 : C;              // weight rows (output channels) one CTA holds
     static constexpr int CHUNK_BYTES = NRB * 128;             // [NRB][64] bf16, 128B-swizzled
