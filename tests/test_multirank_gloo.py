@@ -51,3 +51,21 @@ def test_single_rank_needs_no_process_group():
     v, t = bench.aggregate_throughput(4.0, 1024, 1)
     assert t == 4.0 and v == 1024 / 4e-3
     assert bench.batch_seed(0, 0) == 1002 and len({bench.batch_seed(r, k) for r in range(4) for k in range(8)}) == 32
+
+
+def test_work_accounting_matches_the_survey_figures():
+    """bench.work(): algorithmic MACs per particle: base arch F = 7, k_eff = 16: stated 4 118 976, minimal
+    (layer 1 factorised) 2 876 736; head 66 048 MAC per jet; wide arch minimal 11 504 256; Tiny (k = 4): 9 344 / 8 576."""
+    a = synth.ARCHS["particlenet"]
+    w = bench.work(a, [17])                            # one jet of 17 particles: k_eff = 16 for every particle
+    assert w["stated"] == 2 * (17 * 4118976 + 66048)
+    assert w["min"] == 2 * (17 * 2876736 + 66048)
+    assert w["blocks_min"] == [2 * 17 * 132416, 2 * 17 * 548864, 2 * 17 * 2195456]
+    assert w["blocks_edge"][2] == 2 * 17 * 16 * (256 * 256 * 2)
+    ww = bench.work(synth.ARCHS["wide"], [17])
+    assert ww["min"] == 2 * (17 * 11504256 + 263168)
+    t = bench.work(synth.ARCHS["tiny"], [16])
+    assert t["stated"] == 2 * (16 * 9344 + 64) and t["min"] == 2 * (16 * 8576 + 64)
+    # k_eff = min(k, n - 1): a jet of 5 particles has 4 neighbours per particle, a single particle none
+    w5 = bench.work(a, [5, 1])
+    assert w5["blocks_edge"][0] == 2 * (5 * 4) * (64 * 64 * 2)
