@@ -28,7 +28,7 @@ struct Workspace {
     float* xa = nullptr;        // [Nmax, Cmax] ping
     float* xb = nullptr;        // [Nmax, Cmax] pong
     int32_t* idx = nullptr;     // [Nmax, k] global particle indices, -1 = none
-    int32_t* pjet = nullptr;    // [Nmax] particle -> jet (kNN)
+    int2* pjet = nullptr;       // [Nmax] particle -> (start, n) of its jet (kNN selection: one load instead of three)
     float* dm = nullptr;        // [Nmax, max_particles rounded to 4] per-jet pairwise squared distances (kNN)
     int32_t* jet_start = nullptr;  // [Bmax] sanitised CSR
     int32_t* jet_n = nullptr;      // [Bmax] sanitised multiplicities (< 0 = offending jet; -n if it owns n packed rows)

@@ -60,14 +60,14 @@ __device__ __forceinline__ void topk_insert(KT (&best)[K], KT key) {
 __global__ void __launch_bounds__(KNN_THREADS)
 knn_dist_kernel(const float* __restrict__ space, int D, const int32_t* __restrict__ jet_start,
                 const int32_t* __restrict__ jet_n, const int32_t* __restrict__ meta, float* __restrict__ dm, int pld,
-                int32_t* __restrict__ pjet, int tiles_per_jet) {
+                int2* __restrict__ pjet, int tiles_per_jet) {
     extern __shared__ __align__(16) float smem[];
     if (meta[0]) return;
     const int b = blockIdx.x / tiles_per_jet, qt = blockIdx.x - b * tiles_per_jet;
     const int n = jet_n[b];
     const int start = jet_start[b];
     if (n < -1) {                             // offending ragged jet: owns -n rows; only the particle -> jet map is needed
-        for (int r = qt * KNN_THREADS + threadIdx.x; r < -n; r += tiles_per_jet * KNN_THREADS) pjet[start + r] = b;
+        for (int r = qt * KNN_THREADS + threadIdx.x; r < -n; r += tiles_per_jet * KNN_THREADS) pjet[start + r] = make_int2(start, n);
         return;
     }
     if (n <= 0) return;                       // empty jet (or offending padded jet, which owns no rows)
@@ -78,7 +78,7 @@ knn_dist_kernel(const float* __restrict__ space, int D, const int32_t* __restric
     const int gpc = min(nG, 256 / nG);
     const int q0 = qt * 4 * gpc;
     if (q0 >= n) return;
-    if ((int)threadIdx.x < 4 * gpc && q0 + (int)threadIdx.x < n) pjet[start + q0 + threadIdx.x] = b;
+    if ((int)threadIdx.x < 4 * gpc && q0 + (int)threadIdx.x < n) pjet[start + q0 + threadIdx.x] = make_int2(start, n);
     float* S0 = smem;                         // [2][n4][KNN_LD] double-buffered chunk of dimensions of every row of the jet
     float* Dm = dm + (size_t)(start + q0) * pld;  // rows of this tile's queries in the global distance matrix
     const float* src = space + (size_t)start * D;
@@ -185,15 +185,15 @@ constexpr int KSEL_THREADS = 128;
 // `space` with the arithmetic of knn_dist_kernel (t = s_i - s_j, d = fma(t, t, d) in index order), so both give the same bits.
 template <int K, typename KEY, bool FLY>
 __global__ void __launch_bounds__(KSEL_THREADS)
-knn_select_kernel(const float* __restrict__ dm, int pld, const float* __restrict__ space, int D, int k, const int32_t* __restrict__ pjet, const int32_t* __restrict__ jet_start,
+knn_select_kernel(const float* __restrict__ dm, int pld, const float* __restrict__ space, int D, int k, const int2* __restrict__ pjet, const int32_t* __restrict__ jet_start,
                   const int32_t* __restrict__ jet_n, const int32_t* __restrict__ meta, int32_t* __restrict__ idx_out,
                   int local_out) {
     if (meta[0]) return;
     const int t = blockIdx.x * KSEL_THREADS + threadIdx.x;
     const int q = t >> 1, half = t & 1;
     if (q >= meta[1]) return;                                   // both lanes of a pair leave together
-    const int lo = __ldg(pjet + q);                             // the jet that owns row q (written by knn_dist_kernel)
-    const int n = jet_n[lo], start = jet_start[lo];
+    const int2 pi = __ldg(pjet + q);                            // (start, n) of the jet that owns row q, written with the distances
+    const int n = pi.y, start = pi.x;
     int32_t* out = idx_out + (size_t)q * k;
     if (n < 0) {                              // offending ragged jet (jet_n = -multiplicity): its packed rows exist and the
         for (int m = half; m < k; m += 2) out[m] = -1;            // point-tiled EdgeConv walks them: no neighbours
@@ -220,12 +220,18 @@ knn_select_kernel(const float* __restrict__ dm, int pld, const float* __restrict
     // in registers (a sorted insert costs ~100 instructions, the whole K = 16 network ~500); later ones are inserted
     typedef typename KEY::T KT;
     KT best[K];
+    float dn[8];                              // the eight candidates after the first K ride the same round trip to memory
     {
         float d[K];
 #pragma unroll
         for (int u = 0; u < K; ++u) {
             const int j = half + 2 * u;
             d[u] = (j < n) ? dist(j) : 0.0f;
+        }
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            const int j = half + 2 * (K + u);
+            dn[u] = (j < n) ? dist(j) : 0.0f;
         }
 #pragma unroll
         for (int u = 0; u < K; ++u) {
@@ -248,7 +254,14 @@ knn_select_kernel(const float* __restrict__ dm, int pld, const float* __restrict
                     best[o] = sw ? a : c;
                 }
             }
-    int j = half + 2 * K;
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+        const int j = half + 2 * (K + u);
+        if (j >= n || j == i) continue;
+        const KT key = KEY::make(dn[u], j);
+        if (key < best[K - 1]) topk_insert<K, KT>(best, key);
+    }
+    int j = half + 2 * (K + 8);
     for (; j + 14 < n; j += 16) {             // eight loads in flight per thread
         float d[8];
 #pragma unroll
@@ -299,13 +312,13 @@ knn_select_kernel(const float* __restrict__ dm, int pld, const float* __restrict
 
 // particle -> jet map for the on-the-fly selection: one thread per jet writes its rows (offending ragged jets own rows too)
 __global__ void pjet_kernel(int B, const int32_t* __restrict__ jet_start, const int32_t* __restrict__ jet_n,
-                            const int32_t* __restrict__ meta, int32_t* __restrict__ pjet) {
+                            const int32_t* __restrict__ meta, int2* __restrict__ pjet) {
     if (meta[0]) return;
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= B) return;
     const int n = jet_n[b], start = jet_start[b];
     const int rows = n < -1 ? -n : (n > 0 ? n : 0);
-    for (int r = 0; r < rows; ++r) pjet[start + r] = b;
+    for (int r = 0; r < rows; ++r) pjet[start + r] = make_int2(start, n);
 }
 
 size_t knn_smem_bytes(int P) {

@@ -28,7 +28,7 @@ struct KnnTcCfg {
 template <int D>
 __global__ void __launch_bounds__(KTC_THREADS)
 knn_gram_kernel(const float* __restrict__ space, const int32_t* __restrict__ jet_start, const int32_t* __restrict__ jet_n,
-                const int32_t* __restrict__ meta, float* __restrict__ dm, int pld, int32_t* __restrict__ pjet) {
+                const int32_t* __restrict__ meta, float* __restrict__ dm, int pld, int2* __restrict__ pjet) {
     using Cfg = KnnTcCfg<D>;
     constexpr int KBD = Cfg::KBD;
     extern __shared__ __align__(1024) uint8_t smem_raw[];
@@ -38,7 +38,7 @@ knn_gram_kernel(const float* __restrict__ space, const int32_t* __restrict__ jet
     const int start = jet_start[b];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     if (n < -1) {                             // offending ragged jet: owns -n rows; only the particle -> jet map is needed
-        for (int r = tid; r < -n; r += KTC_THREADS) pjet[start + r] = b;
+        for (int r = tid; r < -n; r += KTC_THREADS) pjet[start + r] = make_int2(start, n);
         return;
     }
     if (n <= 0) return;
@@ -51,7 +51,7 @@ knn_gram_kernel(const float* __restrict__ space, const int32_t* __restrict__ jet
     uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(bars + 2);
     if (tid == 0) { mbar_init(d_full, 1); fence_mbar_init(); }
     if (warp == 4) tmem_alloc(tmem_ptr, 128);
-    if (tid < n) pjet[start + tid] = b;
+    if (tid < n) pjet[start + tid] = make_int2(start, n);
     const float* src = space + (size_t)start * D;
     // (1) the jet's rows, raw fp32, into the tile buffer with ONE round trip to memory: 16-byte cp.async per (row, chunk),
     //     all in flight (x of the previous block has usually left L2 by now: a dependent walk costs ~1 us per step)
