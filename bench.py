@@ -49,6 +49,7 @@ def parse_args():
     p.add_argument("--batch", type=int, default=1024)
     p.add_argument("--no-cpu-baseline", action="store_true")
     p.add_argument("--no-extras", action="store_true", help="skip the e2e / latency / cpu_baseline legs (profiling runs)")
+    p.add_argument("--no-l2-flush", action="store_true", help="diagnostic: do not evict L2 between steps (says so in config.l2)")
     return p.parse_args()
 
 
@@ -318,7 +319,8 @@ def run_ours(args):
     wall0 = time.perf_counter()
     for i in range(args.steps):
         f, c, o = dbat[i % N_BATCHES]
-        flush.zero_()                               # outside the timed events: evicts the previous step from L2
+        if not args.no_l2_flush:
+            flush.zero_()                           # outside the timed events: evicts the previous step from L2
         ev[i][0].record(stream)
         model.infer(f, c, o, logits=logits)
         ev[i][1].record(stream)
@@ -369,7 +371,8 @@ def run_ours(args):
         "config": {"workload": WORKLOAD, "batch_jets": B, "particles_per_batch": [int(b.n_particles) for b in batches],
                    "entry": "gnn_infer (ragged, device-resident)", "precision": args.precision,
                    "parallelism": "replicas only (jets sharded, no collective)" if world > 1 else "1 GPU",
-                   "l2": "flushed between steps (256 MiB memset outside the per-step CUDA events); %d batches rotate" % N_BATCHES},
+                   "l2": ("NOT flushed (diagnostic run); %d batches rotate" if args.no_l2_flush else
+                          "flushed between steps (256 MiB memset outside the per-step CUDA events); %d batches rotate") % N_BATCHES},
         "roofline": roofline, "forward": fwd, "stages_ms": {k: v for k, v in stages},
         "gpu_launches": int(launches), "wall_s_timed_region": wall,
     }

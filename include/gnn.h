@@ -110,6 +110,8 @@ int gnn_infer_slice(gnn_model* m, int32_t slice, const float* feats_dev, const f
  * more than max_particles real particles raises GNN_ERR_JET_TOO_LARGE.  B*P <= max_batch_jets * GNN_MAX_PARTICLES. */
 int gnn_infer_padded(gnn_model* m, const float* feats_dev, const float* coords_dev, const float* mask_dev,
                      int32_t B, int32_t P, float* logits_dev, void* cuda_stream);
+int gnn_infer_padded_slice(gnn_model* m, int32_t slice, const float* feats_dev, const float* coords_dev,
+                           const float* mask_dev, int32_t B, int32_t P, float* logits_dev, void* cuda_stream);
 
 /* Synchronises `cuda_stream`, returns and clears the sticky device status of `slice` (GNN_OK, GNN_ERR_BAD_OFFSETS,
  * GNN_ERR_JET_TOO_LARGE, or GNN_ERR_CUDA if the stream reports an error). */
@@ -146,6 +148,12 @@ int gnn_debug_knn(gnn_model* m, const float* space_dev, int32_t D, const int32_t
  * in the model's precision mode. */
 int gnn_debug_edgeconv(gnn_model* m, int32_t block, const float* x_dev, const int32_t* idx_dev,
                        const int32_t* offsets_dev, int32_t B, int32_t N, float* y_dev, void* cuda_stream);
+/* GNN_BF16, k = 16, C_last <= 256 only (else GNN_ERR_BAD_ARG): the LAST EdgeConv block with the pooling epilogue the
+ * forward uses in that mode (block output never stored; per-jet channel sums accumulated as exact 2^-32 fixed-point
+ * integers): x_dev [N, C_in of the last block], jet-local idx_dev [N, k] -> g_dev [B, C_last] = mean over the jet's
+ * particles of the block output (0 for an empty jet) = the input of the FC head. */
+int gnn_debug_edgeconv_pool(gnn_model* m, const float* x_dev, const int32_t* idx_dev, const int32_t* offsets_dev,
+                            int32_t B, int32_t N, float* g_dev, void* cuda_stream);
 /* masked global average pool + FC head: x_dev [N, C_last] -> logits_dev [B, n_classes] */
 int gnn_debug_pool_head(gnn_model* m, const float* x_dev, const int32_t* offsets_dev, int32_t B, int32_t N,
                         float* logits_dev, void* cuda_stream);

@@ -48,6 +48,7 @@ def lib():
         L.gnn_infer.argtypes = [vp, f32p, f32p, i32p, i32, i32, f32p, vp]
         L.gnn_infer_slice.argtypes = [vp, i32, f32p, f32p, i32p, i32, i32, f32p, vp]
         L.gnn_infer_padded.argtypes = [vp, f32p, f32p, f32p, i32, i32, f32p, vp]
+        L.gnn_infer_padded_slice.argtypes = [vp, i32, f32p, f32p, f32p, i32, i32, f32p, vp]
         L.gnn_status_check.argtypes = [vp, i32, vp]
         L.gnn_infer_host.argtypes = [vp, i32, vp, vp, vp, i32, i32, vp, vp]
         L.gnn_profile_enable.argtypes = [vp, i32, i32]
@@ -58,6 +59,7 @@ def lib():
         L.gnn_debug_knn.argtypes = [vp, f32p, i32, i32p, i32, i32, i32, i32p, vp]
         L.gnn_debug_edgeconv.argtypes = [vp, i32, f32p, i32p, i32p, i32, i32, f32p, vp]
         L.gnn_debug_pool_head.argtypes = [vp, f32p, i32p, i32, i32, f32p, vp]
+        L.gnn_debug_edgeconv_pool.argtypes = [vp, f32p, i32p, i32p, i32, i32, f32p, vp]
         L.gnn_batcher_create.argtypes = [vp, C.POINTER(BatcherOpts), C.POINTER(vp)]
         L.gnn_batcher_submit.argtypes = [vp, vp, vp, vp, i32, vp, C.POINTER(Ticket)]
         L.gnn_batcher_wait.argtypes = [vp, Ticket, C.c_int64, C.POINTER(C.c_double), C.POINTER(C.c_double)]
@@ -149,13 +151,13 @@ class Model:
                                           _stream(stream)), "gnn_infer")
         return logits
 
-    def infer_padded(self, feats, coords, mask, logits=None, stream=None):
+    def infer_padded(self, feats, coords, mask, logits=None, stream=None, slice=0):
         import torch
         B, P = mask.shape
         if logits is None:
             logits = torch.empty((B, self.arch.n_classes), dtype=torch.float32, device=mask.device)
-        self._check(lib().gnn_infer_padded(self.h, _ptr(feats), _ptr(coords), _ptr(mask), B, P, _ptr(logits),
-                                           _stream(stream)), "gnn_infer_padded")
+        self._check(lib().gnn_infer_padded_slice(self.h, slice, _ptr(feats), _ptr(coords), _ptr(mask), B, P, _ptr(logits),
+                                                 _stream(stream)), "gnn_infer_padded")
         return logits
 
     def infer_host(self, feats, coords, offsets, logits, stream=None, slice=0):
@@ -198,6 +200,15 @@ class Model:
         self._check(lib().gnn_debug_edgeconv(self.h, block, _ptr(x), _ptr(idx), _ptr(offsets), offsets.numel() - 1, N,
                                              _ptr(y), _stream(stream)), "gnn_debug_edgeconv")
         return y
+
+    def debug_edgeconv_pool(self, x, idx, offsets, stream=None):
+        import torch
+        B = offsets.numel() - 1
+        C_last = self.arch.channels[self.arch.n_blocks - 1][2]
+        g = torch.empty((B, C_last), dtype=torch.float32, device=x.device)
+        self._check(lib().gnn_debug_edgeconv_pool(self.h, _ptr(x), _ptr(idx), _ptr(offsets), B, x.shape[0], _ptr(g),
+                                                  _stream(stream)), "gnn_debug_edgeconv_pool")
+        return g
 
     def debug_pool_head(self, x, offsets, stream=None):
         import torch

@@ -30,7 +30,7 @@ def needs_build():
 def build(force=False, verbose=False):
     if not force and not needs_build():
         return LIB
-    flags = [f for f in FLAGS if not f.startswith("--use_fast_math")]
+    flags = [f for f in FLAGS if not f.startswith("--use_fast_math")] + os.environ.get("GNN_NVCC_DEFS", "").split()
     objs = []
     os.makedirs(os.path.join(HERE, "build"), exist_ok=True)
     procs = []

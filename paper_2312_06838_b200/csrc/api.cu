@@ -2,6 +2,7 @@
 // launch plan of one forward pass.  Host code only enqueues kernels; every step of the path runs on the GPU.
 #include "gnn_internal.h"
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -12,6 +13,7 @@ int launch_edgeconv_bf16(gnn_model& m, int block, const float* x, const int32_t*
                          cudaStream_t s);
 int launch_pre_bf16(gnn_model& m, int block, const float* x, int N, Workspace& w, cudaStream_t s);
 int launch_edge_bf16(gnn_model& m, int block, const int32_t* idx, int N, float* y, Workspace& w, cudaStream_t s);
+bool edgeconv_bf16_can_pool(const gnn_model& m, int block);
 
 namespace {
 
@@ -137,17 +139,25 @@ int alloc_workspace(gnn_model* m, Workspace& w) {
     if ((rc = dev_alloc(m, &w.jet_start, Bmax)) != GNN_OK) return rc;
     if ((rc = dev_alloc(m, &w.jet_n, Bmax)) != GNN_OK) return rc;
     if ((rc = dev_alloc(m, &w.status, 1)) != GNN_OK) return rc;
-    if ((rc = dev_alloc(m, &w.meta, 2)) != GNN_OK) return rc;
+    if ((rc = dev_alloc(m, &w.meta, 4)) != GNN_OK) return rc;
+    if ((rc = dev_alloc(m, &w.groups, Bmax)) != GNN_OK) return rc;
+    if ((rc = dev_alloc(m, &w.pjid, Nmax)) != GNN_OK) return rc;
+    if ((rc = dev_alloc(m, &w.pool, Bmax * (size_t)a.channels[a.n_blocks - 1][2])) != GNN_OK) return rc;
     if ((rc = dev_alloc(m, &w.pfeats, Nmax * a.in_features)) != GNN_OK) return rc;
     if ((rc = dev_alloc(m, &w.pcoords, Nmax * a.coord_dims)) != GNN_OK) return rc;
     if ((rc = dev_alloc(m, &w.poffsets, Bmax + 1)) != GNN_OK) return rc;
     if ((rc = dev_alloc(m, &w.pcounts, Bmax)) != GNN_OK) return rc;
     if ((rc = dev_alloc(m, &w.hlogits, Bmax * a.n_classes)) != GNN_OK) return rc;
-    GNN_CUDA_TRY(cudaStreamCreateWithFlags(&w.aux, cudaStreamNonBlocking));
+    // the auxiliary stream carries the per-particle pre kernels, which must reach the SMs BEFORE the kNN CTAs of the caller's
+    // stream (one pre CTA per SM, kNN CTAs in the room that is left; the other way round the kNN CTAs fill every SM and the
+    // two kernels run one after the other): highest priority, which the block scheduler honours between ready grids
+    int prio_lo = 0, prio_hi = 0;
+    GNN_CUDA_TRY(cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi));
+    GNN_CUDA_TRY(cudaStreamCreateWithPriority(&w.aux, cudaStreamNonBlocking, prio_hi));
     GNN_CUDA_TRY(cudaEventCreateWithFlags(&w.ev_x, cudaEventDisableTiming));
     GNN_CUDA_TRY(cudaEventCreateWithFlags(&w.ev_pre, cudaEventDisableTiming));
     GNN_CUDA_TRY(cudaMemset(w.status, 0, sizeof(unsigned)));
-    GNN_CUDA_TRY(cudaMemset(w.meta, 0, 2 * sizeof(int32_t)));
+    GNN_CUDA_TRY(cudaMemset(w.meta, 0, 4 * sizeof(int32_t)));
     return GNN_OK;
 }
 
@@ -186,26 +196,44 @@ int forward(gnn_model* m, Workspace& w, const float* feats, const float* coords,
     tm.mark("ingest");
     const float* x = feats;
     float* bufs[2] = {w.xa, w.xb};
+    const bool bf16 = a.precision == GNN_BF16;
+    static const bool no_fork = std::getenv("GNN_NO_FORK") != nullptr;           // developer knob: everything on one stream
+    const bool fork = bf16 && !no_fork && w.aux != nullptr;
+    // bf16 mode: the last block adds its output straight into the per-jet channel sums (step a7 inside E3 of step a6)
+    static const bool no_fuse = std::getenv("GNN_NO_POOL_FUSE") != nullptr;     // developer knob: A/B of the pooling epilogue
+    const bool fuse_pool = bf16 && !no_fuse && edgeconv_bf16_can_pool(*m, a.n_blocks - 1);
     for (int l = 0; l < a.n_blocks; ++l) {
         const float* space = (l == 0) ? coords : x;
         int D = (l == 0) ? a.coord_dims : block_in(a, l);
-        float* y = bufs[l & 1];
-        const bool fork = a.precision == GNN_BF16 && w.aux != nullptr;
-        if (fork && (cudaEventRecord(w.ev_x, s) != cudaSuccess || cudaStreamWaitEvent(w.aux, w.ev_x, 0) != cudaSuccess)) return GNN_ERR_CUDA;
-        if ((rc = launch_knn(space, D, a.k, B, a.max_particles, w, w.idx, 0, a.precision == GNN_BF16 ? 1 : 0, s)) < 0) return rc;
-        n += rc;
-        tm.mark("knn", l);
-        if (fork) {                         // u, v, shortcut of this block depend on x only: beside the kNN, on the aux stream
-            // (enqueued after the kNN kernels so that the short distance kernel gets the SMs first and the pre kernel,
-            // which fills every SM's shared memory, runs beside the selection kernel, which uses none)
-            if ((rc = launch_pre_bf16(*m, l, x, N_upper, w, w.aux)) < 0) return rc;
-            n += rc;
-            if (cudaEventRecord(w.ev_pre, w.aux) != cudaSuccess) return GNN_ERR_CUDA;
-        }
+        float* y = (fuse_pool && l == a.n_blocks - 1) ? nullptr : bufs[l & 1];
+        // bf16 mode: u, v, shortcut of this block depend on x only, so the per-particle pre kernel runs beside the kNN of the
+        // block on the slice's auxiliary stream (fork: aux waits for x; join: `s` waits for the pre kernel before the edge
+        // kernel).  The join is enqueued on every path out of the fork, error or not, so aux never outlives the call.
+        int rc_pre = 0;
+        bool joined = true;
         if (fork) {
-            if (cudaStreamWaitEvent(s, w.ev_pre, 0) != cudaSuccess) return GNN_ERR_CUDA;
-            rc = launch_edge_bf16(*m, l, w.idx, N_upper, y, w, s);
-        } else if (a.precision == GNN_BF16) rc = launch_edgeconv_bf16(*m, l, x, w.idx, N_upper, y, w, s);
+            if (cudaEventRecord(w.ev_x, s) != cudaSuccess || cudaStreamWaitEvent(w.aux, w.ev_x, 0) != cudaSuccess) return GNN_ERR_CUDA;
+            rc_pre = launch_pre_bf16(*m, l, x, N_upper, w, w.aux);
+            joined = cudaEventRecord(w.ev_pre, w.aux) == cudaSuccess;
+            // the per-jet channel sums are zeroed behind the first pre kernel on the auxiliary stream: off the critical path
+            // (it runs under the first edge kernel) and ordered before the last block by the later forks / joins.  The fork
+            // above also orders it after everything already enqueued on `s` (an earlier forward reading the sums).
+            if (fuse_pool && l == 0 && a.n_blocks > 1 &&
+                cudaMemsetAsync(w.pool, 0, (size_t)B * a.channels[a.n_blocks - 1][2] * sizeof(unsigned long long), w.aux) != cudaSuccess)
+                joined = false;
+        }
+        if (fuse_pool && l == 0 && a.n_blocks == 1 &&          // a single block: nothing to hide it under
+            cudaMemsetAsync(w.pool, 0, (size_t)B * a.channels[0][2] * sizeof(unsigned long long), s) != cudaSuccess)
+            return GNN_ERR_CUDA;
+        const int rc_knn = launch_knn(space, D, a.k, B, a.max_particles, w, w.idx, 0, bf16 ? 1 : 0, s);
+        if (fork) joined = joined && cudaStreamWaitEvent(s, w.ev_pre, 0) == cudaSuccess;
+        if (rc_pre < 0) return rc_pre;
+        if (rc_knn < 0) return rc_knn;
+        if (!joined) return GNN_ERR_CUDA;
+        n += rc_pre + rc_knn;
+        tm.mark("knn", l);
+        if (fork) rc = launch_edge_bf16(*m, l, w.idx, N_upper, y, w, s);
+        else if (bf16) rc = launch_edgeconv_bf16(*m, l, x, w.idx, N_upper, y, w, s);
         else rc = launch_edgeconv_f32(m->blocks[l], a.k, x, w.idx, N_upper, y, w, s);
         if (rc < 0) return rc;
         n += rc;
@@ -258,7 +286,7 @@ int gnn_create(const void* weights_host, size_t bytes, const gnn_arch* arch, int
     m->Nmax = (int64_t)arch->max_batch_jets * arch->max_particles;
     m->Cmax = 8;
     for (int l = 0; l < arch->n_blocks; ++l) m->Cmax = std::max(m->Cmax, arch->channels[l][2]);
-    if ((rc = knn_configure()) != GNN_OK || (rc = pool_head_configure()) != GNN_OK || (rc = knn_tc_configure()) != GNN_OK || (rc = edgeconv_f32_configure()) != GNN_OK ||
+    if ((rc = knn_configure()) != GNN_OK || (rc = pool_head_configure()) != GNN_OK || (rc = knn_group_configure()) != GNN_OK || (rc = edgeconv_f32_configure()) != GNN_OK ||
         (rc = build_model(m, static_cast<const float*>(weights_host))) != GNN_OK) {
         gnn_destroy(m);
         return rc;
@@ -308,15 +336,16 @@ int gnn_infer(gnn_model* m, const float* feats_dev, const float* coords_dev, con
     return gnn_infer_slice(m, 0, feats_dev, coords_dev, offsets_dev, B, N, logits_dev, cuda_stream);
 }
 
-int gnn_infer_padded(gnn_model* m, const float* feats_dev, const float* coords_dev, const float* mask_dev, int32_t B,
-                     int32_t P, float* logits_dev, void* cuda_stream) {
+int gnn_infer_padded_slice(gnn_model* m, int32_t slice, const float* feats_dev, const float* coords_dev, const float* mask_dev,
+                           int32_t B, int32_t P, float* logits_dev, void* cuda_stream) {
     if (!m) return GNN_ERR_NULL;
     if (B < 0 || P < 0) return GNN_ERR_BAD_ARG;
+    if (slice < 0 || slice >= (int)m->ws.size()) return GNN_ERR_BATCH_TOO_LARGE;
     if (B > m->arch.max_batch_jets || (int64_t)B * P > (int64_t)m->arch.max_batch_jets * GNN_MAX_PARTICLES)
         return GNN_ERR_BATCH_TOO_LARGE;
     if (B == 0) return GNN_OK;
     if (!logits_dev || (P > 0 && (!feats_dev || !coords_dev || !mask_dev))) return GNN_ERR_NULL;
-    Workspace& w = m->ws[0];
+    Workspace& w = m->ws[slice];
     cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
     int rc = launch_compact_padded(feats_dev, coords_dev, mask_dev, B, P, m->arch.in_features, m->arch.coord_dims,
                                    m->arch.max_particles, w, s);
@@ -324,6 +353,11 @@ int gnn_infer_padded(gnn_model* m, const float* feats_dev, const float* coords_d
     m->launches.fetch_add(rc, std::memory_order_relaxed);
     int64_t upper = std::min<int64_t>((int64_t)B * std::min<int>(P, m->arch.max_particles), m->Nmax);
     return forward(m, w, w.pfeats, w.pcoords, w.poffsets, w.pcounts, B, -1, (int)upper, logits_dev, s);
+}
+
+int gnn_infer_padded(gnn_model* m, const float* feats_dev, const float* coords_dev, const float* mask_dev, int32_t B,
+                     int32_t P, float* logits_dev, void* cuda_stream) {
+    return gnn_infer_padded_slice(m, 0, feats_dev, coords_dev, mask_dev, B, P, logits_dev, cuda_stream);
 }
 
 int gnn_infer_host(gnn_model* m, int32_t slice, const float* feats_host, const float* coords_host,
@@ -445,7 +479,8 @@ int gnn_debug_knn(gnn_model* m, const float* space_dev, int32_t D, const int32_t
     int n = 0, rc;
     if ((rc = launch_ingest(offsets_dev, nullptr, B, N, (int)m->Nmax, m->arch.max_particles, w, s)) < 0) return rc;
     n += rc;
-    if ((rc = launch_knn(space_dev, D, k, B, m->arch.max_particles, w, idx_dev, 1, 0, s)) < 0) return rc;
+    // a GNN_BF16 model runs what its forward runs (grouped kernels: Gram distances for D = 64 / 128 / 256, 32-bit keys)
+    if ((rc = launch_knn(space_dev, D, k, B, m->arch.max_particles, w, idx_dev, 1, m->arch.precision == GNN_BF16 ? 1 : 0, s)) < 0) return rc;
     n += rc;
     m->launches.fetch_add(n, std::memory_order_relaxed);
     return cudaGetLastError() == cudaSuccess ? GNN_OK : GNN_ERR_CUDA;
@@ -468,6 +503,36 @@ int gnn_debug_edgeconv(gnn_model* m, int32_t block, const float* x_dev, const in
     if (m->arch.precision == GNN_BF16) rc = launch_edgeconv_bf16(*m, block, x_dev, w.idx, N, y_dev, w, s);
     else rc = launch_edgeconv_f32(m->blocks[block], m->arch.k, x_dev, w.idx, N, y_dev, w, s);
     if (rc < 0) return rc;
+    n += rc;
+    m->launches.fetch_add(n, std::memory_order_relaxed);
+    return cudaGetLastError() == cudaSuccess ? GNN_OK : GNN_ERR_CUDA;
+}
+
+int gnn_debug_edgeconv_pool(gnn_model* m, const float* x_dev, const int32_t* idx_dev, const int32_t* offsets_dev, int32_t B,
+                            int32_t N, float* g_dev, void* cuda_stream) {
+    if (!m) return GNN_ERR_NULL;
+    if (B < 0 || N < 0) return GNN_ERR_BAD_ARG;
+    if (B > m->arch.max_batch_jets || (int64_t)N > m->Nmax) return GNN_ERR_BATCH_TOO_LARGE;
+    const int block = m->arch.n_blocks - 1;
+    if (m->arch.precision != GNN_BF16 || !edgeconv_bf16_can_pool(*m, block)) return GNN_ERR_BAD_ARG;
+    if (B == 0) return GNN_OK;
+    if (!offsets_dev || !g_dev || (N > 0 && (!idx_dev || !x_dev))) return GNN_ERR_NULL;
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    Workspace& w = m->ws[0];
+    const int C = m->arch.channels[block][2];
+    int n = 0, rc;
+    if ((rc = launch_ingest(offsets_dev, nullptr, B, N, (int)m->Nmax, m->arch.max_particles, w, s)) < 0) return rc;
+    n += rc;
+    GNN_CUDA_TRY(cudaMemsetAsync(w.pool, 0, (size_t)B * C * sizeof(unsigned long long), s));
+    if (N > 0) {
+        if ((rc = launch_globalize_idx(idx_dev, m->arch.k, B, w, w.idx, s)) < 0) return rc;
+        n += rc;
+        if ((rc = launch_pre_bf16(*m, block, x_dev, N, w, s)) < 0) return rc;
+        n += rc;
+        if ((rc = launch_edge_bf16(*m, block, w.idx, N, nullptr, w, s)) < 0) return rc;
+        n += rc;
+    }
+    if ((rc = launch_pooled_mean(*m, B, w, g_dev, s)) < 0) return rc;
     n += rc;
     m->launches.fetch_add(n, std::memory_order_relaxed);
     return cudaGetLastError() == cudaSuccess ? GNN_OK : GNN_ERR_CUDA;

@@ -28,6 +28,7 @@
 #include "gnn_internal.h"
 #include "tc05.cuh"
 #include <cuda_bf16.h>
+#include <cstdlib>
 #include <cstring>
 
 namespace {
@@ -35,8 +36,18 @@ namespace {
 using namespace tc05;
 
 constexpr int TILE_ROWS = 128;
+// developer knobs (python -m paper_2312_06838_b200.build reads GNN_NVCC_DEFS): which widths run E2 / E3 on separate warp sets
+#ifndef EDGE_SPLIT_MASK
+#define EDGE_SPLIT_MASK 0
+#endif
+#ifndef EDGE_MAXREG_128
+#define EDGE_MAXREG_128 80
+#endif
 
-template <int C>
+// SPLIT_: E2 and E3 on separate warp sets with per-role register budgets (compiled for k = 16 only)
+__host__ __device__ constexpr bool edge_split(int C, int LOGK) { return (((EDGE_SPLIT_MASK) & C) != 0) && LOGK == 4; }
+
+template <int C, bool SPLIT_ = false>
 struct EdgeCfg {
     static constexpr bool PAIR = C >= 256;                    // CTA pair: the weights, split over two SMs, stay resident
     static constexpr int KB = (C + 63) / 64;                  // 64-wide K blocks per layer
@@ -46,11 +57,26 @@ struct EdgeCfg {
     static constexpr int GH = 2;                              // row parts of the gather
     static constexpr int NG = GH * KB;                        // gather warps: K block g % KB, row part g / KB
     static constexpr int RW = TILE_ROWS / GH;                 // rows per gather warp
-    static constexpr bool SPLIT = false;                        // E2 and E3 on separate warp sets: E2(t+1) need not wait for E3(t)
+    static constexpr bool SPLIT = SPLIT_;                      // E2 and E3 on separate warp sets: E2(t+1) need not wait for E3(t)
     static constexpr int NEP = SPLIT ? 2 * NE : NE;           // epilogue warps in total: [0, NE) run E2, [NE, 2 NE) run E3
     static constexpr int MMA_WARP = NEP + NG;
-    static constexpr int THREADS = 32 * (NEP + NG + 1);
-    static constexpr int MAXREG = C >= 256 ? 96 : (C >= 128 ? 80 : 64);   // registers are per SM quarter: ceil(warps / 4) * 32 * MAXREG * MIN_CTAS <= 16384
+    // SPLIT: the roles get different register budgets (setmaxnreg, per warpgroup of four warps), so every role starts on a
+    // warpgroup boundary and the MMA warp brings three idle warps along
+    static constexpr int THREADS = SPLIT ? 32 * (NEP + NG + 4) : 32 * (NEP + NG + 1);
+    static constexpr int MAXREG = SPLIT ? (C >= 256 ? 72 : 64)  // SPLIT: registers at launch (THREADS * MAXREG * MIN_CTAS <= 65536)
+                                        : (C >= 256 ? 96 : (C >= 128 ? (EDGE_MAXREG_128) : 64));   // registers are per SM quarter: ceil(warps / 4) * 32 * MAXREG * MIN_CTAS <= 16384
+    // SPLIT register budgets per role (sum over the warps <= THREADS * MAXREG): gather, MMA warpgroup, E2, E3
+#ifndef RGG
+#define RGG (C >= 256 ? 56 : 48)
+#define RGM (C >= 256 ? 40 : 32)
+#define RGE2 64
+#define RGE3 112
+#endif
+    static constexpr int RG_G = RGG, RG_MMA = RGM, RG_E2 = RGE2, RG_E3 = RGE3;
+    static_assert(!SPLIT || (NE % 4 == 0 && NG % 4 == 0), "SPLIT needs warpgroup-aligned roles");
+#ifndef RG_NOCHECK
+    static_assert(!SPLIT || 32 * (NG * RG_G + 4 * RG_MMA + NE * RG_E2 + NE * RG_E3) <= THREADS * MAXREG, "SPLIT register budget");
+#endif
     static constexpr int KSTEPS_LAST = ((C - (KB - 1) * 64) + 15) / 16;
     static constexpr int NRB = PAIR ? C / 2 : C;              // weight rows (output channels) one CTA holds
     static constexpr int CHUNK_BYTES = NRB * 128;             // [NRB][64] bf16, 128B-swizzled
@@ -61,6 +87,9 @@ struct EdgeCfg {
     static constexpr int NBAR = 3 * KB + 6;
     static constexpr int SMALL_BYTES = 2 * C * 4 + NBAR * 8 + 16;
     static constexpr int SMEM_BYTES = W_BYTES + H_BYTES + SMALL_BYTES + 1024;
+    // POOL variant (last block, k = 16): per epilogue warp and 32-column slab, two 64-bit fixed-point accumulators per lane
+    static constexpr int POOL_BYTES = NE * (CWE / 32) * 32 * 16;
+    static constexpr int SMEM_BYTES_POOL = SMEM_BYTES + POOL_BYTES;
     static constexpr int MIN_CTAS = C >= 256 ? 1 : (C >= 128 ? 2 : 4);
     static constexpr int NRANKS = PAIR ? 2 : 1;
     // shift pre-loaded into the accumulators (tcgen05.st by the epilogue that drains them) or added in the epilogues: the
@@ -68,22 +97,46 @@ struct EdgeCfg {
     static constexpr bool BIAS_ACC = false;
 };
 
+// y >= 0 (post-ReLU) -> unsigned 32.32 fixed point, EXACT for y < 2^32 whose ulp is >= 2^-32 (y >= 2^-8; below that the
+// bits under 2^-32 are cut: an absolute error < 2.4e-10 per addend): integer part by truncation, fraction y - floor(y) (exact
+// in fp32, at most 24 significant bits, so frac * 2^32 is an integer below 2^32).  Two 32-bit conversions: the 64-bit
+// conversion instructions are far slower.  y >= 2^32 saturates the integer part; NaN converts to 0.
+__device__ __forceinline__ unsigned long long to_fixed_32_32(float y) {
+    const unsigned hi = __float2uint_rz(y);
+    const unsigned lo = __float2uint_rz((y - __uint2float_rz(hi)) * 4294967296.0f);
+    return ((unsigned long long)hi << 32) | lo;
+}
+
 struct EdgeParams {
     const __nv_bfloat16* U;      // [N, C]
     const __nv_bfloat16* V;      // [N, C]
     const float* R;              // [N, C] shortcut
     const int32_t* idx;          // [N, k] global neighbour rows, -1 = none
-    float* y;                    // [N, C]
+    float* y;                    // [N, C] (null in the POOL variant)
+    const int32_t* pjid;         // POOL: [N] particle -> jet
+    unsigned long long* pool;    // POOL: [B, C] per-jet channel sums of the block output, 2^-32 fixed point (pre-zeroed)
     const int32_t* meta;         // meta[0] poisoned batch, meta[1] = N
     const uint8_t* wimg;         // per CTA rank: 2*KB chunk images in consumption order
     const float* shifts;         // [t2 | t3]
     int k, logk, TP, n_tiles;
+    int chunk;                   // consecutive (pair) tiles a unit takes at a time
 };
 
 // LOGK >= 0: k = 2^LOGK known at compile time (lets the gather keep one u chunk per particle in registers); -1: runtime
-template <int C, int LOGK>
-__global__ void __launch_bounds__(EdgeCfg<C>::THREADS) __maxnreg__(EdgeCfg<C>::MAXREG) edge_kernel(EdgeParams p) {
-    using Cfg = EdgeCfg<C>;
+// POOL (last block, LOGK = 4 only): the block output is not stored; E3 adds it into the per-jet channel sums of step a7
+// (masked global average pool) instead.  Sums are exact: every value is converted to 2^-32 fixed point first and added as a
+// 64-bit integer (per-lane accumulators in shared memory across the consecutive tiles of a jet, one red.global.add.u64
+// per (lane, column) when the jet changes), so the result does not depend on tile boundaries, CTA assignment or the
+// order of the atomics: batch-composition invariance stays bitwise.
+template <int N>
+__device__ __forceinline__ void setmaxnreg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
+template <int N>
+__device__ __forceinline__ void setmaxnreg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
+
+template <int C, int LOGK, bool POOL>
+__device__ __forceinline__ void edge_body(const EdgeParams& p) {
+    static_assert(!POOL || LOGK == 4, "the pooling epilogue is written for k = 16");
+    using Cfg = EdgeCfg<C, edge_split(C, LOGK)>;
     constexpr bool PAIR = Cfg::PAIR;
     constexpr int KB = Cfg::KB, NE = Cfg::NE, CWE = Cfg::CWE;
     extern __shared__ __align__(1024) uint8_t smem_raw[];
@@ -94,8 +147,15 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS) __maxnreg__(EdgeCfg<C>::M
     const int unit = PAIR ? (int)cluster_id_x() : (int)blockIdx.x;     // scheduling unit: a CTA or a CTA pair
     const int n_units = PAIR ? (int)gridDim.x / 2 : (int)gridDim.x;
     const int n_work = PAIR ? (n_tiles + 1) / 2 : n_tiles;              // (pair) tiles
-    if (unit >= n_work) return;                                  // uniform over the pair
-    const int T = (n_work - unit + n_units - 1) / n_units;       // (pair) tiles of this unit: unit, unit + n_units, ...
+    // a unit owns CHUNKS of p.chunk consecutive (pair) tiles, chunks dealt round-robin over the units: at any time the units
+    // work inside one window of the packed batch (the gathered rows of neighbouring tiles share L2 lines and DRAM pages),
+    // and inside a chunk consecutive tiles mostly belong to the same jet (the POOL epilogue keeps a jet's partial sums on
+    // chip across them).  Only the globally last chunk may be partial.
+    const int CH = p.chunk;
+    const int n_chunks = (n_work + CH - 1) / CH;
+    if (unit >= n_chunks) return;                                // uniform over the pair
+    const int owned = (n_chunks - unit + n_units - 1) / n_units;
+    const int T = owned * CH - (((n_chunks - 1) % n_units) == unit ? n_chunks * CH - n_work : 0);
     const int k = LOGK >= 0 ? (1 << LOGK) : p.k, logk = LOGK >= 0 ? LOGK : p.logk;
 
     // no pointer arithmetic through integers here: the compiler must keep the shared address space (STS/LDS, not generic
@@ -114,6 +174,7 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS) __maxnreg__(EdgeCfg<C>::M
     uint64_t* w_full = d_free + 2;            // weights of this CTA landed
     uint64_t* w_peer = w_full + 1;            // pair mode: the peer's weights landed (leader's copy is used)
     uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(w_peer + 1);
+    ulonglong2* pool_s = reinterpret_cast<ulonglong2*>(smem + ((Cfg::SMEM_BYTES - 1024 + 15) & ~15));   // POOL only
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     if (tid == 0) {
@@ -134,14 +195,23 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS) __maxnreg__(EdgeCfg<C>::M
     tc_fence_after();
     const uint32_t tmem = *tmem_ptr;
 
-    auto tile_p0 = [&](int t) { const int w = unit + t * n_units; return (PAIR ? 2 * w + (int)rank : w) * p.TP; };
+    auto tile_p0 = [&](int t) {
+        int w = unit + t * n_units;                              // CH = 1: round-robin
+        if (CH != 1) { const int kc = t / CH; w = (unit + kc * n_units) * CH + (t - kc * CH); }
+        return (PAIR ? 2 * w + (int)rank : w) * p.TP;
+    };
     auto arrive_leader = [&](uint64_t* bar) {
         __syncwarp();
         if (lane == 0) { if constexpr (PAIR) mbar_arrive_cluster(bar, 0); else mbar_arrive(bar); }
     };
 
-    if (warp == Cfg::MMA_WARP) {
+    // SPLIT: register budgets per role, set at the top of each (warpgroup-uniform) role branch so that the code a budget
+    // governs is exactly the code the setmaxnreg dominates: the E3 warps, whose row reduction is the longest serial piece of
+    // a tile, get what the gather, E2 and MMA warps give back
+    if (warp >= Cfg::MMA_WARP) {
+        if constexpr (Cfg::SPLIT) setmaxnreg_dec<Cfg::RG_MMA>();   // (the three idle warps of this warpgroup fall through)
         // ===== weight load (every chunk once, resident for the life of the CTA), then MMA issuer (leader CTA of a pair) ====
+        if (warp == Cfg::MMA_WARP) {
         if (lane == 0) {
             mbar_arrive_expect_tx(w_full, Cfg::W_BYTES);
             const uint8_t* src = p.wimg + (size_t)rank * Cfg::W_BYTES;
@@ -174,7 +244,9 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS) __maxnreg__(EdgeCfg<C>::M
                 }
             }
         }
+        }
     } else if (warp >= Cfg::NEP) {
+        if constexpr (Cfg::SPLIT) setmaxnreg_dec<Cfg::RG_G>();
         // ===== gather warps: H1 = bf16(relu(u_i + v_j)) for K block gk, rows 64*half .. +63; they run one tile ahead of the
         // epilogue (their only dependency is h_free of the previous tile), so the L2 latency of the gather is off the
         // MMA <-> epilogue critical path ===============================================================================
@@ -263,6 +335,10 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS) __maxnreg__(EdgeCfg<C>::M
             for (int a = 0; a < NI; ++a) idx_r[a] = idx_n[a];
         }
     } else {
+        if constexpr (Cfg::SPLIT) {
+            if (warp < NE) { if constexpr (Cfg::RG_E2 < Cfg::MAXREG) setmaxnreg_dec<Cfg::RG_E2>(); }
+            else setmaxnreg_inc<Cfg::RG_E3>();
+        }
         // ===== epilogue warps: E2 (D0 -> H2) and E3 (D1 -> mean -> y) for lane quadrant q, columns [cg*CWE, +CWE) ==========
         const int q = warp & 3, cg = (warp % NE) >> 2;
         const bool doE2 = !Cfg::SPLIT || warp < NE, doE3 = !Cfg::SPLIT || warp >= NE;
@@ -303,6 +379,28 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS) __maxnreg__(EdgeCfg<C>::M
         if (doE2) reset_acc(0);
         if (doE3) reset_acc(1);
         int idx_cur = load_idx(tile_p0(0));
+        // POOL: this lane's accumulators (slab s -> columns col0 + 32 s + cb, + 1) of the jet `jid_acc` it is walking
+        ulonglong2* acc_s = pool_s + ((warp % NE) * SLABS) * 32 + lane;
+        int jid_acc = -1, jid_cur = -1;
+        auto pool_flush = [&]() {
+            if (jid_acc >= 0) {
+                unsigned long long* dst = p.pool + (size_t)jid_acc * C + col0 + cb;
+#pragma unroll
+                for (int s = 0; s < SLABS; ++s) {
+                    const ulonglong2 a = acc_s[s * 32];
+                    atomicAdd(dst + s * 32, a.x);
+                    atomicAdd(dst + s * 32 + 1, a.y);
+                }
+            }
+#pragma unroll
+            for (int s = 0; s < SLABS; ++s) acc_s[s * 32] = make_ulonglong2(0ull, 0ull);
+        };
+        if constexpr (POOL) {
+#pragma unroll
+            for (int s = 0; s < SLABS; ++s) acc_s[s * 32] = make_ulonglong2(0ull, 0ull);
+            const int pt0 = tile_p0(0) + (row >> logk);
+            jid_cur = pt0 < N ? __ldg(p.pjid + pt0) : -1;
+        }
         for (int t = 0; t < T; ++t) {
             const uint32_t ph = t & 1;
             const int p0 = tile_p0(t);
@@ -352,6 +450,11 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS) __maxnreg__(EdgeCfg<C>::M
             // (two columns per register): a halving butterfly over the k rows of a particle, fp32 again for the mean ------------
             if (doE3) {
             const int idx_next = (t + 1 < T) ? load_idx(tile_p0(t + 1)) : -1;
+            int jid_next = -1;
+            if constexpr (POOL) {
+                if (t + 1 < T) { const int ptn = tile_p0(t + 1) + (row >> logk); jid_next = ptn < N ? __ldg(p.pjid + ptn) : -1; }
+                if (jid_cur != jid_acc) { pool_flush(); jid_acc = jid_cur; }
+            }
             float2 rr[SLABS];
 #pragma unroll
             for (int s = 0; s < SLABS; ++s) {
@@ -367,7 +470,7 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS) __maxnreg__(EdgeCfg<C>::M
                 const bool valid = idx_cur >= 0;
                 const unsigned vmask = __ballot_sync(0xffffffffu, valid);
                 const int cnt = __popc(vmask & gmask);
-                const float inv = cnt > 0 ? 1.0f / (float)cnt : 0.0f;
+                const float inv = cnt > 0 ? (float)k / (float)cnt : 0.0f;   // W3', t3 carry 1/k (host): the f16 row sum is the mean
                 float v[32];
                 tmem_ld32(tbase + C, v);
 #pragma unroll
@@ -411,8 +514,15 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS) __maxnreg__(EdgeCfg<C>::M
                     } else if (pt < N) {
                         if (nout == 2) {
                             const float2 f = unpack_f16x2(w[0]);
-                            *reinterpret_cast<float2*>(p.y + o) =
-                                make_float2(fmaxf(fmaf(f.x, inv, rr[s].x), 0.0f), fmaxf(fmaf(f.y, inv, rr[s].y), 0.0f));
+                            const float y0 = fmaxf(fmaf(f.x, inv, rr[s].x), 0.0f), y1 = fmaxf(fmaf(f.y, inv, rr[s].y), 0.0f);
+                            if constexpr (POOL) {
+                                ulonglong2 a = acc_s[s * 32];
+                                a.x += to_fixed_32_32(y0);
+                                a.y += to_fixed_32_32(y1);
+                                acc_s[s * 32] = a;
+                            } else {
+                                *reinterpret_cast<float2*>(p.y + o) = make_float2(y0, y1);
+                            }
                         } else {
 #pragma unroll
                             for (int i = 0; i < 16; i += 2)
@@ -429,13 +539,27 @@ __global__ void __launch_bounds__(EdgeCfg<C>::THREADS) __maxnreg__(EdgeCfg<C>::M
             }
             if (t + 1 < T) reset_acc(1);
             idx_cur = idx_next;
+            if constexpr (POOL) jid_cur = jid_next;
             }
         }
+        if constexpr (POOL) pool_flush();
     }
     tc_fence_before();
     if constexpr (PAIR) cluster_sync_all(); else __syncthreads();
     if (warp == Cfg::MMA_WARP) tmem_dealloc_g<PAIR>(tmem, Cfg::TMEM_COLS);
 }
+
+// two entry points: one register budget for every warp (__maxnreg__), or the budget at launch with setmaxnreg per role
+template <int C, int LOGK, bool POOL>
+__global__ void __launch_bounds__((EdgeCfg<C, false>::THREADS)) __maxnreg__((EdgeCfg<C, false>::MAXREG)) edge_kernel(EdgeParams p) {
+    if constexpr (!edge_split(C, LOGK)) edge_body<C, LOGK, POOL>(p);
+}
+template <int C, int LOGK, bool POOL>
+__global__ void __launch_bounds__((EdgeCfg<C, true>::THREADS), (EdgeCfg<C, true>::MIN_CTAS)) edge_kernel_ws(EdgeParams p) {
+    if constexpr (edge_split(C, LOGK)) edge_body<C, LOGK, POOL>(p);
+}
+template <int C, int LOGK, bool POOL>
+auto edge_entry() { if constexpr (edge_split(C, LOGK)) return edge_kernel_ws<C, LOGK, POOL>; else return edge_kernel<C, LOGK, POOL>; }
 
 // ---- wide blocks (C = 512, configs[4] wide variant): the 1 MB of W2', W3' cannot be resident even split over a CTA pair,
 // and two 512-column accumulators exceed TMEM.  This kernel is the simple, sequential form: one CTA per SM, one tile at a
@@ -624,7 +748,7 @@ __global__ void __launch_bounds__(WIDE_THREADS, 1) edge_wide_kernel(EdgeParams p
                 const bool valid = idx_s[row] >= 0;
                 const unsigned gmask = (k >= 32) ? 0xffffffffu : (((1u << k) - 1u) << (lane & ~(k - 1)));
                 const int cnt = __popc(__ballot_sync(0xffffffffu, valid) & gmask);
-                const float inv = cnt > 0 ? 1.0f / (float)cnt : 0.0f;
+                const float inv = cnt > 0 ? (float)k / (float)cnt : 0.0f;   // W3', t3 carry 1/k (host)
                 const int pt = p0 + (row >> logk);
                 int cb = 0;                                      // first of the 32 >> logk columns this lane ends up with
                 for (int s = 0; s < logk; ++s) cb += ((lane >> s) & 1) * (16 >> s);
@@ -737,6 +861,48 @@ __global__ void __launch_bounds__(PRE_THREADS) pre_kernel(PreParams p) {
             } else {
                 *reinterpret_cast<float4*>(p.R + (size_t)row * p.C3 + (col - 2 * p.C1)) = make_float4(o0, o1, o2, o3);
             }
+        }
+    }
+}
+
+// Narrow inputs (block 1: C_in = F <= 16): thread (x = column quad, y) computes four output columns of PRS_ROWS consecutive
+// particles; the rows and the weight column quad come straight from L1 / L2 (a CTA shares 16 rows and the 5 KB weight matrix),
+// no staging, no barrier.
+constexpr int PRS_ROWS = 4;      // rows per thread
+constexpr int PRS_TY = 4;        // blockDim.y
+
+template <int KP>
+__global__ void __launch_bounds__(1024) pre_small_kernel(PreParams p) {
+    if (p.meta[0]) return;
+    const int N = p.meta[1];
+    const int cg = threadIdx.x;                                  // blockDim.x = NC / 4
+    const int row0 = (blockIdx.x * PRS_TY + threadIdx.y) * PRS_ROWS;
+    if (row0 >= N) return;
+    float4 w[KP];
+    const float* w0 = p.Wt + cg * 4;
+#pragma unroll
+    for (int kk = 0; kk < KP; ++kk) w[kk] = kk < p.cin ? __ldg(reinterpret_cast<const float4*>(w0 + (size_t)kk * p.NC)) : make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+    const float4 b = __ldg(reinterpret_cast<const float4*>(p.bias + cg * 4));
+    const int col = cg * 4;
+#pragma unroll
+    for (int r = 0; r < PRS_ROWS; ++r) {
+        const int row = row0 + r;
+        if (row >= N) break;
+        float4 acc = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+#pragma unroll
+        for (int kk = 0; kk < KP; ++kk) {
+            if (kk < p.cin) {
+                const float x = __ldg(p.x + (size_t)row * p.cin + kk);
+                acc.x = fmaf(x, w[kk].x, acc.x); acc.y = fmaf(x, w[kk].y, acc.y);
+                acc.z = fmaf(x, w[kk].z, acc.z); acc.w = fmaf(x, w[kk].w, acc.w);
+            }
+        }
+        const float o0 = acc.x + b.x, o1 = acc.y + b.y, o2 = acc.z + b.z, o3 = acc.w + b.w;
+        if (col < 2 * p.C1) {
+            __nv_bfloat16* dst = (col < p.C1) ? p.U + (size_t)row * p.C1 + col : p.V + (size_t)row * p.C1 + (col - p.C1);
+            *reinterpret_cast<uint2*>(dst) = make_uint2(pack_bf16x2(o0, o1), pack_bf16x2(o2, o3));
+        } else {
+            *reinterpret_cast<float4*>(p.R + (size_t)row * p.C3 + (col - 2 * p.C1)) = make_float4(o0, o1, o2, o3);
         }
     }
 }
@@ -956,7 +1122,7 @@ struct Bf16BlockDev {
     const float* pre_bias = nullptr;
     const uint8_t* pre_wimg = nullptr;   // tf32 chunk images of the tensor-core pre kernel (null: SIMT pre kernel)
     int cin = 0, Kp = 0, C = 0, NC = 0;
-    int grid_cap = 148;
+    int grid_cap = 148, grid_cap_pool = 148;
 };
 struct Bf16Scratch {
     __nv_bfloat16* U = nullptr;
@@ -998,51 +1164,75 @@ void pack_layer(const std::vector<float>& W, int C, int NRB, int row0, std::vect
     }
 }
 
-template <int C, int LOGK>
+template <int C, int LOGK, bool POOL>
 int configure_edge(Bf16BlockDev& b, int n_sms) {
-    using Cfg = EdgeCfg<C>;
-    auto* kern = edge_kernel<C, LOGK>;
-    GNN_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::SMEM_BYTES));
+    using Cfg = EdgeCfg<C, edge_split(C, LOGK)>;
+    constexpr int SMEM = POOL ? Cfg::SMEM_BYTES_POOL : Cfg::SMEM_BYTES;
+    auto* kern = edge_entry<C, LOGK, POOL>();
+    GNN_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM));
     GNN_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+    int cap;
     if (Cfg::PAIR) {
         cudaLaunchConfig_t cfg{};
-        cfg.gridDim = dim3(n_sms & ~1); cfg.blockDim = dim3(Cfg::THREADS); cfg.dynamicSmemBytes = Cfg::SMEM_BYTES;
+        cfg.gridDim = dim3(n_sms & ~1); cfg.blockDim = dim3(Cfg::THREADS); cfg.dynamicSmemBytes = SMEM;
         cudaLaunchAttribute at[1];
         at[0].id = cudaLaunchAttributeClusterDimension;
         at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
         cfg.attrs = at; cfg.numAttrs = 1;
         int ncl = 0;
         GNN_CUDA_TRY(cudaOccupancyMaxActiveClusters(&ncl, kern, &cfg));
-        if (ncl < 1) { std::fprintf(stderr, "libgnn: edge_kernel<%d>: no resident cluster (threads %d, smem %d)\n", C, Cfg::THREADS, Cfg::SMEM_BYTES); return GNN_ERR_BAD_ARCH; }
-        b.grid_cap = 2 * std::min(ncl, n_sms / 2);
+        if (ncl < 1) { std::fprintf(stderr, "libgnn: edge_kernel<%d>: no resident cluster (threads %d, smem %d)\n", C, Cfg::THREADS, SMEM); return GNN_ERR_BAD_ARCH; }
+        cap = 2 * std::min(ncl, n_sms / 2);
     } else {
         int occ = 0;
-        GNN_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, Cfg::THREADS, Cfg::SMEM_BYTES));
-        if (occ < 1) { std::fprintf(stderr, "libgnn: edge_kernel<%d>: occupancy 0 (threads %d, smem %d)\n", C, Cfg::THREADS, Cfg::SMEM_BYTES); return GNN_ERR_BAD_ARCH; }
+        GNN_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, Cfg::THREADS, SMEM));
+        if (occ < 1) { std::fprintf(stderr, "libgnn: edge_kernel<%d>: occupancy 0 (threads %d, smem %d)\n", C, Cfg::THREADS, SMEM); return GNN_ERR_BAD_ARCH; }
         occ = std::max(occ, Cfg::MIN_CTAS);                    // the kernel is compiled for MIN_CTAS resident CTAs per SM
         const int tmem_cap = 512 / Cfg::TMEM_COLS;              // co-resident CTAs must all fit their TMEM columns
-        b.grid_cap = n_sms * std::min(occ, tmem_cap);
+        cap = n_sms * std::min(occ, tmem_cap);
     }
+    (POOL ? b.grid_cap_pool : b.grid_cap) = cap;
     return GNN_OK;
 }
 
-template <int C, int LOGK>
-int launch_edge_t(const EdgeParams& p, int grid_cap, cudaStream_t s) {
-    using Cfg = EdgeCfg<C>;
+template <int C>
+int configure_edge_c(Bf16BlockDev& b, int n_sms, int k) {
+    if (k != 16) return configure_edge<C, -1, false>(b, n_sms);
+    const int rc = configure_edge<C, 4, false>(b, n_sms);
+    return rc != GNN_OK ? rc : configure_edge<C, 4, true>(b, n_sms);
+}
+
+template <int C, int LOGK, bool POOL>
+int launch_edge_t(const EdgeParams& p_in, int grid_cap, cudaStream_t s) {
+    using Cfg = EdgeCfg<C, edge_split(C, LOGK)>;
+    constexpr int SMEM = POOL ? Cfg::SMEM_BYTES_POOL : Cfg::SMEM_BYTES;
+    EdgeParams p = p_in;
+    const int n_work = Cfg::PAIR ? (p.n_tiles + 1) / 2 : p.n_tiles;
+    const int n_units = Cfg::PAIR ? std::min(n_work, grid_cap / 2) : std::min(n_work, grid_cap);
+    // tiles a unit takes at a time (GNN_EDGE_CHUNK overrides, developer knob).  Measured on configs[1]: without the pooling
+    // epilogue tile-by-tile round-robin is best (39 / 72 us for C = 64 / 128 against 42 / 72 us with one contiguous range per
+    // unit); the pooling epilogue wants ONE contiguous range per unit -- a jet's partial sums then stay on chip across
+    // its tiles (161 us against 176 us round-robin, where every tile flushes 2048 atomics)
+    if (p.chunk <= 0) p.chunk = POOL ? (n_work + n_units - 1) / n_units : 1;
     if (Cfg::PAIR) {
-        const int n_work = (p.n_tiles + 1) / 2;
         cudaLaunchConfig_t cfg{};
-        cfg.gridDim = dim3(2 * std::min(n_work, grid_cap / 2)); cfg.blockDim = dim3(Cfg::THREADS);
-        cfg.dynamicSmemBytes = Cfg::SMEM_BYTES; cfg.stream = s;
+        cfg.gridDim = dim3(2 * n_units); cfg.blockDim = dim3(Cfg::THREADS);
+        cfg.dynamicSmemBytes = SMEM; cfg.stream = s;
         cudaLaunchAttribute at[1];
         at[0].id = cudaLaunchAttributeClusterDimension;
         at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
         cfg.attrs = at; cfg.numAttrs = 1;
-        GNN_CUDA_TRY(cudaLaunchKernelEx(&cfg, edge_kernel<C, LOGK>, p));
+        GNN_CUDA_TRY(cudaLaunchKernelEx(&cfg, edge_entry<C, LOGK, POOL>(), p));
     } else {
-        edge_kernel<C, LOGK><<<std::min(p.n_tiles, grid_cap), Cfg::THREADS, Cfg::SMEM_BYTES, s>>>(p);
+        edge_entry<C, LOGK, POOL>()<<<n_units, Cfg::THREADS, SMEM, s>>>(p);
     }
     return GNN_OK;
+}
+
+template <int C>
+int launch_edge_c(const EdgeParams& p, const Bf16BlockDev& b, int k, bool pool, cudaStream_t s) {
+    if (k != 16) return launch_edge_t<C, -1, false>(p, b.grid_cap, s);
+    return pool ? launch_edge_t<C, 4, true>(p, b.grid_cap_pool, s) : launch_edge_t<C, 4, false>(p, b.grid_cap, s);
 }
 
 }  // namespace
@@ -1080,12 +1270,16 @@ int edgeconv_bf16_prepare(gnn_model& m, const float* blob) {
             bias[o] = t1[o]; bias[2 * C + o] = ts[o];
         }
         std::vector<float> W2f((size_t)C * C), W3f((size_t)C * C), sh((size_t)2 * C);
+        // Layer 3 carries 1/k (k is a power of two in this mode, so the scaling is exact in fp32 and bf16): E3 sums the k rows
+        // of relu(D1 + t3) in packed fp16, and with the factor inside, the sum IS the mean -- it stays below the largest
+        // activation, so fp16's range (65504, conversions saturate) bounds single activations, not k times the mean.
+        const float rk = 1.0f / (float)a.k;
         for (int o = 0; o < C; ++o) {
             for (int c = 0; c < C; ++c) {
                 W2f[(size_t)o * C + c] = s2[o] * W2[(size_t)o * C + c];
-                W3f[(size_t)o * C + c] = s3[o] * W3[(size_t)o * C + c];
+                W3f[(size_t)o * C + c] = s3[o] * W3[(size_t)o * C + c] * rk;
             }
-            sh[o] = t2[o]; sh[C + o] = t3[o];
+            sh[o] = t2[o]; sh[C + o] = t3[o] * rk;
         }
         std::vector<uint8_t> img;                              // per CTA rank: [W2' chunks | W3' chunks] of its output rows
         if (C > 256) {                                          // streamed: layer-major, N halves of 256 rows, K blocks
@@ -1103,7 +1297,7 @@ int edgeconv_bf16_prepare(gnn_model& m, const float* blob) {
             (rc = upload(m, img, &b.wimg)) != GNN_OK || (rc = upload(m, sh, &b.shifts)) != GNN_OK)
             return rc;
         if ((cin == 64 && C == 128) || (cin == 128 && C == 256)) {
-            // tensor-core pre kernel: per slice (u, v, r) and K block of 32: [C][32] tf32 (RNA), 128B-swizzled
+            // tensor-core pre kernel: per slice of C output columns (u, v, r) and K block of 32: [C][32] tf32 (RNA), 128B-swizzled
             std::vector<uint8_t> pimg((size_t)3 * C * cin * 4, 0);
             size_t base = 0;
             for (int sl = 0; sl < 3; ++sl)
@@ -1118,14 +1312,21 @@ int edgeconv_bf16_prepare(gnn_model& m, const float* blob) {
                             std::memcpy(&pimg[off], &u, 4);
                         }
             if ((rc = upload(m, pimg, &b.pre_wimg)) != GNN_OK) return rc;
-            if (C == 128) GNN_CUDA_TRY(cudaFuncSetAttribute(pre_tc_kernel<64, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize, PreTcCfg<64, 128>::SMEM_BYTES));
-            else GNN_CUDA_TRY(cudaFuncSetAttribute(pre_tc_kernel<128, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, PreTcCfg<128, 256>::SMEM_BYTES));
+            // (largest shared-memory carve-out: the split is per-SM state that only changes on an idle SM, so a kernel that asks
+            // for less would keep the kNN CTAs of the other stream off its SMs)
+            if (C == 128) {
+                GNN_CUDA_TRY(cudaFuncSetAttribute(pre_tc_kernel<64, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize, PreTcCfg<64, 128>::SMEM_BYTES));
+                GNN_CUDA_TRY(cudaFuncSetAttribute(pre_tc_kernel<64, 128>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+            } else {
+                GNN_CUDA_TRY(cudaFuncSetAttribute(pre_tc_kernel<128, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, PreTcCfg<128, 256>::SMEM_BYTES));
+                GNN_CUDA_TRY(cudaFuncSetAttribute(pre_tc_kernel<128, 256>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+            }
         }
         switch (C) {
-            case 32: rc = a.k == 16 ? configure_edge<32, 4>(b, m.n_sms) : configure_edge<32, -1>(b, m.n_sms); break;
-            case 64: rc = a.k == 16 ? configure_edge<64, 4>(b, m.n_sms) : configure_edge<64, -1>(b, m.n_sms); break;
-            case 128: rc = a.k == 16 ? configure_edge<128, 4>(b, m.n_sms) : configure_edge<128, -1>(b, m.n_sms); break;
-            case 256: rc = a.k == 16 ? configure_edge<256, 4>(b, m.n_sms) : configure_edge<256, -1>(b, m.n_sms); break;
+            case 32: rc = configure_edge_c<32>(b, m.n_sms, a.k); break;
+            case 64: rc = configure_edge_c<64>(b, m.n_sms, a.k); break;
+            case 128: rc = configure_edge_c<128>(b, m.n_sms, a.k); break;
+            case 256: rc = configure_edge_c<256>(b, m.n_sms, a.k); break;
             case 512:
                 rc = cudaFuncSetAttribute(edge_wide_kernel<512>, cudaFuncAttributeMaxDynamicSharedMemorySize, WideCfg<512>::SMEM_BYTES) == cudaSuccess ? GNN_OK : GNN_ERR_CUDA;
                 b.grid_cap = m.n_sms;
@@ -1169,30 +1370,49 @@ int launch_pre_bf16(gnn_model& m, int block, const float* x, int N, Workspace& w
         PreParams pp;
         pp.x = x; pp.Wt = b.pre_Wt; pp.bias = b.pre_bias; pp.U = sc.U; pp.V = sc.V; pp.R = sc.R; pp.meta = w.meta;
         pp.cin = b.cin; pp.Kp = b.Kp; pp.C1 = b.C; pp.C3 = b.C; pp.NC = b.NC;
-        const size_t pre_smem = (size_t)PRE_ROWS * (b.Kp + 4) * sizeof(float);
-        pre_kernel<<<(N + PRE_ROWS - 1) / PRE_ROWS, PRE_THREADS, pre_smem, s>>>(pp);
+        if (b.cin <= 16 && (b.NC >> 2) * PRS_TY <= 1024) {
+            const dim3 blk(b.NC >> 2, PRS_TY);
+            const unsigned grid = (unsigned)((N + PRS_TY * PRS_ROWS - 1) / (PRS_TY * PRS_ROWS));
+            if (b.cin <= 8) pre_small_kernel<8><<<grid, blk, 0, s>>>(pp);
+            else pre_small_kernel<16><<<grid, blk, 0, s>>>(pp);
+        } else {
+            const size_t pre_smem = (size_t)PRE_ROWS * (b.Kp + 4) * sizeof(float);
+            pre_kernel<<<(N + PRE_ROWS - 1) / PRE_ROWS, PRE_THREADS, pre_smem, s>>>(pp);
+        }
     }
     return 1;
 }
 
-// per-edge part: gather, layers 2-3 on the tensor cores, mean, shortcut (needs idx and the pre kernel's U, V, R)
+// the POOL epilogue exists for k = 16 and the resident-weight kernels (C <= 256)
+bool edgeconv_bf16_can_pool(const gnn_model& m, int block) {
+    const Bf16BlockDev& b = static_cast<const Bf16BlockDev*>(m.bf16_blocks)[block];
+    return m.arch.k == 16 && b.C <= 256;
+}
+
+// per-edge part: gather, layers 2-3 on the tensor cores, mean, shortcut (needs idx and the pre kernel's U, V, R).
+// y != null: the block output [N, C] is stored; y == null (edgeconv_bf16_can_pool only): it is added into w.pool instead
 int launch_edge_bf16(gnn_model& m, int block, const int32_t* idx, int N, float* y, Workspace& w, cudaStream_t s) {
     if (N == 0) return 0;
     const Bf16BlockDev& b = static_cast<const Bf16BlockDev*>(m.bf16_blocks)[block];
     const Bf16Scratch& sc = *static_cast<const Bf16Scratch*>(w.bf16_scratch);
     const int k = m.arch.k;
+    const bool pool = y == nullptr;
+    if (pool && !edgeconv_bf16_can_pool(m, block)) return GNN_ERR_BAD_ARG;
     EdgeParams ep;
-    ep.U = sc.U; ep.V = sc.V; ep.R = sc.R; ep.idx = idx; ep.y = y; ep.meta = w.meta; ep.wimg = b.wimg; ep.shifts = b.shifts;
+    ep.U = sc.U; ep.V = sc.V; ep.R = sc.R; ep.idx = idx; ep.y = y; ep.pjid = w.pjid; ep.pool = w.pool; ep.meta = w.meta;
+    ep.wimg = b.wimg; ep.shifts = b.shifts;
     ep.k = k; ep.logk = 0;
     while ((1 << ep.logk) < k) ++ep.logk;
     ep.TP = TILE_ROWS / k;
     ep.n_tiles = (N + ep.TP - 1) / ep.TP;
+    static const int chunk_env = [] { const char* e = std::getenv("GNN_EDGE_CHUNK"); return e ? std::atoi(e) : 0; }();
+    ep.chunk = chunk_env;                                       // <= 0: chosen per kernel in launch_edge_t
     int rc;
     switch (b.C) {
-        case 32: rc = k == 16 ? launch_edge_t<32, 4>(ep, b.grid_cap, s) : launch_edge_t<32, -1>(ep, b.grid_cap, s); break;
-        case 64: rc = k == 16 ? launch_edge_t<64, 4>(ep, b.grid_cap, s) : launch_edge_t<64, -1>(ep, b.grid_cap, s); break;
-        case 128: rc = k == 16 ? launch_edge_t<128, 4>(ep, b.grid_cap, s) : launch_edge_t<128, -1>(ep, b.grid_cap, s); break;
-        case 256: rc = k == 16 ? launch_edge_t<256, 4>(ep, b.grid_cap, s) : launch_edge_t<256, -1>(ep, b.grid_cap, s); break;
+        case 32: rc = launch_edge_c<32>(ep, b, k, pool, s); break;
+        case 64: rc = launch_edge_c<64>(ep, b, k, pool, s); break;
+        case 128: rc = launch_edge_c<128>(ep, b, k, pool, s); break;
+        case 256: rc = launch_edge_c<256>(ep, b, k, pool, s); break;
         case 512:
             edge_wide_kernel<512><<<std::min(ep.n_tiles, b.grid_cap), WIDE_THREADS, WideCfg<512>::SMEM_BYTES, s>>>(ep);
             rc = GNN_OK;
@@ -1210,4 +1430,3 @@ int launch_edgeconv_bf16(gnn_model& m, int block, const float* x, const int32_t*
     const int b = launch_edge_bf16(m, block, idx, N, y, w, s);
     return b < 0 ? b : a + b;
 }
-

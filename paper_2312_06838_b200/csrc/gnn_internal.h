@@ -33,7 +33,10 @@ struct Workspace {
     int32_t* jet_start = nullptr;  // [Bmax] sanitised CSR
     int32_t* jet_n = nullptr;      // [Bmax] sanitised multiplicities (< 0 = offending jet; -n if it owns n packed rows)
     unsigned* status = nullptr;    // [1] sticky device status word
-    int32_t* meta = nullptr;       // [2] per call: meta[0] = batch poisoned, meta[1] = particles in the batch
+    int32_t* meta = nullptr;       // [4] per call: meta[0] = batch poisoned, meta[1] = particles in the batch, meta[2] = kNN groups
+    int2* groups = nullptr;        // [Bmax] kNN group schedule: (first jet, jets) of runs of whole jets that fit one 128-row tile
+    int32_t* pjid = nullptr;       // [Nmax] particle -> jet index (written by the grouped kNN, read by the pooling EdgeConv epilogue)
+    unsigned long long* pool = nullptr;  // [Bmax, C_last] bf16 mode: per-jet channel sums of the last block's output, 2^-32 fixed point
     // padded entry
     float* pfeats = nullptr;    // [Nmax, F]
     float* pcoords = nullptr;   // [Nmax, CD]
@@ -84,16 +87,19 @@ int launch_ingest(const int32_t* offsets, const int32_t* counts, int B, int N_ex
 int launch_compact_padded(const float* feats, const float* coords, const float* mask, int B, int P, int F, int CD,
                           int max_particles, Workspace& w, cudaStream_t s);
 // kNN: space [N, D]; out [N, k] global indices (local_out = 0) or jet-local (local_out = 1)
-// gram != 0 (bf16 mode, R28): distances may take the tensor-core Gram form where D has one, and the selection
-// orders 32-bit keys (d to 16 mantissa bits | j); 0: exact direct differences and exact (d, j) order
+// gram != 0 (bf16 mode, R28): the grouped kernels of knn_group.cu where they have a form for D (Gram distances on
+// the tensor cores for feature spaces, 32-bit keys: d to 16 mantissa bits | j); 0: exact direct differences, exact (d, j) order
 int launch_knn(const float* space, int D, int k, int B, int max_particles, const Workspace& w, int32_t* idx_out,
                int local_out, int gram, cudaStream_t s);
 int launch_edgeconv_f32(const BlockDev& b, int k, const float* x, const int32_t* idx, int N, float* y,
                         const Workspace& w, cudaStream_t s);
 int launch_globalize_idx(const int32_t* idx_local, int k, int B, const Workspace& w, int32_t* idx_global, cudaStream_t s);
 int launch_pool_head(const gnn_model& m, const float* x, int B, const Workspace& w, float* logits, cudaStream_t s);
+int launch_pooled_mean(const gnn_model& m, int B, const Workspace& w, float* g, cudaStream_t s);
 int knn_configure();
 int pool_head_configure();
-int knn_tc_configure();
+int knn_group_configure();
+int launch_knn_group(const float* space, int D, int k, int B, int max_particles, const Workspace& w, int32_t* idx_out,
+                     int local_out, cudaStream_t s);
 int edgeconv_f32_configure();
 

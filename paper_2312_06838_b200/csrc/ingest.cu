@@ -7,11 +7,24 @@
 // offsets hold.  Globally inconsistent offsets poison the whole batch (meta[0] = 1, GNN_DEV_BAD_OFFSETS); a jet
 // larger than max_particles poisons only itself (jet_n < 0, GNN_DEV_JET_TOO_LARGE).  meta[1] = number of particles
 // later kernels may touch.  `counts` (padded entry only) carries -1 for jets whose mask selected too many slots.
+//
+// Second phase: the GROUP SCHEDULE of the grouped kNN kernels (knn_group.cu).  A group is a run of consecutive whole jets
+// whose rows fit one 128-row tile (at most GROUP_MAX_JETS jets; an offending ragged jet, which owns more rows than a
+// tile, is a group of its own).  Greedy packing is sequential, so it is done per chunk of 32 consecutive jets by one
+// warp: lane l finds next(l) = the first jet of the chunk that no longer fits a group starting at l, the group starts are
+// the orbit of lane 0 under next (five pointer-doubling steps on ballots), and a block-wide scan of the chunks' group
+// counts gives every group its slot.  groups[g] = (first jet, number of jets), meta[2] = number of groups.
+constexpr int GROUP_ROWS = 128;
+constexpr int GROUP_MAX_JETS = 16;
+
 __global__ void __launch_bounds__(1024) ingest_kernel(const int32_t* __restrict__ offsets,
                                                       const int32_t* __restrict__ counts, int B, int N_exact, int N_cap,
                                                       int max_particles, int32_t* __restrict__ jet_start,
                                                       int32_t* __restrict__ jet_n, int32_t* __restrict__ meta,
-                                                      unsigned* status) {
+                                                      unsigned* status, int2* __restrict__ groups) {
+    __shared__ int chunk_cnt[1024];                // groups per chunk of 32 jets, then its exclusive scan
+    __shared__ int warp_tot[32];
+    __shared__ unsigned char rows_s[32768];        // rows a jet brings to a group (GROUP_ROWS + 1: never shares one)
     int any_bad = 0, any_big = 0;
     for (int b = threadIdx.x; b < B; b += blockDim.x) {
         int s = offsets[b], e = offsets[b + 1];
@@ -22,6 +35,7 @@ __global__ void __launch_bounds__(1024) ingest_kernel(const int32_t* __restrict_
         else if (n > max_particles) { any_big = 1; n = -n; }                        // ragged: jet_n = -multiplicity
         jet_start[b] = s;
         jet_n[b] = n;
+        rows_s[b] = (unsigned char)(n > 0 ? min(n, GROUP_ROWS + 1) : (n < -1 ? GROUP_ROWS + 1 : 0));   // offending ragged jet: alone
     }
     any_bad = __syncthreads_or(any_bad);
     any_big = __syncthreads_or(any_big);
@@ -31,11 +45,81 @@ __global__ void __launch_bounds__(1024) ingest_kernel(const int32_t* __restrict_
         if (any_bad) atomicOr(status, GNN_DEV_BAD_OFFSETS);
         if (any_big) atomicOr(status, GNN_DEV_JET_TOO_LARGE);
     }
+    if (groups == nullptr || any_bad) { if (threadIdx.x == 0) meta[2] = 0; return; }
+    // ---- group schedule (from the rows kept in shared memory: no global round trip) ------------------------------------------
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    const int n_chunks = (B + 31) >> 5;                         // <= 1024 for B <= 32768 (checked by the launcher)
+    // pass 1: group starts per chunk -> chunk_cnt; the per-lane results are recomputed in pass 2 (cheaper than keeping them)
+    auto chunk_groups = [&](int chunk, int& njets_out, unsigned& marks_out) {
+        const int b = chunk * 32 + lane;
+        const int rows = b < B ? (int)rows_s[b] : 0;
+        int P = rows;                                           // inclusive prefix of rows inside the chunk
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, P, o); if (lane >= o) P += v; }
+        const int S = P - rows;
+        int next = 32;                                          // first lane that does not fit a group starting here
+#pragma unroll
+        for (int d = 1; d <= GROUP_MAX_JETS; ++d) {
+            const int l2 = lane + d;
+            const int Pv = __shfl_sync(0xffffffffu, P, l2 & 31);
+            if (next == 32 && l2 < 32 && (Pv - S > GROUP_ROWS || d == GROUP_MAX_JETS)) next = l2;
+        }
+        if (b >= B) next = 32;
+        njets_out = min(next, 32) - lane;
+        if (b < B && chunk * 32 + next > B) njets_out = B - b;
+        unsigned marks = 1u;                                    // lane 0 starts a group (chunk is non-empty)
+        int nx = next;
+#pragma unroll
+        for (int it = 0; it < 5; ++it) {
+            const bool mine = (marks >> lane) & 1u;
+            marks |= __reduce_or_sync(0xffffffffu, (mine && nx < 32) ? (1u << nx) : 0u);
+            const int n2 = __shfl_sync(0xffffffffu, nx, nx & 31);
+            nx = nx < 32 ? n2 : 32;
+        }
+        const int nb = min(32, B - chunk * 32);                 // lanes past the batch start no group
+        marks_out = nb >= 32 ? marks : (marks & ((1u << nb) - 1u));
+    };
+    for (int chunk = warp; chunk < n_chunks; chunk += nwarps) {
+        int nj; unsigned marks;
+        chunk_groups(chunk, nj, marks);
+        if (lane == 0) chunk_cnt[chunk] = __popc(marks);
+    }
+    __syncthreads();
+    // exclusive scan of chunk_cnt (n_chunks <= 1024 = blockDim): warp scans + scan of the warp totals
+    {
+        const int v = (int)threadIdx.x < n_chunks ? chunk_cnt[threadIdx.x] : 0;
+        int incl = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const int u = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += u; }
+        if (lane == 31) warp_tot[warp] = incl;
+        __syncthreads();
+        if (warp == 0) {
+            const int t = lane < nwarps ? warp_tot[lane] : 0;
+            int ti = t;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) { const int u = __shfl_up_sync(0xffffffffu, ti, o); if (lane >= o) ti += u; }
+            warp_tot[lane] = ti - t;                            // exclusive
+            if (lane == 31) meta[2] = ti;                       // total number of groups
+        }
+        __syncthreads();
+        if ((int)threadIdx.x < n_chunks) chunk_cnt[threadIdx.x] = warp_tot[warp] + incl - v;
+        __syncthreads();
+    }
+    for (int chunk = warp; chunk < n_chunks; chunk += nwarps) {
+        int nj; unsigned marks;
+        chunk_groups(chunk, nj, marks);
+        if ((marks >> lane) & 1u) {
+            const int slot = chunk_cnt[chunk] + __popc(marks & ((1u << lane) - 1u));
+            groups[slot] = make_int2(chunk * 32 + lane, nj);
+        }
+    }
 }
 
 int launch_ingest(const int32_t* offsets, const int32_t* counts, int B, int N_exact, int N_cap, int max_particles,
                   Workspace& w, cudaStream_t s) {
-    ingest_kernel<<<1, 1024, 0, s>>>(offsets, counts, B, N_exact, N_cap, max_particles, w.jet_start, w.jet_n, w.meta, w.status);
+    if (B > 32768) return GNN_ERR_BATCH_TOO_LARGE;               // group schedule: one CTA, 1024 chunks of 32 jets
+    ingest_kernel<<<1, 1024, 0, s>>>(offsets, counts, B, N_exact, N_cap, max_particles, w.jet_start, w.jet_n, w.meta, w.status,
+                                     w.groups);
     return 1;
 }
 
@@ -121,3 +205,4 @@ int launch_compact_padded(const float* feats, const float* coords, const float* 
     scatter_padded_kernel<<<B, 128, 0, s>>>(feats, coords, mask, P, F, CD, max_particles, w.poffsets, w.pcounts, w.pfeats, w.pcoords);
     return 3;
 }
+

@@ -2,24 +2,22 @@
 // "dynamic graph"; BASELINE.json north_star (1): pairwise distances in shared memory, top-k with ties broken by the
 // lower index; on (eta, phi) for block 1 and on the features for later blocks).
 //
-// One CTA per (jet, tile of 32 queries): a jet of n particles occupies ceil(n/32) small CTAs, so an SM holds many
-// (the selection phase is a serial insertion per query; its latency is hidden by CTAs, not by threads of one CTA).
+// Exact path (GNN_FP32_VALIDATION, and gnn_debug_knn on spaces the grouped kernels of knn_group.cu do not take).
 // Readings: R3 squared Euclidean, direct differences (R18: no Gram form -- its cancellation error
 // exceeds the 1e-5 near-tie band); R4 self excluded by index; R5 strict order on (d, j); R6 k_eff = min(k, n-1).
 // fp32 arithmetic, d = fma(t, t, d) with t = s_i - s_j, dimensions summed in index order.
 //
-// Phase 1 (ALU-bound): the jet's rows are staged 32 dimensions at a time ([n4][36] floats: with this row stride the
-//   eight lanes of a quarter-warp reading eight consecutive rows with LDS.128 hit eight different bank groups); each
-//   thread owns up to two 4x4 (query x candidate) register tiles that accumulate over the chunks; chunks are
-//   double-buffered and staged with cp.async so that the next one lands while this one is used.  Distances of the 32
-//   queries go to a [32][n|1] matrix in shared memory with d_ii = +inf.
-// Phase 2: one thread per query walks its row and keeps the k smallest 64-bit keys (float bits of d << 32 | j) in a
-//   sorted register list -- d >= 0, so unsigned order on the bits is numeric order and equal distances fall back
-//   to the lower index for free.  (The paper-era "warp-level top-k" is replaced by this: see DESIGN.md.)
+// knn_dist_kernel (spaces of more than 4 dimensions): one CTA per (jet, group of query rows), groups sized so that a
+//   typical jet is one CTA with ~100 busy threads; the jet's rows are staged 32 dimensions at a time ([n4][36] floats,
+//   double-buffered with cp.async); each thread owns up to two 4x4 (query x candidate) register tiles; distances go to the
+//   global (L2-resident) matrix dm [N][pld] and the particle -> jet map pjet is written on the way.
+// knn_select_kernel: TWO threads per particle of the packed batch (even / odd candidates).  Each orders its first K
+//   candidates with a bitonic network in registers and inserts the rest into the sorted list of 64-bit keys
+//   (float bits of d << 32 | j: d >= 0, so unsigned order on the bits is numeric order and equal distances fall back to the
+//   lower index); the halves are merged through one shuffle per slot.  Spaces of <= 4 dimensions (the coordinates of
+//   block 1) skip the matrix: the selection computes d(i, j) on the fly with the same arithmetic.
 #include "gnn_internal.h"
 #include <cfloat>
-
-int launch_knn_gram(const float* space, int D, int B, int max_particles, const Workspace& w, cudaStream_t s);   // knn_tc.cu
 
 namespace {
 
@@ -28,20 +26,13 @@ constexpr int KNN_QT = 32;      // queries per CTA
 constexpr int KNN_DC = 32;      // dimensions staged per chunk
 constexpr int KNN_LD = KNN_DC + 4;
 
-// Selection keys.  Key64 = (float bits of d) << 32 | j: exact lexicographic (d, j) order (d >= 0, so unsigned order on the
-// bits is numeric order).  Key32 (GNN_BF16 mode only, R28) = float bits with the low 7 mantissa bits replaced
-// by j (j < 128): d to 16 mantissa bits -- finer than the tf32 inputs it was computed from -- at half the instructions.
+// Selection keys: (float bits of d) << 32 | j -- exact lexicographic (d, j) order (d >= 0, so unsigned order on the bits is
+// numeric order).
 struct Key64 {
     typedef unsigned long long T;
     static __device__ __forceinline__ T none() { return ~0ull; }
     static __device__ __forceinline__ T make(float d, int j) { return ((T)__float_as_uint(d) << 32) | (unsigned)j; }
     static __device__ __forceinline__ int index(T k) { return (int)(k & 0xffffffffull); }
-};
-struct Key32 {
-    typedef unsigned T;
-    static __device__ __forceinline__ T none() { return ~0u; }
-    static __device__ __forceinline__ T make(float d, int j) { return (__float_as_uint(d) & ~0x7fu) | (unsigned)j; }
-    static __device__ __forceinline__ int index(T k) { return (int)(k & 0x7fu); }
 };
 
 template <int K, typename KT>
@@ -191,8 +182,13 @@ knn_select_kernel(const float* __restrict__ dm, int pld, const float* __restrict
     if (meta[0]) return;
     const int t = blockIdx.x * KSEL_THREADS + threadIdx.x;
     const int q = t >> 1, half = t & 1;
-    if (q >= meta[1]) return;                                   // both lanes of a pair leave together
-    const int2 pi = __ldg(pjet + q);                            // (start, n) of the jet that owns row q, written with the distances
+    const bool live = q < meta[1];
+    int2 pi = make_int2(0, -1);
+    if (live) pi = __ldg(pjet + q);                             // (start, n) of the jet that owns row q, written with the distances
+    // lanes that reach the pair merge below, decided while the warp is still converged (the per-lane loops over n diverge,
+    // and independent thread scheduling does not promise reconvergence before the shuffle)
+    const unsigned pm = __ballot_sync(0xffffffffu, live && pi.y >= 0);
+    if (!live) return;                                          // both lanes of a pair leave together
     const int n = pi.y, start = pi.x;
     int32_t* out = idx_out + (size_t)q * k;
     if (n < 0) {                              // offending ragged jet (jet_n = -multiplicity): its packed rows exist and the
@@ -285,7 +281,7 @@ knn_select_kernel(const float* __restrict__ dm, int pld, const float* __restrict
         }
     }
     // merge with the partner lane: slot m of the merge is min(A[m], B[K-1-m]); both lanes end up with the same set
-    const unsigned pm = __activemask();
+    __syncwarp(pm);
     const int base = local_out ? 0 : start;
     KT r[K];
 #pragma unroll
@@ -328,7 +324,7 @@ size_t knn_smem_bytes(int P) {
 
 template <int K>
 int launch_knn_t(const float* space, int D, int k, int B, int P, const Workspace& w, int32_t* idx_out, int local_out,
-                 int gram, cudaStream_t s) {
+                 cudaStream_t s) {
     const int tiles = (P + KNN_QT - 1) / KNN_QT;
     const int pld = (P + 3) & ~3;
     const long long n_upper = 2ll * B * P;                     // two threads per particle slot
@@ -336,20 +332,11 @@ int launch_knn_t(const float* space, int D, int k, int B, int P, const Workspace
     if (D <= 4) {
         // coordinates (block 1): distances on the fly inside the selection; the particle -> jet map comes from its own kernel
         pjet_kernel<<<(B + 127) / 128, 128, 0, s>>>(B, w.jet_start, w.jet_n, w.meta, w.pjet);
-        if (gram && P <= 128)
-            knn_select_kernel<K, Key32, true><<<grid, KSEL_THREADS, 0, s>>>(w.dm, pld, space, D, k, w.pjet, w.jet_start, w.jet_n, w.meta, idx_out, local_out);
-        else
-            knn_select_kernel<K, Key64, true><<<grid, KSEL_THREADS, 0, s>>>(w.dm, pld, space, D, k, w.pjet, w.jet_start, w.jet_n, w.meta, idx_out, local_out);
+        knn_select_kernel<K, Key64, true><<<grid, KSEL_THREADS, 0, s>>>(w.dm, pld, space, D, k, w.pjet, w.jet_start, w.jet_n, w.meta, idx_out, local_out);
         return 2;
     }
-    // distances: the Gram form on the tensor cores where the caller allows it (bf16 mode, feature spaces) and D has one,
-    // else the exact direct-difference kernel
-    if (!(gram && launch_knn_gram(space, D, B, P, w, s) == 1))
-        knn_dist_kernel<<<B * tiles, KNN_THREADS, knn_smem_bytes(P), s>>>(space, D, w.jet_start, w.jet_n, w.meta, w.dm, pld, w.pjet, tiles);
-    if (gram && P <= 128)                    // bf16 mode: 32-bit keys (R28)
-        knn_select_kernel<K, Key32, false><<<grid, KSEL_THREADS, 0, s>>>(w.dm, pld, space, D, k, w.pjet, w.jet_start, w.jet_n, w.meta, idx_out, local_out);
-    else
-        knn_select_kernel<K, Key64, false><<<grid, KSEL_THREADS, 0, s>>>(w.dm, pld, space, D, k, w.pjet, w.jet_start, w.jet_n, w.meta, idx_out, local_out);
+    knn_dist_kernel<<<B * tiles, KNN_THREADS, knn_smem_bytes(P), s>>>(space, D, w.jet_start, w.jet_n, w.meta, w.dm, pld, w.pjet, tiles);
+    knn_select_kernel<K, Key64, false><<<grid, KSEL_THREADS, 0, s>>>(w.dm, pld, space, D, k, w.pjet, w.jet_start, w.jet_n, w.meta, idx_out, local_out);
     return 2;
 }
 
@@ -358,17 +345,22 @@ int launch_knn_t(const float* space, int D, int k, int B, int P, const Workspace
 int launch_knn(const float* space, int D, int k, int B, int max_particles, const Workspace& w, int32_t* idx_out,
                int local_out, int gram, cudaStream_t s) {
     if (B == 0) return 0;
+    if (gram) {                               // bf16 mode: grouped kernels where they have a form for this space
+        const int n = launch_knn_group(space, D, k, B, max_particles, w, idx_out, local_out, s);
+        if (n != 0) return n;
+    }
     if (knn_smem_bytes(max_particles) > 227 * 1024) return GNN_ERR_BAD_ARG;
-    if (k <= 4) return launch_knn_t<4>(space, D, k, B, max_particles, w, idx_out, local_out, gram, s);
-    if (k <= 8) return launch_knn_t<8>(space, D, k, B, max_particles, w, idx_out, local_out, gram, s);
-    if (k <= 16) return launch_knn_t<16>(space, D, k, B, max_particles, w, idx_out, local_out, gram, s);
-    return launch_knn_t<32>(space, D, k, B, max_particles, w, idx_out, local_out, gram, s);
+    if (k <= 4) return launch_knn_t<4>(space, D, k, B, max_particles, w, idx_out, local_out, s);
+    if (k <= 8) return launch_knn_t<8>(space, D, k, B, max_particles, w, idx_out, local_out, s);
+    if (k <= 16) return launch_knn_t<16>(space, D, k, B, max_particles, w, idx_out, local_out, s);
+    return launch_knn_t<32>(space, D, k, B, max_particles, w, idx_out, local_out, s);
 }
 
-// debug entry: jet-local neighbour indices -> the global ones the EdgeConv kernels read (out-of-jet values -> -1)
+// debug entry: jet-local neighbour indices -> the global ones the EdgeConv kernels read (out-of-jet values -> -1), and the
+// particle -> jet map the pooling epilogue reads (the forward gets both from the kNN kernels)
 __global__ void globalize_idx_kernel(const int32_t* __restrict__ idx_local, int k, const int32_t* __restrict__ jet_start,
                                      const int32_t* __restrict__ jet_n, const int32_t* __restrict__ meta,
-                                     int32_t* __restrict__ idx_global) {
+                                     int32_t* __restrict__ idx_global, int32_t* __restrict__ pjid) {
     if (meta[0]) return;
     const int b = blockIdx.x;
     int n = jet_n[b];
@@ -378,11 +370,12 @@ __global__ void globalize_idx_kernel(const int32_t* __restrict__ idx_local, int 
         int j = idx_local[(size_t)start * k + e];
         idx_global[(size_t)start * k + e] = (n > 0 && j >= 0 && j < n) ? j + start : -1;
     }
+    for (int r = threadIdx.x; r < rows; r += blockDim.x) pjid[start + r] = b;
 }
 
 int launch_globalize_idx(const int32_t* idx_local, int k, int B, const Workspace& w, int32_t* idx_global, cudaStream_t s) {
     if (B == 0) return 0;
-    globalize_idx_kernel<<<B, 128, 0, s>>>(idx_local, k, w.jet_start, w.jet_n, w.meta, idx_global);
+    globalize_idx_kernel<<<B, 128, 0, s>>>(idx_local, k, w.jet_start, w.jet_n, w.meta, idx_global, w.pjid);
     return 1;
 }
 

@@ -166,8 +166,140 @@ pool_head_kernel(const float* __restrict__ x, const int32_t* __restrict__ jet_st
     }
 }
 
+// ---- GNN_BF16 with the pooling EdgeConv epilogue: the head alone, on the per-jet channel sums -----------------------------
+// The sums arrive as exact 2^-32 fixed-point integers (edge_kernel<.., POOL>).  One CTA per HD_JETS jets; activations are kept
+// TRANSPOSED in shared memory (zT[k][jet]) so that one 16-byte load feeds four jets; a thread owns four outputs x HD_JETS
+// jets of one K slice of a wide layer (weights Wt[in][out] read once per CTA, eight 16-byte loads in flight), slices are
+// summed through shared memory in a fixed order; the narrow final layer runs one warp per (jet, output).
+// sum (unsigned 32.32 fixed point) / n in fp32: integer and fraction parts convert separately (no 64-bit or fp64 conversions,
+// which are slow); the result is within 1.5 ulp of the exact mean and depends on nothing but (sum, n)
+__device__ __forceinline__ float fixed_mean(unsigned long long v, int n) {
+    const float s = fmaf((float)(unsigned)(v & 0xffffffffull), 1.0f / 4294967296.0f, (float)(unsigned)(v >> 32));
+    return s / (float)n;
+}
+
+constexpr int HD_THREADS = 256;
+constexpr int HD_JETS = 8;
+
+__global__ void __launch_bounds__(HD_THREADS)
+head_kernel(const unsigned long long* __restrict__ pooled, const int32_t* __restrict__ jet_n, const int32_t* __restrict__ meta,
+            HeadParams hp, int B, float* __restrict__ logits) {
+    extern __shared__ __align__(16) float hs[];      // zT0 [wmax][HD_JETS] | zT1 [wmax][HD_JETS] | partials [KS][HD_JETS][ld]
+    __shared__ int s_n[HD_JETS];
+    const int b0 = blockIdx.x * HD_JETS;
+    const int nj = min(HD_JETS, B - b0);
+    const int C = hp.C, W = hp.wmax;
+    float* z0 = hs;
+    float* z1 = hs + W * HD_JETS;
+    float* part = z1 + W * HD_JETS;
+    const bool poisoned = meta[0] != 0;
+    if (threadIdx.x < HD_JETS) {
+        const int jb = threadIdx.x;
+        int n = (jb < nj && !poisoned) ? jet_n[b0 + jb] : 0;
+        s_n[jb] = n < 0 ? 0 : n;                     // offending jet: pools nothing (its logits become NaN below)
+    }
+    __syncthreads();
+    for (int it = threadIdx.x; it < HD_JETS * C; it += HD_THREADS) {
+        const int jb = it / C, c = it - jb * C;
+        const int n = s_n[jb];
+        float g = 0.0f;                              // R12: empty jet pools to 0
+        if (n > 0) g = fixed_mean(__ldg(pooled + (size_t)(b0 + jb) * C + c), n);
+        z0[c * HD_JETS + jb] = g;
+    }
+    __syncthreads();
+    float* zin = z0; float* zout = z1;
+    for (int l = 0; l < hp.n_fc; ++l) {
+        const LinF32 L = hp.fc[l];
+        const bool last = (l == hp.n_fc - 1);
+        const int OQ = L.ld >> 2;
+        if (OQ >= 16 && OQ <= HD_THREADS) {
+            const int KS = HD_THREADS / OQ;                      // K slices
+            const int oq = (int)threadIdx.x % OQ, ks = (int)threadIdx.x / OQ;
+            if (ks < KS) {
+                const int kper = (L.K + KS - 1) / KS, k0 = ks * kper, k1 = min(L.K, k0 + kper);
+                float4 acc[HD_JETS];
+#pragma unroll
+                for (int jb = 0; jb < HD_JETS; ++jb) acc[jb] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+                const float4* wp = reinterpret_cast<const float4*>(L.Wt) + oq;
+                auto load8 = [&](float4 (&wv)[8], int c) {
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) {
+                        wv[u] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+                        if (c + u < k1) wv[u] = __ldg(wp + (size_t)(c + u) * OQ);
+                    }
+                };
+                auto fma8 = [&](const float4 (&wv)[8], int c) {
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) {
+                        if (c + u < k1) {
+                            const float4 za = *reinterpret_cast<const float4*>(zin + (c + u) * HD_JETS);
+                            const float4 zb = *reinterpret_cast<const float4*>(zin + (c + u) * HD_JETS + 4);
+                            const float zv[HD_JETS] = {za.x, za.y, za.z, za.w, zb.x, zb.y, zb.z, zb.w};
+#pragma unroll
+                            for (int jb = 0; jb < HD_JETS; ++jb) {
+                                acc[jb].x = fmaf(zv[jb], wv[u].x, acc[jb].x); acc[jb].y = fmaf(zv[jb], wv[u].y, acc[jb].y);
+                                acc[jb].z = fmaf(zv[jb], wv[u].z, acc[jb].z); acc[jb].w = fmaf(zv[jb], wv[u].w, acc[jb].w);
+                            }
+                        }
+                    }
+                };
+                // two batches of eight weight rows alternate: the loads of one are in flight while the other is multiplied
+                float4 wa[8], wb[8];
+                load8(wa, k0);
+                for (int c = k0; c < k1; c += 16) {
+                    load8(wb, c + 8);
+                    fma8(wa, c);
+                    load8(wa, c + 16);
+                    fma8(wb, c + 8);
+                }
+#pragma unroll
+                for (int jb = 0; jb < HD_JETS; ++jb)
+                    *reinterpret_cast<float4*>(part + ((size_t)ks * HD_JETS + jb) * L.ld + 4 * oq) = acc[jb];
+            }
+            __syncthreads();
+            for (int it = threadIdx.x; it < HD_JETS * L.N; it += HD_THREADS) {
+                const int jb = it / L.N, o = it - jb * L.N;
+                float v = __ldg(L.shift + o);
+                for (int k2 = 0; k2 < KS; ++k2) v += part[((size_t)k2 * HD_JETS + jb) * L.ld + o];
+                if (last) {
+                    if (jb < nj) {
+                        const bool bad = poisoned || jet_n[b0 + jb] < 0;
+                        logits[(size_t)(b0 + jb) * hp.n_classes + o] = bad ? __int_as_float(0x7fc00000) : v;
+                    }
+                } else {
+                    zout[o * HD_JETS + jb] = fmaxf(v, 0.0f);
+                }
+            }
+        } else {
+            // narrow layer (the final one): one WARP per (jet, output), lanes split K, fixed-order shuffle reduction
+            const int wid = threadIdx.x >> 5, ln = threadIdx.x & 31;
+            for (int it = wid; it < HD_JETS * L.N; it += HD_THREADS / 32) {
+                const int jb = it / L.N, o = it - jb * L.N;
+                float a0 = 0.0f;
+                for (int c = ln; c < L.K; c += 32) a0 = fmaf(zin[c * HD_JETS + jb], __ldg(L.Wt + (size_t)c * L.ld + o), a0);
+#pragma unroll
+                for (int sh = 16; sh > 0; sh >>= 1) a0 += __shfl_xor_sync(0xffffffffu, a0, sh);
+                const float v = a0 + __ldg(L.shift + o);
+                if (ln == 0) {
+                    if (last) {
+                        if (jb < nj) {
+                            const bool bad = poisoned || jet_n[b0 + jb] < 0;
+                            logits[(size_t)(b0 + jb) * hp.n_classes + o] = bad ? __int_as_float(0x7fc00000) : v;
+                        }
+                    } else {
+                        zout[o * HD_JETS + jb] = fmaxf(v, 0.0f);
+                    }
+                }
+            }
+        }
+        __syncthreads();
+        float* t = zin; zin = zout; zout = t;
+    }
+}
+
 }  // namespace
 
+// x != null: pool the stored block output [N, C]; x == null: the channel sums are in w.pool (pooling EdgeConv epilogue)
 int launch_pool_head(const gnn_model& m, const float* x, int B, const Workspace& w, float* logits, cudaStream_t s) {
     if (B == 0) return 0;
     HeadParams hp;
@@ -177,6 +309,16 @@ int launch_pool_head(const gnn_model& m, const float* x, int B, const Workspace&
     hp.n_classes = m.arch.n_classes;
     hp.wmax = hp.C;
     for (int i = 0; i < m.n_fc; ++i) hp.wmax = std::max(hp.wmax, (m.fc[i].N + 3) & ~3);
+    if (x == nullptr) {
+        size_t part = 4;
+        for (int i = 0; i < m.n_fc; ++i) {
+            const int OQ = m.fc[i].ld / 4;
+            if (OQ >= 16 && OQ <= HD_THREADS) part = std::max(part, (size_t)(HD_THREADS / OQ) * HD_JETS * m.fc[i].ld);
+        }
+        const size_t smem = ((size_t)2 * HD_JETS * hp.wmax + part) * sizeof(float);
+        head_kernel<<<(B + HD_JETS - 1) / HD_JETS, HD_THREADS, smem, s>>>(w.pool, w.jet_n, w.meta, hp, B, logits);
+        return 1;
+    }
     const int G = std::max(1, PH_THREADS / (hp.C / 4));
     size_t part = (size_t)G * PH_JETS * hp.C;                    // pooling partials, reused as the split-K partials
     for (int i = 0; i < m.n_fc; ++i) {
@@ -188,7 +330,24 @@ int launch_pool_head(const gnn_model& m, const float* x, int B, const Workspace&
     return 1;
 }
 
+// debug entry of the pooling EdgeConv epilogue: fixed-point channel sums -> g [B, C] = mean over the jet's particles
+__global__ void pooled_mean_kernel(const unsigned long long* __restrict__ pooled, const int32_t* __restrict__ jet_n,
+                                   const int32_t* __restrict__ meta, int B, int C, float* __restrict__ g) {
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= B * C) return;
+    const int n = meta[0] ? 0 : jet_n[e / C];
+    g[e] = n > 0 ? fixed_mean(pooled[e], n) : 0.0f;
+}
+
+int launch_pooled_mean(const gnn_model& m, int B, const Workspace& w, float* g, cudaStream_t s) {
+    if (B == 0) return 0;
+    const int C = m.arch.channels[m.arch.n_blocks - 1][2];
+    pooled_mean_kernel<<<(B * C + 255) / 256, 256, 0, s>>>(w.pool, w.jet_n, w.meta, B, C, g);
+    return 1;
+}
+
 int pool_head_configure() {
-    return cudaFuncSetAttribute(pool_head_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024) == cudaSuccess
+    return cudaFuncSetAttribute(pool_head_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024) == cudaSuccess &&
+                   cudaFuncSetAttribute(head_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024) == cudaSuccess
                ? GNN_OK : GNN_ERR_CUDA;
 }

@@ -30,11 +30,24 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
         : "memory");
     return ok != 0;
 }
-// Bounded spin: a protocol bug traps (launch failure reported to the host) instead of hanging the GPU.
+// Bounded wait: a protocol bug traps (launch failure reported to the host) instead of hanging the GPU.  The bound is TIME
+// (%globaltimer, 4 s), not a poll count, so a sanitizer, a debugger, ncu replay or a time-sliced GPU cannot trip it; the
+// timer is only read once every 4096 failed polls (try_wait itself suspends the warp for a hardware-chosen interval).
+__device__ __forceinline__ uint64_t global_timer_ns() {
+    uint64_t t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    if (mbar_try_wait(bar, parity)) return;
     uint32_t spins = 0;
+    uint64_t t0 = 0;
     while (!mbar_try_wait(bar, parity)) {
-        if (++spins > (1u << 22)) __trap();
+        if ((++spins & 4095u) == 0u) {
+            const uint64_t now = global_timer_ns();
+            if (t0 == 0) t0 = now;
+            else if (now - t0 > 4000000000ull) __trap();
+        }
     }
 }
 
@@ -212,10 +225,10 @@ __device__ __forceinline__ void tmem_st32(uint32_t taddr, const float (&v)[32]) 
 __device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 
 // ---- packed fp16 helpers (E3 row reduction) ---------------------------------------------------------------------------------
-// {lo, hi} fp32 -> f16x2 with ReLU folded into the conversion (RNE)
+// {lo, hi} fp32 -> f16x2 with ReLU folded into the conversion (RNE), saturating at the largest finite fp16
 __device__ __forceinline__ uint32_t pack_relu_f16x2(float lo, float hi) {
     uint32_t d;
-    asm("cvt.rn.relu.f16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(hi), "f"(lo));
+    asm("cvt.rn.relu.satfinite.f16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(hi), "f"(lo));
     return d;
 }
 __device__ __forceinline__ uint32_t add_f16x2(uint32_t a, uint32_t b) {

@@ -117,15 +117,22 @@ def test_particlenet_end_to_end_256(pn):
 
 
 def test_particlenet_full_batch_1024(pn):
-    """BASELINE configs[1] at its full size, in the launch configuration bench.py times (one gnn_infer)."""
+    """BASELINE configs[1] at its full size, in the launch configuration bench.py times (one gnn_infer).  R21 to the
+    letter: the staged run gives the GPU's neighbour sets of every block; a jet may miss the 1e-4 bar only if it holds
+    an ambiguous point (oracle gap < 1e-5 relative) whose GPU set actually differs, and every such jet is counted."""
     a, w, m = pn
     b = synth.make_particlenet_batch()
+    staged, r, report, excluded = staged_fp32(m, a, w, b)
+    assert all(bad == 0 for bad, _ in report), report          # no set differs outside the near-tie band
     lg = run_ragged(m, b)
-    ref = oracle.forward(a, w, b.feats, b.coords, b.offsets)
-    err = np.abs(lg - ref).max(1)
-    assert (err < LOGIT_TOL).mean() >= 0.995                   # jets hit by an ambiguous flip (R21) may exceed
+    assert np.array_equal(lg, staged)                          # gnn_infer == the staged entry points, bitwise
+    err = np.abs(lg - r["logits"]).max(1)
+    print("fp32 B=1024: max |dlogit| over non-excluded jets %.2e, excluded jets %d, ambiguous flips per block %s" %
+          (err[~excluded].max(), excluded.sum(), [f for _, f in report]))
+    assert (err[~excluded] < LOGIT_TOL).all()
+    assert excluded.sum() <= 8                                 # expected ~1-2e-4 of the points per block (SURVEY 8(c) R21)
     assert np.median(err) < 2e-5
-    assert (np.argmax(lg, 1) == np.argmax(ref, 1)).all()
+    assert (np.argmax(lg, 1) == np.argmax(r["logits"], 1)).all()
 
 
 def test_edge_case_set(pn):
