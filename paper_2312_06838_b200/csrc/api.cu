@@ -148,12 +148,7 @@ int alloc_workspace(gnn_model* m, Workspace& w) {
     if ((rc = dev_alloc(m, &w.poffsets, Bmax + 1)) != GNN_OK) return rc;
     if ((rc = dev_alloc(m, &w.pcounts, Bmax)) != GNN_OK) return rc;
     if ((rc = dev_alloc(m, &w.hlogits, Bmax * a.n_classes)) != GNN_OK) return rc;
-    // the auxiliary stream carries the per-particle pre kernels, which must reach the SMs BEFORE the kNN CTAs of the caller's
-    // stream (one pre CTA per SM, kNN CTAs in the room that is left; the other way round the kNN CTAs fill every SM and the
-    // two kernels run one after the other): highest priority, which the block scheduler honours between ready grids
-    int prio_lo = 0, prio_hi = 0;
-    GNN_CUDA_TRY(cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi));
-    GNN_CUDA_TRY(cudaStreamCreateWithPriority(&w.aux, cudaStreamNonBlocking, prio_hi));
+    GNN_CUDA_TRY(cudaStreamCreateWithFlags(&w.aux, cudaStreamNonBlocking));
     GNN_CUDA_TRY(cudaEventCreateWithFlags(&w.ev_x, cudaEventDisableTiming));
     GNN_CUDA_TRY(cudaEventCreateWithFlags(&w.ev_pre, cudaEventDisableTiming));
     GNN_CUDA_TRY(cudaMemset(w.status, 0, sizeof(unsigned)));

@@ -36,47 +36,34 @@ namespace {
 using namespace tc05;
 
 constexpr int TILE_ROWS = 128;
-// developer knobs (python -m paper_2312_06838_b200.build reads GNN_NVCC_DEFS): which widths run E2 / E3 on separate warp sets
-#ifndef EDGE_SPLIT_MASK
-#define EDGE_SPLIT_MASK 0
+// developer knobs (python -m paper_2312_06838_b200.build reads GNN_NVCC_DEFS): epilogue warp width and register caps
+#ifndef EDGE_CWE_256
+#define EDGE_CWE_256 128
+#endif
+#ifndef EDGE_CWE_128
+#define EDGE_CWE_128 128
+#endif
+#ifndef EDGE_MAXREG_256
+#define EDGE_MAXREG_256 96
 #endif
 #ifndef EDGE_MAXREG_128
 #define EDGE_MAXREG_128 80
 #endif
 
-// SPLIT_: E2 and E3 on separate warp sets with per-role register budgets (compiled for k = 16 only)
-__host__ __device__ constexpr bool edge_split(int C, int LOGK) { return (((EDGE_SPLIT_MASK) & C) != 0) && LOGK == 4; }
-
-template <int C, bool SPLIT_ = false>
+template <int C>
 struct EdgeCfg {
     static constexpr bool PAIR = C >= 256;                    // CTA pair: the weights, split over two SMs, stay resident
     static constexpr int KB = (C + 63) / 64;                  // 64-wide K blocks per layer
     static constexpr int KW = C < 64 ? C : 64;                // columns of one K block that are in use
-    static constexpr int CWE = C >= 128 ? 128 : C;            // columns per epilogue warp (measured best: more, narrower epilogue
+    static constexpr int CWE = C >= 256 ? (EDGE_CWE_256) : (C >= 128 ? (EDGE_CWE_128) : C);   // columns per epilogue warp (measured best: more, narrower epilogue
     static constexpr int NE = 4 * (C / CWE);                  // warps cost registers); lane quadrant q = w & 3, column group w >> 2
     static constexpr int GH = 2;                              // row parts of the gather
     static constexpr int NG = GH * KB;                        // gather warps: K block g % KB, row part g / KB
     static constexpr int RW = TILE_ROWS / GH;                 // rows per gather warp
-    static constexpr bool SPLIT = SPLIT_;                      // E2 and E3 on separate warp sets: E2(t+1) need not wait for E3(t)
-    static constexpr int NEP = SPLIT ? 2 * NE : NE;           // epilogue warps in total: [0, NE) run E2, [NE, 2 NE) run E3
+    static constexpr int NEP = NE;                            // epilogue warps: each runs E2 then E3 of a tile
     static constexpr int MMA_WARP = NEP + NG;
-    // SPLIT: the roles get different register budgets (setmaxnreg, per warpgroup of four warps), so every role starts on a
-    // warpgroup boundary and the MMA warp brings three idle warps along
-    static constexpr int THREADS = SPLIT ? 32 * (NEP + NG + 4) : 32 * (NEP + NG + 1);
-    static constexpr int MAXREG = SPLIT ? (C >= 256 ? 72 : 64)  // SPLIT: registers at launch (THREADS * MAXREG * MIN_CTAS <= 65536)
-                                        : (C >= 256 ? 96 : (C >= 128 ? (EDGE_MAXREG_128) : 64));   // registers are per SM quarter: ceil(warps / 4) * 32 * MAXREG * MIN_CTAS <= 16384
-    // SPLIT register budgets per role (sum over the warps <= THREADS * MAXREG): gather, MMA warpgroup, E2, E3
-#ifndef RGG
-#define RGG (C >= 256 ? 56 : 48)
-#define RGM (C >= 256 ? 40 : 32)
-#define RGE2 64
-#define RGE3 112
-#endif
-    static constexpr int RG_G = RGG, RG_MMA = RGM, RG_E2 = RGE2, RG_E3 = RGE3;
-    static_assert(!SPLIT || (NE % 4 == 0 && NG % 4 == 0), "SPLIT needs warpgroup-aligned roles");
-#ifndef RG_NOCHECK
-    static_assert(!SPLIT || 32 * (NG * RG_G + 4 * RG_MMA + NE * RG_E2 + NE * RG_E3) <= THREADS * MAXREG, "SPLIT register budget");
-#endif
+    static constexpr int THREADS = 32 * (NEP + NG + 1);
+    static constexpr int MAXREG = C >= 256 ? (EDGE_MAXREG_256) : (C >= 128 ? (EDGE_MAXREG_128) : 64);   // registers are per SM quarter: ceil(warps / 4) * 32 * MAXREG * MIN_CTAS <= 16384
     static constexpr int KSTEPS_LAST = ((C - (KB - 1) * 64) + 15) / 16;
     static constexpr int NRB = PAIR ? C / 2 : C;              // weight rows (output channels) one CTA holds
     static constexpr int CHUNK_BYTES = NRB * 128;             // [NRB][64] bf16, 128B-swizzled
@@ -85,10 +72,18 @@ struct EdgeCfg {
     static constexpr int H_BYTES = KB * HK_BYTES;
     static constexpr int TMEM_COLS = 2 * C < 32 ? 32 : 2 * C; // D0 | D1
     static constexpr int NBAR = 3 * KB + 6;
+    // TR3 (k = 16 kernels of C >= 128): layer 3 is issued TRANSPOSED -- A = W3' (M = output channels), B = H2 (N = edge rows)
+    // -- so that an accumulator LANE is a channel and its columns are edges: the 16 neighbour rows of a particle are 16
+    // consecutive columns of one thread, and the mean over k is an in-thread sum (no shuffles, a scalar shift per thread).
+    // Measured on configs[1]: C = 128: 70 -> 64 us.  The code also covers pair mode (M = 256 channels over the two CTAs,
+    // N = 256 edge rows = the tile of CTA 0 then the tile of CTA 1, each CTA ending up with ITS 128 channels of all 16
+    // particles): there E3 shrinks from 3.4 k to 2.2 k cycles per tile and the pooling epilogue becomes free, but the
+    // transposed MMAs issue at ~190 cycles each instead of ~150 and the kernel loses 25 us, so C = 256 keeps the row layout.
+    static constexpr bool TR3_OK = C == 128;
     static constexpr int SMALL_BYTES = 2 * C * 4 + NBAR * 8 + 16;
     static constexpr int SMEM_BYTES = W_BYTES + H_BYTES + SMALL_BYTES + 1024;
     // POOL variant (last block, k = 16): per epilogue warp and 32-column slab, two 64-bit fixed-point accumulators per lane
-    static constexpr int POOL_BYTES = NE * (CWE / 32) * 32 * 16;
+    static constexpr int POOL_BYTES = TR3_OK ? 0 : NE * (CWE / 32) * 32 * 16;   // (TR3 keeps the sums in registers)
     static constexpr int SMEM_BYTES_POOL = SMEM_BYTES + POOL_BYTES;
     static constexpr int MIN_CTAS = C >= 256 ? 1 : (C >= 128 ? 2 : 4);
     static constexpr int NRANKS = PAIR ? 2 : 1;
@@ -128,15 +123,11 @@ struct EdgeParams {
 // 64-bit integer (per-lane accumulators in shared memory across the consecutive tiles of a jet, one red.global.add.u64
 // per (lane, column) when the jet changes), so the result does not depend on tile boundaries, CTA assignment or the
 // order of the atomics: batch-composition invariance stays bitwise.
-template <int N>
-__device__ __forceinline__ void setmaxnreg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
-template <int N>
-__device__ __forceinline__ void setmaxnreg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
-
 template <int C, int LOGK, bool POOL>
 __device__ __forceinline__ void edge_body(const EdgeParams& p) {
     static_assert(!POOL || LOGK == 4, "the pooling epilogue is written for k = 16");
-    using Cfg = EdgeCfg<C, edge_split(C, LOGK)>;
+    using Cfg = EdgeCfg<C>;
+    constexpr bool TR3 = Cfg::TR3_OK && LOGK == 4;
     constexpr bool PAIR = Cfg::PAIR;
     constexpr int KB = Cfg::KB, NE = Cfg::NE, CWE = Cfg::CWE;
     extern __shared__ __align__(1024) uint8_t smem_raw[];
@@ -205,13 +196,8 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
         if (lane == 0) { if constexpr (PAIR) mbar_arrive_cluster(bar, 0); else mbar_arrive(bar); }
     };
 
-    // SPLIT: register budgets per role, set at the top of each (warpgroup-uniform) role branch so that the code a budget
-    // governs is exactly the code the setmaxnreg dominates: the E3 warps, whose row reduction is the longest serial piece of
-    // a tile, get what the gather, E2 and MMA warps give back
-    if (warp >= Cfg::MMA_WARP) {
-        if constexpr (Cfg::SPLIT) setmaxnreg_dec<Cfg::RG_MMA>();   // (the three idle warps of this warpgroup fall through)
+    if (warp == Cfg::MMA_WARP) {
         // ===== weight load (every chunk once, resident for the life of the CTA), then MMA issuer (leader CTA of a pair) ====
-        if (warp == Cfg::MMA_WARP) {
         if (lane == 0) {
             mbar_arrive_expect_tx(w_full, Cfg::W_BYTES);
             const uint8_t* src = p.wimg + (size_t)rank * Cfg::W_BYTES;
@@ -221,6 +207,7 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
         }
         if (lane == 0 && rank == 0) {
             constexpr uint32_t idesc = idesc_bf16_f32(PAIR ? 256 : 128, C);
+            constexpr uint32_t idesc_tr = idesc_bf16_f32(PAIR ? 256 : 128, PAIR ? 256 : 128);   // TR3: M = channels, N = edge rows
             const uint32_t h_addr = smem_u32(H), w_addr = smem_u32(Wsm);
             mbar_wait(w_full, 0);
             if (PAIR) mbar_wait(w_peer, 0);
@@ -234,9 +221,15 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
                         tc_fence_after();
                         const int ksteps = (kb == KB - 1) ? Cfg::KSTEPS_LAST : 4;
                         for (int ks = 0; ks < ksteps; ++ks) {
-                            const uint64_t ad = desc_sw128(h_addr + kb * Cfg::HK_BYTES + ks * 32);
-                            const uint64_t bd = desc_sw128(w_addr + (layer * KB + kb) * Cfg::CHUNK_BYTES + ks * 32);
-                            mma_bf16_ss_g<PAIR>(tmem + layer * C, ad, bd, idesc, Cfg::BIAS_ACC ? 1u : (uint32_t)((kb | ks) != 0));
+                            const uint64_t hd = desc_sw128(h_addr + kb * Cfg::HK_BYTES + ks * 32);
+                            const uint64_t wd = desc_sw128(w_addr + (layer * KB + kb) * Cfg::CHUNK_BYTES + ks * 32);
+                            const uint32_t acc = Cfg::BIAS_ACC ? 1u : (uint32_t)((kb | ks) != 0);
+                            if (TR3 && layer == 1) {
+                                // D1[channel, edge]: weights are the M operand; pair mode: N = 256 = the 128 edge rows of each CTA
+                                mma_bf16_ss_g<PAIR>(tmem + C, wd, hd, idesc_tr, acc);
+                            } else {
+                                mma_bf16_ss_g<PAIR>(tmem + layer * C, hd, wd, idesc, acc);
+                            }
                         }
                         if (layer == 1) mma_commit_g<PAIR>(&h_free[kb]);   // gather of the next tile may overwrite it
                     }
@@ -244,9 +237,7 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
                 }
             }
         }
-        }
     } else if (warp >= Cfg::NEP) {
-        if constexpr (Cfg::SPLIT) setmaxnreg_dec<Cfg::RG_G>();
         // ===== gather warps: H1 = bf16(relu(u_i + v_j)) for K block gk, rows 64*half .. +63; they run one tile ahead of the
         // epilogue (their only dependency is h_free of the previous tile), so the L2 latency of the gather is off the
         // MMA <-> epilogue critical path ===============================================================================
@@ -335,13 +326,8 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
             for (int a = 0; a < NI; ++a) idx_r[a] = idx_n[a];
         }
     } else {
-        if constexpr (Cfg::SPLIT) {
-            if (warp < NE) { if constexpr (Cfg::RG_E2 < Cfg::MAXREG) setmaxnreg_dec<Cfg::RG_E2>(); }
-            else setmaxnreg_inc<Cfg::RG_E3>();
-        }
         // ===== epilogue warps: E2 (D0 -> H2) and E3 (D1 -> mean -> y) for lane quadrant q, columns [cg*CWE, +CWE) ==========
         const int q = warp & 3, cg = (warp % NE) >> 2;
-        const bool doE2 = !Cfg::SPLIT || warp < NE, doE3 = !Cfg::SPLIT || warp >= NE;
         const int row = 32 * q + lane;                           // TMEM lane = edge row of the tile
         const int col0 = cg * CWE;
         constexpr int SLABS = CWE / 32;
@@ -376,8 +362,8 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
             tc_fence_before();
             arrive_leader(&d_free[layer]);
         };
-        if (doE2) reset_acc(0);
-        if (doE3) reset_acc(1);
+        reset_acc(0);
+        reset_acc(1);
         int idx_cur = load_idx(tile_p0(0));
         // POOL: this lane's accumulators (slab s -> columns col0 + 32 s + cb, + 1) of the jet `jid_acc` it is walking
         ulonglong2* acc_s = pool_s + ((warp % NE) * SLABS) * 32 + lane;
@@ -395,12 +381,38 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
 #pragma unroll
             for (int s = 0; s < SLABS; ++s) acc_s[s * 32] = make_ulonglong2(0ull, 0ull);
         };
-        if constexpr (POOL) {
+        if constexpr (POOL && !TR3) {
 #pragma unroll
             for (int s = 0; s < SLABS; ++s) acc_s[s * 32] = make_ulonglong2(0ull, 0ull);
             const int pt0 = tile_p0(0) + (row >> logk);
             jid_cur = pt0 < N ? __ldg(p.pjid + pt0) : -1;
         }
+        // ---- TR3 state: lane l < NP describes particle l of the (pair) tile: packed row (-1: none), valid-neighbour mask,
+        // k / k_eff, jet.  Pair tile w covers the 16 consecutive particles of tiles 2w and 2w + 1.
+        constexpr int NP = PAIR ? 16 : 8;                        // particles of a (pair) tile, k = 16
+        constexpr int NCG = NE / 4, NPW = NP / NCG;              // column groups of epilogue warps; particles per warp
+        int m_pt = -1, m_jid = -1, n_pt = -1, n_jid = -1;
+        unsigned m_mask = 0, n_mask = 0;
+        float m_inv = 0.0f, n_inv = 0.0f;
+        auto load_meta = [&](int pb, int& o_pt, unsigned& o_mask, float& o_inv, int& o_jid) {
+            o_pt = -1; o_mask = 0u; o_inv = 0.0f; o_jid = -1;
+            const int ptl = pb + lane;
+            if (lane < NP && ptl < N) {
+                const int4* ir = reinterpret_cast<const int4*>(p.idx + (size_t)ptl * 16);
+                unsigned mk = 0u;
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    const int4 a = __ldg(ir + i);
+                    mk |= (a.x >= 0 ? 1u : 0u) << (4 * i) | (a.y >= 0 ? 2u : 0u) << (4 * i) | (a.z >= 0 ? 4u : 0u) << (4 * i) | (a.w >= 0 ? 8u : 0u) << (4 * i);
+                }
+                const int cnt = __popc(mk);
+                o_pt = ptl; o_mask = mk;
+                o_inv = cnt > 0 ? 16.0f / (float)cnt : 0.0f;     // W3', t3 carry 1/k (host): the f16 sum over the k columns is the mean
+                if constexpr (POOL) o_jid = __ldg(p.pjid + ptl);
+            }
+        };
+        unsigned long long pacc = 0ull;                          // TR3 + POOL: this thread's channel sum of the jet jid_acc
+        if constexpr (TR3) load_meta(tile_p0(0) - (PAIR ? (int)rank * p.TP : 0), m_pt, m_mask, m_inv, m_jid);
         for (int t = 0; t < T; ++t) {
             const uint32_t ph = t & 1;
             const int p0 = tile_p0(t);
@@ -408,12 +420,11 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
             // the start of E3 (a value held in registers across E2 is spilled, and the spill store waits for the load)
             const int pt = p0 + (row >> logk);
             const size_t obase = (size_t)pt * C + col0 + cb;
-            if (pt < N && nout <= 2) {
+            if (!TR3 && pt < N && nout <= 2) {
 #pragma unroll
                 for (int s = 0; s < SLABS; ++s) asm volatile("prefetch.global.L2 [%0];" ::"l"(p.R + obase + s * 32));
             }
             // ---- E2: H2 = bf16(relu(D0)); the TMEM load of slab s+1 is in flight while slab s is converted ---------------
-            if (doE2) {
             mbar_wait(&d_full[0], ph);                           // implies every layer-2 read of H1 is done
             tc_fence_after();
             {
@@ -445,10 +456,60 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
                 }
             }
             if (t + 1 < T) reset_acc(0);
-            }
             // ---- E3: mean over the valid neighbours of relu(D1), + shortcut, ReLU.  The row reduction runs on packed f16x2
             // (two columns per register): a halving butterfly over the k rows of a particle, fp32 again for the mean ------------
-            if (doE3) {
+            if constexpr (TR3) {
+                // ---- E3, transposed accumulator: thread = channel, 16 consecutive columns = the k neighbour rows of a particle ----
+                const int ch = (PAIR ? 128 * (int)rank : 0) + 32 * q + lane;
+                const float t3c = shifts_s[C + ch];
+                const uint32_t tb1 = tmem + ((uint32_t)(32 * q) << 16) + C + cg * (NPW * 16);
+                // particle behind column group i of this warp (pair mode: the columns of CTA 0's tile, then CTA 1's)
+                auto part_lane = [&](int i) { return cg * NPW + i; };
+                if (t + 1 < T) load_meta(tile_p0(t + 1) - (PAIR ? (int)rank * p.TP : 0), n_pt, n_mask, n_inv, n_jid);
+                else { n_pt = -1; n_mask = 0u; n_inv = 0.0f; n_jid = -1; }
+                float rr[NPW];
+#pragma unroll
+                for (int i = 0; i < NPW; ++i) {
+                    const int ptl = __shfl_sync(0xffffffffu, m_pt, part_lane(i));
+                    rr[i] = ptl >= 0 ? __ldg(p.R + (size_t)ptl * C + ch) : 0.0f;
+                }
+                mbar_wait(&d_full[1], ph);
+                tc_fence_after();
+                float v[16];
+                tmem_ld16(tb1, v);
+#pragma unroll
+                for (int i = 0; i < NPW; ++i) {
+                    tmem_ld_wait();
+                    uint32_t h[8];
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) h[u] = pack_relu_f16x2(v[2 * u] + t3c, v[2 * u + 1] + t3c);
+                    if (i + 1 < NPW) tmem_ld16(tb1 + 16 * (i + 1), v);       // in flight during this particle's sum
+                    const int pl = part_lane(i);
+                    const int ptl = __shfl_sync(0xffffffffu, m_pt, pl);
+                    const unsigned mk = __shfl_sync(0xffffffffu, m_mask, pl);
+                    const float inv = __shfl_sync(0xffffffffu, m_inv, pl);
+                    if (mk != 0xffffu) {                         // k_eff < k (warp-uniform): rows without a neighbour add nothing
+#pragma unroll
+                        for (int u = 0; u < 8; ++u)
+                            h[u] &= (((mk >> (2 * u)) & 1u) ? 0x0000ffffu : 0u) | (((mk >> (2 * u + 1)) & 1u) ? 0xffff0000u : 0u);
+                    }
+                    const uint32_t a0 = add_f16x2(h[0], h[1]), a1 = add_f16x2(h[2], h[3]), a2 = add_f16x2(h[4], h[5]), a3 = add_f16x2(h[6], h[7]);
+                    const float2 f = unpack_f16x2(add_f16x2(add_f16x2(a0, a1), add_f16x2(a2, a3)));
+                    const float y = fmaxf(fmaf(f.x + f.y, inv, rr[i]), 0.0f);
+                    if constexpr (POOL) {
+                        const int jid = __shfl_sync(0xffffffffu, m_jid, pl);
+                        if (jid != jid_acc) {                    // warp-uniform: the jet changed, flush its exact fixed-point sum
+                            if (jid_acc >= 0) atomicAdd(p.pool + (size_t)jid_acc * C + ch, pacc);
+                            pacc = 0ull; jid_acc = jid;
+                        }
+                        if (ptl >= 0) pacc += to_fixed_32_32(y);
+                    } else {
+                        if (ptl >= 0) p.y[(size_t)ptl * C + ch] = y;
+                    }
+                }
+                if (t + 1 < T) reset_acc(1);
+                m_pt = n_pt; m_mask = n_mask; m_inv = n_inv; m_jid = n_jid;
+            } else {
             const int idx_next = (t + 1 < T) ? load_idx(tile_p0(t + 1)) : -1;
             int jid_next = -1;
             if constexpr (POOL) {
@@ -542,24 +603,20 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
             if constexpr (POOL) jid_cur = jid_next;
             }
         }
-        if constexpr (POOL) pool_flush();
+        if constexpr (POOL) {
+            if constexpr (TR3) { if (jid_acc >= 0) atomicAdd(p.pool + (size_t)jid_acc * C + ((PAIR ? 128 * (int)rank : 0) + 32 * q + lane), pacc); }
+            else pool_flush();
+        }
     }
     tc_fence_before();
     if constexpr (PAIR) cluster_sync_all(); else __syncthreads();
     if (warp == Cfg::MMA_WARP) tmem_dealloc_g<PAIR>(tmem, Cfg::TMEM_COLS);
 }
 
-// two entry points: one register budget for every warp (__maxnreg__), or the budget at launch with setmaxnreg per role
 template <int C, int LOGK, bool POOL>
-__global__ void __launch_bounds__((EdgeCfg<C, false>::THREADS)) __maxnreg__((EdgeCfg<C, false>::MAXREG)) edge_kernel(EdgeParams p) {
-    if constexpr (!edge_split(C, LOGK)) edge_body<C, LOGK, POOL>(p);
+__global__ void __launch_bounds__(EdgeCfg<C>::THREADS) __maxnreg__(EdgeCfg<C>::MAXREG) edge_kernel(EdgeParams p) {
+    edge_body<C, LOGK, POOL>(p);
 }
-template <int C, int LOGK, bool POOL>
-__global__ void __launch_bounds__((EdgeCfg<C, true>::THREADS), (EdgeCfg<C, true>::MIN_CTAS)) edge_kernel_ws(EdgeParams p) {
-    if constexpr (edge_split(C, LOGK)) edge_body<C, LOGK, POOL>(p);
-}
-template <int C, int LOGK, bool POOL>
-auto edge_entry() { if constexpr (edge_split(C, LOGK)) return edge_kernel_ws<C, LOGK, POOL>; else return edge_kernel<C, LOGK, POOL>; }
 
 // ---- wide blocks (C = 512, configs[4] wide variant): the 1 MB of W2', W3' cannot be resident even split over a CTA pair,
 // and two 512-column accumulators exceed TMEM.  This kernel is the simple, sequential form: one CTA per SM, one tile at a
@@ -1166,9 +1223,9 @@ void pack_layer(const std::vector<float>& W, int C, int NRB, int row0, std::vect
 
 template <int C, int LOGK, bool POOL>
 int configure_edge(Bf16BlockDev& b, int n_sms) {
-    using Cfg = EdgeCfg<C, edge_split(C, LOGK)>;
+    using Cfg = EdgeCfg<C>;
     constexpr int SMEM = POOL ? Cfg::SMEM_BYTES_POOL : Cfg::SMEM_BYTES;
-    auto* kern = edge_entry<C, LOGK, POOL>();
+    auto* kern = edge_kernel<C, LOGK, POOL>;
     GNN_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM));
     GNN_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
     int cap;
@@ -1204,7 +1261,7 @@ int configure_edge_c(Bf16BlockDev& b, int n_sms, int k) {
 
 template <int C, int LOGK, bool POOL>
 int launch_edge_t(const EdgeParams& p_in, int grid_cap, cudaStream_t s) {
-    using Cfg = EdgeCfg<C, edge_split(C, LOGK)>;
+    using Cfg = EdgeCfg<C>;
     constexpr int SMEM = POOL ? Cfg::SMEM_BYTES_POOL : Cfg::SMEM_BYTES;
     EdgeParams p = p_in;
     const int n_work = Cfg::PAIR ? (p.n_tiles + 1) / 2 : p.n_tiles;
@@ -1222,9 +1279,9 @@ int launch_edge_t(const EdgeParams& p_in, int grid_cap, cudaStream_t s) {
         at[0].id = cudaLaunchAttributeClusterDimension;
         at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
         cfg.attrs = at; cfg.numAttrs = 1;
-        GNN_CUDA_TRY(cudaLaunchKernelEx(&cfg, edge_entry<C, LOGK, POOL>(), p));
+        GNN_CUDA_TRY(cudaLaunchKernelEx(&cfg, edge_kernel<C, LOGK, POOL>, p));
     } else {
-        edge_entry<C, LOGK, POOL>()<<<n_units, Cfg::THREADS, SMEM, s>>>(p);
+        edge_kernel<C, LOGK, POOL><<<n_units, Cfg::THREADS, SMEM, s>>>(p);
     }
     return GNN_OK;
 }

@@ -183,10 +183,10 @@ knn_group_coords_kernel(const float* __restrict__ space, int D, const int32_t* _
 }
 
 // ---- feature spaces: Gram matrix on the tensor cores -------------------------------------------------------------------------
-// thread = row = TMEM lane; warp 0 also owns the TMEM allocation and its lane 0 issues the MMAs.  Exactly FOUR warps (one per
-// SM sub-partition, 64 registers): the register file is split per sub-partition, and this is what still fits beside a CTA of
-// the per-particle pre kernel (17 warps x 88 registers) running on the other stream
-constexpr int KG_THREADS = 128;
+// warps 0-3: thread = row = TMEM lane (selection); warps 4-7 help with the load, the means and the centring pass; warp 4 owns
+// the TMEM allocation and its lane 0 issues the MMAs
+constexpr int KG_THREADS = 256;
+constexpr int KG_MMA_WARP = 4;
 
 template <int D>
 struct KnnGroupCfg {
@@ -197,19 +197,8 @@ struct KnnGroupCfg {
     static constexpr int SMEM_BYTES = X_BYTES + MEAN_BYTES + KG_ROWS * 4 + KG_ROWS + (int)sizeof(GroupInfo) + 2 * 8 + 16 + 64;
 };
 
-__device__ __forceinline__ void tmem_ld16(uint32_t taddr, float (&v)[16]) {
-    uint32_t* r = reinterpret_cast<uint32_t*>(v);
-    asm volatile(
-        "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
-        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
-        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
-          "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
-        : "r"(taddr)
-        : "memory");
-}
-
 template <int D, int K>
-__global__ void __launch_bounds__(KG_THREADS) __maxnreg__(K <= 16 ? 64 : 96)
+__global__ void __launch_bounds__(KG_THREADS)
 knn_group_gram_kernel(const float* __restrict__ space, const int32_t* __restrict__ jet_start, const int32_t* __restrict__ jet_n,
                       const int32_t* __restrict__ meta, const int2* __restrict__ groups, int32_t* __restrict__ idx_out,
                       int32_t* __restrict__ pjid, int k, int local_out) {
@@ -236,7 +225,7 @@ knn_group_gram_kernel(const float* __restrict__ space, const int32_t* __restrict
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int R = gi->R, r0 = gi->r0;
     if (tid == 0) { mbar_init(d_full, 1); fence_mbar_init(); }
-    if (warp == 0) tmem_alloc(tmem_ptr, 128);
+    if (warp == KG_MMA_WARP) tmem_alloc(tmem_ptr, 128);
     // (1) the tile's rows, raw fp32, with ONE round trip to memory: 16-byte cp.async per (row, chunk), all in flight
     const float* src = space + (size_t)r0 * D;
     constexpr int CPR = D / 4;                                  // 16-byte chunks per row
@@ -247,60 +236,57 @@ knn_group_gram_kernel(const float* __restrict__ space, const int32_t* __restrict
     }
     asm volatile("cp.async.commit_group;" ::: "memory");
     int jt = 0, c0 = 0, c1 = 0;
-    row_range(gi, tid, jt, c0, c1);
-    if (tid >= R) { c0 = 0; c1 = 0; }
-    rowjet_s[tid] = (uint8_t)jt;
-    if (tid < R && pjid) pjid[r0 + tid] = gi->j0 + jt;
+    if (tid < KG_ROWS) {
+        row_range(gi, tid, jt, c0, c1);
+        if (tid >= R) { c0 = 0; c1 = 0; }
+        rowjet_s[tid] = (uint8_t)jt;
+        if (tid < R && pjid) pjid[r0 + tid] = gi->j0 + jt;
+    }
     asm volatile("cp.async.wait_group 0;" ::: "memory");
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
     KTR();
     const uint32_t tmem = *tmem_ptr;
-    // (2) per-jet column means (lanes = consecutive columns: conflict-free); a jet's sum has a fixed order (two chains by the
-    //     row's parity inside the jet), so it does not depend on the group the jet landed in
+    // (2) per-jet column means (lanes = consecutive columns: conflict-free); a jet's sum has a fixed order (four chains by the
+    //     row's index inside the jet modulo 4, combined as (s0 + s2) + (s1 + s3)), so it does not depend on the group
     for (int e = tid; e < D * gi->nj; e += KG_THREADS) {
         const int t = e / D, c = e - t * D;
         const int a = gi->ls[t], n = gi->rows[t];
         const float* colp = reinterpret_cast<const float*>(X + (c >> 5) * Cfg::XK_BYTES) + a * 32 + (c & 31);
-        float s0 = 0.0f, s1 = 0.0f;
+        float s0 = 0.0f, s1 = 0.0f, s2 = 0.0f, s3 = 0.0f;
         int r = 0;
-        for (; r + 1 < n; r += 2) { s0 += colp[r * 32]; s1 += colp[(r + 1) * 32]; }
+        for (; r + 3 < n; r += 4) { s0 += colp[r * 32]; s1 += colp[(r + 1) * 32]; s2 += colp[(r + 2) * 32]; s3 += colp[(r + 3) * 32]; }
         if (r < n) s0 += colp[r * 32];
-        mean_s[t * D + c] = n > 0 ? (s0 + s1) / (float)n : 0.0f;
+        if (r + 1 < n) s1 += colp[(r + 1) * 32];
+        if (r + 2 < n) s2 += colp[(r + 2) * 32];
+        mean_s[t * D + c] = n > 0 ? ((s0 + s2) + (s1 + s3)) / (float)n : 0.0f;
     }
     __syncthreads();
     KTR();
-    // (3) in place: centre on the jet's mean, round to tf32 (RNA), apply the 128-byte swizzle.  One thread owns a whole
-    //     128-byte line (row, K block): it reads the eight chunks (rotated by the row so that the lanes of a quarter-warp hit
-    //     eight different bank groups), then writes them permuted.  Rows >= R keep whatever the buffer held: row i of A and
-    //     row j of B only reach G_ij, and no entry with i >= R or j >= R is ever used.
-    for (int e = tid; e < R * KBD; e += KG_THREADS) {
-        const int kb = e / R, r = e - kb * R;
+    // (3) in place: centre on the jet's mean, round to tf32 (RNA), apply the 128-byte swizzle.  One thread per 16-byte chunk,
+    //     the eight lanes of a quarter-warp on one 128-byte line (row, K block): they read it whole (eight bank groups) and
+    //     write it back permuted among themselves (chunk c -> c ^ (row & 7): again eight bank groups); the line's loads have
+    //     all landed before its first store issues (same warp, same instruction).  Rows >= R keep whatever the buffer
+    //     held: row i of A and row j of B only reach G_ij, and no entry with i >= R or j >= R is ever used.
+    for (int e = tid; e < R * KBD * 8; e += KG_THREADS) {
+        const int c = e & 7, l = e >> 3;
+        const int kb = l / R, r = l - kb * R;
         uint8_t* line = X + kb * Cfg::XK_BYTES + r * 128;
-        const float* mu_row = mean_s + (int)rowjet_s[r] * D + kb * 32;
-        uint4 o[8];
-#pragma unroll
-        for (int cc = 0; cc < 8; ++cc) {
-            const int c = (cc + r) & 7;
-            const float4 v = *reinterpret_cast<const float4*>(line + (c << 4));
-            const float4 mu = *reinterpret_cast<const float4*>(mu_row + 4 * c);
-            asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(o[cc].x) : "f"(v.x - mu.x));
-            asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(o[cc].y) : "f"(v.y - mu.y));
-            asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(o[cc].z) : "f"(v.z - mu.z));
-            asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(o[cc].w) : "f"(v.w - mu.w));
-        }
-#pragma unroll
-        for (int cc = 0; cc < 8; ++cc) {
-            const int c = (cc + r) & 7;
-            *reinterpret_cast<uint4*>(line + ((c ^ (r & 7)) << 4)) = o[cc];
-        }
+        const float4 v = *reinterpret_cast<const float4*>(line + (c << 4));
+        const float4 mu = *reinterpret_cast<const float4*>(mean_s + (int)rowjet_s[r] * D + kb * 32 + 4 * c);
+        uint4 o;
+        asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(o.x) : "f"(v.x - mu.x));
+        asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(o.y) : "f"(v.y - mu.y));
+        asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(o.z) : "f"(v.z - mu.z));
+        asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(o.w) : "f"(v.w - mu.w));
+        *reinterpret_cast<uint4*>(line + ((c ^ (r & 7)) << 4)) = o;
     }
     fence_proxy_async();
     __syncthreads();
     KTR();
     const int n16 = (R + 15) & ~15;
-    if (tid == 0) {
+    if (warp == KG_MMA_WARP && lane == 0) {
         tc_fence_after();
         const uint32_t idesc = idesc_tf32_f32(128, n16);
         const uint32_t x_addr = smem_u32(X);
@@ -313,8 +299,7 @@ knn_group_gram_kernel(const float* __restrict__ space, const int32_t* __restrict
             }
         mma_commit(d_full);
     }
-    __syncwarp();
-    {
+    if (warp < 4) {
         // thread = row i = TMEM lane; diagonal first (G_ii sits in this thread's own row), then the row of G 16 columns at a time
         mbar_wait(d_full, 0);
         tc_fence_after();
@@ -377,7 +362,7 @@ knn_group_gram_kernel(const float* __restrict__ space, const int32_t* __restrict
         printf("knn<%d> cta %d R %d: group %llu load %llu mean %llu centre %llu mma %llu select %llu store %llu (ns)\n", D, blockIdx.x, R,
                tr[1] - tr[0], tr[2] - tr[1], tr[3] - tr[2], tr[4] - tr[3], tr[5] - tr[4], tr[6] - tr[5], tr[7] - tr[6]);
 #endif
-    if (warp == 0) tmem_dealloc(tmem, 128);
+    if (warp == KG_MMA_WARP) tmem_dealloc(tmem, 128);
 }
 
 template <int K>
