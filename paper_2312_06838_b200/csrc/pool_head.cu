@@ -11,6 +11,24 @@
 
 namespace {
 
+// thread-block cluster helpers of head_split_kernel
+__device__ __forceinline__ unsigned tc_cluster_rank() {
+    unsigned r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ void tc_cluster_sync() {
+    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// generic address of `p` (a shared-memory object of this CTA) in CTA `rank` of the cluster
+template <typename T>
+__device__ __forceinline__ T* tc_map_shared_rank(T* p, unsigned rank) {
+    unsigned long long out;
+    asm volatile("mapa.u64 %0, %1, %2;" : "=l"(out) : "l"((unsigned long long)p), "r"(rank));
+    return reinterpret_cast<T*>(out);
+}
+
 constexpr int PH_THREADS = 256;
 constexpr int PH_JETS = 4;
 
@@ -173,10 +191,10 @@ pool_head_kernel(const float* __restrict__ x, const int32_t* __restrict__ jet_st
 // summed through shared memory in a fixed order; the narrow final layer runs one warp per (jet, output).
 // sum (unsigned 32.32 fixed point) / n in fp32: integer and fraction parts convert separately (no 64-bit or fp64 conversions,
 // which are slow); the result is within 1.5 ulp of the exact mean and depends on nothing but (sum, n)
-__device__ __forceinline__ float fixed_mean(unsigned long long v, int n) {
-    const float s = fmaf((float)(unsigned)(v & 0xffffffffull), 1.0f / 4294967296.0f, (float)(unsigned)(v >> 32));
-    return s / (float)n;
+__device__ __forceinline__ float fixed_value(unsigned long long v) {
+    return fmaf((float)(unsigned)(v & 0xffffffffull), 1.0f / 4294967296.0f, (float)(unsigned)(v >> 32));
 }
+__device__ __forceinline__ float fixed_mean(unsigned long long v, int n) { return fixed_value(v) / (float)n; }
 
 constexpr int HD_THREADS = 256;
 constexpr int HD_JETS = 8;
@@ -297,6 +315,152 @@ head_kernel(const unsigned long long* __restrict__ pooled, const int32_t* __rest
     }
 }
 
+
+// ---- the head with ONE hidden layer (every BASELINE config), outputs of the hidden layer split over a CLUSTER of CTAs -------
+// head_kernel above gives one CTA all of FC-1 for its jets: at B = 1024 that is 128 CTAs of 8 warps, one per SM, each walking
+// a 256 KB weight matrix through dependent batches of loads (ncu: 12 % warps active, 24 us).  Here a CTA owns HS_JETS jets x
+// HS_OUT hidden units and the H / HS_OUT CTAs of a jet group form a thread-block cluster: grid (jet groups, H / HS_OUT), one
+// wave at B = 1024.  Thread (oq, ks) holds 4 hidden units of K slice ks (C / 16 rows of Wt, all its loads in flight at once:
+// one round trip, kept in registers for both passes of 8 jets), slices are summed through shared memory in a fixed order,
+// bias + ReLU, then this CTA's share of the final layer (HS_OUT terms per logit, one warp per (jet, class), fixed shuffle
+// tree).  The shares go to the cluster's first CTA through distributed shared memory and are added there in rank order, so a
+// logit depends neither on CTA timing nor on the batch mates: batch-composition invariance stays bitwise.
+constexpr int HS_THREADS = 256;
+constexpr int HS_PASS = 8;                            // jets per pass (accumulators in registers)
+constexpr int HS_PASSES = 2;
+constexpr int HS_JETS = HS_PASS * HS_PASSES;
+constexpr int HS_OUT = 64;
+constexpr int HS_KS = HS_THREADS / (HS_OUT / 4);     // 16 K slices
+constexpr int HS_MAX_SPLIT = 8;                       // portable cluster size
+constexpr int HS_MAX_CLASSES = 4;
+
+template <int KPER>                                   // rows of Wt per K slice = C / HS_KS
+__global__ void __launch_bounds__(HS_THREADS)
+head_split_kernel(const unsigned long long* __restrict__ pooled, const int32_t* __restrict__ jet_n, const int32_t* __restrict__ meta,
+                  LinF32 L1, LinF32 L2, int B, int n_classes, float* __restrict__ logits) {
+    constexpr int C = KPER * HS_KS;
+    __shared__ __align__(16) float zT[C * HS_PASS];                  // pooled means of one pass, [channel][jet]
+    __shared__ __align__(16) float part[HS_KS * HS_PASS * HS_OUT];   // [ks][jet][out]
+    __shared__ float hT[HS_JETS * HS_OUT];                           // hidden activations of this CTA, [jet][out]
+    __shared__ float s_inv[HS_JETS];                                 // 1 / n (0 for empty, offending or absent jets)
+    __shared__ float cl_share[HS_MAX_SPLIT * HS_JETS * HS_MAX_CLASSES];   // rank 0: [rank][jet][class]
+    const unsigned rank = tc_cluster_rank(), n_rank = gridDim.y;
+    const int b0 = blockIdx.x * HS_JETS, o0 = blockIdx.y * HS_OUT;
+    const int nj = min(HS_JETS, B - b0);
+    const int tid = threadIdx.x, oq = tid % (HS_OUT / 4), ks = tid / (HS_OUT / 4);
+    const int wid = tid >> 5, ln = tid & 31;
+    // this thread's weights first: they depend on nothing
+    float4 wv[KPER];
+    const float4* wp = reinterpret_cast<const float4*>(L1.Wt + (size_t)(ks * KPER) * L1.ld + o0) + oq;
+#pragma unroll
+    for (int u = 0; u < KPER; ++u) wv[u] = __ldg(wp + (size_t)u * (L1.ld >> 2));
+    // the jets' channel sums of a pass: every load of a thread in flight before the first conversion (one round trip)
+    constexpr int CPT = (C + HS_THREADS - 1) / HS_THREADS;
+    unsigned long long pv[CPT][HS_PASS];
+    auto load_pooled = [&](int pass) {
+#pragma unroll
+        for (int i = 0; i < CPT; ++i)
+#pragma unroll
+            for (int jb = 0; jb < HS_PASS; ++jb) {
+                const int c = tid + i * HS_THREADS, j = pass * HS_PASS + jb;
+                pv[i][jb] = (c < C && j < nj) ? __ldg(pooled + (size_t)(b0 + j) * C + c) : 0ull;
+            }
+    };
+    load_pooled(0);
+    const bool poisoned = meta[0] != 0;
+    if (tid < HS_JETS) {
+        int n = (tid < nj && !poisoned) ? jet_n[b0 + tid] : 0;
+        s_inv[tid] = n > 0 ? 1.0f / (float)n : 0.0f;   // offending jet: pools nothing (its logits become NaN below); R12: empty jet pools to 0
+    }
+    // this warp's weights of the final layer (warp = (jet, class) items, lanes = hidden units ln and 32 + ln)
+    float w2a[HS_MAX_CLASSES], w2b[HS_MAX_CLASSES];
+#pragma unroll
+    for (int o = 0; o < HS_MAX_CLASSES; ++o) {
+        w2a[o] = o < n_classes ? __ldg(L2.Wt + (size_t)(o0 + ln) * L2.ld + o) : 0.0f;
+        w2b[o] = o < n_classes ? __ldg(L2.Wt + (size_t)(o0 + 32 + ln) * L2.ld + o) : 0.0f;
+    }
+    const float shift1 = __ldg(L1.shift + o0 + (tid % HS_OUT));
+    __syncthreads();
+#pragma unroll 1
+    for (int pass = 0; pass < HS_PASSES; ++pass) {
+#pragma unroll
+        for (int i = 0; i < CPT; ++i) {
+            const int c = tid + i * HS_THREADS;
+            if (c < C) {
+                float z[HS_PASS];
+#pragma unroll
+                for (int jb = 0; jb < HS_PASS; ++jb) z[jb] = fixed_value(pv[i][jb]) * s_inv[pass * HS_PASS + jb];
+                *reinterpret_cast<float4*>(zT + c * HS_PASS) = make_float4(z[0], z[1], z[2], z[3]);
+                *reinterpret_cast<float4*>(zT + c * HS_PASS + 4) = make_float4(z[4], z[5], z[6], z[7]);
+            }
+        }
+        if (pass + 1 < HS_PASSES) load_pooled(pass + 1);          // in flight during this pass's products
+        __syncthreads();
+        float4 acc[HS_PASS];
+#pragma unroll
+        for (int jb = 0; jb < HS_PASS; ++jb) acc[jb] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+#pragma unroll
+        for (int u = 0; u < KPER; ++u) {
+            const float4 za = *reinterpret_cast<const float4*>(zT + (ks * KPER + u) * HS_PASS);
+            const float4 zb = *reinterpret_cast<const float4*>(zT + (ks * KPER + u) * HS_PASS + 4);
+            const float zv[HS_PASS] = {za.x, za.y, za.z, za.w, zb.x, zb.y, zb.z, zb.w};
+#pragma unroll
+            for (int jb = 0; jb < HS_PASS; ++jb) {
+                acc[jb].x = fmaf(zv[jb], wv[u].x, acc[jb].x); acc[jb].y = fmaf(zv[jb], wv[u].y, acc[jb].y);
+                acc[jb].z = fmaf(zv[jb], wv[u].z, acc[jb].z); acc[jb].w = fmaf(zv[jb], wv[u].w, acc[jb].w);
+            }
+        }
+#pragma unroll
+        for (int jb = 0; jb < HS_PASS; ++jb)
+            *reinterpret_cast<float4*>(part + (ks * HS_PASS + jb) * HS_OUT + 4 * oq) = acc[jb];
+        __syncthreads();
+        for (int it = tid; it < HS_PASS * HS_OUT; it += HS_THREADS) {      // it = jb * HS_OUT + o, o = tid % HS_OUT
+            float v = shift1;
+#pragma unroll
+            for (int k2 = 0; k2 < HS_KS; ++k2) v += part[k2 * HS_PASS * HS_OUT + it];
+            hT[pass * HS_PASS * HS_OUT + it] = fmaxf(v, 0.0f);
+        }
+        __syncthreads();                                            // zT and part are rewritten by the next pass
+    }
+    // final layer, this CTA's HS_OUT terms: one warp per jet (all classes), then into the first CTA's shared memory
+    float* dst = tc_map_shared_rank(cl_share, 0) + rank * (HS_JETS * HS_MAX_CLASSES);
+    for (int jb = wid; jb < HS_JETS; jb += HS_THREADS / 32) {
+        const float ha = hT[jb * HS_OUT + ln], hb = hT[jb * HS_OUT + 32 + ln];
+#pragma unroll
+        for (int o = 0; o < HS_MAX_CLASSES; ++o) {
+            float a0 = fmaf(hb, w2b[o], ha * w2a[o]);
+#pragma unroll
+            for (int sh = 16; sh > 0; sh >>= 1) a0 += __shfl_xor_sync(0xffffffffu, a0, sh);
+            if (ln == 0) dst[jb * HS_MAX_CLASSES + o] = a0;
+        }
+    }
+    tc_cluster_sync();                                              // release / acquire: the shares are visible to rank 0
+    if (rank != 0) return;
+    for (int it = tid; it < nj * n_classes; it += HS_THREADS) {
+        const int jb = it / n_classes, o = it - jb * n_classes;
+        float v = __ldg(L2.shift + o);
+        for (unsigned y = 0; y < n_rank; ++y) v += cl_share[(y * HS_JETS + jb) * HS_MAX_CLASSES + o];
+        const bool bad = poisoned || jet_n[b0 + jb] < 0;
+        logits[(size_t)(b0 + jb) * n_classes + o] = bad ? __int_as_float(0x7fc00000) : v;
+    }
+}
+
+template <int KPER>
+int launch_head_split(const HeadParams& hp, int B, const Workspace& w, float* logits, cudaStream_t s) {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((B + HS_JETS - 1) / HS_JETS, hp.fc[0].N / HS_OUT);
+    cfg.blockDim = dim3(HS_THREADS);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = 1; at[0].val.clusterDim.y = cfg.gridDim.y; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    GNN_CUDA_TRY(cudaLaunchKernelEx(&cfg, head_split_kernel<KPER>, (const unsigned long long*)w.pool, (const int32_t*)w.jet_n,
+                                    (const int32_t*)w.meta, hp.fc[0], hp.fc[1], B, hp.n_classes, logits));
+    return 1;
+}
+
 }  // namespace
 
 // x != null: pool the stored block output [N, C]; x == null: the channel sums are in w.pool (pooling EdgeConv epilogue)
@@ -309,6 +473,14 @@ int launch_pool_head(const gnn_model& m, const float* x, int B, const Workspace&
     hp.n_classes = m.arch.n_classes;
     hp.wmax = hp.C;
     for (int i = 0; i < m.n_fc; ++i) hp.wmax = std::max(hp.wmax, (m.fc[i].N + 3) & ~3);
+    if (x == nullptr && hp.n_fc == 2 && hp.fc[0].N % HS_OUT == 0 && hp.fc[0].N / HS_OUT <= HS_MAX_SPLIT &&
+        hp.n_classes <= HS_MAX_CLASSES && (hp.C == 256 || hp.C == 128 || hp.C == 64)) {   // (C = 512: beyond 48 KB of static shared memory)
+        switch (hp.C) {
+            case 64: return launch_head_split<64 / HS_KS>(hp, B, w, logits, s);
+            case 128: return launch_head_split<128 / HS_KS>(hp, B, w, logits, s);
+            default: return launch_head_split<256 / HS_KS>(hp, B, w, logits, s);
+        }
+    }
     if (x == nullptr) {
         size_t part = 4;
         for (int i = 0; i < m.n_fc; ++i) {
