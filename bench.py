@@ -164,75 +164,117 @@ def cpu_baseline(arch, weights, batch, target_s=12.0):
                       (n, int(batch.offsets[n]), t)}
 
 
-def serving_leg(gnn, synth, arch, weights, device, n_clients=64, warm_s=0.5, run_s=2.0):
-    """BASELINE.json configs[3]: synchronous clients (submit -> wait -> next), batcher with
-    max_batch 1024, max queue delay 1 ms, 2 instances.  Client threads are Python threads (ctypes releases the GIL in
-    submit / wait), so the Python side is part of the measured request latency."""
-    model = gnn.Model(gnn.arch_struct(arch, max_batch_jets=1024, precision=gnn.BF16, workspace_slices=2, max_particles=100),
-                      weights, device=device)
-    bt = gnn.Batcher(model, max_batch_jets=1024, max_queue_delay_us=1000, n_instances=2)
+def serving_leg(gnn, synth, arch, weights, device, n_clients=64, warm_ms=500, run_ms=2000):
+    """BASELINE.json configs[3]: 64 synchronous clients (submit -> wait -> next) x 16-jet
+    requests, batcher with max_batch 1024 and max queue delay 1 ms, n_instances 1 / 2 / 4 (2 is the config,
+    1 and 4 reported beside it).  Clients are the library's native closed-loop load generator (gnn_loadgen_run), so the
+    latency is the batcher's and the GPU's; request latency = submit -> logits in client memory."""
     pools = [synth.make_client_pool(c, n_requests=16) for c in range(n_clients)]
-    lat, qs, cs, stop, t_start = [[] for _ in range(n_clients)], [[] for _ in range(n_clients)], [[] for _ in range(n_clients)], [False], [0.0]
+    # one ragged host batch; request r = client r % n_clients, its (r // n_clients)-th request (the load generator's client c
+    # walks requests c, c + n_clients, ...)
+    reqs = [pools[c][i] for i in range(16) for c in range(n_clients)]
+    feats = np.concatenate([r.feats for r in reqs]); coords = np.concatenate([r.coords for r in reqs])
+    counts = np.concatenate([r.counts() for r in reqs])
+    offsets = np.zeros(counts.size + 1, np.int32); offsets[1:] = np.cumsum(counts)
+    rfj = np.arange(len(reqs) + 1, dtype=np.int32) * 16
+    out = {}
+    for n_inst in (2, 1, 4):
+        model = gnn.Model(gnn.arch_struct(arch, max_batch_jets=1024, precision=gnn.BF16, workspace_slices=n_inst, max_particles=100),
+                          weights, device=device)
+        bt = gnn.Batcher(model, max_batch_jets=1024, max_queue_delay_us=1000, n_instances=n_inst)
+        r = bt.loadgen(feats, coords, offsets, rfj, n_clients, warm_ms, run_ms)
+        bt.close()
+        model.close()
+        out[n_inst] = {"value": r["jets_per_s"], "unit": UNIT, "requests": int(r["n_requests"]), "p50_us": r["p50_us"],
+                       "p90_us": r["p90_us"], "p99_us": r["p99_us"], "mean_us": r["mean_us"], "queue_us_mean": r["queue_us_mean"],
+                       "compute_us_mean": r["compute_us_mean"], "mean_coalesced_batch_jets": r["mean_batch_jets"],
+                       "seconds": r["seconds"]}
+    res = dict(out[2])
+    res["workload"] = ("configs[3]: %d closed-loop native client threads x 16 jets (gnn_loadgen_run), batcher max_batch 1024, "
+                       "max delay 1 ms, 2 instances" % n_clients)
+    res["n_instances_1"] = out[1]
+    res["n_instances_4"] = out[4]
+    return res
 
-    def client(c):
-        i = 0
-        while not stop[0]:
-            r = pools[c][i % len(pools[c])]
-            t0 = time.perf_counter()
-            tk, _ = bt.submit(r.feats, r.coords, r.offsets)
-            rc, q_us, c_us = bt.wait(tk)
-            t1 = time.perf_counter()
-            if rc == 0 and t0 >= t_start[0] > 0.0:
-                lat[c].append((t1 - t0) * 1e6); qs[c].append(q_us); cs[c].append(c_us)
-            i += 1
 
-    th = [threading.Thread(target=client, args=(c,), daemon=True) for c in range(n_clients)]
-    for t in th:
-        t.start()
-    time.sleep(warm_s)
-    t_start[0] = time.perf_counter()
-    time.sleep(run_s)
-    stop[0] = True
-    t_end = time.perf_counter()
-    for t in th:
-        t.join(10.0)
-    st = bt.stats()
-    bt.close()
+def time_forward(torch, model, b, dev, n_classes, reps, warm=3):
+    """median / p99 CUDA-event milliseconds of gnn_infer on one device-resident ragged batch"""
+    f, c, o = (torch.from_numpy(x).to(dev) for x in (b.feats, b.coords, b.offsets))
+    lg = torch.empty((b.n_jets, n_classes), dtype=torch.float32, device=dev)
+    for _ in range(warm):
+        model.infer(f, c, o, logits=lg)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(reps)]
+    torch.cuda.synchronize()
+    for a, e in ev:
+        a.record(torch.cuda.current_stream()); model.infer(f, c, o, logits=lg); e.record(torch.cuda.current_stream())
+    torch.cuda.synchronize()
+    t = np.array([a.elapsed_time(e) for a, e in ev])
+    return float(np.median(t)), float(np.percentile(t, 99))
+
+
+def ragged_leg(torch, gnn, synth, work_fn, peak_tf, device, reps=20):
+    """BASELINE.json configs[2]: 4096 ragged jets (multiplicity ~ clip(Poisson(40), 5, 128)), F = 9, CSR offsets only, bf16.
+    The 164 k-particle batch's intermediates (> 300 MB) exceed L2 by themselves, so L2 is not flushed between launches."""
+    dev = torch.device("cuda", device)
+    arch = synth.ARCHS["particlenet_f9"]
+    b = synth.make_ragged_batch()
+    model = gnn.Model(gnn.arch_struct(arch, max_batch_jets=b.n_jets, precision=gnn.BF16, max_particles=128),
+                      synth.make_weights(arch), device=device)
+    ms, p99 = time_forward(torch, model, b, dev, arch.n_classes, reps)
+    assert model.status_check() == 0
     model.close()
-    allv = np.concatenate([np.asarray(v) for v in lat if v]) if any(lat) else np.zeros(1)
-    return {"workload": "configs[3]: %d closed-loop clients x 16 jets, batcher max_batch 1024, max delay 1 ms, 2 instances" % n_clients,
-            "value": 16 * allv.size / (t_end - t_start[0]), "unit": UNIT, "requests": int(allv.size),
-            "p50_us": float(np.percentile(allv, 50)), "p99_us": float(np.percentile(allv, 99)),
-            "queue_us_mean": float(np.mean(np.concatenate([np.asarray(v) for v in qs if v]))) if any(qs) else None,
-            "compute_us_mean": float(np.mean(np.concatenate([np.asarray(v) for v in cs if v]))) if any(cs) else None,
-            "mean_coalesced_batch_jets": st["mean_batch_jets"], "seconds": t_end - t_start[0]}
+    fl = work_fn(arch, b.counts())["min"]
+    return {"workload": "configs[2]: %d ragged jets, %d particles, F = 9, k = 16, gnn_infer (device-resident)" % (b.n_jets, b.n_particles),
+            "value": b.n_jets / (ms * 1e-3), "unit": UNIT, "ms_p50": ms, "ms_p99": p99, "flops_min": fl,
+            "frac_of_bf16_peak": fl / (ms * 1e-3) / 1e12 / peak_tf, "launches_timed": reps}
 
 
-def sweep_leg(torch, gnn, synth, work_fn, peak_tf, device, reps=5):
+def fig4_leg(gnn, synth, model, arch, n_classes, oracle_jets_per_s, n_jets=10000, batch=1024):
+    """Fig-4 analogue (the paper's GPU server was O(50) x its CPU on ParticleNet at batch 1024):
+    10 000 jets (configs[1] recipe, seed 1006) from HOST memory in batches of 1024 through gnn_infer_host (H2D + forward +
+    D2H per batch), cumulative wall time vs jets processed, beside the oracle's time at its measured jets/s."""
+    import torch
+    full = synth.make_particlenet_batch(seed=1006, n_jets=n_jets)
+    cuts = list(range(0, n_jets, batch)) + [n_jets]
+    parts = []
+    for i in range(len(cuts) - 1):
+        sub = full.select(range(cuts[i], cuts[i + 1]))
+        parts.append((torch.from_numpy(sub.feats).pin_memory(), torch.from_numpy(sub.coords).pin_memory(),
+                      torch.from_numpy(sub.offsets).pin_memory(), torch.empty((sub.n_jets, n_classes), dtype=torch.float32).pin_memory()))
+    for f, c, o, lg in parts[:2]:
+        model.infer_host(f, c, o, lg)
+    cum = []
+    t0 = time.perf_counter()
+    for f, c, o, lg in parts:
+        model.infer_host(f, c, o, lg)
+        cum.append(time.perf_counter() - t0)
+    out = {"workload": "%d jets (configs[1] recipe, seed 1006) in batches of %d from pinned host memory, gnn_infer_host" % (n_jets, batch),
+           "jets_processed": cuts[1:], "cumulative_wall_ms": [t * 1e3 for t in cum], "jets_per_s": n_jets / cum[-1]}
+    if oracle_jets_per_s:
+        out["oracle_wall_s_at_measured_rate"] = n_jets / oracle_jets_per_s
+        out["ratio_vs_oracle"] = (n_jets / cum[-1]) / oracle_jets_per_s
+        out["paper_context"] = "PAPER.md L121: GPU server O(50) x CPU for ParticleNet at batch 1024 (A100 MIG slice vs an unspecified CPU)"
+    return out
+
+
+def sweep_leg(torch, gnn, synth, work_fn, peak_tf, device):
     """BASELINE.json configs[4]: saturation sweep, nested batches of one 16 384-jet sequence (multiplicity ~ clip(Poisson(60),
-    5, 128)), base and wide architecture, bf16; jets/s, p50 of a few launches and the fraction of the forward's bf16 roofline."""
+    5, 128)), base and wide architecture, bf16; jets/s, p50 / p99 of the launches and the fraction of the forward's bf16 roofline."""
     dev = torch.device("cuda", device)
     out = {}
     full = synth.make_sweep_batch(n_jets=16384)
-    for name, sizes in (("particlenet", (1, 16, 256, 1024, 4096, 16384)), ("wide", (16, 256, 1024))):
+    sizes = (1, 16, 256, 1024, 4096, 16384)
+    for name in ("particlenet", "wide"):
         arch = synth.ARCHS[name]
         model = gnn.Model(gnn.arch_struct(arch, max_batch_jets=max(sizes), precision=gnn.BF16, max_particles=128),
                           synth.make_weights(arch), device=device)
         rows = []
         for B in sizes:
             b = full.head(B)
-            f, c, o = (torch.from_numpy(x).to(dev) for x in (b.feats, b.coords, b.offsets))
-            lg = torch.empty((B, arch.n_classes), dtype=torch.float32, device=dev)
-            for _ in range(2):
-                model.infer(f, c, o, logits=lg)
-            ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(reps)]
-            torch.cuda.synchronize()
-            for a, e in ev:
-                a.record(torch.cuda.current_stream()); model.infer(f, c, o, logits=lg); e.record(torch.cuda.current_stream())
-            torch.cuda.synchronize()
-            ms = float(np.median([a.elapsed_time(e) for a, e in ev]))
+            ms, p99 = time_forward(torch, model, b, dev, arch.n_classes, reps=20 if B <= 1024 else 5, warm=2)
             fl = work_fn(arch, b.counts())["min"]
-            rows.append({"batch_jets": B, "ms_p50": ms, "jets_per_s": B / (ms * 1e-3), "frac_of_bf16_peak": fl / (ms * 1e-3) / 1e12 / peak_tf})
+            rows.append({"batch_jets": B, "ms_p50": ms, "ms_p99": p99, "jets_per_s": B / (ms * 1e-3),
+                         "frac_of_bf16_peak": fl / (ms * 1e-3) / 1e12 / peak_tf})
         assert model.status_check() == 0
         model.close()
         out[name] = rows
@@ -348,10 +390,14 @@ def run_ours(args):
     # kNN of the block (its time is inside "knn<l>"), so the kernel's algorithmic FLOPs are the per-edge layers 2-3
     dom_flops = mean_of("blocks_edge", dom_l)
     roof_peak = pk["bf16_tflops"]
-    traffic = None                                   # dram bytes per launch of that kernel, from the committed ncu capture
-    tpath = os.path.join(ROOT, "profiles", "r01_traffic.txt")
+    # dram bytes per launch of that kernel: from the committed `ncu --set full` capture of this same command, extracted by
+    # `python ncu_summary.py <report> --traffic profiles/r02_traffic.json` (profiles/r02_bf16.md names the commands)
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "r02_traffic.json")
     if os.path.exists(tpath):
-        traffic = json.load(open(tpath)).get("edge_kernel_c%d_dram_bytes_per_launch" % arch.channels[dom_l][0])
+        tj = json.load(open(tpath))
+        key = [k for k in tj if k.startswith("edge_kernel<%d," % arch.channels[dom_l][0])]
+        traffic = tj[key[0]] if key else None
     roofline = {"bound": "tensor", "kernel": "edge_kernel<%d> (stage %s: EdgeConv block %d, per-edge layers 2-3)" % (arch.channels[dom_l][0], dom[0], dom_l + 1),
                 "achieved": dom_flops / (dom[1] * 1e-3) / 1e12, "peak": roof_peak,
                 "unit": "TFLOP/s", "frac": dom_flops / (dom[1] * 1e-3) / 1e12 / roof_peak, "traffic": traffic,
@@ -417,10 +463,13 @@ def run_ours(args):
         # ---- configs[3]: 64 closed-loop clients x 16-jet requests through the host dynamic batcher (bf16) -------------
         if rank == 0 and args.precision == "bf16":
             out["serving"] = serving_leg(gnn, synth, arch, weights, local)
+            out["ragged_4096_f9"] = ragged_leg(torch, gnn, synth, work, roof_peak, local)
             out["sweep"] = sweep_leg(torch, gnn, synth, work, roof_peak, local)
     out["clocks"] = sampler.summary()
     if rank == 0 and world == 1 and not args.no_cpu_baseline and not args.no_extras:
         out["cpu_baseline"] = cpu_baseline(arch, weights, batches[0])
+    if rank == 0 and not args.no_extras and args.precision == "bf16":
+        out["fig4"] = fig4_leg(gnn, synth, model, arch, arch.n_classes, out.get("cpu_baseline", {}).get("value"))
     model.close()
     if world > 1:
         dist.barrier()

@@ -181,6 +181,27 @@ int gnn_batcher_stats(gnn_batcher* b, uint64_t* n_requests, uint64_t* n_jets, ui
                       double* mean_batch_jets);
 void gnn_batcher_destroy(gnn_batcher* b);   /* drains pending tickets first */
 
+/* ---- closed-loop load generator (App. C: perf_analyzer in synchronous mode; Table C2 sweep) ----------
+ * n_clients native threads; client c cycles through requests c, c + n_clients, ... of the pool: submit -> wait -> next.
+ * The pool is one ragged batch in HOST memory (layouts as gnn_infer: feats [N, F], coords [N, CD], offsets [J + 1] absolute)
+ * cut into requests of consecutive jets: request r = jets [request_first_jet[r], request_first_jet[r + 1]).  After
+ * warmup_ms the harness measures run_ms: jets/s, request latency (submit -> logits in client memory) mean / p50 / p90 /
+ * p99, its split into queue and compute time (Fig. C3) and the mean coalesced batch size.  Blocking; returns the first
+ * failing request's status, else GNN_OK. */
+typedef struct {
+    const float* feats_host;
+    const float* coords_host;
+    const int32_t* offsets_host;
+    const int32_t* request_first_jet;   /* [n_requests + 1] */
+    int32_t n_requests, in_features, coord_dims, n_classes;
+} gnn_loadgen_pool;
+typedef struct { int32_t n_clients, warmup_ms, run_ms; } gnn_loadgen_opts;
+typedef struct {
+    uint64_t n_requests, n_jets;
+    double seconds, jets_per_s, mean_us, p50_us, p90_us, p99_us, queue_us_mean, compute_us_mean, mean_batch_jets;
+} gnn_loadgen_result;
+int gnn_loadgen_run(gnn_batcher* b, const gnn_loadgen_pool* pool, const gnn_loadgen_opts* opts, gnn_loadgen_result* out);
+
 #ifdef __cplusplus
 }
 #endif

@@ -33,6 +33,22 @@ class Ticket(C.Structure):
     _fields_ = [("id", C.c_uint64)]
 
 
+class LoadgenPool(C.Structure):
+    _fields_ = [("feats_host", C.c_void_p), ("coords_host", C.c_void_p), ("offsets_host", C.c_void_p),
+                ("request_first_jet", C.c_void_p), ("n_requests", C.c_int32), ("in_features", C.c_int32),
+                ("coord_dims", C.c_int32), ("n_classes", C.c_int32)]
+
+
+class LoadgenOpts(C.Structure):
+    _fields_ = [("n_clients", C.c_int32), ("warmup_ms", C.c_int32), ("run_ms", C.c_int32)]
+
+
+class LoadgenResult(C.Structure):
+    _fields_ = [("n_requests", C.c_uint64), ("n_jets", C.c_uint64)] + [(k, C.c_double) for k in (
+        "seconds", "jets_per_s", "mean_us", "p50_us", "p90_us", "p99_us", "queue_us_mean", "compute_us_mean",
+        "mean_batch_jets")]
+
+
 def lib():
     """Loads libgnn.so (built in-tree by `python -m paper_2312_06838_b200.build`).  No fallback."""
     global _lib
@@ -66,6 +82,7 @@ def lib():
         L.gnn_batcher_stats.argtypes = [vp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64), C.POINTER(C.c_uint64),
                                         C.POINTER(C.c_double)]
         L.gnn_batcher_destroy.argtypes = [vp]; L.gnn_batcher_destroy.restype = None
+        L.gnn_loadgen_run.argtypes = [vp, C.POINTER(LoadgenPool), C.POINTER(LoadgenOpts), C.POINTER(LoadgenResult)]
         _lib = L
     return _lib
 
@@ -254,6 +271,21 @@ class Batcher:
         a, b, c, d = C.c_uint64(0), C.c_uint64(0), C.c_uint64(0), C.c_double(0)
         lib().gnn_batcher_stats(self.h, C.byref(a), C.byref(b), C.byref(c), C.byref(d))
         return {"n_requests": a.value, "n_jets": b.value, "n_launches": c.value, "mean_batch_jets": d.value}
+
+    def loadgen(self, feats: np.ndarray, coords: np.ndarray, offsets: np.ndarray, request_first_jet: np.ndarray,
+                n_clients: int, warmup_ms: int = 500, run_ms: int = 2000) -> dict:
+        """gnn_loadgen_run: closed-loop native client threads over a pool of requests cut from one ragged host batch."""
+        feats = np.ascontiguousarray(feats, np.float32); coords = np.ascontiguousarray(coords, np.float32)
+        offsets = np.ascontiguousarray(offsets, np.int32); rfj = np.ascontiguousarray(request_first_jet, np.int32)
+        a = self.model.arch
+        pool = LoadgenPool(feats.ctypes.data, coords.ctypes.data, offsets.ctypes.data, rfj.ctypes.data, rfj.size - 1,
+                           a.in_features, a.coord_dims, a.n_classes)
+        o = LoadgenOpts(n_clients, warmup_ms, run_ms)
+        r = LoadgenResult()
+        rc = lib().gnn_loadgen_run(self.h, C.byref(pool), C.byref(o), C.byref(r))
+        if rc != 0:
+            raise GnnError(rc, "gnn_loadgen_run")
+        return {k: getattr(r, k) for k, _ in LoadgenResult._fields_}
 
     def close(self):
         if getattr(self, "h", None):

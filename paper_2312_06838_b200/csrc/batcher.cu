@@ -11,6 +11,7 @@
 #include <condition_variable>
 #include <cstring>
 #include <deque>
+#include <memory>
 #include <mutex>
 #include <thread>
 #include <unordered_map>
@@ -19,13 +20,20 @@ namespace {
 
 using Clock = std::chrono::steady_clock;
 
+// One allocation per request: [feats | coords | offsets] copied once at submit.  Completion is per request (its own mutex
+// and condition variable): a finished batch wakes exactly the clients whose tickets were in it, and a waking client takes
+// the batcher's mutex only to erase its ticket.
 struct Request {
     uint64_t id = 0;
     int n_jets = 0, n_particles = 0;
-    std::vector<float> feats, coords;
-    std::vector<int32_t> offsets;      // [n_jets + 1], relative to the request
+    std::unique_ptr<unsigned char[]> store;
+    const float* feats = nullptr;
+    const float* coords = nullptr;
+    const int32_t* offsets = nullptr;  // [n_jets + 1], relative to the request
     float* out = nullptr;
     Clock::time_point t_submit, t_launch, t_done;
+    std::mutex mu;
+    std::condition_variable cv;
     bool done = false;
     int status = GNN_OK;
 };
@@ -45,7 +53,7 @@ struct gnn_batcher {
     gnn_model* m = nullptr;
     gnn_batcher_opts opts{};
     std::mutex mu;
-    std::condition_variable cv_work, cv_done;
+    std::condition_variable cv_work;
     std::deque<Request*> queue;
     int queued_jets = 0;
     std::unordered_map<uint64_t, Request*> tickets;
@@ -58,12 +66,14 @@ struct gnn_batcher {
 namespace {
 
 void finish(gnn_batcher* b, std::vector<Request*>& batch, int status, Clock::time_point t_launch) {
+    (void)b;
     auto now = Clock::now();
-    std::lock_guard<std::mutex> lk(b->mu);
     for (Request* r : batch) {
+        // notify under the request's lock: once it is released the waiter may delete r, so r is not touched again
+        std::lock_guard<std::mutex> lk(r->mu);
         r->status = status; r->t_launch = t_launch; r->t_done = now; r->done = true;
+        r->cv.notify_one();
     }
-    b->cv_done.notify_all();
 }
 
 void worker_main(gnn_batcher* b, int wi) {
@@ -102,8 +112,8 @@ void worker_main(gnn_batcher* b, int wi) {
         int B = 0, N = 0;
         I.h_offsets[0] = 0;
         for (Request* r : batch) {
-            std::memcpy(I.h_feats + (size_t)N * F, r->feats.data(), (size_t)r->n_particles * F * sizeof(float));
-            std::memcpy(I.h_coords + (size_t)N * CD, r->coords.data(), (size_t)r->n_particles * CD * sizeof(float));
+            std::memcpy(I.h_feats + (size_t)N * F, r->feats, (size_t)r->n_particles * F * sizeof(float));
+            std::memcpy(I.h_coords + (size_t)N * CD, r->coords, (size_t)r->n_particles * CD * sizeof(float));
             for (int j = 0; j < r->n_jets; ++j) I.h_offsets[B + j + 1] = N + r->offsets[j + 1];
             B += r->n_jets; N += r->n_particles;
         }
@@ -202,9 +212,16 @@ int gnn_batcher_submit(gnn_batcher* b, const float* feats_host, const float* coo
     Request* r = new (std::nothrow) Request();
     if (!r) return GNN_ERR_CUDA;
     r->n_jets = n_jets; r->n_particles = N; r->out = logits_host_out;
-    r->feats.assign(feats_host, feats_host + (size_t)N * a.in_features);
-    r->coords.assign(coords_host, coords_host + (size_t)N * a.coord_dims);
-    r->offsets.assign(offsets_host, offsets_host + n_jets + 1);
+    const size_t fb = (size_t)N * a.in_features * sizeof(float), cb = (size_t)N * a.coord_dims * sizeof(float);
+    const size_t ob = (size_t)(n_jets + 1) * sizeof(int32_t);
+    r->store.reset(new (std::nothrow) unsigned char[fb + cb + ob]);
+    if (!r->store) { delete r; return GNN_ERR_CUDA; }
+    if (fb) std::memcpy(r->store.get(), feats_host, fb);
+    if (cb) std::memcpy(r->store.get() + fb, coords_host, cb);
+    std::memcpy(r->store.get() + fb + cb, offsets_host, ob);
+    r->feats = reinterpret_cast<const float*>(r->store.get());
+    r->coords = reinterpret_cast<const float*>(r->store.get() + fb);
+    r->offsets = reinterpret_cast<const int32_t*>(r->store.get() + fb + cb);
     {
         std::lock_guard<std::mutex> lk(b->mu);
         if (b->stop || (int)b->tickets.size() >= b->opts.max_pending_requests) {
@@ -225,18 +242,34 @@ int gnn_batcher_submit(gnn_batcher* b, const float* feats_host, const float* coo
 
 int gnn_batcher_wait(gnn_batcher* b, gnn_ticket t, int64_t timeout_us, double* queue_us, double* compute_us) {
     if (!b) return GNN_ERR_NULL;
-    std::unique_lock<std::mutex> lk(b->mu);
-    auto it = b->tickets.find(t.id);
-    if (it == b->tickets.end()) return GNN_ERR_BAD_TICKET;
-    Request* r = it->second;
-    if (timeout_us < 0) b->cv_done.wait(lk, [&] { return r->done; });
-    else if (!b->cv_done.wait_for(lk, std::chrono::microseconds(timeout_us), [&] { return r->done; })) return GNN_ERR_TIMEOUT;
-    using us = std::chrono::duration<double, std::micro>;
-    if (queue_us) *queue_us = us(r->t_launch - r->t_submit).count();
-    if (compute_us) *compute_us = us(r->t_done - r->t_launch).count();
-    int status = r->status;
-    b->tickets.erase(it);
-    lk.unlock();
+    Request* r = nullptr;
+    {
+        std::lock_guard<std::mutex> lk(b->mu);
+        auto it = b->tickets.find(t.id);
+        if (it == b->tickets.end()) return GNN_ERR_BAD_TICKET;
+        r = it->second;
+        if (r->id == 0) return GNN_ERR_BAD_TICKET;             // another thread is already waiting on this ticket
+        r->id = 0;                                             // claimed: a ticket has one waiter
+    }
+    int status;
+    {
+        std::unique_lock<std::mutex> lk(r->mu);
+        if (timeout_us < 0) r->cv.wait(lk, [&] { return r->done; });
+        else if (!r->cv.wait_for(lk, std::chrono::microseconds(timeout_us), [&] { return r->done; })) {
+            lk.unlock();
+            std::lock_guard<std::mutex> g(b->mu);
+            r->id = t.id;                                      // unclaimed again: the ticket can be waited on later
+            return GNN_ERR_TIMEOUT;
+        }
+        using us = std::chrono::duration<double, std::micro>;
+        if (queue_us) *queue_us = us(r->t_launch - r->t_submit).count();
+        if (compute_us) *compute_us = us(r->t_done - r->t_launch).count();
+        status = r->status;
+    }
+    {
+        std::lock_guard<std::mutex> lk(b->mu);
+        b->tickets.erase(t.id);
+    }
     delete r;
     return status;
 }
