@@ -28,6 +28,7 @@
 #include "gnn_internal.h"
 #include "tc05.cuh"
 #include <cuda_bf16.h>
+#include <cuda_fp16.h>
 #include <cstdlib>
 #include <cstring>
 
@@ -105,7 +106,7 @@ __device__ __forceinline__ unsigned long long to_fixed_32_32(float y) {
 struct EdgeParams {
     const __nv_bfloat16* U;      // [N, C]
     const __nv_bfloat16* V;      // [N, C]
-    const float* R;              // [N, C] shortcut
+    const __half* R;             // [N, C] shortcut (fp16: 11 significant bits, three more than the bf16 operands of the edge MLP)
     const int32_t* idx;          // [N, k] global neighbour rows, -1 = none
     float* y;                    // [N, C] (null in the POOL variant)
     const int32_t* pjid;         // POOL: [N] particle -> jet
@@ -467,11 +468,11 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
                 auto part_lane = [&](int i) { return cg * NPW + i; };
                 if (t + 1 < T) load_meta(tile_p0(t + 1) - (PAIR ? (int)rank * p.TP : 0), n_pt, n_mask, n_inv, n_jid);
                 else { n_pt = -1; n_mask = 0u; n_inv = 0.0f; n_jid = -1; }
-                float rr[NPW];
-#pragma unroll
+                unsigned short rr[NPW];                          // fp16 bits: converted where they are used, so that nothing waits for
+#pragma unroll                                                   // these loads before the accumulator is complete
                 for (int i = 0; i < NPW; ++i) {
                     const int ptl = __shfl_sync(0xffffffffu, m_pt, part_lane(i));
-                    rr[i] = ptl >= 0 ? __ldg(p.R + (size_t)ptl * C + ch) : 0.0f;
+                    rr[i] = ptl >= 0 ? __ldg(reinterpret_cast<const unsigned short*>(p.R) + (size_t)ptl * C + ch) : (unsigned short)0;
                 }
                 mbar_wait(&d_full[1], ph);
                 tc_fence_after();
@@ -495,7 +496,7 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
                     }
                     const uint32_t a0 = add_f16x2(h[0], h[1]), a1 = add_f16x2(h[2], h[3]), a2 = add_f16x2(h[4], h[5]), a3 = add_f16x2(h[6], h[7]);
                     const float2 f = unpack_f16x2(add_f16x2(add_f16x2(a0, a1), add_f16x2(a2, a3)));
-                    const float y = fmaxf(fmaf(f.x + f.y, inv, rr[i]), 0.0f);
+                    const float y = fmaxf(fmaf(f.x + f.y, inv, __half2float(__ushort_as_half(rr[i]))), 0.0f);
                     if constexpr (POOL) {
                         const int jid = __shfl_sync(0xffffffffu, m_jid, pl);
                         if (jid != jid_acc) {                    // warp-uniform: the jet changed, flush its exact fixed-point sum
@@ -516,17 +517,23 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
                 if (t + 1 < T) { const int ptn = tile_p0(t + 1) + (row >> logk); jid_next = ptn < N ? __ldg(p.pjid + ptn) : -1; }
                 if (jid_cur != jid_acc) { pool_flush(); jid_acc = jid_cur; }
             }
-            float2 rr[SLABS];
+            uint32_t rr[SLABS];                                  // shortcut values, packed fp16 until they are used
+            auto load_rr = [&]() {
 #pragma unroll
-            for (int s = 0; s < SLABS; ++s) {
-                rr[s] = make_float2(0.0f, 0.0f);
-                if (pt < N) {
-                    if (nout == 2) rr[s] = __ldg(reinterpret_cast<const float2*>(p.R + obase + s * 32));
-                    else if (nout == 1) rr[s].x = __ldg(p.R + obase + s * 32);
+                for (int s = 0; s < SLABS; ++s) {
+                    rr[s] = 0u;
+                    if (pt < N) {
+                        if (nout == 2) rr[s] = __ldg(reinterpret_cast<const uint32_t*>(p.R + obase + s * 32));
+                        else if (nout == 1) rr[s] = (uint32_t)__ldg(reinterpret_cast<const uint16_t*>(p.R + obase + s * 32));
+                    }
                 }
-            }
+            };
+            // C <= 64 runs at 64 registers (four CTAs per SM): loads in flight across the wait get spilled, and the spill store
+            // waits for them; there they are issued behind the wait (L2 hits: prefetched at the top of the tile)
+            if constexpr (C > 64) load_rr();
             mbar_wait(&d_full[1], ph);
             tc_fence_after();
+            if constexpr (C <= 64) load_rr();
             {
                 const bool valid = idx_cur >= 0;
                 const unsigned vmask = __ballot_sync(0xffffffffu, valid);
@@ -571,11 +578,11 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
                         const float2 f = unpack_f16x2(w[0]);
                         const bool up = (lane >> 4) & 1;
                         const float sum = (up ? f.y : f.x) + __shfl_xor_sync(0xffffffffu, up ? f.x : f.y, 16);
-                        if (pt < N) p.y[o] = fmaxf(fmaf(sum, inv, rr[s].x), 0.0f);
+                        if (pt < N) p.y[o] = fmaxf(fmaf(sum, inv, unpack_f16x2(rr[s]).x), 0.0f);
                     } else if (pt < N) {
                         if (nout == 2) {
-                            const float2 f = unpack_f16x2(w[0]);
-                            const float y0 = fmaxf(fmaf(f.x, inv, rr[s].x), 0.0f), y1 = fmaxf(fmaf(f.y, inv, rr[s].y), 0.0f);
+                            const float2 f = unpack_f16x2(w[0]), rs = unpack_f16x2(rr[s]);
+                            const float y0 = fmaxf(fmaf(f.x, inv, rs.x), 0.0f), y1 = fmaxf(fmaf(f.y, inv, rs.y), 0.0f);
                             if constexpr (POOL) {
                                 ulonglong2 a = acc_s[s * 32];
                                 a.x += to_fixed_32_32(y0);
@@ -589,7 +596,9 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
                             for (int i = 0; i < 16; i += 2)
                                 if (2 * i < nout) {
                                     const float2 f0 = unpack_f16x2(w[i]), f1 = unpack_f16x2(w[i + 1]);
-                                    const float4 r4 = __ldg(reinterpret_cast<const float4*>(p.R + o + 2 * i));
+                                    const uint2 rh = __ldg(reinterpret_cast<const uint2*>(p.R + o + 2 * i));
+                                    const float2 ra = unpack_f16x2(rh.x), rb = unpack_f16x2(rh.y);
+                                    const float4 r4 = make_float4(ra.x, ra.y, rb.x, rb.y);
                                     *reinterpret_cast<float4*>(p.y + o + 2 * i) =
                                         make_float4(fmaxf(fmaf(f0.x, inv, r4.x), 0.0f), fmaxf(fmaf(f0.y, inv, r4.y), 0.0f),
                                                     fmaxf(fmaf(f1.x, inv, r4.z), 0.0f), fmaxf(fmaf(f1.y, inv, r4.w), 0.0f));
@@ -839,7 +848,7 @@ __global__ void __launch_bounds__(WIDE_THREADS, 1) edge_wide_kernel(EdgeParams p
                         const size_t o = (size_t)pt * C + col + cb;
 #pragma unroll
                         for (int i = 0; i < 32; ++i)
-                            if (i < nout) p.y[o + i] = fmaxf(fmaf(v[i], inv, __ldg(p.R + o + i)), 0.0f);
+                            if (i < nout) p.y[o + i] = fmaxf(fmaf(v[i], inv, __half2float(__ldg(p.R + o + i))), 0.0f);
                     }
                 }
             }
@@ -862,7 +871,7 @@ struct PreParams {
     const float* bias;       // [NC] = [t1 | 0 | ts]
     __nv_bfloat16* U;        // [N, C1]
     __nv_bfloat16* V;        // [N, C1]
-    float* R;                // [N, C3]
+    __half* R;               // [N, C3]
     const int32_t* meta;
     int cin, Kp, C1, C3, NC;
 };
@@ -916,7 +925,7 @@ __global__ void __launch_bounds__(PRE_THREADS) pre_kernel(PreParams p) {
                 __nv_bfloat16* dst = (col < p.C1) ? p.U + (size_t)row * p.C1 + col : p.V + (size_t)row * p.C1 + (col - p.C1);
                 *reinterpret_cast<uint2*>(dst) = make_uint2(pack_bf16x2(o0, o1), pack_bf16x2(o2, o3));
             } else {
-                *reinterpret_cast<float4*>(p.R + (size_t)row * p.C3 + (col - 2 * p.C1)) = make_float4(o0, o1, o2, o3);
+                *reinterpret_cast<uint2*>(p.R + (size_t)row * p.C3 + (col - 2 * p.C1)) = make_uint2(pack_f16x2(o0, o1), pack_f16x2(o2, o3));
             }
         }
     }
@@ -959,35 +968,39 @@ __global__ void __launch_bounds__(1024) pre_small_kernel(PreParams p) {
             __nv_bfloat16* dst = (col < p.C1) ? p.U + (size_t)row * p.C1 + col : p.V + (size_t)row * p.C1 + (col - p.C1);
             *reinterpret_cast<uint2*>(dst) = make_uint2(pack_bf16x2(o0, o1), pack_bf16x2(o2, o3));
         } else {
-            *reinterpret_cast<float4*>(p.R + (size_t)row * p.C3 + (col - 2 * p.C1)) = make_float4(o0, o1, o2, o3);
+            *reinterpret_cast<uint2*>(p.R + (size_t)row * p.C3 + (col - 2 * p.C1)) = make_uint2(pack_f16x2(o0, o1), pack_f16x2(o2, o3));
         }
     }
 }
 
-// ---- pre kernel on the tensor cores (blocks whose input width is a multiple of 32): [u | v | r] = x * Wpre^T + bias --------
-// One GEMM [N, CIN] x [CIN, 3C] in tf32 (kind::tf32, fp32 accumulate in TMEM): x is rounded to tf32 (RNA) on its way
-// into shared memory, Wpre is rounded once on the host.  The 3C output columns are three slices of C columns (u, v,
-// r); a CTA keeps ONE slice of the weights resident ([C][CIN] tf32 as 128B-swizzled K blocks of 32 floats) and walks
-// the 128-row tiles of its slice group, so per tile only the x rows move (L2 -> smem).  A is single-buffered and handed
-// over per K block (a_ready / a_free), the accumulator is double-buffered (2 x C TMEM columns): epilogue(t) and the
-// loads of tile t+1 run under MMA(t+1) / MMA(t).
-// Warps: 0-7 epilogue (thread = row = TMEM lane), 8-15 x loaders (a whole tile in flight in registers), 16 MMA issuer +
-// TMEM owner + weight load.
-constexpr int PTC_THREADS = 544;
-constexpr int PTC_EPI_WARPS = 8;          // lane quadrant w & 3, slabs of parity w >> 2
-constexpr int PTC_MMA_WARP = 16;
+// ---- pre kernel on the tensor cores (blocks whose input width is a multiple of 64): [u | v | r] = x * Wpre^T + bias ---------
+// One GEMM [N, CIN] x [CIN, 3C], fp16 operands (x and the folded weights rounded RNE: 10 mantissa bits as tf32, at twice
+// the rate and half the shared memory), fp32 accumulation in TMEM.  The 3C output columns are three slices of C columns
+// (u, v, r); a CTA keeps ONE slice of the weights resident ([C][CIN] fp16 as 128B-swizzled K blocks of 64) and walks
+// the 128-row tiles of its slice group.  The 128 rows of a tile are contiguous in x, so a tile arrives with ONE bulk (TMA)
+// copy into a raw fp32 buffer, issued a tile ahead by the MMA thread: no registers hold loads in flight, and the next tile
+// streams in while this one is converted, multiplied and stored.  Converter warps turn the raw rows into the swizzled fp16
+// operand tile; the accumulator is double-buffered (2 x C TMEM columns), so epilogue(t) runs under convert / MMA (t + 1).
+// Shared memory (169 KB for 128 -> 256) and registers leave room for a kNN CTA of the same block on the SM: the forward
+// runs the two kernels side by side on two streams.
+// Warps: 0-7 epilogue (thread = row = TMEM lane, slabs of parity w >> 2), 8-11 converters, 12 TMA + MMA issuer + TMEM owner.
+constexpr int PTC_EPI_WARPS = 8;
+constexpr int PTC_CVT_WARPS = 4;
+constexpr int PTC_MMA_WARP = PTC_EPI_WARPS + PTC_CVT_WARPS;
+constexpr int PTC_THREADS = 32 * (PTC_MMA_WARP + 1);
 
 template <int CIN, int C>
 struct PreTcCfg {
-    static constexpr int KBA = CIN / 32;                      // K blocks of 32 tf32 (128 bytes per row)
+    static constexpr int KBA = CIN / 64;                      // K blocks of 64 fp16 (128 bytes per row)
     static constexpr int AK_BYTES = TILE_ROWS * 128;
     static constexpr int A_BYTES = KBA * AK_BYTES;
-    static constexpr int WK_BYTES = C * 128;                  // [C][32] tf32 chunk
+    static constexpr int WK_BYTES = C * 128;                  // [C][64] fp16 chunk
     static constexpr int W_BYTES = KBA * WK_BYTES;            // one slice
+    static constexpr int RAW_BYTES = TILE_ROWS * CIN * 4;     // one tile of raw fp32 rows
     static constexpr int TMEM_COLS = 2 * C;
-    static constexpr int NBAR = 2 * KBA + 5;
-    static constexpr int STAGE_BYTES = PTC_EPI_WARPS * 4096;  // per epilogue warp: [32 rows][32 cols] fp32, swizzled
-    static constexpr int SMEM_BYTES = W_BYTES + A_BYTES + STAGE_BYTES + C * 4 + NBAR * 8 + 16;
+    static constexpr int NBAR = 8;
+    static constexpr int STAGE_BYTES = PTC_EPI_WARPS * 2048;  // per epilogue warp: [32 rows][32 cols] 16-bit, swizzled
+    static constexpr int SMEM_BYTES = W_BYTES + A_BYTES + RAW_BYTES + STAGE_BYTES + C * 4 + NBAR * 8 + 16;
 };
 
 struct PreTcParams {
@@ -996,19 +1009,13 @@ struct PreTcParams {
     const float* bias;           // [3C] = [t1 | 0 | ts]
     __nv_bfloat16* U;            // [N, C]
     __nv_bfloat16* V;            // [N, C]
-    float* R;                    // [N, C]
+    __half* R;                   // [N, C]
     const int32_t* meta;
     int n_tiles;
 };
 
-__device__ __forceinline__ uint32_t f32_to_tf32_rna(float f) {
-    uint32_t r;
-    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(f));
-    return r;
-}
-
 template <int CIN, int C>
-__global__ void __launch_bounds__(PTC_THREADS, 1) pre_tc_kernel(PreTcParams p) {
+__global__ void __maxnreg__(80) pre_tc_kernel(PreTcParams p) {
     using Cfg = PreTcCfg<CIN, C>;
     constexpr int KBA = Cfg::KBA;
     extern __shared__ __align__(1024) uint8_t smem_raw[];
@@ -1025,19 +1032,23 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) pre_tc_kernel(PreTcParams p) {
     if ((smem_u32(smem) & 1023u) != 0u) __trap();
     uint8_t* Wsm = smem;
     uint8_t* A = Wsm + Cfg::W_BYTES;
-    uint8_t* stage = A + Cfg::A_BYTES;
+    uint8_t* raw = A + Cfg::A_BYTES;
+    uint8_t* stage = raw + Cfg::RAW_BYTES;
     float* bias_s = reinterpret_cast<float*>(stage + Cfg::STAGE_BYTES);
     uint64_t* bars = reinterpret_cast<uint64_t*>(bias_s + C);
-    uint64_t* a_ready = bars;                 // [KBA] loaders -> MMA
-    uint64_t* a_free = bars + KBA;            // [KBA] MMA -> loaders
-    uint64_t* d_full = bars + 2 * KBA;        // [2]
-    uint64_t* d_free = d_full + 2;            // [2]
-    uint64_t* w_full = d_free + 2;
-    uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(w_full + 1);
+    uint64_t* raw_full = bars;                // TMA -> converters: the tile's raw rows landed
+    uint64_t* a_ready = bars + 1;             // converters -> MMA: operand tile written (and the raw buffer is free again)
+    uint64_t* a_free = bars + 2;              // MMA -> converters: the operand tile has been read
+    uint64_t* d_full = bars + 3;              // [2]
+    uint64_t* d_free = bars + 5;              // [2]
+    uint64_t* w_full = bars + 7;
+    uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(bars + Cfg::NBAR);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     if (tid == 0) {
-        for (int i = 0; i < KBA; ++i) { mbar_init(&a_ready[i], 8); mbar_init(&a_free[i], 1); }
+        mbar_init(raw_full, 1);
+        mbar_init(a_ready, PTC_CVT_WARPS);
+        mbar_init(a_free, 1);
         for (int i = 0; i < 2; ++i) { mbar_init(&d_full[i], 1); mbar_init(&d_free[i], PTC_EPI_WARPS); }
         mbar_init(w_full, 1);
         fence_mbar_init();
@@ -1048,70 +1059,70 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) pre_tc_kernel(PreTcParams p) {
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tmem_ptr;
+    auto tile_bytes = [&](int t) {
+        const int r0 = (gi + t * ng) * TILE_ROWS;
+        return (uint32_t)(min(TILE_ROWS, N - r0) * CIN * 4);
+    };
 
     if (warp == PTC_MMA_WARP) {
-        // ===== weight load + MMA issuer =================================================================================
+        // ===== weight load, tile loads (one tile ahead) and MMA issue ===================================================
         if (lane == 0) {
+            mbar_arrive_expect_tx(raw_full, tile_bytes(0));
+            bulk_g2s(raw, p.x + (size_t)gi * TILE_ROWS * CIN, tile_bytes(0), raw_full);
             mbar_arrive_expect_tx(w_full, Cfg::W_BYTES);
             const uint8_t* src = p.wimg + (size_t)slice * Cfg::W_BYTES;
             for (int c = 0; c < KBA; ++c)
                 bulk_g2s(Wsm + (size_t)c * Cfg::WK_BYTES, src + (size_t)c * Cfg::WK_BYTES, Cfg::WK_BYTES, w_full);
-            constexpr uint32_t idesc = idesc_tf32_f32(128, C);
+            constexpr uint32_t idesc = idesc_f16_f32(128, C);
             const uint32_t a_addr = smem_u32(A), w_addr = smem_u32(Wsm);
             mbar_wait(w_full, 0);
             for (int t = 0; t < T; ++t) {
                 const int acc = t & 1;
+                mbar_wait(a_ready, t & 1);                       // operand tile t written: the raw buffer is free
+                if (t + 1 < T) {
+                    mbar_arrive_expect_tx(raw_full, tile_bytes(t + 1));
+                    bulk_g2s(raw, p.x + (size_t)(gi + (t + 1) * ng) * TILE_ROWS * CIN, tile_bytes(t + 1), raw_full);
+                }
                 mbar_wait(&d_free[acc], ((t >> 1) & 1) ^ 1);
                 tc_fence_after();
 #pragma unroll
-                for (int kb = 0; kb < KBA; ++kb) {
-                    mbar_wait(&a_ready[kb], t & 1);
-                    tc_fence_after();
+                for (int kb = 0; kb < KBA; ++kb)
 #pragma unroll
-                    for (int ks = 0; ks < 4; ++ks) {             // K = 8 tf32 = 32 bytes per step
+                    for (int ks = 0; ks < 4; ++ks) {             // K = 16 fp16 = 32 bytes per step
                         const uint64_t ad = desc_sw128(a_addr + kb * Cfg::AK_BYTES + ks * 32);
                         const uint64_t bd = desc_sw128(w_addr + kb * Cfg::WK_BYTES + ks * 32);
-                        mma_tf32_ss(tmem + acc * C, ad, bd, idesc, (kb | ks) != 0);
+                        mma_bf16_ss(tmem + acc * C, ad, bd, idesc, (kb | ks) != 0);   // kind::f16; the descriptor says fp16
                     }
-                    mma_commit(&a_free[kb]);
-                }
+                mma_commit(a_free);
                 mma_commit(&d_full[acc]);
             }
         }
     } else if (warp >= PTC_EPI_WARPS) {
-        // ===== x loaders: rows 16*lw .. +15 of every K block, 8 lanes per row (one 128-byte line); all K blocks of a tile
-        // are requested before the first store, so a whole tile per CTA is in flight while the previous one is multiplied
-        const int lw = warp - PTC_EPI_WARPS;
-        const int gc = lane & 7, grs = lane >> 3;
+        // ===== converters: raw fp32 rows -> fp16 (RNE, saturating), 128B-swizzled K blocks.  One item = 8 columns of a row
+        // (32 bytes in, one 16-byte chunk out); the eight lanes of a quarter-warp write one 128-byte line ====================
+        const int ct = tid - PTC_EPI_WARPS * 32;
+        constexpr int IPR = CIN / 8;                             // items per row
+        constexpr int ITEMS = TILE_ROWS * IPR / (PTC_CVT_WARPS * 32);
         for (int t = 0; t < T; ++t) {
-            const int r0 = (gi + t * ng) * TILE_ROWS;
-            float4 v[KBA][4];
-#pragma unroll
-            for (int kb = 0; kb < KBA; ++kb)
-#pragma unroll
-                for (int it = 0; it < 4; ++it) {
-                    const int r = 16 * lw + it * 4 + grs;
-                    v[kb][it] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-                    if (r0 + r < N) v[kb][it] = __ldg(reinterpret_cast<const float4*>(p.x + (size_t)(r0 + r) * CIN + kb * 32) + gc);
-                }
-#pragma unroll
-            for (int kb = 0; kb < KBA; ++kb) {
-                mbar_wait(&a_free[kb], (t & 1) ^ 1);
-#pragma unroll
-                for (int it = 0; it < 4; ++it) {
-                    const int r = 16 * lw + it * 4 + grs;
-                    const uint4 w = make_uint4(f32_to_tf32_rna(v[kb][it].x), f32_to_tf32_rna(v[kb][it].y),
-                                               f32_to_tf32_rna(v[kb][it].z), f32_to_tf32_rna(v[kb][it].w));
-                    *reinterpret_cast<uint4*>(A + kb * Cfg::AK_BYTES + r * 128 + ((gc ^ (r & 7)) << 4)) = w;
-                }
-                fence_proxy_async();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&a_ready[kb]);
+            mbar_wait(raw_full, t & 1);
+            if (t > 0) mbar_wait(a_free, (t - 1) & 1);
+#pragma unroll 4
+            for (int i = 0; i < ITEMS; ++i) {
+                const int e = ct + i * (PTC_CVT_WARPS * 32);
+                const int r = e / IPR, c = e - r * IPR;
+                const float4 a = *reinterpret_cast<const float4*>(raw + (size_t)r * (CIN * 4) + c * 32);
+                const float4 b = *reinterpret_cast<const float4*>(raw + (size_t)r * (CIN * 4) + c * 32 + 16);
+                const uint4 o = make_uint4(pack_f16x2(a.x, a.y), pack_f16x2(a.z, a.w), pack_f16x2(b.x, b.y), pack_f16x2(b.z, b.w));
+                *reinterpret_cast<uint4*>(A + (c >> 3) * Cfg::AK_BYTES + r * 128 + (((c & 7) ^ (r & 7)) << 4)) = o;
             }
+            fence_proxy_async();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(a_ready);
         }
     } else {
-        // ===== epilogue: thread = row = TMEM lane; slice 0 -> U (bf16), 1 -> V (bf16), 2 -> R (fp32) ======================
+        // ===== epilogue: thread = row = TMEM lane; slice 0 -> U (bf16), 1 -> V (bf16), 2 -> R (fp16) ======================
         const int q = warp & 3, eh = warp >> 2;
+        uint16_t* outp = reinterpret_cast<uint16_t*>(slice == 0 ? (void*)p.U : (slice == 1 ? (void*)p.V : (void*)p.R));
         for (int t = 0; t < T; ++t) {
             const int acc = t & 1;
             mbar_wait(&d_full[acc], (t >> 1) & 1);
@@ -1131,36 +1142,27 @@ __global__ void __launch_bounds__(PTC_THREADS, 1) pre_tc_kernel(PreTcParams p) {
                     const float4 b = *reinterpret_cast<const float4*>(bias_s + s * 32 + 4 * i);
                     v[4 * i] += b.x; v[4 * i + 1] += b.y; v[4 * i + 2] += b.z; v[4 * i + 3] += b.w;
                 }
-                // transpose through this warp's staging tile so that global stores are whole 128-byte (fp32) / 64-byte
-                // (bf16) row segments: thread = row writes swizzled 16-byte chunks, then 8 (4) lanes read one row back
-                uint8_t* st = stage + warp * 4096;
+                // transpose through this warp's staging tile so that global stores are whole 64-byte row segments: thread =
+                // row writes swizzled 16-byte chunks, then 4 lanes read one row back
+                uint8_t* st = stage + warp * 2048;
                 const int tr0 = (gi + t * ng) * TILE_ROWS + 32 * q;
-                if (slice == 2) {
 #pragma unroll
-                    for (int i = 0; i < 8; ++i)
-                        *reinterpret_cast<float4*>(st + lane * 128 + ((i ^ (lane & 7)) << 4)) =
-                            make_float4(v[4 * i], v[4 * i + 1], v[4 * i + 2], v[4 * i + 3]);
-                    __syncwarp();
-#pragma unroll
-                    for (int it = 0; it < 8; ++it) {
-                        const int r = it * 4 + (lane >> 3), c = lane & 7;
-                        const float4 o = *reinterpret_cast<const float4*>(st + r * 128 + ((c ^ (r & 7)) << 4));
-                        if (tr0 + r < N) *(reinterpret_cast<float4*>(p.R + (size_t)(tr0 + r) * C + s * 32) + c) = o;
-                    }
-                } else {
-#pragma unroll
-                    for (int i = 0; i < 4; ++i)
-                        *reinterpret_cast<uint4*>(st + lane * 64 + ((i ^ ((lane >> 1) & 3)) << 4)) =
-                            make_uint4(pack_bf16x2(v[8 * i], v[8 * i + 1]), pack_bf16x2(v[8 * i + 2], v[8 * i + 3]),
+                for (int i = 0; i < 4; ++i) {
+                    uint4 o;
+                    if (slice == 2)
+                        o = make_uint4(pack_f16x2(v[8 * i], v[8 * i + 1]), pack_f16x2(v[8 * i + 2], v[8 * i + 3]),
+                                       pack_f16x2(v[8 * i + 4], v[8 * i + 5]), pack_f16x2(v[8 * i + 6], v[8 * i + 7]));
+                    else
+                        o = make_uint4(pack_bf16x2(v[8 * i], v[8 * i + 1]), pack_bf16x2(v[8 * i + 2], v[8 * i + 3]),
                                        pack_bf16x2(v[8 * i + 4], v[8 * i + 5]), pack_bf16x2(v[8 * i + 6], v[8 * i + 7]));
-                    __syncwarp();
-                    __nv_bfloat16* outp = slice == 0 ? p.U : p.V;
+                    *reinterpret_cast<uint4*>(st + lane * 64 + ((i ^ ((lane >> 1) & 3)) << 4)) = o;
+                }
+                __syncwarp();
 #pragma unroll
-                    for (int it = 0; it < 4; ++it) {
-                        const int r = it * 8 + (lane >> 2), c = lane & 3;
-                        const uint4 o = *reinterpret_cast<const uint4*>(st + r * 64 + ((c ^ ((r >> 1) & 3)) << 4));
-                        if (tr0 + r < N) *(reinterpret_cast<uint4*>(outp + (size_t)(tr0 + r) * C + s * 32) + c) = o;
-                    }
+                for (int it = 0; it < 4; ++it) {
+                    const int r = it * 8 + (lane >> 2), c = lane & 3;
+                    const uint4 o = *reinterpret_cast<const uint4*>(st + r * 64 + ((c ^ ((r >> 1) & 3)) << 4));
+                    if (tr0 + r < N) *(reinterpret_cast<uint4*>(outp + (size_t)(tr0 + r) * C + s * 32) + c) = o;
                 }
                 __syncwarp();
             }
@@ -1180,11 +1182,12 @@ struct Bf16BlockDev {
     const uint8_t* pre_wimg = nullptr;   // tf32 chunk images of the tensor-core pre kernel (null: SIMT pre kernel)
     int cin = 0, Kp = 0, C = 0, NC = 0;
     int grid_cap = 148, grid_cap_pool = 148;
+    int pre_ctas_per_sm = 1;
 };
 struct Bf16Scratch {
     __nv_bfloat16* U = nullptr;
     __nv_bfloat16* V = nullptr;
-    float* R = nullptr;
+    __half* R = nullptr;
 };
 
 uint16_t f32_to_bf16_rne(float f) {
@@ -1354,30 +1357,31 @@ int edgeconv_bf16_prepare(gnn_model& m, const float* blob) {
             (rc = upload(m, img, &b.wimg)) != GNN_OK || (rc = upload(m, sh, &b.shifts)) != GNN_OK)
             return rc;
         if ((cin == 64 && C == 128) || (cin == 128 && C == 256)) {
-            // tensor-core pre kernel: per slice of C output columns (u, v, r) and K block of 32: [C][32] tf32 (RNA), 128B-swizzled
-            std::vector<uint8_t> pimg((size_t)3 * C * cin * 4, 0);
+            // tensor-core pre kernel: per slice of C output columns (u, v, r) and K block of 64: [C][64] fp16 (RNE), 128B-swizzled
+            std::vector<uint8_t> pimg((size_t)3 * C * cin * 2, 0);
             size_t base = 0;
             for (int sl = 0; sl < 3; ++sl)
-                for (int kb = 0; kb < cin / 32; ++kb, base += (size_t)C * 128)
+                for (int kb = 0; kb < cin / 64; ++kb, base += (size_t)C * 128)
                     for (int nl = 0; nl < C; ++nl)
-                        for (int kk = 0; kk < 32; ++kk) {
-                            const float f = Wt[(size_t)(kb * 32 + kk) * b.NC + sl * C + nl];
-                            uint32_t u;
-                            std::memcpy(&u, &f, 4);
-                            u = (u + 0x1000u) & ~0x1fffu;
-                            const size_t off = base + (size_t)nl * 128 + (size_t)(((kk >> 2) ^ (nl & 7)) << 4) + (kk & 3) * 4;
-                            std::memcpy(&pimg[off], &u, 4);
+                        for (int kk = 0; kk < 64; ++kk) {
+                            const __half h = __float2half_rn(Wt[(size_t)(kb * 64 + kk) * b.NC + sl * C + nl]);
+                            const size_t off = base + (size_t)nl * 128 + (size_t)(((kk >> 3) ^ (nl & 7)) << 4) + (kk & 7) * 2;
+                            std::memcpy(&pimg[off], &h, 2);
                         }
             if ((rc = upload(m, pimg, &b.pre_wimg)) != GNN_OK) return rc;
             // (largest shared-memory carve-out: the split is per-SM state that only changes on an idle SM, so a kernel that asks
             // for less would keep the kNN CTAs of the other stream off its SMs)
+            int occ = 0;
             if (C == 128) {
                 GNN_CUDA_TRY(cudaFuncSetAttribute(pre_tc_kernel<64, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize, PreTcCfg<64, 128>::SMEM_BYTES));
                 GNN_CUDA_TRY(cudaFuncSetAttribute(pre_tc_kernel<64, 128>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+                GNN_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pre_tc_kernel<64, 128>, PTC_THREADS, PreTcCfg<64, 128>::SMEM_BYTES));
             } else {
                 GNN_CUDA_TRY(cudaFuncSetAttribute(pre_tc_kernel<128, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, PreTcCfg<128, 256>::SMEM_BYTES));
                 GNN_CUDA_TRY(cudaFuncSetAttribute(pre_tc_kernel<128, 256>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+                GNN_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pre_tc_kernel<128, 256>, PTC_THREADS, PreTcCfg<128, 256>::SMEM_BYTES));
             }
+            b.pre_ctas_per_sm = std::max(1, std::min(occ, 512 / (2 * C)));   // co-resident CTAs must all fit their TMEM columns
         }
         switch (C) {
             case 32: rc = configure_edge_c<32>(b, m.n_sms, a.k); break;
@@ -1399,7 +1403,7 @@ int edgeconv_bf16_prepare(gnn_model& m, const float* blob) {
         void* d = nullptr;
         GNN_CUDA_TRY(cudaMalloc(&d, (size_t)m.Nmax * m.Cmax * sizeof(__nv_bfloat16))); m.allocs.push_back(d); sc->U = (__nv_bfloat16*)d;
         GNN_CUDA_TRY(cudaMalloc(&d, (size_t)m.Nmax * m.Cmax * sizeof(__nv_bfloat16))); m.allocs.push_back(d); sc->V = (__nv_bfloat16*)d;
-        GNN_CUDA_TRY(cudaMalloc(&d, (size_t)m.Nmax * m.Cmax * sizeof(float))); m.allocs.push_back(d); sc->R = (float*)d;
+        GNN_CUDA_TRY(cudaMalloc(&d, (size_t)m.Nmax * m.Cmax * sizeof(__half))); m.allocs.push_back(d); sc->R = (__half*)d;
     }
     return GNN_OK;
 }
@@ -1420,7 +1424,7 @@ int launch_pre_bf16(gnn_model& m, int block, const float* x, int N, Workspace& w
         PreTcParams tp;
         tp.x = x; tp.wimg = b.pre_wimg; tp.bias = b.pre_bias; tp.U = sc.U; tp.V = sc.V; tp.R = sc.R; tp.meta = w.meta;
         tp.n_tiles = (N + TILE_ROWS - 1) / TILE_ROWS;
-        const int grid = 3 * std::min(tp.n_tiles, std::max(1, m.n_sms / 3));
+        const int grid = 3 * std::min(tp.n_tiles, std::max(1, m.n_sms * b.pre_ctas_per_sm / 3));
         if (b.C == 128) pre_tc_kernel<64, 128><<<grid, PTC_THREADS, PreTcCfg<64, 128>::SMEM_BYTES, s>>>(tp);
         else pre_tc_kernel<128, 256><<<grid, PTC_THREADS, PreTcCfg<128, 256>::SMEM_BYTES, s>>>(tp);
     } else {

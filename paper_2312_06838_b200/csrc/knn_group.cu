@@ -7,11 +7,11 @@
 // ~3 jets of the configs' <n> = 40 per group, so ~110 of the 128 rows are busy instead of 40 with one jet per CTA).
 // thread = row = one particle; its candidates are the columns [c0, c1) of its own jet inside the tile.
 //   knn_group_gram_kernel<D, K>   feature spaces, D = 64 / 128 / 256 (R28): the tile's pairwise inner products as
-//       ONE tcgen05.mma chain (kind::tf32, M = 128, N = rows rounded up to 16, K = D, A = B = the tile) into TMEM;
-//       d(i, j) = G_ii + G_jj - 2 G_ij on rows centred on their JET's mean (centring keeps the cancellation error of the
-//       Gram form below the neighbour gaps, and per-jet means keep a jet's result independent of its group mates, so
-//       batch-composition invariance stays bitwise).  The distance matrix never leaves the SM: each thread reads its row
-//       of G from TMEM 16 columns at a time and selects in registers.
+//       ONE tcgen05.mma chain (kind::f16 on fp16 operands, M = 128, N = rows rounded up to 16, K = D, A = B = the tile) into
+//       TMEM; d(i, j) = G_ii + G_jj - 2 G_ij on rows centred on the FIRST ROW OF THEIR JET (a reference inside the jet keeps
+//       the cancellation error of the Gram form below the neighbour gaps, costs no pass over the tile, and depends on
+//       nothing but the jet, so batch-composition invariance stays bitwise).  The distance matrix never leaves the SM: each
+//       thread reads its row of G from TMEM 16 columns at a time and selects in registers.
 //   knn_group_coords_kernel<K>    spaces of <= 4 dimensions (the coordinates of block 1): exact direct differences in
 //       fp32 from shared memory, same selection.
 // Selection: 32-bit keys (float bits of d with the low 7 mantissa bits replaced by the jet-local index j < 128: d to 16
@@ -190,11 +190,10 @@ constexpr int KG_MMA_WARP = 4;
 
 template <int D>
 struct KnnGroupCfg {
-    static constexpr int KBD = D / 32;                         // K blocks of 32 tf32 (128 bytes per row)
+    static constexpr int KBD = D / 64;                         // K blocks of 64 fp16 (128 bytes per row)
     static constexpr int XK_BYTES = KG_ROWS * 128;
     static constexpr int X_BYTES = KBD * XK_BYTES;
-    static constexpr int MEAN_BYTES = KG_MAX_JETS * D * 4;
-    static constexpr int SMEM_BYTES = X_BYTES + MEAN_BYTES + KG_ROWS * 4 + KG_ROWS + (int)sizeof(GroupInfo) + 2 * 8 + 16 + 64;
+    static constexpr int SMEM_BYTES = X_BYTES + KG_ROWS * 4 + KG_ROWS * 4 + (int)sizeof(GroupInfo) + 2 * 8 + 16 + 64;
 };
 
 template <int D, int K>
@@ -205,11 +204,10 @@ knn_group_gram_kernel(const float* __restrict__ space, const int32_t* __restrict
     using Cfg = KnnGroupCfg<D>;
     constexpr int KBD = Cfg::KBD;
     extern __shared__ __align__(1024) uint8_t smem_raw[];
-    uint8_t* X = smem_raw;                    // [KBD][128 rows][32 tf32], 128B-swizzled after the centring pass
-    float* mean_s = reinterpret_cast<float*>(X + Cfg::X_BYTES);                 // [KG_MAX_JETS][D]
-    float* diag_s = mean_s + KG_MAX_JETS * D;                                   // [128]
-    uint8_t* rowjet_s = reinterpret_cast<uint8_t*>(diag_s + KG_ROWS);           // [128] jet slot of a row
-    GroupInfo* gi = reinterpret_cast<GroupInfo*>(rowjet_s + KG_ROWS);
+    uint8_t* X = smem_raw;                    // [KBD][128 rows][64 fp16], 128B-swizzled: the centred rows
+    float* diag_s = reinterpret_cast<float*>(X + Cfg::X_BYTES);                 // [128]
+    int* ref_s = reinterpret_cast<int*>(diag_s + KG_ROWS);                      // [128] first row (inside the tile) of a row's jet
+    GroupInfo* gi = reinterpret_cast<GroupInfo*>(ref_s + KG_ROWS);
     uint64_t* d_full = reinterpret_cast<uint64_t*>(reinterpret_cast<uint8_t*>(gi) + ((sizeof(GroupInfo) + 7) & ~7));
     uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(d_full + 1);
 #ifdef KNN_TRACE
@@ -226,61 +224,56 @@ knn_group_gram_kernel(const float* __restrict__ space, const int32_t* __restrict
     const int R = gi->R, r0 = gi->r0;
     if (tid == 0) { mbar_init(d_full, 1); fence_mbar_init(); }
     if (warp == KG_MMA_WARP) tmem_alloc(tmem_ptr, 128);
-    // (1) the tile's rows, raw fp32, with ONE round trip to memory: 16-byte cp.async per (row, chunk), all in flight
-    const float* src = space + (size_t)r0 * D;
-    constexpr int CPR = D / 4;                                  // 16-byte chunks per row
-    for (int e = tid; e < R * CPR; e += KG_THREADS) {
-        const int r = e / CPR, c = e - r * CPR;                  // chunk c of row r: K block c / 8, chunk c % 8 of its line
-        const unsigned sa = smem_u32(X + (c >> 3) * Cfg::XK_BYTES + r * 128 + ((c & 7) << 4));
-        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(src + (size_t)r * D + 4 * c) : "memory");
-    }
-    asm volatile("cp.async.commit_group;" ::: "memory");
     int jt = 0, c0 = 0, c1 = 0;
     if (tid < KG_ROWS) {
         row_range(gi, tid, jt, c0, c1);
         if (tid >= R) { c0 = 0; c1 = 0; }
-        rowjet_s[tid] = (uint8_t)jt;
+        ref_s[tid] = c0;
         if (tid < R && pjid) pjid[r0 + tid] = gi->j0 + jt;
     }
-    asm volatile("cp.async.wait_group 0;" ::: "memory");
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
     KTR();
     const uint32_t tmem = *tmem_ptr;
-    // (2) per-jet column means (lanes = consecutive columns: conflict-free); a jet's sum has a fixed order (four chains by the
-    //     row's index inside the jet modulo 4, combined as (s0 + s2) + (s1 + s3)), so it does not depend on the group
-    for (int e = tid; e < D * gi->nj; e += KG_THREADS) {
-        const int t = e / D, c = e - t * D;
-        const int a = gi->ls[t], n = gi->rows[t];
-        const float* colp = reinterpret_cast<const float*>(X + (c >> 5) * Cfg::XK_BYTES) + a * 32 + (c & 31);
-        float s0 = 0.0f, s1 = 0.0f, s2 = 0.0f, s3 = 0.0f;
-        int r = 0;
-        for (; r + 3 < n; r += 4) { s0 += colp[r * 32]; s1 += colp[(r + 1) * 32]; s2 += colp[(r + 2) * 32]; s3 += colp[(r + 3) * 32]; }
-        if (r < n) s0 += colp[r * 32];
-        if (r + 1 < n) s1 += colp[(r + 1) * 32];
-        if (r + 2 < n) s2 += colp[(r + 2) * 32];
-        mean_s[t * D + c] = n > 0 ? ((s0 + s2) + (s1 + s3)) / (float)n : 0.0f;
-    }
-    __syncthreads();
-    KTR();
-    // (3) in place: centre on the jet's mean, round to tf32 (RNA), apply the 128-byte swizzle.  One thread per 16-byte chunk,
-    //     the eight lanes of a quarter-warp on one 128-byte line (row, K block): they read it whole (eight bank groups) and
-    //     write it back permuted among themselves (chunk c -> c ^ (row & 7): again eight bank groups); the line's loads have
-    //     all landed before its first store issues (same warp, same instruction).  Rows >= R keep whatever the buffer
-    //     held: row i of A and row j of B only reach G_ij, and no entry with i >= R or j >= R is ever used.
-    for (int e = tid; e < R * KBD * 8; e += KG_THREADS) {
-        const int c = e & 7, l = e >> 3;
-        const int kb = l / R, r = l - kb * R;
-        uint8_t* line = X + kb * Cfg::XK_BYTES + r * 128;
-        const float4 v = *reinterpret_cast<const float4*>(line + (c << 4));
-        const float4 mu = *reinterpret_cast<const float4*>(mean_s + (int)rowjet_s[r] * D + kb * 32 + 4 * c);
-        uint4 o;
-        asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(o.x) : "f"(v.x - mu.x));
-        asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(o.y) : "f"(v.y - mu.y));
-        asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(o.z) : "f"(v.z - mu.z));
-        asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(o.w) : "f"(v.w - mu.w));
-        *reinterpret_cast<uint4*>(line + ((c ^ (r & 7)) << 4)) = o;
+    // (1) the tile's rows CENTRED ON THE FIRST ROW OF THEIR JET, rounded to fp16 (RNE; 10 mantissa bits as tf32) and stored with
+    //     the 128-byte swizzle.  d(i, j) is translation invariant, so any per-jet reference point is legitimate; moving the
+    //     origin into the jet keeps the cancellation error of the Gram form (G_ii + G_jj - 2 G_ij) below the neighbour gaps,
+    //     and a reference that is a row of the jet itself needs no pass over the tile (no column sums, no staging of the
+    //     raw rows) and depends on nothing but the jet: batch-composition invariance stays bitwise.  One item = 8 columns
+    //     of a row: its own 32 bytes and the reference row's, all loads of a thread in flight together (one round trip).
+    //     Rows >= R keep whatever the buffer held: row i of A and row j of B only reach G_ij, and no entry with i >= R or
+    //     j >= R is ever used.
+    const float* src = space + (size_t)r0 * D;
+    constexpr int IPR = D / 8;                                  // items per row
+    constexpr int ITEMS = (KG_ROWS * IPR + KG_THREADS - 1) / KG_THREADS;
+    const int n_items = R * IPR;
+#pragma unroll
+    for (int i0 = 0; i0 < ITEMS; i0 += 4) {
+        float4 xa[4], xb[4], ra[4], rb[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int e = tid + (i0 + u) * KG_THREADS;
+            if (i0 + u < ITEMS && e < n_items) {
+                const int r = e / IPR, c = e - r * IPR;
+                const float4* xp = reinterpret_cast<const float4*>(src + (size_t)r * D + 8 * c);
+                const float4* rp = reinterpret_cast<const float4*>(src + (size_t)ref_s[r] * D + 8 * c);
+                xa[u] = __ldg(xp); xb[u] = __ldg(xp + 1); ra[u] = __ldg(rp); rb[u] = __ldg(rp + 1);
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int e = tid + (i0 + u) * KG_THREADS;
+            if (i0 + u < ITEMS && e < n_items) {
+                const int r = e / IPR, c = e - r * IPR;
+                uint4 o;
+                o.x = pack_f16x2(xa[u].x - ra[u].x, xa[u].y - ra[u].y);
+                o.y = pack_f16x2(xa[u].z - ra[u].z, xa[u].w - ra[u].w);
+                o.z = pack_f16x2(xb[u].x - rb[u].x, xb[u].y - rb[u].y);
+                o.w = pack_f16x2(xb[u].z - rb[u].z, xb[u].w - rb[u].w);
+                *reinterpret_cast<uint4*>(X + (c >> 3) * Cfg::XK_BYTES + r * 128 + (((c & 7) ^ (r & 7)) << 4)) = o;
+            }
+        }
     }
     fence_proxy_async();
     __syncthreads();
@@ -288,14 +281,14 @@ knn_group_gram_kernel(const float* __restrict__ space, const int32_t* __restrict
     const int n16 = (R + 15) & ~15;
     if (warp == KG_MMA_WARP && lane == 0) {
         tc_fence_after();
-        const uint32_t idesc = idesc_tf32_f32(128, n16);
+        const uint32_t idesc = idesc_f16_f32(128, n16);
         const uint32_t x_addr = smem_u32(X);
 #pragma unroll
         for (int kb = 0; kb < KBD; ++kb)
 #pragma unroll
-            for (int ks = 0; ks < 4; ++ks) {
+            for (int ks = 0; ks < 4; ++ks) {                     // K = 16 fp16 = 32 bytes per step
                 const uint64_t ad = desc_sw128(x_addr + kb * Cfg::XK_BYTES + ks * 32);
-                mma_tf32_ss(tmem, ad, ad, idesc, (kb | ks) != 0);
+                mma_bf16_ss(tmem, ad, ad, idesc, (kb | ks) != 0);    // kind::f16; the descriptor says fp16 operands
             }
         mma_commit(d_full);
     }
@@ -359,8 +352,8 @@ knn_group_gram_kernel(const float* __restrict__ space, const int32_t* __restrict
     KTR();
 #ifdef KNN_TRACE
     if (threadIdx.x == 0 && (blockIdx.x % 97) == 5)
-        printf("knn<%d> cta %d R %d: group %llu load %llu mean %llu centre %llu mma %llu select %llu store %llu (ns)\n", D, blockIdx.x, R,
-               tr[1] - tr[0], tr[2] - tr[1], tr[3] - tr[2], tr[4] - tr[3], tr[5] - tr[4], tr[6] - tr[5], tr[7] - tr[6]);
+        printf("knn<%d> cta %d R %d: group %llu rows %llu centre %llu mma %llu select %llu store %llu (ns)\n", D, blockIdx.x, R,
+               tr[1] - tr[0], tr[2] - tr[1], tr[3] - tr[2], tr[4] - tr[3], tr[5] - tr[4], tr[6] - tr[5]);
 #endif
     if (warp == KG_MMA_WARP) tmem_dealloc(tmem, 128);
 }
