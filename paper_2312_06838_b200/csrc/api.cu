@@ -11,7 +11,8 @@ int edgeconv_bf16_prepare(gnn_model& m, const float* blob_host);       // edgeco
 void edgeconv_bf16_release(gnn_model& m);
 int launch_edgeconv_bf16(gnn_model& m, int block, const float* x, const int32_t* idx, int N, float* y, Workspace& w,
                          cudaStream_t s);
-int launch_pre_bf16(gnn_model& m, int block, const float* x, int N, Workspace& w, cudaStream_t s);
+int launch_pre_bf16(gnn_model& m, int block, const float* x, int N, Workspace& w, cudaStream_t s, int dep);
+bool pre_bf16_single_wave(const gnn_model& m, int block);
 int launch_edge_bf16(gnn_model& m, int block, const int32_t* idx, int N, float* y, Workspace& w, cudaStream_t s);
 bool edgeconv_bf16_can_pool(const gnn_model& m, int block);
 
@@ -148,9 +149,7 @@ int alloc_workspace(gnn_model* m, Workspace& w) {
     if ((rc = dev_alloc(m, &w.poffsets, Bmax + 1)) != GNN_OK) return rc;
     if ((rc = dev_alloc(m, &w.pcounts, Bmax)) != GNN_OK) return rc;
     if ((rc = dev_alloc(m, &w.hlogits, Bmax * a.n_classes)) != GNN_OK) return rc;
-    GNN_CUDA_TRY(cudaStreamCreateWithFlags(&w.aux, cudaStreamNonBlocking));
-    GNN_CUDA_TRY(cudaEventCreateWithFlags(&w.ev_x, cudaEventDisableTiming));
-    GNN_CUDA_TRY(cudaEventCreateWithFlags(&w.ev_pre, cudaEventDisableTiming));
+    GNN_CUDA_TRY(cudaMemset(w.pool, 0, Bmax * (size_t)a.channels[a.n_blocks - 1][2] * sizeof(unsigned long long)));
     GNN_CUDA_TRY(cudaMemset(w.status, 0, sizeof(unsigned)));
     GNN_CUDA_TRY(cudaMemset(w.meta, 0, 4 * sizeof(int32_t)));
     return GNN_OK;
@@ -192,50 +191,50 @@ int forward(gnn_model* m, Workspace& w, const float* feats, const float* coords,
     const float* x = feats;
     float* bufs[2] = {w.xa, w.xb};
     const bool bf16 = a.precision == GNN_BF16;
-    static const bool no_fork = std::getenv("GNN_NO_FORK") != nullptr;           // developer knob: everything on one stream
-    const bool fork = bf16 && !no_fork && w.aux != nullptr;
-    // bf16 mode: the last block adds its output straight into the per-jet channel sums (step a7 inside E3 of step a6)
+    // bf16 mode: the last block adds its output straight into the per-jet channel sums (step a7 inside E3 of step a6).  The
+    // sums are zero between forwards: the head kernel that reads them clears them (head_split_kernel), else they are cleared here.
     static const bool no_fuse = std::getenv("GNN_NO_POOL_FUSE") != nullptr;     // developer knob: A/B of the pooling epilogue
     const bool fuse_pool = bf16 && !no_fuse && edgeconv_bf16_can_pool(*m, a.n_blocks - 1);
+    if (fuse_pool && !w.pool_self_cleaning &&
+        cudaMemsetAsync(w.pool, 0, (size_t)B * a.channels[a.n_blocks - 1][2] * sizeof(unsigned long long), s) != cudaSuccess)
+        return GNN_ERR_CUDA;
     for (int l = 0; l < a.n_blocks; ++l) {
         const float* space = (l == 0) ? coords : x;
         int D = (l == 0) ? a.coord_dims : block_in(a, l);
         float* y = (fuse_pool && l == a.n_blocks - 1) ? nullptr : bufs[l & 1];
-        // bf16 mode: u, v, shortcut of this block depend on x only, so the per-particle pre kernel runs beside the kNN of the
-        // block on the slice's auxiliary stream (fork: aux waits for x; join: `s` waits for the pre kernel before the edge
-        // kernel).  The join is enqueued on every path out of the fork, error or not, so aux never outlives the call.
-        int rc_pre = 0;
-        bool joined = true;
-        if (fork) {
-            if (cudaEventRecord(w.ev_x, s) != cudaSuccess || cudaStreamWaitEvent(w.aux, w.ev_x, 0) != cudaSuccess) return GNN_ERR_CUDA;
-            rc_pre = launch_pre_bf16(*m, l, x, N_upper, w, w.aux);
-            joined = cudaEventRecord(w.ev_pre, w.aux) == cudaSuccess;
-            // the per-jet channel sums are zeroed behind the first pre kernel on the auxiliary stream: off the critical path
-            // (it runs under the first edge kernel) and ordered before the last block by the later forks / joins.  The fork
-            // above also orders it after everything already enqueued on `s` (an earlier forward reading the sums).
-            if (fuse_pool && l == 0 && a.n_blocks > 1 &&
-                cudaMemsetAsync(w.pool, 0, (size_t)B * a.channels[a.n_blocks - 1][2] * sizeof(unsigned long long), w.aux) != cudaSuccess)
-                joined = false;
+        if (bf16) {
+            // One stream, programmatic dependent launches.  u, v and the shortcut of a block depend on x only, as does its kNN,
+            // so the two kernels run SIDE BY SIDE as a primary / secondary pair (gnn_internal.h, DEP_*); the primary is the one
+            // whose CTAs are all resident at once: the tensor-core pre kernel (blocks >= 2), else the grouped kNN kernel.  The
+            // primary's prologue (weights, TMEM) runs under the tail of the kernel before it.  edge_l is a normal launch: it
+            // starts when the secondary, hence the pair, has completed.
+            int rc_pre, rc_knn;
+            if (N_upper == 0 || !knn_group_supported(D, a.max_particles)) {          // no pair: ordinary launches
+                if ((rc_pre = launch_pre_bf16(*m, l, x, N_upper, w, s, DEP_NONE)) < 0) return rc_pre;
+                if ((rc_knn = launch_knn(space, D, a.k, B, a.max_particles, w, w.idx, 0, 1, s)) < 0) return rc_knn;
+            } else if (pre_bf16_single_wave(*m, l)) {
+                if ((rc_pre = launch_pre_bf16(*m, l, x, N_upper, w, s, DEP_PRIMARY)) < 0) return rc_pre;
+                if ((rc_knn = launch_knn(space, D, a.k, B, a.max_particles, w, w.idx, 0, 1, s, DEP_SECONDARY)) < 0) return rc_knn;
+            } else {
+                if ((rc_knn = launch_knn(space, D, a.k, B, a.max_particles, w, w.idx, 0, 1, s, DEP_PRIMARY)) < 0) return rc_knn;
+                if ((rc_pre = launch_pre_bf16(*m, l, x, N_upper, w, s, DEP_SECONDARY)) < 0) return rc_pre;
+            }
+            n += rc_pre + rc_knn;
+            tm.mark("knn", l);
+            rc = launch_edge_bf16(*m, l, w.idx, N_upper, y, w, s);
+        } else {
+            const int rc_knn = launch_knn(space, D, a.k, B, a.max_particles, w, w.idx, 0, 0, s);
+            if (rc_knn < 0) return rc_knn;
+            n += rc_knn;
+            tm.mark("knn", l);
+            rc = launch_edgeconv_f32(m->blocks[l], a.k, x, w.idx, N_upper, y, w, s);
         }
-        if (fuse_pool && l == 0 && a.n_blocks == 1 &&          // a single block: nothing to hide it under
-            cudaMemsetAsync(w.pool, 0, (size_t)B * a.channels[0][2] * sizeof(unsigned long long), s) != cudaSuccess)
-            return GNN_ERR_CUDA;
-        const int rc_knn = launch_knn(space, D, a.k, B, a.max_particles, w, w.idx, 0, bf16 ? 1 : 0, s);
-        if (fork) joined = joined && cudaStreamWaitEvent(s, w.ev_pre, 0) == cudaSuccess;
-        if (rc_pre < 0) return rc_pre;
-        if (rc_knn < 0) return rc_knn;
-        if (!joined) return GNN_ERR_CUDA;
-        n += rc_pre + rc_knn;
-        tm.mark("knn", l);
-        if (fork) rc = launch_edge_bf16(*m, l, w.idx, N_upper, y, w, s);
-        else if (bf16) rc = launch_edgeconv_bf16(*m, l, x, w.idx, N_upper, y, w, s);
-        else rc = launch_edgeconv_f32(m->blocks[l], a.k, x, w.idx, N_upper, y, w, s);
         if (rc < 0) return rc;
         n += rc;
         tm.mark("edgeconv", l);
         x = y;
     }
-    if ((rc = launch_pool_head(*m, x, B, w, logits, s)) < 0) return rc;
+    if ((rc = launch_pool_head(*m, x, B, w, logits, s, bf16)) < 0) return rc;
     n += rc;
     tm.mark("pool_head");
     m->launches.fetch_add(n, std::memory_order_relaxed);
@@ -248,6 +247,11 @@ int forward(gnn_model* m, Workspace& w, const float* feats, const float* coords,
 }
 
 }  // namespace
+
+bool gnn_pdl_enabled() {
+    static const bool on = std::getenv("GNN_NO_PDL") == nullptr;
+    return on;
+}
 
 extern "C" {
 
@@ -287,8 +291,10 @@ int gnn_create(const void* weights_host, size_t bytes, const gnn_arch* arch, int
         return rc;
     }
     m->ws.resize(m->arch.workspace_slices);
-    for (auto& w : m->ws)
+    for (auto& w : m->ws) {
         if ((rc = alloc_workspace(m, w)) != GNN_OK) { gnn_destroy(m); return rc; }
+        w.pool_self_cleaning = head_clears_pool(*m);
+    }
     if (m->arch.precision == GNN_BF16 &&
         (rc = edgeconv_bf16_prepare(*m, static_cast<const float*>(weights_host))) != GNN_OK) {
         gnn_destroy(m);
@@ -307,9 +313,6 @@ void gnn_destroy(gnn_model* m) {
     edgeconv_bf16_release(*m);
     for (auto& w : m->ws) {
         for (cudaEvent_t e : w.prof_events) cudaEventDestroy(e);
-        if (w.ev_x) cudaEventDestroy(w.ev_x);
-        if (w.ev_pre) cudaEventDestroy(w.ev_pre);
-        if (w.aux) cudaStreamDestroy(w.aux);
     }
     delete m;
 }
@@ -522,13 +525,14 @@ int gnn_debug_edgeconv_pool(gnn_model* m, const float* x_dev, const int32_t* idx
     if (N > 0) {
         if ((rc = launch_globalize_idx(idx_dev, m->arch.k, B, w, w.idx, s)) < 0) return rc;
         n += rc;
-        if ((rc = launch_pre_bf16(*m, block, x_dev, N, w, s)) < 0) return rc;
+        if ((rc = launch_pre_bf16(*m, block, x_dev, N, w, s, DEP_NONE)) < 0) return rc;
         n += rc;
         if ((rc = launch_edge_bf16(*m, block, w.idx, N, nullptr, w, s)) < 0) return rc;
         n += rc;
     }
     if ((rc = launch_pooled_mean(*m, B, w, g_dev, s)) < 0) return rc;
     n += rc;
+    GNN_CUDA_TRY(cudaMemsetAsync(w.pool, 0, (size_t)B * C * sizeof(unsigned long long), s));   // the sums are zero between calls
     m->launches.fetch_add(n, std::memory_order_relaxed);
     return cudaGetLastError() == cudaSuccess ? GNN_OK : GNN_ERR_CUDA;
 }

@@ -186,6 +186,7 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
     if constexpr (PAIR) cluster_sync_all(); else __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tmem_ptr;
+    grid_dep_launch();                                           // the next kernel's prologue may run under this kernel's tail
 
     auto tile_p0 = [&](int t) {
         int w = unit + t * n_units;                              // CH = 1: round-robin
@@ -243,6 +244,8 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
         // epilogue (their only dependency is h_free of the previous tile), so the L2 latency of the gather is off the
         // MMA <-> epilogue critical path ===============================================================================
         const int g = warp - Cfg::NEP, gk = g % KB, half = g / KB;
+        grid_dep_wait();                                         // idx, U, V come from the kernels before this one; the set-up
+                                                                 // above and the weight load ran under their tail
         constexpr int CPR = Cfg::KW / 8;                         // 16-byte chunks per row of a K block
         constexpr int RPI = 32 / CPR;                            // rows per warp iteration
         constexpr int RW = Cfg::RW, NI = RW / 32;
@@ -329,6 +332,7 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
     } else {
         // ===== epilogue warps: E2 (D0 -> H2) and E3 (D1 -> mean -> y) for lane quadrant q, columns [cg*CWE, +CWE) ==========
         const int q = warp & 3, cg = (warp % NE) >> 2;
+        grid_dep_wait();                                         // idx, R, pjid come from the kernels before this one
         const int row = 32 * q + lane;                           // TMEM lane = edge row of the tile
         const int col0 = cg * CWE;
         constexpr int SLABS = CWE / 32;
@@ -874,9 +878,10 @@ struct PreParams {
     __half* R;               // [N, C3]
     const int32_t* meta;
     int cin, Kp, C1, C3, NC;
+    int dep;                 // DEP_* of gnn_internal.h
 };
 
-__global__ void __launch_bounds__(PRE_THREADS) pre_kernel(PreParams p) {
+__device__ __forceinline__ void pre_body(const PreParams& p) {
     extern __shared__ __align__(16) float xs[];      // [PRE_ROWS][Kp + 4]
     if (p.meta[0]) return;
     const int N = p.meta[1];
@@ -931,6 +936,13 @@ __global__ void __launch_bounds__(PRE_THREADS) pre_kernel(PreParams p) {
     }
 }
 
+// dep: the kernel's role in a primary / secondary pair with the kNN of the block (gnn_internal.h)
+__global__ void __launch_bounds__(PRE_THREADS) pre_kernel(PreParams p) {
+    if (p.dep != DEP_SECONDARY) { grid_dep_wait(); grid_dep_launch(); }      // x and meta come from the kernels before this one
+    pre_body(p);
+    if (p.dep == DEP_SECONDARY && blockIdx.x == 0) grid_dep_wait();
+}
+
 // Narrow inputs (block 1: C_in = F <= 16): thread (x = column quad, y) computes four output columns of PRS_ROWS consecutive
 // particles; the rows and the weight column quad come straight from L1 / L2 (a CTA shares 16 rows and the 5 KB weight matrix),
 // no staging, no barrier.
@@ -938,7 +950,7 @@ constexpr int PRS_ROWS = 4;      // rows per thread
 constexpr int PRS_TY = 4;        // blockDim.y
 
 template <int KP>
-__global__ void __launch_bounds__(1024) pre_small_kernel(PreParams p) {
+__device__ __forceinline__ void pre_small_body(const PreParams& p) {
     if (p.meta[0]) return;
     const int N = p.meta[1];
     const int cg = threadIdx.x;                                  // blockDim.x = NC / 4
@@ -973,21 +985,31 @@ __global__ void __launch_bounds__(1024) pre_small_kernel(PreParams p) {
     }
 }
 
+template <int KP>
+__global__ void __launch_bounds__(1024) pre_small_kernel(PreParams p) {
+    if (p.dep != DEP_SECONDARY) { grid_dep_wait(); grid_dep_launch(); }      // x and meta come from the kernels before this one
+    pre_small_body<KP>(p);
+    if (p.dep == DEP_SECONDARY && blockIdx.x == 0) grid_dep_wait();
+}
+
 // ---- pre kernel on the tensor cores (blocks whose input width is a multiple of 64): [u | v | r] = x * Wpre^T + bias ---------
 // One GEMM [N, CIN] x [CIN, 3C], fp16 operands (x and the folded weights rounded RNE: 10 mantissa bits as tf32, at twice
 // the rate and half the shared memory), fp32 accumulation in TMEM.  The 3C output columns are three slices of C columns
 // (u, v, r); a CTA keeps ONE slice of the weights resident ([C][CIN] fp16 as 128B-swizzled K blocks of 64) and walks
-// the 128-row tiles of its slice group.  The 128 rows of a tile are contiguous in x, so a tile arrives with ONE bulk (TMA)
-// copy into a raw fp32 buffer, issued a tile ahead by the MMA thread: no registers hold loads in flight, and the next tile
-// streams in while this one is converted, multiplied and stored.  Converter warps turn the raw rows into the swizzled fp16
-// operand tile; the accumulator is double-buffered (2 x C TMEM columns), so epilogue(t) runs under convert / MMA (t + 1).
-// Shared memory (169 KB for 128 -> 256) and registers leave room for a kNN CTA of the same block on the SM: the forward
-// runs the two kernels side by side on two streams.
-// Warps: 0-7 epilogue (thread = row = TMEM lane, slabs of parity w >> 2), 8-11 converters, 12 TMA + MMA issuer + TMEM owner.
-constexpr int PTC_EPI_WARPS = 8;
+// the 128-row tiles of its slice group.  The 128 rows of a tile are contiguous in x, so a tile arrives as two bulk (TMA)
+// copies of 64 rows into a raw fp32 buffer, each re-issued for the next tile by the MMA thread as soon as the converter
+// warps have read that half: no registers hold loads in flight, and the next tile streams in while this one is
+// converted, multiplied and stored.  Converter warps turn the raw rows into the swizzled fp16 operand tile.  A tile is
+// multiplied as two N halves of C / 2 columns, each with its own accumulator (C TMEM columns in all): the epilogue of one
+// half runs under the MMAs of the other and of the next tile.
+// Shared memory (161 KB for 128 -> 256), registers (288 threads x 80) and TMEM (C columns) leave room for kNN CTAs of the
+// same block on the SM: the forward runs the two kernels side by side on two streams.
+// Warps: 0-3 epilogue (thread = row = TMEM lane), 4-7 converters, 8 TMA + MMA issuer + TMEM owner.
+constexpr int PTC_EPI_WARPS = 4;
 constexpr int PTC_CVT_WARPS = 4;
 constexpr int PTC_MMA_WARP = PTC_EPI_WARPS + PTC_CVT_WARPS;
 constexpr int PTC_THREADS = 32 * (PTC_MMA_WARP + 1);
+constexpr int PTC_HALF_ROWS = TILE_ROWS / 2;
 
 template <int CIN, int C>
 struct PreTcCfg {
@@ -996,9 +1018,10 @@ struct PreTcCfg {
     static constexpr int A_BYTES = KBA * AK_BYTES;
     static constexpr int WK_BYTES = C * 128;                  // [C][64] fp16 chunk
     static constexpr int W_BYTES = KBA * WK_BYTES;            // one slice
-    static constexpr int RAW_BYTES = TILE_ROWS * CIN * 4;     // one tile of raw fp32 rows
-    static constexpr int TMEM_COLS = 2 * C;
-    static constexpr int NBAR = 8;
+    static constexpr int RAW_BYTES = TILE_ROWS * CIN * 4;     // one tile of raw fp32 rows (two halves of 64 rows)
+    static constexpr int NH = C / 2;                          // columns of an N half
+    static constexpr int TMEM_COLS = C;
+    static constexpr int NBAR = 10;
     static constexpr int STAGE_BYTES = PTC_EPI_WARPS * 2048;  // per epilogue warp: [32 rows][32 cols] 16-bit, swizzled
     static constexpr int SMEM_BYTES = W_BYTES + A_BYTES + RAW_BYTES + STAGE_BYTES + C * 4 + NBAR * 8 + 16;
 };
@@ -1017,14 +1040,9 @@ struct PreTcParams {
 template <int CIN, int C>
 __global__ void __maxnreg__(80) pre_tc_kernel(PreTcParams p) {
     using Cfg = PreTcCfg<CIN, C>;
-    constexpr int KBA = Cfg::KBA;
+    constexpr int KBA = Cfg::KBA, NH = Cfg::NH;
     extern __shared__ __align__(1024) uint8_t smem_raw[];
-    if (p.meta[0]) return;
-    const int N = p.meta[1];
-    const int n_tiles = min(p.n_tiles, (N + TILE_ROWS - 1) / TILE_ROWS);
     const int slice = blockIdx.x % 3, gi = blockIdx.x / 3, ng = gridDim.x / 3;
-    if (gi >= n_tiles) return;
-    const int T = (n_tiles - gi + ng - 1) / ng;
 
     // no pointer arithmetic through integers here: the compiler must keep the shared address space (STS/LDS, not generic
     // ST/LD); these kernels have no static shared memory, so the dynamic window starts 1024-byte aligned (checked)
@@ -1036,20 +1054,26 @@ __global__ void __maxnreg__(80) pre_tc_kernel(PreTcParams p) {
     uint8_t* stage = raw + Cfg::RAW_BYTES;
     float* bias_s = reinterpret_cast<float*>(stage + Cfg::STAGE_BYTES);
     uint64_t* bars = reinterpret_cast<uint64_t*>(bias_s + C);
-    uint64_t* raw_full = bars;                // TMA -> converters: the tile's raw rows landed
-    uint64_t* a_ready = bars + 1;             // converters -> MMA: operand tile written (and the raw buffer is free again)
-    uint64_t* a_free = bars + 2;              // MMA -> converters: the operand tile has been read
-    uint64_t* d_full = bars + 3;              // [2]
-    uint64_t* d_free = bars + 5;              // [2]
-    uint64_t* w_full = bars + 7;
+    uint64_t* raw_full = bars;                // [2] TMA -> converters: rows [64 h, 64 h + 64) of the tile landed
+    uint64_t* cv_done = bars + 2;             // [2] converters -> MMA: that half is converted (its raw buffer is free again;
+                                              //     [1] also says the whole operand tile is written)
+    uint64_t* a_free = bars + 4;              // MMA -> converters: the operand tile has been read
+    uint64_t* d_full = bars + 5;              // [2] accumulator of N half h complete
+    uint64_t* d_free = bars + 7;              // [2] ... drained
+    uint64_t* w_full = bars + 9;
     uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(bars + Cfg::NBAR);
 
+    // ---- prologue: nothing here depends on the kernels before this one (weights, barriers, TMEM), so as a programmatic
+    // dependent it runs under their tail ------------------------------------------------------------------------------------
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     if (tid == 0) {
-        mbar_init(raw_full, 1);
-        mbar_init(a_ready, PTC_CVT_WARPS);
+        for (int i = 0; i < 2; ++i) {
+            mbar_init(&raw_full[i], 1);
+            mbar_init(&cv_done[i], PTC_CVT_WARPS);
+            mbar_init(&d_full[i], 1);
+            mbar_init(&d_free[i], PTC_EPI_WARPS);
+        }
         mbar_init(a_free, 1);
-        for (int i = 0; i < 2; ++i) { mbar_init(&d_full[i], 1); mbar_init(&d_free[i], PTC_EPI_WARPS); }
         mbar_init(w_full, 1);
         fence_mbar_init();
     }
@@ -1059,42 +1083,55 @@ __global__ void __maxnreg__(80) pre_tc_kernel(PreTcParams p) {
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tmem_ptr;
-    auto tile_bytes = [&](int t) {
-        const int r0 = (gi + t * ng) * TILE_ROWS;
-        return (uint32_t)(min(TILE_ROWS, N - r0) * CIN * 4);
-    };
+    if (warp == PTC_MMA_WARP && lane == 0) {
+        mbar_arrive_expect_tx(w_full, Cfg::W_BYTES);
+        const uint8_t* src = p.wimg + (size_t)slice * Cfg::W_BYTES;
+        for (int c = 0; c < KBA; ++c)
+            bulk_g2s(Wsm + (size_t)c * Cfg::WK_BYTES, src + (size_t)c * Cfg::WK_BYTES, Cfg::WK_BYTES, w_full);
+    }
+    grid_dep_wait();                          // x and meta come from the kernels before this one
+    grid_dep_launch();                        // the kNN of the block runs beside this kernel (forward() in api.cu)
+    const int N = p.meta[0] ? 0 : p.meta[1];
+    const int n_tiles = min(p.n_tiles, (N + TILE_ROWS - 1) / TILE_ROWS);
+    const int T = gi < n_tiles ? (n_tiles - gi + ng - 1) / ng : 0;      // 0: nothing to do, but the weight copy must land first
 
     if (warp == PTC_MMA_WARP) {
-        // ===== weight load, tile loads (one tile ahead) and MMA issue ===================================================
+        // ===== weight load, tile loads and MMA issue ====================================================================
         if (lane == 0) {
-            mbar_arrive_expect_tx(raw_full, tile_bytes(0));
-            bulk_g2s(raw, p.x + (size_t)gi * TILE_ROWS * CIN, tile_bytes(0), raw_full);
-            mbar_arrive_expect_tx(w_full, Cfg::W_BYTES);
-            const uint8_t* src = p.wimg + (size_t)slice * Cfg::W_BYTES;
-            for (int c = 0; c < KBA; ++c)
-                bulk_g2s(Wsm + (size_t)c * Cfg::WK_BYTES, src + (size_t)c * Cfg::WK_BYTES, Cfg::WK_BYTES, w_full);
-            constexpr uint32_t idesc = idesc_f16_f32(128, C);
+            auto load_half = [&](int t, int h) {                 // rows [64 h, 64 h + 64) of tile t (fewer, or none, at the end)
+                const int r0 = (gi + t * ng) * TILE_ROWS + h * PTC_HALF_ROWS;
+                const int rows = max(0, min(PTC_HALF_ROWS, N - r0));
+                if (rows > 0) {
+                    mbar_arrive_expect_tx(&raw_full[h], (uint32_t)(rows * CIN * 4));
+                    bulk_g2s(raw + h * (Cfg::RAW_BYTES / 2), p.x + (size_t)r0 * CIN, (uint32_t)(rows * CIN * 4), &raw_full[h]);
+                } else {
+                    mbar_arrive(&raw_full[h]);
+                }
+            };
+            if (T > 0) { load_half(0, 0); load_half(0, 1); }
+            constexpr uint32_t idesc = idesc_f16_f32(128, NH);
             const uint32_t a_addr = smem_u32(A), w_addr = smem_u32(Wsm);
             mbar_wait(w_full, 0);
             for (int t = 0; t < T; ++t) {
-                const int acc = t & 1;
-                mbar_wait(a_ready, t & 1);                       // operand tile t written: the raw buffer is free
-                if (t + 1 < T) {
-                    mbar_arrive_expect_tx(raw_full, tile_bytes(t + 1));
-                    bulk_g2s(raw, p.x + (size_t)(gi + (t + 1) * ng) * TILE_ROWS * CIN, tile_bytes(t + 1), raw_full);
+                mbar_wait(&cv_done[0], t & 1);
+                if (t + 1 < T) load_half(t + 1, 0);
+                mbar_wait(&cv_done[1], t & 1);                   // operand tile t written
+                if (t + 1 < T) load_half(t + 1, 1);
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    mbar_wait(&d_free[h], (t & 1) ^ 1);
+                    tc_fence_after();
+#pragma unroll
+                    for (int kb = 0; kb < KBA; ++kb)
+#pragma unroll
+                        for (int ks = 0; ks < 4; ++ks) {         // K = 16 fp16 = 32 bytes per step
+                            const uint64_t ad = desc_sw128(a_addr + kb * Cfg::AK_BYTES + ks * 32);
+                            const uint64_t bd = desc_sw128(w_addr + kb * Cfg::WK_BYTES + h * (NH * 128) + ks * 32);
+                            mma_bf16_ss(tmem + h * NH, ad, bd, idesc, (kb | ks) != 0);   // kind::f16; the descriptor says fp16
+                        }
+                    if (h == 1) mma_commit(a_free);
+                    mma_commit(&d_full[h]);
                 }
-                mbar_wait(&d_free[acc], ((t >> 1) & 1) ^ 1);
-                tc_fence_after();
-#pragma unroll
-                for (int kb = 0; kb < KBA; ++kb)
-#pragma unroll
-                    for (int ks = 0; ks < 4; ++ks) {             // K = 16 fp16 = 32 bytes per step
-                        const uint64_t ad = desc_sw128(a_addr + kb * Cfg::AK_BYTES + ks * 32);
-                        const uint64_t bd = desc_sw128(w_addr + kb * Cfg::WK_BYTES + ks * 32);
-                        mma_bf16_ss(tmem + acc * C, ad, bd, idesc, (kb | ks) != 0);   // kind::f16; the descriptor says fp16
-                    }
-                mma_commit(a_free);
-                mma_commit(&d_full[acc]);
             }
         }
     } else if (warp >= PTC_EPI_WARPS) {
@@ -1102,69 +1139,75 @@ __global__ void __maxnreg__(80) pre_tc_kernel(PreTcParams p) {
         // (32 bytes in, one 16-byte chunk out); the eight lanes of a quarter-warp write one 128-byte line ====================
         const int ct = tid - PTC_EPI_WARPS * 32;
         constexpr int IPR = CIN / 8;                             // items per row
-        constexpr int ITEMS = TILE_ROWS * IPR / (PTC_CVT_WARPS * 32);
+        constexpr int ITEMS = PTC_HALF_ROWS * IPR / (PTC_CVT_WARPS * 32);
         for (int t = 0; t < T; ++t) {
-            mbar_wait(raw_full, t & 1);
             if (t > 0) mbar_wait(a_free, (t - 1) & 1);
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                mbar_wait(&raw_full[h], t & 1);
 #pragma unroll 4
-            for (int i = 0; i < ITEMS; ++i) {
-                const int e = ct + i * (PTC_CVT_WARPS * 32);
-                const int r = e / IPR, c = e - r * IPR;
-                const float4 a = *reinterpret_cast<const float4*>(raw + (size_t)r * (CIN * 4) + c * 32);
-                const float4 b = *reinterpret_cast<const float4*>(raw + (size_t)r * (CIN * 4) + c * 32 + 16);
-                const uint4 o = make_uint4(pack_f16x2(a.x, a.y), pack_f16x2(a.z, a.w), pack_f16x2(b.x, b.y), pack_f16x2(b.z, b.w));
-                *reinterpret_cast<uint4*>(A + (c >> 3) * Cfg::AK_BYTES + r * 128 + (((c & 7) ^ (r & 7)) << 4)) = o;
+                for (int i = 0; i < ITEMS; ++i) {
+                    const int e = ct + i * (PTC_CVT_WARPS * 32);
+                    const int r = h * PTC_HALF_ROWS + e / IPR, c = e % IPR;
+                    const float4 a = *reinterpret_cast<const float4*>(raw + (size_t)r * (CIN * 4) + c * 32);
+                    const float4 b = *reinterpret_cast<const float4*>(raw + (size_t)r * (CIN * 4) + c * 32 + 16);
+                    const uint4 o = make_uint4(pack_f16x2(a.x, a.y), pack_f16x2(a.z, a.w), pack_f16x2(b.x, b.y), pack_f16x2(b.z, b.w));
+                    *reinterpret_cast<uint4*>(A + (c >> 3) * Cfg::AK_BYTES + r * 128 + (((c & 7) ^ (r & 7)) << 4)) = o;
+                }
+                fence_proxy_async();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&cv_done[h]);
             }
-            fence_proxy_async();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(a_ready);
         }
     } else {
         // ===== epilogue: thread = row = TMEM lane; slice 0 -> U (bf16), 1 -> V (bf16), 2 -> R (fp16) ======================
-        const int q = warp & 3, eh = warp >> 2;
+        const int q = warp;
         uint16_t* outp = reinterpret_cast<uint16_t*>(slice == 0 ? (void*)p.U : (slice == 1 ? (void*)p.V : (void*)p.R));
+        uint8_t* st = stage + warp * 2048;
         for (int t = 0; t < T; ++t) {
-            const int acc = t & 1;
-            mbar_wait(&d_full[acc], (t >> 1) & 1);
-            tc_fence_after();
+            const int tr0 = (gi + t * ng) * TILE_ROWS + 32 * q;
 #pragma unroll 1
-            for (int s = eh; s < C / 32; s += 2) {
-                float v[32];
-                tmem_ld32(tmem + ((uint32_t)(32 * q) << 16) + acc * C + s * 32, v);
-                tmem_ld_wait();
-                if (s + 2 >= C / 32) {
-                    tc_fence_before();
+            for (int h = 0; h < 2; ++h) {
+                mbar_wait(&d_full[h], t & 1);
+                tc_fence_after();
+#pragma unroll 1
+                for (int s = 0; s < NH / 32; ++s) {
+                    const int col = h * NH + s * 32;
+                    float v[32];
+                    tmem_ld32(tmem + ((uint32_t)(32 * q) << 16) + col, v);
+                    tmem_ld_wait();
+                    if (s == NH / 32 - 1) {
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(&d_free[h]);
+                    }
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const float4 b = *reinterpret_cast<const float4*>(bias_s + col + 4 * i);
+                        v[4 * i] += b.x; v[4 * i + 1] += b.y; v[4 * i + 2] += b.z; v[4 * i + 3] += b.w;
+                    }
+                    // transpose through this warp's staging tile so that global stores are whole 64-byte row segments: thread =
+                    // row writes swizzled 16-byte chunks, then 4 lanes read one row back
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        uint4 o;
+                        if (slice == 2)
+                            o = make_uint4(pack_f16x2(v[8 * i], v[8 * i + 1]), pack_f16x2(v[8 * i + 2], v[8 * i + 3]),
+                                           pack_f16x2(v[8 * i + 4], v[8 * i + 5]), pack_f16x2(v[8 * i + 6], v[8 * i + 7]));
+                        else
+                            o = make_uint4(pack_bf16x2(v[8 * i], v[8 * i + 1]), pack_bf16x2(v[8 * i + 2], v[8 * i + 3]),
+                                           pack_bf16x2(v[8 * i + 4], v[8 * i + 5]), pack_bf16x2(v[8 * i + 6], v[8 * i + 7]));
+                        *reinterpret_cast<uint4*>(st + lane * 64 + ((i ^ ((lane >> 1) & 3)) << 4)) = o;
+                    }
                     __syncwarp();
-                    if (lane == 0) mbar_arrive(&d_free[acc]);
-                }
 #pragma unroll
-                for (int i = 0; i < 8; ++i) {
-                    const float4 b = *reinterpret_cast<const float4*>(bias_s + s * 32 + 4 * i);
-                    v[4 * i] += b.x; v[4 * i + 1] += b.y; v[4 * i + 2] += b.z; v[4 * i + 3] += b.w;
+                    for (int it = 0; it < 4; ++it) {
+                        const int r = it * 8 + (lane >> 2), c = lane & 3;
+                        const uint4 o = *reinterpret_cast<const uint4*>(st + r * 64 + ((c ^ ((r >> 1) & 3)) << 4));
+                        if (tr0 + r < N) *(reinterpret_cast<uint4*>(outp + (size_t)(tr0 + r) * C + col) + c) = o;
+                    }
+                    __syncwarp();
                 }
-                // transpose through this warp's staging tile so that global stores are whole 64-byte row segments: thread =
-                // row writes swizzled 16-byte chunks, then 4 lanes read one row back
-                uint8_t* st = stage + warp * 2048;
-                const int tr0 = (gi + t * ng) * TILE_ROWS + 32 * q;
-#pragma unroll
-                for (int i = 0; i < 4; ++i) {
-                    uint4 o;
-                    if (slice == 2)
-                        o = make_uint4(pack_f16x2(v[8 * i], v[8 * i + 1]), pack_f16x2(v[8 * i + 2], v[8 * i + 3]),
-                                       pack_f16x2(v[8 * i + 4], v[8 * i + 5]), pack_f16x2(v[8 * i + 6], v[8 * i + 7]));
-                    else
-                        o = make_uint4(pack_bf16x2(v[8 * i], v[8 * i + 1]), pack_bf16x2(v[8 * i + 2], v[8 * i + 3]),
-                                       pack_bf16x2(v[8 * i + 4], v[8 * i + 5]), pack_bf16x2(v[8 * i + 6], v[8 * i + 7]));
-                    *reinterpret_cast<uint4*>(st + lane * 64 + ((i ^ ((lane >> 1) & 3)) << 4)) = o;
-                }
-                __syncwarp();
-#pragma unroll
-                for (int it = 0; it < 4; ++it) {
-                    const int r = it * 8 + (lane >> 2), c = lane & 3;
-                    const uint4 o = *reinterpret_cast<const uint4*>(st + r * 64 + ((c ^ ((r >> 1) & 3)) << 4));
-                    if (tr0 + r < N) *(reinterpret_cast<uint4*>(outp + (size_t)(tr0 + r) * C + s * 32) + c) = o;
-                }
-                __syncwarp();
             }
         }
     }
@@ -1278,13 +1321,15 @@ int launch_edge_t(const EdgeParams& p_in, int grid_cap, cudaStream_t s) {
         cudaLaunchConfig_t cfg{};
         cfg.gridDim = dim3(2 * n_units); cfg.blockDim = dim3(Cfg::THREADS);
         cfg.dynamicSmemBytes = SMEM; cfg.stream = s;
-        cudaLaunchAttribute at[1];
+        cudaLaunchAttribute at[2];
         at[0].id = cudaLaunchAttributeClusterDimension;
         at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
-        cfg.attrs = at; cfg.numAttrs = 1;
+        at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[1].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = at; cfg.numAttrs = gnn_pdl_enabled() ? 2 : 1;
         GNN_CUDA_TRY(cudaLaunchKernelEx(&cfg, edge_kernel<C, LOGK, POOL>, p));
     } else {
-        edge_kernel<C, LOGK, POOL><<<n_units, Cfg::THREADS, SMEM, s>>>(p);
+        GNN_CUDA_TRY(launch_k(edge_kernel<C, LOGK, POOL>, dim3(n_units), dim3(Cfg::THREADS), SMEM, s, true, p));
     }
     return GNN_OK;
 }
@@ -1381,7 +1426,7 @@ int edgeconv_bf16_prepare(gnn_model& m, const float* blob) {
                 GNN_CUDA_TRY(cudaFuncSetAttribute(pre_tc_kernel<128, 256>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
                 GNN_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pre_tc_kernel<128, 256>, PTC_THREADS, PreTcCfg<128, 256>::SMEM_BYTES));
             }
-            b.pre_ctas_per_sm = std::max(1, std::min(occ, 512 / (2 * C)));   // co-resident CTAs must all fit their TMEM columns
+            b.pre_ctas_per_sm = std::max(1, std::min(occ, 2));   // (TMEM: C columns per CTA, and the kNN CTAs of the block want theirs)
         }
         switch (C) {
             case 32: rc = configure_edge_c<32>(b, m.n_sms, a.k); break;
@@ -1416,29 +1461,34 @@ void edgeconv_bf16_release(gnn_model& m) {
 
 // per-particle part of a block (u, v, shortcut): depends on x only, so the forward runs it on the workspace's auxiliary
 // stream next to the kNN of the same block
-int launch_pre_bf16(gnn_model& m, int block, const float* x, int N, Workspace& w, cudaStream_t s) {
+// dep: DEP_* of gnn_internal.h (DEP_NONE = an ordinary launch); the tensor-core kernel can only be a primary
+bool pre_bf16_single_wave(const gnn_model& m, int block) { return static_cast<const Bf16BlockDev*>(m.bf16_blocks)[block].pre_wimg != nullptr; }
+
+int launch_pre_bf16(gnn_model& m, int block, const float* x, int N, Workspace& w, cudaStream_t s, int dep) {
+    const bool pdl = dep != DEP_NONE;
     if (N == 0) return 0;
     const Bf16BlockDev& b = static_cast<const Bf16BlockDev*>(m.bf16_blocks)[block];
     const Bf16Scratch& sc = *static_cast<const Bf16Scratch*>(w.bf16_scratch);
     if (b.pre_wimg) {
+        if (dep == DEP_SECONDARY) return GNN_ERR_BAD_ARG;
         PreTcParams tp;
         tp.x = x; tp.wimg = b.pre_wimg; tp.bias = b.pre_bias; tp.U = sc.U; tp.V = sc.V; tp.R = sc.R; tp.meta = w.meta;
         tp.n_tiles = (N + TILE_ROWS - 1) / TILE_ROWS;
         const int grid = 3 * std::min(tp.n_tiles, std::max(1, m.n_sms * b.pre_ctas_per_sm / 3));
-        if (b.C == 128) pre_tc_kernel<64, 128><<<grid, PTC_THREADS, PreTcCfg<64, 128>::SMEM_BYTES, s>>>(tp);
-        else pre_tc_kernel<128, 256><<<grid, PTC_THREADS, PreTcCfg<128, 256>::SMEM_BYTES, s>>>(tp);
+        if (b.C == 128) GNN_CUDA_TRY(launch_k(pre_tc_kernel<64, 128>, dim3(grid), dim3(PTC_THREADS), PreTcCfg<64, 128>::SMEM_BYTES, s, pdl, tp));
+        else GNN_CUDA_TRY(launch_k(pre_tc_kernel<128, 256>, dim3(grid), dim3(PTC_THREADS), PreTcCfg<128, 256>::SMEM_BYTES, s, pdl, tp));
     } else {
         PreParams pp;
         pp.x = x; pp.Wt = b.pre_Wt; pp.bias = b.pre_bias; pp.U = sc.U; pp.V = sc.V; pp.R = sc.R; pp.meta = w.meta;
-        pp.cin = b.cin; pp.Kp = b.Kp; pp.C1 = b.C; pp.C3 = b.C; pp.NC = b.NC;
+        pp.cin = b.cin; pp.Kp = b.Kp; pp.C1 = b.C; pp.C3 = b.C; pp.NC = b.NC; pp.dep = dep;
         if (b.cin <= 16 && (b.NC >> 2) * PRS_TY <= 1024) {
             const dim3 blk(b.NC >> 2, PRS_TY);
             const unsigned grid = (unsigned)((N + PRS_TY * PRS_ROWS - 1) / (PRS_TY * PRS_ROWS));
-            if (b.cin <= 8) pre_small_kernel<8><<<grid, blk, 0, s>>>(pp);
-            else pre_small_kernel<16><<<grid, blk, 0, s>>>(pp);
+            if (b.cin <= 8) GNN_CUDA_TRY(launch_k(pre_small_kernel<8>, dim3(grid), blk, 0, s, pdl, pp));
+            else GNN_CUDA_TRY(launch_k(pre_small_kernel<16>, dim3(grid), blk, 0, s, pdl, pp));
         } else {
             const size_t pre_smem = (size_t)PRE_ROWS * (b.Kp + 4) * sizeof(float);
-            pre_kernel<<<(N + PRE_ROWS - 1) / PRE_ROWS, PRE_THREADS, pre_smem, s>>>(pp);
+            GNN_CUDA_TRY(launch_k(pre_kernel, dim3((N + PRE_ROWS - 1) / PRE_ROWS), dim3(PRE_THREADS), pre_smem, s, pdl, pp));
         }
     }
     return 1;
@@ -1486,7 +1536,7 @@ int launch_edge_bf16(gnn_model& m, int block, const int32_t* idx, int N, float* 
 
 int launch_edgeconv_bf16(gnn_model& m, int block, const float* x, const int32_t* idx, int N, float* y, Workspace& w,
                          cudaStream_t s) {
-    const int a = launch_pre_bf16(m, block, x, N, w, s);
+    const int a = launch_pre_bf16(m, block, x, N, w, s, DEP_NONE);
     if (a < 0) return a;
     const int b = launch_edge_bf16(m, block, idx, N, y, w, s);
     return b < 0 ? b : a + b;

@@ -43,8 +43,7 @@ struct Workspace {
     int32_t* poffsets = nullptr;  // [Bmax + 1]
     int32_t* pcounts = nullptr;   // [Bmax]
     void* bf16_scratch = nullptr;  // per-slice scratch of the bf16 path
-    cudaStream_t aux = nullptr;    // second stream of the forward: the pre kernel of a block runs beside its kNN
-    cudaEvent_t ev_x = nullptr, ev_pre = nullptr;
+    bool pool_self_cleaning = false;   // the head kernel of this model clears `pool` after reading it (else forward() does)
     float* hlogits = nullptr;      // [Bmax, n_classes] device staging of gnn_infer_host (inputs stage in pfeats/pcoords/poffsets)
     // stage timing (gnn_profile_*): events of up to PROF_MAX_FORWARDS forwards, (n_stages + 1) per forward
     bool prof_on = false;
@@ -89,17 +88,54 @@ int launch_compact_padded(const float* feats, const float* coords, const float* 
 // kNN: space [N, D]; out [N, k] global indices (local_out = 0) or jet-local (local_out = 1)
 // gram != 0 (bf16 mode, R28): the grouped kernels of knn_group.cu where they have a form for D (Gram distances on
 // the tensor cores for feature spaces, 32-bit keys: d to 16 mantissa bits | j); 0: exact direct differences, exact (d, j) order
+// dep (forward only, grouped kernels only): role of the kernel in a pair of programmatic dependent launches, see DEP_* below
 int launch_knn(const float* space, int D, int k, int B, int max_particles, const Workspace& w, int32_t* idx_out,
-               int local_out, int gram, cudaStream_t s);
+               int local_out, int gram, cudaStream_t s, int dep = 0);
 int launch_edgeconv_f32(const BlockDev& b, int k, const float* x, const int32_t* idx, int N, float* y,
                         const Workspace& w, cudaStream_t s);
 int launch_globalize_idx(const int32_t* idx_local, int k, int B, const Workspace& w, int32_t* idx_global, cudaStream_t s);
-int launch_pool_head(const gnn_model& m, const float* x, int B, const Workspace& w, float* logits, cudaStream_t s);
+int launch_pool_head(const gnn_model& m, const float* x, int B, const Workspace& w, float* logits, cudaStream_t s, bool pdl = false);
+bool head_clears_pool(const gnn_model& m);
 int launch_pooled_mean(const gnn_model& m, int B, const Workspace& w, float* g, cudaStream_t s);
 int knn_configure();
 int pool_head_configure();
 int knn_group_configure();
 int launch_knn_group(const float* space, int D, int k, int B, int max_particles, const Workspace& w, int32_t* idx_out,
-                     int local_out, cudaStream_t s);
+                     int local_out, int dep, cudaStream_t s);
+bool knn_group_supported(int D, int max_particles);
 int edgeconv_f32_configure();
 
+
+// ---- programmatic dependent launch (PDL) --------------------------------------------------------------------------------
+// A kernel launched with `pdl` may start while the kernel before it in the stream is still running, once every CTA of that
+// kernel has executed grid_dep_launch() (or exited).  It must execute grid_dep_wait() before it touches anything the earlier
+// kernel writes (or reads and this kernel overwrites); what it does before that -- barrier and TMEM set-up, weight loads --
+// overlaps the earlier kernel's tail.  Both instructions are no-ops in a kernel launched without the attribute.
+// Two kernels that both depend only on the kernel before them (the per-particle pre kernel and the kNN of a block) run side
+// by side as a PRIMARY / SECONDARY pair on one stream:
+//   DEP_PRIMARY    launched as a dependent of the kernel before it; waits for it (after its own prologue), then at once
+//                  releases its dependents.  It must be the kernel whose CTAs are all resident at once, because the
+//                  secondary can only launch when every primary CTA has got that far.
+//   DEP_SECONDARY  launched as a dependent of the primary; does NOT wait before reading its inputs -- a secondary CTA exists
+//                  only after every primary CTA has passed its wait, i.e. the inputs of both are complete -- but its CTA 0
+//                  waits for the primary before it exits, so that the pair is complete when the secondary is: the next
+//                  kernel, a normal launch, then starts after both.
+enum { DEP_NONE = 0, DEP_PRIMARY = 1, DEP_SECONDARY = 2 };
+#ifdef __CUDACC__
+__device__ __forceinline__ void grid_dep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void grid_dep_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+bool gnn_pdl_enabled();       // false with GNN_NO_PDL in the environment (developer knob: A/B of the overlap)
+
+template <typename... KArgs, typename... Args>
+cudaError_t launch_k(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s, bool pdl, Args&&... args) {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = (pdl && gnn_pdl_enabled()) ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+}
+#endif

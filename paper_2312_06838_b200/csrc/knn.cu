@@ -343,10 +343,10 @@ int launch_knn_t(const float* space, int D, int k, int B, int P, const Workspace
 }  // namespace
 
 int launch_knn(const float* space, int D, int k, int B, int max_particles, const Workspace& w, int32_t* idx_out,
-               int local_out, int gram, cudaStream_t s) {
+               int local_out, int gram, cudaStream_t s, int dep) {
     if (B == 0) return 0;
     if (gram) {                               // bf16 mode: grouped kernels where they have a form for this space
-        const int n = launch_knn_group(space, D, k, B, max_particles, w, idx_out, local_out, s);
+        const int n = launch_knn_group(space, D, k, B, max_particles, w, idx_out, local_out, dep, s);
         if (n != 0) return n;
     }
     if (knn_smem_bytes(max_particles) > 227 * 1024) return GNN_ERR_BAD_ARG;

@@ -22,6 +22,7 @@
 // Output: idx [N, k] GLOBAL row indices in ascending (d, j) order (R29), -1 = none (k_eff < k); pjid [N] = jet of a row.
 #include "gnn_internal.h"
 #include "tc05.cuh"
+#include <algorithm>
 
 namespace {
 
@@ -77,15 +78,14 @@ struct GroupInfo {
     int special;                  // offending ragged jet (owns more rows than max_particles): no neighbours
 };
 
-// returns false if the CTA has nothing to compute (also handles the offending-jet group: idx = -1, pjid)
+// group `grp` (< meta[2]) -> *gi; returns false if there is nothing to compute (also handles the offending-jet group: idx = -1, pjid)
 __device__ __forceinline__ bool load_group(GroupInfo* gi, const int2* __restrict__ groups, const int32_t* __restrict__ jet_start,
                                            const int32_t* __restrict__ jet_n, const int32_t* __restrict__ meta,
-                                           int32_t* __restrict__ idx_out, int32_t* __restrict__ pjid, int k) {
-    if ((int)blockIdx.x >= meta[2]) return false;               // meta[2] = 0 for a poisoned batch
+                                           int32_t* __restrict__ idx_out, int32_t* __restrict__ pjid, int k, int grp) {
     const int tid = threadIdx.x;
     // one round trip: every thread of the first warp reads the group, lane t then reads jet t (all loads independent)
     if (tid < 32) {
-        const int2 g = __ldg(groups + blockIdx.x);
+        const int2 g = __ldg(groups + grp);
         int n = 0, st = 0;
         if (tid < g.y) { n = __ldg(jet_n + g.x + tid); st = __ldg(jet_start + g.x + tid); }
         const int r0 = __shfl_sync(0xffffffffu, st, 0), n0 = __shfl_sync(0xffffffffu, n, 0);
@@ -139,47 +139,54 @@ template <int K>
 __global__ void __launch_bounds__(KC_THREADS)
 knn_group_coords_kernel(const float* __restrict__ space, int D, const int32_t* __restrict__ jet_start,
                         const int32_t* __restrict__ jet_n, const int32_t* __restrict__ meta, const int2* __restrict__ groups,
-                        int32_t* __restrict__ idx_out, int32_t* __restrict__ pjid, int k, int local_out) {
+                        int32_t* __restrict__ idx_out, int32_t* __restrict__ pjid, int k, int local_out, int dep) {
     __shared__ GroupInfo gi;
     __shared__ float4 xs[KG_ROWS];
-    if (!load_group(&gi, groups, jet_start, jet_n, meta, idx_out, pjid, k)) return;
-    const int i = threadIdx.x, R = gi.R;
-    float4 xi = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-    if (i < R) {
-        const float* src = space + (size_t)(gi.r0 + i) * D;
-        xi.x = __ldg(src);
-        if (D > 1) xi.y = __ldg(src + 1);
-        if (D > 2) xi.z = __ldg(src + 2);
-        if (D > 3) xi.w = __ldg(src + 3);
-    }
-    xs[i] = xi;
-    int t, c0, c1;
-    row_range(&gi, i, t, c0, c1);
-    if (i >= R) { c0 = 0; c1 = 0; }
-    if (i < R && pjid) pjid[gi.r0 + i] = gi.j0 + t;
-    __syncthreads();
-    unsigned best[K];
+    if (dep == DEP_PRIMARY) { grid_dep_wait(); grid_dep_launch(); }
+    const int n_groups = meta[2];                               // 0 for a poisoned batch
+    for (int grp = blockIdx.x; grp < n_groups; grp += gridDim.x) {
+        if (load_group(&gi, groups, jet_start, jet_n, meta, idx_out, pjid, k, grp)) {
+            const int i = threadIdx.x, R = gi.R;
+            float4 xi = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+            if (i < R) {
+                const float* src = space + (size_t)(gi.r0 + i) * D;
+                xi.x = __ldg(src);
+                if (D > 1) xi.y = __ldg(src + 1);
+                if (D > 2) xi.z = __ldg(src + 2);
+                if (D > 3) xi.w = __ldg(src + 3);
+            }
+            xs[i] = xi;
+            int t, c0, c1;
+            row_range(&gi, i, t, c0, c1);
+            if (i >= R) { c0 = 0; c1 = 0; }
+            if (i < R && pjid) pjid[gi.r0 + i] = gi.j0 + t;
+            __syncthreads();
+            unsigned best[K];
 #pragma unroll
-    for (int m = 0; m < K; ++m) best[m] = KEY_NONE;
-    // every lane walks ITS jet's candidates from c0 in chunks of K; the trip count is the warp's largest
-    const int trips = (c1 - c0 + K - 1) / K;
-    const int wtrips = __reduce_max_sync(0xffffffffu, trips);
-    for (int tr = 0; tr < wtrips; ++tr) {
-        unsigned c[K];
+            for (int m = 0; m < K; ++m) best[m] = KEY_NONE;
+            // every lane walks ITS jet's candidates from c0 in chunks of K; the trip count is the warp's largest
+            const int trips = (c1 - c0 + K - 1) / K;
+            const int wtrips = __reduce_max_sync(0xffffffffu, trips);
+            for (int tr = 0; tr < wtrips; ++tr) {
+                unsigned c[K];
 #pragma unroll
-        for (int u = 0; u < K; ++u) {
-            const int j = c0 + tr * K + u;
-            const float4 xj = xs[min(j, KG_ROWS - 1)];
-            // t = s_i - s_j, d = fma(t, t, d) in index order: the arithmetic of the exact path (knn.cu); padded dimensions add 0
-            float tt = xi.x - xj.x, d = tt * tt;
-            tt = xi.y - xj.y; d = fmaf(tt, tt, d);
-            tt = xi.z - xj.z; d = fmaf(tt, tt, d);
-            tt = xi.w - xj.w; d = fmaf(tt, tt, d);
-            c[u] = (j < c1 && j != i) ? make_key(d, j - c0) : KEY_NONE;      // R4: self excluded by index
+                for (int u = 0; u < K; ++u) {
+                    const int j = c0 + tr * K + u;
+                    const float4 xj = xs[min(j, KG_ROWS - 1)];
+                    // t = s_i - s_j, d = fma(t, t, d) in index order: the arithmetic of the exact path (knn.cu); padded dimensions add 0
+                    float tt = xi.x - xj.x, d = tt * tt;
+                    tt = xi.y - xj.y; d = fmaf(tt, tt, d);
+                    tt = xi.z - xj.z; d = fmaf(tt, tt, d);
+                    tt = xi.w - xj.w; d = fmaf(tt, tt, d);
+                    c[u] = (j < c1 && j != i) ? make_key(d, j - c0) : KEY_NONE;      // R4: self excluded by index
+                }
+                merge_chunk<K>(best, c);
+            }
+            if (i < R) write_neighbours<K>(best, idx_out + (size_t)(gi.r0 + i) * k, k, local_out ? 0 : gi.r0 + c0);
         }
-        merge_chunk<K>(best, c);
+        __syncthreads();                                        // gi and xs are rewritten by the next group
     }
-    if (i < R) write_neighbours<K>(best, idx_out + (size_t)(gi.r0 + i) * k, k, local_out ? 0 : gi.r0 + c0);
+    if (dep == DEP_SECONDARY && blockIdx.x == 0) grid_dep_wait();
 }
 
 // ---- feature spaces: Gram matrix on the tensor cores -------------------------------------------------------------------------
@@ -187,6 +194,7 @@ knn_group_coords_kernel(const float* __restrict__ space, int D, const int32_t* _
 // the TMEM allocation and its lane 0 issues the MMAs
 constexpr int KG_THREADS = 256;
 constexpr int KG_MMA_WARP = 4;
+constexpr int KG_BATCH = 2;                // items a thread has in flight (registers: three CTAs per SM, beside the pre kernel)
 
 template <int D>
 struct KnnGroupCfg {
@@ -197,10 +205,10 @@ struct KnnGroupCfg {
 };
 
 template <int D, int K>
-__global__ void __launch_bounds__(KG_THREADS)
+__global__ void __launch_bounds__(KG_THREADS, 3)
 knn_group_gram_kernel(const float* __restrict__ space, const int32_t* __restrict__ jet_start, const int32_t* __restrict__ jet_n,
                       const int32_t* __restrict__ meta, const int2* __restrict__ groups, int32_t* __restrict__ idx_out,
-                      int32_t* __restrict__ pjid, int k, int local_out) {
+                      int32_t* __restrict__ pjid, int k, int local_out, int dep) {
     using Cfg = KnnGroupCfg<D>;
     constexpr int KBD = Cfg::KBD;
     extern __shared__ __align__(1024) uint8_t smem_raw[];
@@ -216,14 +224,23 @@ knn_group_gram_kernel(const float* __restrict__ space, const int32_t* __restrict
 #else
 #define KTR() do { } while (0)
 #endif
-    KTR();
-    if (!load_group(gi, groups, jet_start, jet_n, meta, idx_out, pjid, k)) return;
-    KTR();
     if ((smem_u32(X) & 1023u) != 0u) __trap();
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int R = gi->R, r0 = gi->r0;
     if (tid == 0) { mbar_init(d_full, 1); fence_mbar_init(); }
     if (warp == KG_MMA_WARP) tmem_alloc(tmem_ptr, 128);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = *tmem_ptr;
+    if (dep == DEP_PRIMARY) { grid_dep_wait(); grid_dep_launch(); }   // (DEP_SECONDARY: see gnn_internal.h)
+    const int n_groups = meta[2];                               // 0 for a poisoned batch
+    int iter = 0;
+    for (int grp = blockIdx.x; grp < n_groups; grp += gridDim.x, ++iter) {
+    KTR();
+    const bool work = load_group(gi, groups, jet_start, jet_n, meta, idx_out, pjid, k, grp);
+    KTR();
+    if (work) {
+    const int R = gi->R, r0 = gi->r0;
     int jt = 0, c0 = 0, c1 = 0;
     if (tid < KG_ROWS) {
         row_range(gi, tid, jt, c0, c1);
@@ -231,11 +248,8 @@ knn_group_gram_kernel(const float* __restrict__ space, const int32_t* __restrict
         ref_s[tid] = c0;
         if (tid < R && pjid) pjid[r0 + tid] = gi->j0 + jt;
     }
-    tc_fence_before();
     __syncthreads();
-    tc_fence_after();
     KTR();
-    const uint32_t tmem = *tmem_ptr;
     // (1) the tile's rows CENTRED ON THE FIRST ROW OF THEIR JET, rounded to fp16 (RNE; 10 mantissa bits as tf32) and stored with
     //     the 128-byte swizzle.  d(i, j) is translation invariant, so any per-jet reference point is legitimate; moving the
     //     origin into the jet keeps the cancellation error of the Gram form (G_ii + G_jj - 2 G_ij) below the neighbour gaps,
@@ -249,10 +263,10 @@ knn_group_gram_kernel(const float* __restrict__ space, const int32_t* __restrict
     constexpr int ITEMS = (KG_ROWS * IPR + KG_THREADS - 1) / KG_THREADS;
     const int n_items = R * IPR;
 #pragma unroll
-    for (int i0 = 0; i0 < ITEMS; i0 += 4) {
-        float4 xa[4], xb[4], ra[4], rb[4];
+    for (int i0 = 0; i0 < ITEMS; i0 += KG_BATCH) {
+        float4 xa[KG_BATCH], xb[KG_BATCH], ra[KG_BATCH], rb[KG_BATCH];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
+        for (int u = 0; u < KG_BATCH; ++u) {
             const int e = tid + (i0 + u) * KG_THREADS;
             if (i0 + u < ITEMS && e < n_items) {
                 const int r = e / IPR, c = e - r * IPR;
@@ -262,7 +276,7 @@ knn_group_gram_kernel(const float* __restrict__ space, const int32_t* __restrict
             }
         }
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
+        for (int u = 0; u < KG_BATCH; ++u) {
             const int e = tid + (i0 + u) * KG_THREADS;
             if (i0 + u < ITEMS && e < n_items) {
                 const int r = e / IPR, c = e - r * IPR;
@@ -294,7 +308,7 @@ knn_group_gram_kernel(const float* __restrict__ space, const int32_t* __restrict
     }
     if (warp < 4) {
         // thread = row i = TMEM lane; diagonal first (G_ii sits in this thread's own row), then the row of G 16 columns at a time
-        mbar_wait(d_full, 0);
+        mbar_wait(d_full, iter & 1);
         tc_fence_after();
         KTR();
         const int i = tid;
@@ -346,31 +360,42 @@ knn_group_gram_kernel(const float* __restrict__ space, const int32_t* __restrict
         }
         KTR();
         if (i < R) write_neighbours<K>(best, idx_out + (size_t)(r0 + i) * k, k, local_out ? 0 : r0 + c0);
+        tc_fence_before();
     }
-    tc_fence_before();
-    __syncthreads();
+    }   // work
+    __syncthreads();                                            // the tile, gi, ref_s, diag_s and the accumulator are reused
+    tc_fence_after();
     KTR();
 #ifdef KNN_TRACE
-    if (threadIdx.x == 0 && (blockIdx.x % 97) == 5)
-        printf("knn<%d> cta %d R %d: group %llu rows %llu centre %llu mma %llu select %llu store %llu (ns)\n", D, blockIdx.x, R,
+    if (threadIdx.x == 0 && (blockIdx.x % 97) == 5 && work)
+        printf("knn<%d> cta %d R %d: group %llu rows %llu centre %llu mma %llu select %llu store %llu (ns)\n", D, blockIdx.x, gi->R,
                tr[1] - tr[0], tr[2] - tr[1], tr[3] - tr[2], tr[4] - tr[3], tr[5] - tr[4], tr[6] - tr[5]);
+    trn = 0;
 #endif
+    }   // groups
+    tc_fence_before();
+    __syncthreads();
     if (warp == KG_MMA_WARP) tmem_dealloc(tmem, 128);
+    if (dep == DEP_SECONDARY && blockIdx.x == 0) grid_dep_wait();
 }
 
 template <int K>
-int launch_group_t(const float* space, int D, int k, int B, const Workspace& w, int32_t* idx_out, int local_out, cudaStream_t s) {
+int launch_group_t(const float* space, int D, int k, int B, const Workspace& w, int32_t* idx_out, int local_out, int dep, cudaStream_t s) {
     // one CTA per possible group (at most one per jet); CTAs beyond meta[2] leave at once
+    const bool pdl = dep != DEP_NONE;
+    cudaError_t e;
     if (D <= 4) {
-        knn_group_coords_kernel<K><<<B, KC_THREADS, 0, s>>>(space, D, w.jet_start, w.jet_n, w.meta, w.groups, idx_out, w.pjid, k, local_out);
-        return 1;
+        e = launch_k(knn_group_coords_kernel<K>, dim3(B), dim3(KC_THREADS), 0, s, pdl, space, D, w.jet_start, w.jet_n, w.meta, w.groups, idx_out, w.pjid, k, local_out, dep);
+    } else if (D == 64) {
+        e = launch_k(knn_group_gram_kernel<64, K>, dim3(B), dim3(KG_THREADS), KnnGroupCfg<64>::SMEM_BYTES, s, pdl, space, w.jet_start, w.jet_n, w.meta, w.groups, idx_out, w.pjid, k, local_out, dep);
+    } else if (D == 128) {
+        e = launch_k(knn_group_gram_kernel<128, K>, dim3(B), dim3(KG_THREADS), KnnGroupCfg<128>::SMEM_BYTES, s, pdl, space, w.jet_start, w.jet_n, w.meta, w.groups, idx_out, w.pjid, k, local_out, dep);
+    } else if (D == 256) {
+        e = launch_k(knn_group_gram_kernel<256, K>, dim3(B), dim3(KG_THREADS), KnnGroupCfg<256>::SMEM_BYTES, s, pdl, space, w.jet_start, w.jet_n, w.meta, w.groups, idx_out, w.pjid, k, local_out, dep);
+    } else {
+        return 0;
     }
-    switch (D) {
-        case 64: knn_group_gram_kernel<64, K><<<B, KG_THREADS, KnnGroupCfg<64>::SMEM_BYTES, s>>>(space, w.jet_start, w.jet_n, w.meta, w.groups, idx_out, w.pjid, k, local_out); return 1;
-        case 128: knn_group_gram_kernel<128, K><<<B, KG_THREADS, KnnGroupCfg<128>::SMEM_BYTES, s>>>(space, w.jet_start, w.jet_n, w.meta, w.groups, idx_out, w.pjid, k, local_out); return 1;
-        case 256: knn_group_gram_kernel<256, K><<<B, KG_THREADS, KnnGroupCfg<256>::SMEM_BYTES, s>>>(space, w.jet_start, w.jet_n, w.meta, w.groups, idx_out, w.pjid, k, local_out); return 1;
-        default: return 0;
-    }
+    return e == cudaSuccess ? 1 : GNN_ERR_CUDA;
 }
 
 template <int D, int K>
@@ -385,14 +410,19 @@ bool configure_k() { return configure_one<64, K>() && configure_one<128, K>() &&
 
 // kNN of every jet in `space` [N, D] through the grouped kernels; returns the number of kernels enqueued, or 0 if this
 // (D, max_particles) has no grouped form (the caller then takes the exact path of knn.cu)
+bool knn_group_supported(int D, int max_particles) {
+    return max_particles <= KG_ROWS && (D <= 4 || D == 64 || D == 128 || D == 256);
+}
+
+// dep: DEP_* of gnn_internal.h (forward() only; DEP_NONE = an ordinary launch)
 int launch_knn_group(const float* space, int D, int k, int B, int max_particles, const Workspace& w, int32_t* idx_out,
-                     int local_out, cudaStream_t s) {
-    if (max_particles > KG_ROWS || !(D <= 4 || D == 64 || D == 128 || D == 256)) return 0;
+                     int local_out, int dep, cudaStream_t s) {
+    if (!knn_group_supported(D, max_particles)) return 0;
     if (B == 0) return 0;
-    if (k <= 4) return launch_group_t<4>(space, D, k, B, w, idx_out, local_out, s);
-    if (k <= 8) return launch_group_t<8>(space, D, k, B, w, idx_out, local_out, s);
-    if (k <= 16) return launch_group_t<16>(space, D, k, B, w, idx_out, local_out, s);
-    return launch_group_t<32>(space, D, k, B, w, idx_out, local_out, s);
+    if (k <= 4) return launch_group_t<4>(space, D, k, B, w, idx_out, local_out, dep, s);
+    if (k <= 8) return launch_group_t<8>(space, D, k, B, w, idx_out, local_out, dep, s);
+    if (k <= 16) return launch_group_t<16>(space, D, k, B, w, idx_out, local_out, dep, s);
+    return launch_group_t<32>(space, D, k, B, w, idx_out, local_out, dep, s);
 }
 
 int knn_group_configure() {

@@ -336,9 +336,10 @@ constexpr int HS_MAX_CLASSES = 4;
 
 template <int KPER>                                   // rows of Wt per K slice = C / HS_KS
 __global__ void __launch_bounds__(HS_THREADS)
-head_split_kernel(const unsigned long long* __restrict__ pooled, const int32_t* __restrict__ jet_n, const int32_t* __restrict__ meta,
+head_split_kernel(const unsigned long long* pooled, const int32_t* __restrict__ jet_n, const int32_t* __restrict__ meta,
                   LinF32 L1, LinF32 L2, int B, int n_classes, float* __restrict__ logits) {
     constexpr int C = KPER * HS_KS;
+    unsigned long long* pooled_rw = const_cast<unsigned long long*>(pooled);
     __shared__ __align__(16) float zT[C * HS_PASS];                  // pooled means of one pass, [channel][jet]
     __shared__ __align__(16) float part[HS_KS * HS_PASS * HS_OUT];   // [ks][jet][out]
     __shared__ float hT[HS_JETS * HS_OUT];                           // hidden activations of this CTA, [jet][out]
@@ -363,15 +364,9 @@ head_split_kernel(const unsigned long long* __restrict__ pooled, const int32_t* 
 #pragma unroll
             for (int jb = 0; jb < HS_PASS; ++jb) {
                 const int c = tid + i * HS_THREADS, j = pass * HS_PASS + jb;
-                pv[i][jb] = (c < C && j < nj) ? __ldg(pooled + (size_t)(b0 + j) * C + c) : 0ull;
+                pv[i][jb] = (c < C && j < nj) ? __ldcg(pooled + (size_t)(b0 + j) * C + c) : 0ull;
             }
     };
-    load_pooled(0);
-    const bool poisoned = meta[0] != 0;
-    if (tid < HS_JETS) {
-        int n = (tid < nj && !poisoned) ? jet_n[b0 + tid] : 0;
-        s_inv[tid] = n > 0 ? 1.0f / (float)n : 0.0f;   // offending jet: pools nothing (its logits become NaN below); R12: empty jet pools to 0
-    }
     // this warp's weights of the final layer (warp = (jet, class) items, lanes = hidden units ln and 32 + ln)
     float w2a[HS_MAX_CLASSES], w2b[HS_MAX_CLASSES];
 #pragma unroll
@@ -380,6 +375,13 @@ head_split_kernel(const unsigned long long* __restrict__ pooled, const int32_t* 
         w2b[o] = o < n_classes ? __ldg(L2.Wt + (size_t)(o0 + 32 + ln) * L2.ld + o) : 0.0f;
     }
     const float shift1 = __ldg(L1.shift + o0 + (tid % HS_OUT));
+    grid_dep_wait();                                 // the weight loads above run under the tail of the last EdgeConv kernel
+    load_pooled(0);
+    const bool poisoned = meta[0] != 0;
+    if (tid < HS_JETS) {
+        int n = (tid < nj && !poisoned) ? jet_n[b0 + tid] : 0;
+        s_inv[tid] = n > 0 ? 1.0f / (float)n : 0.0f;   // offending jet: pools nothing (its logits become NaN below); R12: empty jet pools to 0
+    }
     __syncthreads();
 #pragma unroll 1
     for (int pass = 0; pass < HS_PASSES; ++pass) {
@@ -436,6 +438,8 @@ head_split_kernel(const unsigned long long* __restrict__ pooled, const int32_t* 
     }
     tc_cluster_sync();                                              // release / acquire: the shares are visible to rank 0
     if (rank != 0) return;
+    // every CTA of the cluster has read the jets' channel sums: clear them for the next forward (Workspace::pool_self_cleaning)
+    for (int it = tid; it < nj * C; it += HS_THREADS) pooled_rw[(size_t)b0 * C + it] = 0ull;
     for (int it = tid; it < nj * n_classes; it += HS_THREADS) {
         const int jb = it / n_classes, o = it - jb * n_classes;
         float v = __ldg(L2.shift + o);
@@ -446,16 +450,18 @@ head_split_kernel(const unsigned long long* __restrict__ pooled, const int32_t* 
 }
 
 template <int KPER>
-int launch_head_split(const HeadParams& hp, int B, const Workspace& w, float* logits, cudaStream_t s) {
+int launch_head_split(const HeadParams& hp, int B, const Workspace& w, float* logits, cudaStream_t s, bool pdl) {
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((B + HS_JETS - 1) / HS_JETS, hp.fc[0].N / HS_OUT);
     cfg.blockDim = dim3(HS_THREADS);
     cfg.dynamicSmemBytes = 0;
     cfg.stream = s;
-    cudaLaunchAttribute at[1];
+    cudaLaunchAttribute at[2];
     at[0].id = cudaLaunchAttributeClusterDimension;
     at[0].val.clusterDim.x = 1; at[0].val.clusterDim.y = cfg.gridDim.y; at[0].val.clusterDim.z = 1;
-    cfg.attrs = at; cfg.numAttrs = 1;
+    at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[1].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = (pdl && gnn_pdl_enabled()) ? 2 : 1;
     GNN_CUDA_TRY(cudaLaunchKernelEx(&cfg, head_split_kernel<KPER>, (const unsigned long long*)w.pool, (const int32_t*)w.jet_n,
                                     (const int32_t*)w.meta, hp.fc[0], hp.fc[1], B, hp.n_classes, logits));
     return 1;
@@ -464,7 +470,14 @@ int launch_head_split(const HeadParams& hp, int B, const Workspace& w, float* lo
 }  // namespace
 
 // x != null: pool the stored block output [N, C]; x == null: the channel sums are in w.pool (pooling EdgeConv epilogue)
-int launch_pool_head(const gnn_model& m, const float* x, int B, const Workspace& w, float* logits, cudaStream_t s) {
+// whether launch_pool_head(x == null) takes head_split_kernel, which clears the channel sums after reading them
+bool head_clears_pool(const gnn_model& m) {
+    const int C = m.arch.channels[m.arch.n_blocks - 1][2];
+    return m.n_fc == 2 && m.fc[0].N % HS_OUT == 0 && m.fc[0].N / HS_OUT <= HS_MAX_SPLIT && m.arch.n_classes <= HS_MAX_CLASSES &&
+           (C == 256 || C == 128 || C == 64);          // (C = 512: beyond 48 KB of static shared memory)
+}
+
+int launch_pool_head(const gnn_model& m, const float* x, int B, const Workspace& w, float* logits, cudaStream_t s, bool pdl) {
     if (B == 0) return 0;
     HeadParams hp;
     hp.n_fc = m.n_fc;
@@ -473,12 +486,11 @@ int launch_pool_head(const gnn_model& m, const float* x, int B, const Workspace&
     hp.n_classes = m.arch.n_classes;
     hp.wmax = hp.C;
     for (int i = 0; i < m.n_fc; ++i) hp.wmax = std::max(hp.wmax, (m.fc[i].N + 3) & ~3);
-    if (x == nullptr && hp.n_fc == 2 && hp.fc[0].N % HS_OUT == 0 && hp.fc[0].N / HS_OUT <= HS_MAX_SPLIT &&
-        hp.n_classes <= HS_MAX_CLASSES && (hp.C == 256 || hp.C == 128 || hp.C == 64)) {   // (C = 512: beyond 48 KB of static shared memory)
+    if (x == nullptr && head_clears_pool(m)) {
         switch (hp.C) {
-            case 64: return launch_head_split<64 / HS_KS>(hp, B, w, logits, s);
-            case 128: return launch_head_split<128 / HS_KS>(hp, B, w, logits, s);
-            default: return launch_head_split<256 / HS_KS>(hp, B, w, logits, s);
+            case 64: return launch_head_split<64 / HS_KS>(hp, B, w, logits, s, pdl);
+            case 128: return launch_head_split<128 / HS_KS>(hp, B, w, logits, s, pdl);
+            default: return launch_head_split<256 / HS_KS>(hp, B, w, logits, s, pdl);
         }
     }
     if (x == nullptr) {
