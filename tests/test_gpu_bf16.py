@@ -224,3 +224,28 @@ def test_batcher_bf16_equals_direct():
         assert np.array_equal(out.astype(np.float64), ref)
     bt.close()
     m.close()
+
+
+def test_forward_is_bitwise_repeatable_back_to_back(pn):
+    """The forward runs on one stream with programmatic dependent launches (a kernel's prologue under its predecessor's tail,
+    the pre kernel and the kNN of a block side by side; api.cu forward()).  Back-to-back forwards over batches of different
+    sizes, with and without an L2 eviction in between, must reproduce their first result bit for bit: a missing dependency
+    between two kernels shows up as a sporadic difference."""
+    _, _, m = pn
+    flush = torch.empty(160 << 20, dtype=torch.uint8, device="cuda")
+    bs = []
+    for r, B in enumerate((1024, 16, 1, 300, 77)):
+        b = synth.make_particlenet_batch(seed=5000 + r, n_jets=B)
+        bs.append((dev(b.feats), dev(b.coords), dev(b.offsets)))
+    first = [None] * len(bs)
+    for it in range(150):
+        i = it % len(bs)
+        if it % 3 == 0:
+            flush.zero_()
+        out = m.infer(*bs[i]).clone()
+        if first[i] is None:
+            first[i] = out
+        else:
+            assert torch.equal(out, first[i]), "forward %d (batch %d) differs from its first result" % (it, i)
+    torch.cuda.synchronize()
+    assert m.status_check() == 0
