@@ -181,7 +181,7 @@ struct StageTimer {
 
 // the launch plan of one forward (SURVEY.md call stack (4)): ingest -> per block [kNN, EdgeConv] -> pool + head
 int forward(gnn_model* m, Workspace& w, const float* feats, const float* coords, const int32_t* offsets,
-            const int32_t* counts, int B, int N_exact, int N_upper, float* logits, cudaStream_t s) {
+            const int32_t* counts, int B, int N_exact, int N_upper, float* logits, cudaStream_t s, int* n_launches_out = nullptr) {
     const gnn_arch& a = m->arch;
     int n = 0, rc;
     StageTimer tm(w, s, 2 + 2 * a.n_blocks);
@@ -237,12 +237,76 @@ int forward(gnn_model* m, Workspace& w, const float* feats, const float* coords,
     if ((rc = launch_pool_head(*m, x, B, w, logits, s, bf16)) < 0) return rc;
     n += rc;
     tm.mark("pool_head");
-    m->launches.fetch_add(n, std::memory_order_relaxed);
+    if (n_launches_out) *n_launches_out = n;
+    else m->launches.fetch_add(n, std::memory_order_relaxed);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) {
         std::fprintf(stderr, "libgnn: launch failed: %s\n", cudaGetErrorString(e));
         return GNN_ERR_CUDA;
     }
+    return GNN_OK;
+}
+
+// gnn_infer_slice through the slice's graph cache.  A call is replayed from a graph if its arguments (pointers, B, N) equal
+// an earlier call's; the graph is captured the SECOND time a set of arguments is seen, so one-off calls never pay for a
+// capture.  Not used while stage timing is on (events between the kernels) or while the caller's stream is itself being
+// captured (the forward is then simply recorded into the caller's graph: one stream, no host synchronisation).
+int forward_cached(gnn_model* m, Workspace& w, const float* feats, const float* coords, const int32_t* offsets, int B, int N,
+                   float* logits, cudaStream_t s) {
+    static const bool no_graphs = std::getenv("GNN_NO_GRAPHS") != nullptr;      // developer knob
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (no_graphs || w.prof_on || cudaStreamIsCapturing(s, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone)
+        return forward(m, w, feats, coords, offsets, nullptr, B, N, N, logits, s);
+    Workspace::ForwardGraph* hit = nullptr;
+    for (auto& g : w.graphs)
+        if (g.feats == feats && g.coords == coords && g.offsets == offsets && g.logits == logits && g.B == B && g.N == N) { hit = &g; break; }
+    if (hit && hit->exec) {
+        hit->last_use = ++w.graph_clock;
+        GNN_CUDA_TRY(cudaGraphLaunch(hit->exec, s));
+        m->launches.fetch_add(hit->n_launches, std::memory_order_relaxed);
+        return GNN_OK;
+    }
+    if (!hit) {                                                  // first sighting: remember the arguments, run normally
+        if ((int)w.graphs.size() < GNN_MAX_FORWARD_GRAPHS) w.graphs.emplace_back();
+        else {
+            hit = &w.graphs[0];
+            for (auto& g : w.graphs) if (g.last_use < hit->last_use) hit = &g;
+            if (hit->exec) cudaGraphExecDestroy(hit->exec);
+            *hit = Workspace::ForwardGraph();
+        }
+        Workspace::ForwardGraph& g = hit ? *hit : w.graphs.back();
+        g.feats = feats; g.coords = coords; g.offsets = offsets; g.logits = logits; g.B = B; g.N = N;
+        g.last_use = ++w.graph_clock;
+        return forward(m, w, feats, coords, offsets, nullptr, B, N, N, logits, s);
+    }
+    // second sighting: capture, instantiate, launch
+    hit->last_use = ++w.graph_clock;
+    cudaGraph_t graph = nullptr;
+    if (cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+        cudaGetLastError();
+        return forward(m, w, feats, coords, offsets, nullptr, B, N, N, logits, s);
+    }
+    int n = 0;
+    const int rc = forward(m, w, feats, coords, offsets, nullptr, B, N, N, logits, s, &n);
+    const cudaError_t ec = cudaStreamEndCapture(s, &graph);
+    if (rc != GNN_OK || ec != cudaSuccess || graph == nullptr) {
+        if (graph) cudaGraphDestroy(graph);
+        cudaGetLastError();
+        if (rc != GNN_OK) return rc;
+        *hit = Workspace::ForwardGraph();                        // capture not possible here: keep launching directly
+        return forward(m, w, feats, coords, offsets, nullptr, B, N, N, logits, s);
+    }
+    cudaGraphExec_t exec = nullptr;
+    const cudaError_t ei = cudaGraphInstantiate(&exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (ei != cudaSuccess || exec == nullptr) {
+        cudaGetLastError();
+        *hit = Workspace::ForwardGraph();
+        return forward(m, w, feats, coords, offsets, nullptr, B, N, N, logits, s);
+    }
+    hit->exec = exec; hit->n_launches = n;
+    GNN_CUDA_TRY(cudaGraphLaunch(exec, s));
+    m->launches.fetch_add(n, std::memory_order_relaxed);
     return GNN_OK;
 }
 
@@ -312,6 +376,7 @@ void gnn_destroy(gnn_model* m) {
     for (void* p : m->allocs) cudaFree(p);
     edgeconv_bf16_release(*m);
     for (auto& w : m->ws) {
+        for (auto& g : w.graphs) if (g.exec) cudaGraphExecDestroy(g.exec);
         for (cudaEvent_t e : w.prof_events) cudaEventDestroy(e);
     }
     delete m;
@@ -325,8 +390,7 @@ int gnn_infer_slice(gnn_model* m, int32_t slice, const float* feats_dev, const f
     if (B > m->arch.max_batch_jets || (int64_t)N > m->Nmax) return GNN_ERR_BATCH_TOO_LARGE;
     if (B == 0) return GNN_OK;
     if (!offsets_dev || !logits_dev || (N > 0 && (!feats_dev || !coords_dev))) return GNN_ERR_NULL;
-    return forward(m, m->ws[slice], feats_dev, coords_dev, offsets_dev, nullptr, B, N, N, logits_dev,
-                   static_cast<cudaStream_t>(cuda_stream));
+    return forward_cached(m, m->ws[slice], feats_dev, coords_dev, offsets_dev, B, N, logits_dev, static_cast<cudaStream_t>(cuda_stream));
 }
 
 int gnn_infer(gnn_model* m, const float* feats_dev, const float* coords_dev, const int32_t* offsets_dev, int32_t B,

@@ -43,6 +43,16 @@ struct Workspace {
     int32_t* poffsets = nullptr;  // [Bmax + 1]
     int32_t* pcounts = nullptr;   // [Bmax]
     void* bf16_scratch = nullptr;  // per-slice scratch of the bf16 path
+    // CUDA graphs of whole forwards (gnn_infer_slice): a call whose arguments repeat an earlier call's exactly is replayed as
+    // one graph launch instead of ~11 kernel launches (small batches are bound by the host's launch rate otherwise)
+    struct ForwardGraph {
+        const void *feats = nullptr, *coords = nullptr, *offsets = nullptr, *logits = nullptr;
+        int B = 0, N = 0, n_launches = 0;
+        cudaGraphExec_t exec = nullptr;      // null: seen once, not captured yet
+        uint64_t last_use = 0;
+    };
+    std::vector<ForwardGraph> graphs;
+    uint64_t graph_clock = 0;
     bool pool_self_cleaning = false;   // the head kernel of this model clears `pool` after reading it (else forward() does)
     float* hlogits = nullptr;      // [Bmax, n_classes] device staging of gnn_infer_host (inputs stage in pfeats/pcoords/poffsets)
     // stage timing (gnn_profile_*): events of up to PROF_MAX_FORWARDS forwards, (n_stages + 1) per forward
@@ -52,7 +62,7 @@ struct Workspace {
     std::vector<cudaEvent_t> prof_events;
     std::vector<std::string> prof_names;
 };
-enum { PROF_MAX_FORWARDS = 512 };
+enum { PROF_MAX_FORWARDS = 512, GNN_MAX_FORWARD_GRAPHS = 8 };
 
 struct gnn_model {
     gnn_arch arch{};
