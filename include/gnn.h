@@ -117,6 +117,17 @@ int gnn_infer_padded_slice(gnn_model* m, int32_t slice, const float* feats_dev, 
  * GNN_ERR_JET_TOO_LARGE, or GNN_ERR_CUDA if the stream reports an error). */
 int gnn_status_check(gnn_model* m, int32_t slice, void* cuda_stream);
 
+/* The paper's literal I/O contract ("features", "coordinates" and "mask", all FP32; L285 Table C2: input
+ * shape 8 x 100 per jet = (F + coord_dims + 1) channels x P slots, output 2): CHANNEL-FIRST padded tensors
+ * points_dev [B, coord_dims, P], features_dev [B, F, P], mask_dev [B, 1, P] (slot real iff mask != 0, any slot order,
+ * masked slots may hold anything).  Compacts on the device like gnn_infer_padded, runs the forward on `slice`, and
+ * writes out_dev [B, n_classes]: raw logits, or with softmax != 0 the class probabilities (row-wise softmax in fp32).
+ * Errors as gnn_infer_padded. */
+int gnn_infer_channel_first(gnn_model* m, int32_t slice, const float* points_dev, const float* features_dev,
+                            const float* mask_dev, int32_t B, int32_t P, int32_t softmax, float* out_dev, void* cuda_stream);
+/* row-wise softmax of logits_dev [B, n_classes] into probs_dev (may alias), fp32, maximum subtracted first */
+int gnn_softmax(const float* logits_dev, int32_t B, int32_t n_classes, float* probs_dev, void* cuda_stream);
+
 /* The same forward from HOST buffers (layouts as gnn_infer; pinned memory makes the copies asynchronous): copies the
  * inputs to device staging owned by `slice`, runs the forward, copies logits_host [B, n_classes] back and
  * synchronises `cuda_stream` before returning.  This is the one blocking inference call.  Device-side errors are

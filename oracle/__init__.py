@@ -152,3 +152,11 @@ def forward_padded(a, blob, feats, coords, mask, nthreads: int = 0):
     f = feats.reshape(B * P, -1)[keep.reshape(-1)]
     c = coords.reshape(B * P, -1)[keep.reshape(-1)]
     return forward(a, blob, f, c, offsets, nthreads=nthreads)
+
+
+def softmax(logits):
+    """Class probabilities from logits [B, n_classes], fp64: p_c = exp(z_c - max z) / sum_c' exp(z_c' - max z) (the textbook
+    definition; PAPER.md L262 ends the network in "two nodes", L270 serves their FP32 scores)."""
+    z = np.asarray(logits, np.float64)
+    e = np.exp(z - z.max(axis=1, keepdims=True))
+    return e / e.sum(axis=1, keepdims=True)

@@ -66,6 +66,8 @@ def lib():
         L.gnn_infer_padded.argtypes = [vp, f32p, f32p, f32p, i32, i32, f32p, vp]
         L.gnn_infer_padded_slice.argtypes = [vp, i32, f32p, f32p, f32p, i32, i32, f32p, vp]
         L.gnn_status_check.argtypes = [vp, i32, vp]
+        L.gnn_infer_channel_first.argtypes = [vp, i32, f32p, f32p, f32p, i32, i32, i32, f32p, vp]
+        L.gnn_softmax.argtypes = [f32p, i32, i32, f32p, vp]
         L.gnn_infer_host.argtypes = [vp, i32, vp, vp, vp, i32, i32, vp, vp]
         L.gnn_profile_enable.argtypes = [vp, i32, i32]
         L.gnn_profile_read.argtypes = [vp, i32, i32, C.POINTER(C.c_float), C.POINTER(i32), C.POINTER(i32)]
@@ -176,6 +178,16 @@ class Model:
         self._check(lib().gnn_infer_padded_slice(self.h, slice, _ptr(feats), _ptr(coords), _ptr(mask), B, P, _ptr(logits),
                                                  _stream(stream)), "gnn_infer_padded")
         return logits
+
+    def infer_channel_first(self, points, features, mask, softmax=False, out=None, stream=None, slice=0):
+        """gnn_infer_channel_first: points [B, CD, P], features [B, F, P], mask [B, 1, P] device tensors."""
+        import torch
+        B, P = int(features.shape[0]), int(features.shape[2])
+        if out is None:
+            out = torch.empty((B, self.arch.n_classes), dtype=torch.float32, device=features.device)
+        self._check(lib().gnn_infer_channel_first(self.h, slice, _ptr(points), _ptr(features), _ptr(mask), B, P, int(bool(softmax)),
+                                                  _ptr(out), _stream(stream)), "gnn_infer_channel_first")
+        return out
 
     def infer_host(self, feats, coords, offsets, logits, stream=None, slice=0):
         """gnn_infer_host: host tensors / arrays in (torch CPU tensors, ideally pinned, or numpy), logits written into

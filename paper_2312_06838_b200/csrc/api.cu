@@ -417,6 +417,37 @@ int gnn_infer_padded_slice(gnn_model* m, int32_t slice, const float* feats_dev, 
     return forward(m, w, w.pfeats, w.pcoords, w.poffsets, w.pcounts, B, -1, (int)upper, logits_dev, s);
 }
 
+int gnn_infer_channel_first(gnn_model* m, int32_t slice, const float* points_dev, const float* features_dev, const float* mask_dev,
+                            int32_t B, int32_t P, int32_t softmax, float* out_dev, void* cuda_stream) {
+    if (!m) return GNN_ERR_NULL;
+    if (B < 0 || P < 0) return GNN_ERR_BAD_ARG;
+    if (slice < 0 || slice >= (int)m->ws.size()) return GNN_ERR_BATCH_TOO_LARGE;
+    if (B > m->arch.max_batch_jets || (int64_t)B * P > (int64_t)m->arch.max_batch_jets * GNN_MAX_PARTICLES)
+        return GNN_ERR_BATCH_TOO_LARGE;
+    if (B == 0) return GNN_OK;
+    if (!out_dev || (P > 0 && (!features_dev || !points_dev || !mask_dev))) return GNN_ERR_NULL;
+    Workspace& w = m->ws[slice];
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    int rc = launch_compact_padded(features_dev, points_dev, mask_dev, B, P, m->arch.in_features, m->arch.coord_dims,
+                                   m->arch.max_particles, w, s, true);
+    if (rc < 0) return rc;
+    m->launches.fetch_add(rc, std::memory_order_relaxed);
+    int64_t upper = std::min<int64_t>((int64_t)B * std::min<int>(P, m->arch.max_particles), m->Nmax);
+    rc = forward(m, w, w.pfeats, w.pcoords, w.poffsets, w.pcounts, B, -1, (int)upper, out_dev, s);
+    if (rc != GNN_OK || !softmax) return rc;
+    if ((rc = launch_softmax(out_dev, B, m->arch.n_classes, out_dev, s)) < 0) return rc;
+    m->launches.fetch_add(rc, std::memory_order_relaxed);
+    return cudaGetLastError() == cudaSuccess ? GNN_OK : GNN_ERR_CUDA;
+}
+
+int gnn_softmax(const float* logits_dev, int32_t B, int32_t n_classes, float* probs_dev, void* cuda_stream) {
+    if (B < 0 || n_classes < 1) return GNN_ERR_BAD_ARG;
+    if (B == 0) return GNN_OK;
+    if (!logits_dev || !probs_dev) return GNN_ERR_NULL;
+    if (launch_softmax(logits_dev, B, n_classes, probs_dev, static_cast<cudaStream_t>(cuda_stream)) < 0) return GNN_ERR_CUDA;
+    return cudaGetLastError() == cudaSuccess ? GNN_OK : GNN_ERR_CUDA;
+}
+
 int gnn_infer_padded(gnn_model* m, const float* feats_dev, const float* coords_dev, const float* mask_dev, int32_t B,
                      int32_t P, float* logits_dev, void* cuda_stream) {
     return gnn_infer_padded_slice(m, 0, feats_dev, coords_dev, mask_dev, B, P, logits_dev, cuda_stream);

@@ -94,7 +94,8 @@ static inline int block_in(const gnn_arch& a, int l) { return l == 0 ? a.in_feat
 int launch_ingest(const int32_t* offsets, const int32_t* counts, int B, int N_exact, int N_cap, int max_particles,
                   Workspace& w, cudaStream_t s);
 int launch_compact_padded(const float* feats, const float* coords, const float* mask, int B, int P, int F, int CD,
-                          int max_particles, Workspace& w, cudaStream_t s);
+                          int max_particles, Workspace& w, cudaStream_t s, bool channel_first = false);
+int launch_softmax(const float* logits, int B, int n_classes, float* probs, cudaStream_t s);
 // kNN: space [N, D]; out [N, k] global indices (local_out = 0) or jet-local (local_out = 1)
 // gram != 0 (bf16 mode, R28): the grouped kernels of knn_group.cu where they have a form for D (Gram distances on
 // the tensor cores for feature spaces, 32-bit keys: d to 16 mantissa bits | j); 0: exact direct differences, exact (d, j) order

@@ -168,7 +168,7 @@ __global__ void scan_counts_kernel(const int32_t* __restrict__ counts, int B, in
 __global__ void scatter_padded_kernel(const float* __restrict__ feats, const float* __restrict__ coords,
                                       const float* __restrict__ mask, int P, int F, int CD, int max_particles,
                                       const int32_t* __restrict__ offsets, const int32_t* __restrict__ counts,
-                                      float* __restrict__ pfeats, float* __restrict__ pcoords) {
+                                      float* __restrict__ pfeats, float* __restrict__ pcoords, int channel_first) {
     int b = blockIdx.x;
     int base_out = offsets[b];
     if (counts[b] < 0) return;             // offending jet: ingest flags it, it owns no packed rows
@@ -188,8 +188,13 @@ __global__ void scatter_padded_kernel(const float* __restrict__ feats, const flo
         pre += __popc(bal & ((1u << lane) - 1u));
         if (keep) {
             size_t src = (size_t)b * P + p, dst = (size_t)base_out + pre;
-            for (int c = 0; c < F; ++c) pfeats[dst * F + c] = feats[src * F + c];
-            for (int c = 0; c < CD; ++c) pcoords[dst * CD + c] = coords[src * CD + c];
+            if (channel_first) {             // [B, F, P] / [B, CD, P] (8 x 100 inputs per jet): a warp reads 32 consecutive slots
+                for (int c = 0; c < F; ++c) pfeats[dst * F + c] = feats[((size_t)b * F + c) * P + p];
+                for (int c = 0; c < CD; ++c) pcoords[dst * CD + c] = coords[((size_t)b * CD + c) * P + p];
+            } else {
+                for (int c = 0; c < F; ++c) pfeats[dst * F + c] = feats[src * F + c];
+                for (int c = 0; c < CD; ++c) pcoords[dst * CD + c] = coords[src * CD + c];
+            }
         }
         __syncthreads();
         if (threadIdx.x == 0) running += wsum[0] + wsum[1] + wsum[2] + wsum[3];
@@ -198,11 +203,31 @@ __global__ void scatter_padded_kernel(const float* __restrict__ feats, const flo
 }
 
 int launch_compact_padded(const float* feats, const float* coords, const float* mask, int B, int P, int F, int CD,
-                          int max_particles, Workspace& w, cudaStream_t s) {
+                          int max_particles, Workspace& w, cudaStream_t s, bool channel_first) {
     if (B == 0) return 0;
     count_mask_kernel<<<B, 128, 0, s>>>(mask, B, P, max_particles, w.pcounts);
     scan_counts_kernel<<<1, 1024, 0, s>>>(w.pcounts, B, w.poffsets);
-    scatter_padded_kernel<<<B, 128, 0, s>>>(feats, coords, mask, P, F, CD, max_particles, w.poffsets, w.pcounts, w.pfeats, w.pcoords);
+    scatter_padded_kernel<<<B, 128, 0, s>>>(feats, coords, mask, P, F, CD, max_particles, w.poffsets, w.pcounts, w.pfeats, w.pcoords, channel_first ? 1 : 0);
     return 3;
 }
 
+
+// ---- class probabilities (PAPER.md L262 ends the network in "two nodes"; the served model's FP32 output, L270, is read as
+// softmax scores by the analyses): row-wise softmax of [B, n_classes] logits in fp32, max subtracted first; NaN rows stay NaN
+__global__ void softmax_kernel(const float* __restrict__ logits, int B, int n_classes, float* __restrict__ probs) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= B) return;
+    const float* z = logits + (size_t)b * n_classes;
+    float mx = z[0];
+    for (int c = 1; c < n_classes; ++c) mx = fmaxf(mx, z[c]);
+    float sum = 0.0f;
+    for (int c = 0; c < n_classes; ++c) sum += expf(z[c] - mx);
+    const float inv = 1.0f / sum;
+    for (int c = 0; c < n_classes; ++c) probs[(size_t)b * n_classes + c] = (z[c] != z[c]) ? z[c] : expf(z[c] - mx) * inv;
+}
+
+int launch_softmax(const float* logits, int B, int n_classes, float* probs, cudaStream_t s) {
+    if (B == 0) return 0;
+    softmax_kernel<<<(B + 127) / 128, 128, 0, s>>>(logits, B, n_classes, probs);
+    return 1;
+}

@@ -91,6 +91,20 @@ def make_particlenet_batch(seed: int = 1002, n_jets: int = 1024, nmax: int = 100
     return _physics_jets(np.random.default_rng(seed), n_jets, 40, 5, nmax, 0)
 
 
+def make_paper_f5_batch(seed: int = 1002, n_jets: int = 1024, nmax: int = 100) -> JetBatch:
+    """The paper-literal input width ("five input features"): the configs[1] jets with their first five
+    feature columns (log pT, log E, log pT-rel, log E-rel, dR); the paper does not name its five."""
+    b = make_particlenet_batch(seed=seed, n_jets=n_jets, nmax=nmax)
+    return JetBatch(np.ascontiguousarray(b.feats[:, :5]), b.coords, b.offsets)
+
+
+def to_channel_first(feats, coords, mask):
+    """[B, P, F], [B, P, 2], [B, P] -> the served model's tensors: points [B, 2, P], features [B, F, P],
+    mask [B, 1, P]; a pure relayout."""
+    return (np.ascontiguousarray(np.transpose(coords, (0, 2, 1))), np.ascontiguousarray(np.transpose(feats, (0, 2, 1))),
+            np.ascontiguousarray(mask[:, None, :]))
+
+
 def make_ragged_batch(seed: int = 1003, n_jets: int = 4096) -> JetBatch:
     """configs[2]: clip(Poisson(40),5,128), 9 features (7 kinematic + 2 ~ N(0,1))."""
     return _physics_jets(np.random.default_rng(seed), n_jets, 40, 5, 128, 2)

@@ -1,0 +1,63 @@
+"""-m gpu tests of the paper-literal variants (SURVEY 8(f) "variants"; PAPER.md L262 five input features, L269 / L285 the
+served model's I/O: channel-first padded tensors points [B, 2, P], features [B, F, P], mask [B, 1, P], 8 x 100 FP32 inputs
+per jet, FP32 output of 2 scores): gnn_infer_channel_first with and without softmax, against the fp64 oracle on the
+same jets in ragged form."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import synth
+import paper_2312_06838_b200 as gnn
+from gpu_util import dev, make_model
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.parametrize("precision,tol", [(gnn.FP32_VALIDATION, 1e-4), (gnn.BF16, 5e-2)])
+def test_paper_f5_channel_first_softmax(precision, tol):
+    a = synth.ARCHS["paper_f5"]
+    w = synth.make_weights(a)
+    b = synth.make_paper_f5_batch(n_jets=256)
+    assert b.feats.shape[1] == 5 and 5 + 2 + 1 == 8                     # Table C2: input shape 8 x 100
+    ref = oracle.forward(a, w, b.feats, b.coords, b.offsets)
+    m = make_model(a, w, precision=precision, max_batch_jets=256, max_particles=100)
+    f, c, k = synth.pad_batch(b, 100, interleave=True, garbage=np.nan)
+    pts, fts, msk = synth.to_channel_first(f, c, k)
+    assert pts.shape == (256, 2, 100) and fts.shape == (256, 5, 100) and msk.shape == (256, 1, 100)
+    lg = m.infer_channel_first(dev(pts), dev(fts), dev(msk)).cpu().numpy().astype(np.float64)
+    torch.cuda.synchronize()
+    assert m.status_check() == 0
+    err = np.abs(lg - ref).max(1)
+    if precision == gnn.FP32_VALIDATION:
+        assert (err < tol).mean() >= 0.99                                # near-tie jets: see test_gpu_fp32 (R21)
+    else:
+        assert err.max() < tol and (lg.argmax(1) == ref.argmax(1)).mean() >= 0.999
+    pr = m.infer_channel_first(dev(pts), dev(fts), dev(msk), softmax=True).cpu().numpy().astype(np.float64)
+    assert np.abs(pr.sum(1) - 1).max() < 1e-6 and (pr >= 0).all()
+    # the device softmax of the device logits is the oracle's softmax of the same logits to fp32 rounding ...
+    assert np.abs(pr - oracle.softmax(lg)).max() < 1e-6
+    # ... and of the oracle's logits to the logit tolerance (|dp| <= |dz| / 2 for two classes)
+    ok = err < tol
+    assert np.abs(pr - oracle.softmax(ref))[ok].max() < tol
+    m.close()
+
+
+def test_softmax_entry_and_layout_equivalence():
+    """gnn_softmax on its own; channel-first and channel-last padded entries give bitwise the same logits."""
+    a = synth.ARCHS["particlenet"]
+    w = synth.make_weights(a)
+    b = synth.make_particlenet_batch(n_jets=64)
+    m = make_model(a, w, precision=gnn.BF16, max_batch_jets=64, max_particles=100)
+    f, c, k = synth.pad_batch(b, 100, interleave=True, garbage=1e9)
+    pts, fts, msk = synth.to_channel_first(f, c, k)
+    l_cf = m.infer_channel_first(dev(pts), dev(fts), dev(msk)).cpu().numpy()
+    l_cl = m.infer_padded(dev(f), dev(c), dev(k)).cpu().numpy()
+    assert np.array_equal(l_cf, l_cl)
+    z = np.array([[0.0, 0.0], [1.0, -1.0], [50.0, -50.0], [-3.0, 2.0], [1e4, 1e4 - 1]], np.float32)
+    out = torch.empty((5, 2), dtype=torch.float32, device="cuda")
+    rc = gnn.lib().gnn_softmax(dev(z).data_ptr(), 5, 2, out.data_ptr(), torch.cuda.current_stream().cuda_stream)
+    assert rc == 0
+    torch.cuda.synchronize()
+    assert np.abs(out.cpu().numpy() - oracle.softmax(z)).max() < 1e-6
+    m.close()

@@ -98,3 +98,18 @@ def test_edge_case_set_runs_and_empty_jet_is_head_of_zero():
     assert np.array_equal(r["logits"][0], zero_logits[0])
     ref = forward_np(a, w, b.feats, b.coords, b.offsets)
     assert np.allclose(r["logits"], ref, rtol=0, atol=1e-10)
+
+
+def test_softmax_against_library_and_closed_form():
+    """oracle.softmax (SURVEY 8(f) variants): scipy's routine, rows summing to one, the two-class closed form
+    p_0 = 1 / (1 + exp(z_1 - z_0)), shift invariance."""
+    from scipy.special import softmax as sp_softmax
+    rng = np.random.default_rng(3)
+    z = rng.normal(0, 5, (200, 2))
+    p = oracle.softmax(z)
+    assert np.abs(p - sp_softmax(z, axis=1)).max() < 1e-14
+    assert np.abs(p.sum(1) - 1).max() < 1e-14
+    assert np.abs(p[:, 0] - 1.0 / (1.0 + np.exp(z[:, 1] - z[:, 0]))).max() < 1e-13
+    assert np.abs(oracle.softmax(z + 1000.0) - p).max() < 1e-12
+    z5 = rng.normal(0, 3, (50, 5))
+    assert np.abs(oracle.softmax(z5) - sp_softmax(z5, axis=1)).max() < 1e-14
