@@ -197,6 +197,42 @@ def serving_leg(gnn, synth, arch, weights, device, n_clients=64, warm_ms=500, ru
     return res
 
 
+def serving_extras(gnn, synth, arch, device, serving_jets_per_s):
+    """SURVEY 8(f) NEXT-1 / NEXT-2 / NEXT-3 on top of the batcher and the native load generator:
+    perf_sweep    PAPER.md L279-L291 (Table C2, Fig. C3): concurrency 1-4 x batch {128, 256, 512, 1024}, synchronous clients;
+                  queue / transfer (PCIe: the paper's network) / inference time per request, normalised per FP32 input of the
+                  paper's padded shape ((F + 2 + 1) x 100 per jet) and as fractions of the request time
+    colocation    PAPER.md L163-L177 (section 4.3, Figs. 10-11): n models with different weights served at once, aggregate and
+                  per-model jets/s, per-model throughput over throughput(1) / n
+    autoscale     PAPER.md L105, App. A: the SP2 rule replayed on a client ramp, with this GPU's measured service rate per
+                  instance (requests of 1024 jets per second)"""
+    from paper_2312_06838_b200 import perf, autoscale
+    big = synth.make_particlenet_batch(seed=1007, n_jets=4096)
+    model = gnn.Model(gnn.arch_struct(arch, max_batch_jets=1024, precision=gnn.BF16, workspace_slices=1, max_particles=100),
+                      synth.make_weights(arch), device=device)
+    inputs = (arch.in_features + 2 + 1) * 100
+    rows = perf.sweep(model, big, inputs, warmup_ms=150, run_ms=500)
+    model.close()
+
+    def make_model(i):
+        return gnn.Model(gnn.arch_struct(arch, max_batch_jets=1024, precision=gnn.BF16, workspace_slices=1, max_particles=100),
+                         synth.make_weights(arch, seed=i), device=device)
+
+    colo = perf.colocation(make_model, big, warmup_ms=200, run_ms=800)
+    rate = serving_jets_per_s / 1024.0                                  # requests of 1024 jets per second and instance
+    tr = autoscale.simulate(lambda t: min(40.0 * rate, t * rate / 20.0) if t < 2400 else 0.0, service_rate_per_instance=rate,
+                            request_rate_per_worker=rate / 4.0, duration_s=4200.0)
+    ups = [r["t"] for a, r in zip(tr, tr[1:]) if r["instances"] > a["instances"]]
+    downs = [r["t"] for a, r in zip(tr, tr[1:]) if r["instances"] < a["instances"]]
+    return {"perf_sweep": {"inputs_per_jet": inputs, "rows": rows,
+                           "note": "transfer = host <-> device copies of the coalesced batch (CUDA events), the paper's network latency"},
+            "colocation": colo,
+            "autoscale": {"policy": "SP2 (400 ms, 4 samples up / 180 s, 40 samples down / 60 s, one instance at a time, <= 10)",
+                          "service_rate_requests_per_s_per_instance": rate, "scale_up_times_s": ups, "scale_down_times_s": downs,
+                          "max_instances": max(r["instances"] for r in tr), "peak_throughput_requests_per_s": max(r["throughput"] for r in tr),
+                          "samples": len(tr)}}
+
+
 def time_forward(torch, model, b, dev, n_classes, reps, warm=3):
     """median / p99 CUDA-event milliseconds of gnn_infer on one device-resident ragged batch"""
     f, c, o = (torch.from_numpy(x).to(dev) for x in (b.feats, b.coords, b.offsets))
@@ -479,6 +515,7 @@ def run_ours(args):
         if rank == 0 and args.precision == "bf16":
             out["serving"] = serving_leg(gnn, synth, arch, weights, local)
             out["ragged_4096_f9"] = ragged_leg(torch, gnn, synth, work, roof_peak, local)
+            out.update(serving_extras(gnn, synth, arch, local, out["serving"]["n_instances_1"]["value"]))
             out["sweep"] = sweep_leg(torch, gnn, synth, work, roof_peak, local)
     out["clocks"] = sampler.summary()
     if rank == 0 and world == 1 and not args.no_cpu_baseline and not args.no_extras:

@@ -188,6 +188,11 @@ int gnn_batcher_submit(gnn_batcher* b, const float* feats_host, const float* coo
 /* Blocks until the ticket completes or timeout_us elapses (< 0: forever).  Returns the ticket's status.  queue_us =
  * submit -> launch, compute_us = launch -> logits in host memory (PAPER.md L279 splits request time this way). */
 int gnn_batcher_wait(gnn_batcher* b, gnn_ticket t, int64_t timeout_us, double* queue_us, double* compute_us);
+/* The same with the full split of Fig. C3: compute_us (launch -> logits in host memory, host clock) contains
+ * transfer_us (host -> device and device -> host copies of the coalesced batch: the paper's "network latency", PCIe here)
+ * and inference_us (the forward), both measured with CUDA events on the instance's stream. */
+typedef struct { double queue_us, compute_us, transfer_us, inference_us; } gnn_request_times;
+int gnn_batcher_wait_ex(gnn_batcher* b, gnn_ticket t, int64_t timeout_us, gnn_request_times* times);
 int gnn_batcher_stats(gnn_batcher* b, uint64_t* n_requests, uint64_t* n_jets, uint64_t* n_launches,
                       double* mean_batch_jets);
 void gnn_batcher_destroy(gnn_batcher* b);   /* drains pending tickets first */
@@ -210,6 +215,7 @@ typedef struct { int32_t n_clients, warmup_ms, run_ms; } gnn_loadgen_opts;
 typedef struct {
     uint64_t n_requests, n_jets;
     double seconds, jets_per_s, mean_us, p50_us, p90_us, p99_us, queue_us_mean, compute_us_mean, mean_batch_jets;
+    double transfer_us_mean, inference_us_mean;   /* device-side parts of compute_us (gnn_request_times) */
 } gnn_loadgen_result;
 int gnn_loadgen_run(gnn_batcher* b, const gnn_loadgen_pool* pool, const gnn_loadgen_opts* opts, gnn_loadgen_result* out);
 

@@ -46,7 +46,7 @@ class LoadgenOpts(C.Structure):
 class LoadgenResult(C.Structure):
     _fields_ = [("n_requests", C.c_uint64), ("n_jets", C.c_uint64)] + [(k, C.c_double) for k in (
         "seconds", "jets_per_s", "mean_us", "p50_us", "p90_us", "p99_us", "queue_us_mean", "compute_us_mean",
-        "mean_batch_jets")]
+        "mean_batch_jets", "transfer_us_mean", "inference_us_mean")]
 
 
 def lib():
@@ -81,6 +81,7 @@ def lib():
         L.gnn_batcher_create.argtypes = [vp, C.POINTER(BatcherOpts), C.POINTER(vp)]
         L.gnn_batcher_submit.argtypes = [vp, vp, vp, vp, i32, vp, C.POINTER(Ticket)]
         L.gnn_batcher_wait.argtypes = [vp, Ticket, C.c_int64, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.gnn_batcher_wait_ex.argtypes = [vp, Ticket, C.c_int64, C.c_void_p]
         L.gnn_batcher_stats.argtypes = [vp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64), C.POINTER(C.c_uint64),
                                         C.POINTER(C.c_double)]
         L.gnn_batcher_destroy.argtypes = [vp]; L.gnn_batcher_destroy.restype = None

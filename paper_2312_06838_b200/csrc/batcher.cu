@@ -32,6 +32,7 @@ struct Request {
     const int32_t* offsets = nullptr;  // [n_jets + 1], relative to the request
     float* out = nullptr;
     Clock::time_point t_submit, t_launch, t_done;
+    float transfer_us = 0.0f, inference_us = 0.0f;   // device-side times of the batch the request rode in
     std::mutex mu;
     std::condition_variable cv;
     bool done = false;
@@ -44,6 +45,7 @@ struct Instance {
     int32_t* h_offsets = nullptr;
     float *d_feats = nullptr, *d_coords = nullptr, *d_logits = nullptr;
     int32_t* d_offsets = nullptr;
+    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};   // before H2D, after H2D, after the forward, after D2H
     std::thread worker;
 };
 
@@ -65,13 +67,14 @@ struct gnn_batcher {
 
 namespace {
 
-void finish(gnn_batcher* b, std::vector<Request*>& batch, int status, Clock::time_point t_launch) {
+void finish(gnn_batcher* b, std::vector<Request*>& batch, int status, Clock::time_point t_launch, float transfer_us, float inference_us) {
     (void)b;
     auto now = Clock::now();
     for (Request* r : batch) {
         // notify under the request's lock: once it is released the waiter may delete r, so r is not touched again
         std::lock_guard<std::mutex> lk(r->mu);
-        r->status = status; r->t_launch = t_launch; r->t_done = now; r->done = true;
+        r->status = status; r->t_launch = t_launch; r->t_done = now; r->transfer_us = transfer_us; r->inference_us = inference_us;
+        r->done = true;
         r->cv.notify_one();
     }
 }
@@ -119,19 +122,31 @@ void worker_main(gnn_batcher* b, int wi) {
         }
         auto t_launch = Clock::now();
         int rc = GNN_OK;
-        cudaError_t e = cudaSuccess;
-        if (N > 0) {
+        cudaError_t e = cudaEventRecord(I.ev[0], I.stream);
+        if (e == cudaSuccess && N > 0) {
             e = cudaMemcpyAsync(I.d_feats, I.h_feats, (size_t)N * F * sizeof(float), cudaMemcpyHostToDevice, I.stream);
             if (e == cudaSuccess)
                 e = cudaMemcpyAsync(I.d_coords, I.h_coords, (size_t)N * CD * sizeof(float), cudaMemcpyHostToDevice, I.stream);
         }
         if (e == cudaSuccess)
             e = cudaMemcpyAsync(I.d_offsets, I.h_offsets, (size_t)(B + 1) * sizeof(int32_t), cudaMemcpyHostToDevice, I.stream);
+        if (e == cudaSuccess) e = cudaEventRecord(I.ev[1], I.stream);
         if (e == cudaSuccess) rc = gnn_infer_slice(b->m, wi, I.d_feats, I.d_coords, I.d_offsets, B, N, I.d_logits, I.stream);
+        if (e == cudaSuccess && rc == GNN_OK) e = cudaEventRecord(I.ev[2], I.stream);
         if (e == cudaSuccess && rc == GNN_OK)
             e = cudaMemcpyAsync(I.h_logits, I.d_logits, (size_t)B * NC * sizeof(float), cudaMemcpyDeviceToHost, I.stream);
+        if (e == cudaSuccess && rc == GNN_OK) e = cudaEventRecord(I.ev[3], I.stream);
         if (e == cudaSuccess) e = cudaStreamSynchronize(I.stream);
         if (e != cudaSuccess) rc = GNN_ERR_CUDA;
+        float transfer_us = 0.0f, inference_us = 0.0f;
+        if (rc == GNN_OK) {
+            float h2d = 0.0f, fw = 0.0f, d2h = 0.0f;             // milliseconds on the instance's stream
+            if (cudaEventElapsedTime(&h2d, I.ev[0], I.ev[1]) == cudaSuccess && cudaEventElapsedTime(&fw, I.ev[1], I.ev[2]) == cudaSuccess &&
+                cudaEventElapsedTime(&d2h, I.ev[2], I.ev[3]) == cudaSuccess) {
+                transfer_us = (h2d + d2h) * 1e3f;
+                inference_us = fw * 1e3f;
+            }
+        }
         if (rc == GNN_OK) {
             int j0 = 0;
             for (Request* r : batch) {
@@ -139,7 +154,7 @@ void worker_main(gnn_batcher* b, int wi) {
                 j0 += r->n_jets;
             }
         }
-        finish(b, batch, rc, t_launch);
+        finish(b, batch, rc, t_launch, transfer_us, inference_us);
     }
 }
 
@@ -152,6 +167,7 @@ void free_instance(Instance& I) {
     if (I.d_coords) cudaFree(I.d_coords);
     if (I.d_logits) cudaFree(I.d_logits);
     if (I.d_offsets) cudaFree(I.d_offsets);
+    for (cudaEvent_t e : I.ev) if (e) cudaEventDestroy(e);
     if (I.stream) cudaStreamDestroy(I.stream);
 }
 
@@ -177,6 +193,7 @@ int gnn_batcher_create(gnn_model* m, const gnn_batcher_opts* opts, gnn_batcher**
     bool ok = true;
     for (auto& I : b->inst) {
         ok = ok && cudaStreamCreateWithFlags(&I.stream, cudaStreamNonBlocking) == cudaSuccess;
+        for (auto& e : I.ev) ok = ok && cudaEventCreate(&e) == cudaSuccess;
         ok = ok && cudaMallocHost(&I.h_feats, Nm * a.in_features * sizeof(float)) == cudaSuccess;
         ok = ok && cudaMallocHost(&I.h_coords, Nm * a.coord_dims * sizeof(float)) == cudaSuccess;
         ok = ok && cudaMallocHost(&I.h_logits, Bm * a.n_classes * sizeof(float)) == cudaSuccess;
@@ -240,7 +257,7 @@ int gnn_batcher_submit(gnn_batcher* b, const float* feats_host, const float* coo
     return GNN_OK;
 }
 
-int gnn_batcher_wait(gnn_batcher* b, gnn_ticket t, int64_t timeout_us, double* queue_us, double* compute_us) {
+int gnn_batcher_wait_ex(gnn_batcher* b, gnn_ticket t, int64_t timeout_us, gnn_request_times* times) {
     if (!b) return GNN_ERR_NULL;
     Request* r = nullptr;
     {
@@ -262,8 +279,12 @@ int gnn_batcher_wait(gnn_batcher* b, gnn_ticket t, int64_t timeout_us, double* q
             return GNN_ERR_TIMEOUT;
         }
         using us = std::chrono::duration<double, std::micro>;
-        if (queue_us) *queue_us = us(r->t_launch - r->t_submit).count();
-        if (compute_us) *compute_us = us(r->t_done - r->t_launch).count();
+        if (times) {
+            times->queue_us = us(r->t_launch - r->t_submit).count();
+            times->compute_us = us(r->t_done - r->t_launch).count();
+            times->transfer_us = r->transfer_us;
+            times->inference_us = r->inference_us;
+        }
         status = r->status;
     }
     {
@@ -272,6 +293,16 @@ int gnn_batcher_wait(gnn_batcher* b, gnn_ticket t, int64_t timeout_us, double* q
     }
     delete r;
     return status;
+}
+
+int gnn_batcher_wait(gnn_batcher* b, gnn_ticket t, int64_t timeout_us, double* queue_us, double* compute_us) {
+    gnn_request_times tm{};
+    const int rc = gnn_batcher_wait_ex(b, t, timeout_us, &tm);
+    if (rc != GNN_ERR_BAD_TICKET && rc != GNN_ERR_TIMEOUT && rc != GNN_ERR_NULL) {
+        if (queue_us) *queue_us = tm.queue_us;
+        if (compute_us) *compute_us = tm.compute_us;
+    }
+    return rc;
 }
 
 int gnn_batcher_stats(gnn_batcher* b, uint64_t* n_requests, uint64_t* n_jets, uint64_t* n_launches, double* mean_batch_jets) {

@@ -18,6 +18,7 @@ using Clock = std::chrono::steady_clock;
 
 struct ClientLog {
     std::vector<float> total_us, queue_us, compute_us;
+    double transfer_us = 0.0, inference_us = 0.0;
     uint64_t jets = 0;
     int status = GNN_OK;
 };
@@ -59,14 +60,15 @@ extern "C" int gnn_loadgen_run(gnn_batcher* b, const gnn_loadgen_pool* pool, con
             gnn_ticket tk;
             int rc = gnn_batcher_submit(b, pool->feats_host + (size_t)p0 * pool->in_features,
                                         pool->coords_host + (size_t)p0 * pool->coord_dims, rel.data(), nj, logits.data(), &tk);
-            double q = 0.0, cu = 0.0;
-            if (rc == GNN_OK) rc = gnn_batcher_wait(b, tk, -1, &q, &cu);
+            gnn_request_times tm{};
+            if (rc == GNN_OK) rc = gnn_batcher_wait_ex(b, tk, -1, &tm);
             const auto t1 = Clock::now();
             if (rc != GNN_OK) { L.status = rc; break; }
             if (ph == 1 && phase.load(std::memory_order_acquire) == 1) {
                 L.total_us.push_back(std::chrono::duration<float, std::micro>(t1 - t0).count());
-                L.queue_us.push_back((float)q);
-                L.compute_us.push_back((float)cu);
+                L.queue_us.push_back((float)tm.queue_us);
+                L.compute_us.push_back((float)tm.compute_us);
+                L.transfer_us += tm.transfer_us; L.inference_us += tm.inference_us;
                 L.jets += (uint64_t)nj;
             }
         }
@@ -87,7 +89,9 @@ extern "C" int gnn_loadgen_run(gnn_batcher* b, const gnn_loadgen_pool* pool, con
     std::vector<float> all, q, cu;
     uint64_t jets = 0;
     int status = GNN_OK;
+    double tr = 0.0, inf = 0.0;
     for (auto& L : logs) {
+        tr += L.transfer_us; inf += L.inference_us;
         all.insert(all.end(), L.total_us.begin(), L.total_us.end());
         q.insert(q.end(), L.queue_us.begin(), L.queue_us.end());
         cu.insert(cu.end(), L.compute_us.begin(), L.compute_us.end());
@@ -102,6 +106,8 @@ extern "C" int gnn_loadgen_run(gnn_batcher* b, const gnn_loadgen_pool* pool, con
     out->mean_us = mean(all);
     out->queue_us_mean = mean(q);
     out->compute_us_mean = mean(cu);
+    out->transfer_us_mean = all.empty() ? 0.0 : tr / (double)all.size();
+    out->inference_us_mean = all.empty() ? 0.0 : inf / (double)all.size();
     out->p50_us = percentile(all, 0.50);
     out->p90_us = percentile(all, 0.90);
     out->p99_us = percentile(all, 0.99);

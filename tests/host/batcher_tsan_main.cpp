@@ -23,6 +23,10 @@ cudaError_t cudaFreeHost(void* p) { std::free(p); return cudaSuccess; }
 cudaError_t cudaFree(void* p) { std::free(p); return cudaSuccess; }
 cudaError_t cudaMemcpyAsync(void* d, const void* s, size_t n, cudaMemcpyKind, cudaStream_t) { std::memcpy(d, s, n); return cudaSuccess; }
 const char* cudaGetErrorString(cudaError_t) { return "stub"; }
+cudaError_t cudaEventCreate(cudaEvent_t* e) { *e = reinterpret_cast<cudaEvent_t>(std::malloc(1)); return cudaSuccess; }
+cudaError_t cudaEventDestroy(cudaEvent_t e) { std::free(e); return cudaSuccess; }
+cudaError_t cudaEventRecord(cudaEvent_t, cudaStream_t) { return cudaSuccess; }
+cudaError_t cudaEventElapsedTime(float* ms, cudaEvent_t, cudaEvent_t) { *ms = 0.05f; return cudaSuccess; }
 
 // stand-in forward: logit c of jet j = (c + 1) * sum of the jet's first feature + number of particles; takes a little while
 int gnn_infer_slice(gnn_model* m, int32_t, const float* feats, const float*, const int32_t* offsets, int32_t B, int32_t N,
