@@ -233,6 +233,59 @@ def serving_extras(gnn, synth, arch, device, serving_jets_per_s):
                           "samples": len(tr)}}
 
 
+def bdt_leg(torch, gnn, synth, pk, device, no_cpu=False):
+    """SURVEY 8(f) NEXT-4, PAPER.md L125 / Fig. 6 / Table C2: the 20-feature, 100-tree BDT (synthetic trees, depth 6) at batch
+    10 K ... 2.56 M: events/s device-resident (CUDA events) and through host buffers (gnn_bdt_infer_host, wall clock), the
+    fp64 oracle on the host cores, and the Fig-6 analogue (10 M inputs in batches of 10 000, the paper's counter-example:
+    'more time for inference on the Triton server GPUs than on the local CPUs' once transfers are counted)."""
+    from oracle import bdt as obdt
+    dev = torch.device("cuda", device)
+    f, t, l = synth.make_bdt()
+    m = gnn.Bdt(f, t, l, 20, device=device)
+    x_all = synth.make_bdt_events(2560000)
+    xd = torch.from_numpy(x_all).to(dev)
+    xh = torch.from_numpy(x_all).pin_memory()
+    od = torch.empty((x_all.shape[0], 2), dtype=torch.float32, device=dev)
+    oh = torch.empty((x_all.shape[0], 2), dtype=torch.float32).pin_memory()
+    rows = []
+    for N in (10000, 40000, 160000, 640000, 2560000):
+        for _ in range(3):
+            m.infer(xd[:N], od[:N])
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(10)]
+        torch.cuda.synchronize()
+        for a, e in ev:
+            a.record(torch.cuda.current_stream()); m.infer(xd[:N], od[:N]); e.record(torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        ms = float(np.median([a.elapsed_time(e) for a, e in ev]))
+        m.infer_host(xh[:N], oh[:N])
+        t0 = time.perf_counter()
+        for _ in range(5):
+            m.infer_host(xh[:N], oh[:N])
+        e2e = (time.perf_counter() - t0) / 5
+        steps = 100 * 6                                          # dependent (node, feature, compare) steps per event
+        rows.append({"batch": N, "device_ms": ms, "device_events_per_s": N / (ms * 1e-3), "e2e_ms": e2e * 1e3,
+                     "e2e_events_per_s": N / e2e, "hbm_gbs": N * 88 / (ms * 1e-3) / 1e9, "hbm_frac": N * 88 / (ms * 1e-3) / 1e9 / pk["hbm_gbs"],
+                     "tree_steps_per_s": N * steps / (ms * 1e-3)})
+    out = {"workload": "BDT, 100 random trees of depth 6, 20 features (PAPER.md L125, Table C2), N(0,1) events", "rows": rows,
+           "bound": "shared-memory / ALU issue (600 dependent tree steps per 88 bytes of HBM traffic); hbm_frac is reported, not the bound"}
+    # Fig-6 analogue: 10 M inputs in batches of 10 000 through host buffers
+    t0 = time.perf_counter()
+    for i in range(1000):
+        o = (i % 256) * 10000
+        m.infer_host(xh[o:o + 10000], oh[o:o + 10000])
+    gpu_s = time.perf_counter() - t0
+    out["fig6"] = {"inputs": 10000000, "batch": 10000, "gpu_e2e_s": gpu_s, "gpu_e2e_events_per_s": 1e7 / gpu_s}
+    if not no_cpu:
+        t0 = time.perf_counter()
+        obdt.predict(f, t, l, x_all[:200000])
+        cpu = 200000 / (time.perf_counter() - t0)
+        out["cpu_oracle"] = {"events_per_s": cpu, "kind": "oracle (numpy fp64, one core)", "sample": "first 200 000 events"}
+        out["fig6"]["cpu_oracle_s_at_measured_rate"] = 1e7 / cpu
+        out["fig6"]["paper_context"] = "PAPER.md L125 / Fig. 6: the BDT was slower through the GPU server than on the local CPU (trained XGBoost model, server overheads)"
+    m.close()
+    return out
+
+
 def time_forward(torch, model, b, dev, n_classes, reps, warm=3):
     """median / p99 CUDA-event milliseconds of gnn_infer on one device-resident ragged batch"""
     f, c, o = (torch.from_numpy(x).to(dev) for x in (b.feats, b.coords, b.offsets))
@@ -521,6 +574,7 @@ def run_ours(args):
     if rank == 0 and world == 1 and not args.no_cpu_baseline and not args.no_extras:
         out["cpu_baseline"] = cpu_baseline(arch, weights, batches[0])
     if rank == 0 and not args.no_extras and args.precision == "bf16":
+        out["bdt"] = bdt_leg(torch, gnn, synth, pk, local, no_cpu=args.no_cpu_baseline)
         out["fig4"] = fig4_leg(gnn, synth, model, arch, arch.n_classes, out.get("cpu_baseline", {}).get("value"))
     model.close()
     if world > 1:

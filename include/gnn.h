@@ -219,6 +219,23 @@ typedef struct {
 } gnn_loadgen_result;
 int gnn_loadgen_run(gnn_batcher* b, const gnn_loadgen_pool* pool, const gnn_loadgen_opts* opts, gnn_loadgen_result* out);
 
+/* ---- second workload: boosted-decision-tree inference (section 4.1, Fig. 6: "a small boosted decision tree
+ * (BDT) with 20 input features and 100 trees"; Table C2: input shape 20, output shape 2, batches 10 K ... 2.56 M) ---
+ * n_trees complete binary trees of depth `depth`.  feature_host / threshold_host [n_trees, 2^depth - 1]: internal node i
+ * tests x[feature] < threshold: true -> child 2 i + 1, else (also for NaN) child 2 i + 2; leaf_host [n_trees, 2^depth]: leaf
+ * j of a tree is reached at node 2^depth - 1 + j.  margin = sum over the trees, in tree order, of the reached leaves (fp32);
+ * output row = (1 - p, p), p = 1 / (1 + exp(-margin)).  The arrays are copied; the forest must fit one SM's shared memory
+ * (GNN_ERR_BAD_ARCH otherwise), feature indices are validated (GNN_ERR_BAD_ARG). */
+typedef struct gnn_bdt gnn_bdt;
+int gnn_bdt_create(const int32_t* feature_host, const float* threshold_host, const float* leaf_host, int32_t n_trees,
+                   int32_t depth, int32_t n_features, int device, gnn_bdt** out);
+void gnn_bdt_destroy(gnn_bdt* b);
+/* x_dev [N, n_features] fp32 row-major -> out_dev [N, 2]; asynchronous on cuda_stream */
+int gnn_bdt_infer(gnn_bdt* b, const float* x_dev, int64_t N, float* out_dev, void* cuda_stream);
+/* the same from / to HOST buffers (pinned memory makes the copies asynchronous); blocking; device staging owned by `b` grows
+ * to the largest N seen */
+int gnn_bdt_infer_host(gnn_bdt* b, const float* x_host, int64_t N, float* out_host, void* cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -3,5 +3,5 @@
 Argument marshalling only -- every step of the path runs in the library's CUDA kernels.  torch is used for device
 memory and streams.  There is no CPU fallback: loading fails loudly if libgnn.so is missing.
 """
-from .binding import (GnnArch, Model, Batcher, GnnError, lib, arch_struct, weights_bytes, strerror, LIB_PATH,  # noqa: F401
+from .binding import (GnnArch, Model, Batcher, Bdt, GnnError, lib, arch_struct, weights_bytes, strerror, LIB_PATH,  # noqa: F401
                       FP32_VALIDATION, BF16)

@@ -85,6 +85,10 @@ def lib():
         L.gnn_batcher_stats.argtypes = [vp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64), C.POINTER(C.c_uint64),
                                         C.POINTER(C.c_double)]
         L.gnn_batcher_destroy.argtypes = [vp]; L.gnn_batcher_destroy.restype = None
+        L.gnn_bdt_create.argtypes = [vp, vp, vp, i32, i32, i32, C.c_int, C.POINTER(vp)]
+        L.gnn_bdt_destroy.argtypes = [vp]; L.gnn_bdt_destroy.restype = None
+        L.gnn_bdt_infer.argtypes = [vp, f32p, C.c_int64, f32p, vp]
+        L.gnn_bdt_infer_host.argtypes = [vp, vp, C.c_int64, vp, vp]
         L.gnn_loadgen_run.argtypes = [vp, C.POINTER(LoadgenPool), C.POINTER(LoadgenOpts), C.POINTER(LoadgenResult)]
         _lib = L
     return _lib
@@ -303,6 +307,50 @@ class Batcher:
     def close(self):
         if getattr(self, "h", None):
             lib().gnn_batcher_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class Bdt:
+    """gnn_bdt: boosted-decision-tree inference (include/gnn.h).  Marshalling only."""
+
+    def __init__(self, feature: np.ndarray, threshold: np.ndarray, leaf: np.ndarray, n_features: int, device: int = 0):
+        feature = np.ascontiguousarray(feature, np.int32); threshold = np.ascontiguousarray(threshold, np.float32)
+        leaf = np.ascontiguousarray(leaf, np.float32)
+        n_trees, n_int = feature.shape
+        depth = int(n_int + 1).bit_length() - 1
+        self.n_features = int(n_features)
+        h = C.c_void_p()
+        rc = lib().gnn_bdt_create(feature.ctypes.data, threshold.ctypes.data, leaf.ctypes.data, n_trees, depth, self.n_features,
+                                  device, C.byref(h))
+        if rc != 0:
+            raise GnnError(rc, "gnn_bdt_create")
+        self.h = h
+
+    def infer(self, x, out=None, stream=None):
+        import torch
+        N = int(x.shape[0])
+        if out is None:
+            out = torch.empty((N, 2), dtype=torch.float32, device=x.device)
+        rc = lib().gnn_bdt_infer(self.h, _ptr(x), N, _ptr(out), _stream(stream))
+        if rc != 0:
+            raise GnnError(rc, "gnn_bdt_infer")
+        return out
+
+    def infer_host(self, x, out, stream=None):
+        rc = lib().gnn_bdt_infer_host(self.h, _hptr(x), int(x.shape[0]), _hptr(out), _stream(stream))
+        if rc != 0:
+            raise GnnError(rc, "gnn_bdt_infer_host")
+        return out
+
+    def close(self):
+        if getattr(self, "h", None):
+            lib().gnn_bdt_destroy(self.h)
             self.h = None
 
     def __del__(self):

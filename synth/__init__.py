@@ -9,3 +9,4 @@ from .arch import Arch, ARCHS, weight_count          # noqa: F401
 from .weights import make_weights                    # noqa: F401
 from .jets import (make_tiny, make_particlenet_batch, make_ragged_batch, make_sweep_batch,  # noqa: F401
                    make_client_pool, make_edge_case_batch, pad_batch, JetBatch, make_paper_f5_batch, to_channel_first)
+from .bdt import make_bdt, make_bdt_events           # noqa: F401
