@@ -89,15 +89,38 @@ def test_tiny_end_to_end():
     m.close()
 
 
-def test_particlenet_full_batch_1024(pn):
+def test_particlenet_full_batch_1024(pn, record_property):
     """BASELINE configs[1] at its full size, in the launch configuration bench.py times (one gnn_infer)."""
     a, w, m = pn
     b = synth.make_particlenet_batch()
     lg = run_ragged(m, b)
     assert m.status_check() == 0
-    ref = oracle.forward(a, w, b.feats, b.coords, b.offsets)
+    r = oracle.forward(a, w, b.feats, b.coords, b.offsets, dumps=True)
+    ref = r["logits"]
     err = check_logits(lg, ref)
     assert err.mean() < 2.5e-2
+    # ---- parity protocol of SURVEY 8(c) for this mode (R20, R22): reported, not enforced.  Per-block neighbour flip rate =
+    # share of the points whose neighbour SET, computed by the production kNN on the GPU's own block input, differs from the
+    # oracle's set on the oracle's input (it contains the upstream bf16 noise); and the oracle's logit-gap histogram, which
+    # says how many jets sit close enough to the decision boundary for a 5e-2 logit error to flip their argmax.
+    o = dev(b.offsets)
+    x, space, flips = dev(b.feats), dev(b.coords), []
+    for l in range(len(a.channels)):
+        idx = m.debug_knn(space, o, a.k)
+        gi, oi = np.sort(idx.cpu().numpy(), 1), np.sort(r["nbr"][l], 1)
+        flips.append(float((gi != oi).any(1).mean()))
+        x = m.debug_edgeconv(l, x, idx, o)
+        space = x
+    staged = m.debug_pool_head(x, o).cpu().numpy().astype(np.float64)
+    assert np.abs(staged - lg).max() < 5e-3                 # same kernels up to the pooling route (stored block output vs fused sums)
+    gap = np.abs(ref[:, 1] - ref[:, 0])
+    edges = [0.0, 0.05, 0.1, 0.2, 0.5, 1.0, 2.0, 5.0, np.inf]
+    hist = np.histogram(gap, edges)[0].tolist()
+    print("bf16 B=1024: max |dlogit| %.3e, mean %.3e; neighbour-set flip rate per block %s; oracle |z1 - z0| histogram over edges %s: %s"
+          % (err.max(), err.mean(), ["%.4f" % f for f in flips], edges, hist))
+    record_property("flip_rate_per_block", flips)
+    record_property("oracle_logit_gap_histogram", {"edges": [str(e) for e in edges], "counts": hist})
+    assert flips[0] < 2e-3 and max(flips) < 0.15            # block 1 is exact arithmetic on exact coordinates; later blocks carry bf16 noise
 
 
 def test_ragged_4096_f9_sampled():
