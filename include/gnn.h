@@ -53,9 +53,10 @@ typedef enum {
 
 typedef enum {
     GNN_FP32_VALIDATION = 0,  /* every contraction in fp32 FMA on CUDA cores (R18) */
-    GNN_BF16 = 1              /* edge-MLP GEMMs as bf16 x bf16 -> fp32 tcgen05 MMAs; per-particle GEMM of blocks >= 2 and kNN Gram
-                                 matrices of blocks >= 2 in tf32; neighbour selection on 32-bit keys; E3 row sum in f16x2;
-                                 accumulators, block outputs, pool, head fp32 (R19, R28) */
+    GNN_BF16 = 1              /* edge-MLP GEMMs as bf16 x bf16 -> fp32 tcgen05 MMAs; per-particle GEMM of blocks >= 2, kNN Gram
+                                 matrices of blocks >= 2 and the stored shortcut in fp16 (10 mantissa bits; saturating at 65504:
+                                 activations must stay below that); neighbour selection on 32-bit keys in every block; E3 row
+                                 sum in f16x2; accumulators, block outputs, pool, head fp32 (R19, R28) */
 } gnn_precision;
 
 /* Architecture.  Constraints checked by gnn_create: 1 <= n_blocks <= GNN_MAX_BLOCKS;
@@ -94,8 +95,9 @@ void gnn_destroy(gnn_model* m);
  * row-major fp32, particles of one jet contiguous; offsets_dev int32 [B+1] CSR (offsets[0] = 0, offsets[B] = N);
  * logits_dev fp32 [B, n_classes] (written).  Asynchronous on `cuda_stream` (a cudaStream_t; NULL = default
  * stream).  Uses workspace slice 0 / `slice`: two calls may overlap only on different slices.  B = 0 is legal.
- * (GNN_BF16: part of the work is enqueued on an auxiliary stream owned by the slice, forked from and joined back into
- * `cuda_stream` by events, so the call is still ordered on `cuda_stream` alone; stream capture is not supported.)
+ * Everything is enqueued on `cuda_stream` alone (GNN_BF16: as programmatic dependent launches), so the call may be
+ * captured into a CUDA graph of the caller's; gnn_infer / gnn_infer_slice also replay a graph of their own when a call's
+ * arguments (pointers, B, N) repeat an earlier call's on the slice (captured on the second sighting, up to 8 per slice).
  * Host-checkable errors return at once; device-checkable ones (GNN_ERR_BAD_OFFSETS, GNN_ERR_JET_TOO_LARGE) set a
  * sticky per-slice status word read by gnn_status_check and put NaN into the offending logits.  n_b = 0 is legal
  * (logits = head(0), R12).  NaN / Inf inputs are not checked. */

@@ -1003,7 +1003,7 @@ __global__ void __launch_bounds__(1024) pre_small_kernel(PreParams p) {
 // multiplied as two N halves of C / 2 columns, each with its own accumulator (C TMEM columns in all): the epilogue of one
 // half runs under the MMAs of the other and of the next tile.
 // Shared memory (161 KB for 128 -> 256), registers (288 threads x 80) and TMEM (C columns) leave room for kNN CTAs of the
-// same block on the SM: the forward runs the two kernels side by side on two streams.
+// same block on the SM: the forward runs the two kernels side by side (primary / secondary pair of dependent launches).
 // Warps: 0-3 epilogue (thread = row = TMEM lane), 4-7 converters, 8 TMA + MMA issuer + TMEM owner.
 constexpr int PTC_EPI_WARPS = 4;
 constexpr int PTC_CVT_WARPS = 4;
@@ -1222,7 +1222,7 @@ struct Bf16BlockDev {
     const float* shifts = nullptr;
     const float* pre_Wt = nullptr;
     const float* pre_bias = nullptr;
-    const uint8_t* pre_wimg = nullptr;   // tf32 chunk images of the tensor-core pre kernel (null: SIMT pre kernel)
+    const uint8_t* pre_wimg = nullptr;   // fp16 chunk images of the tensor-core pre kernel (null: SIMT pre kernel)
     int cin = 0, Kp = 0, C = 0, NC = 0;
     int grid_cap = 148, grid_cap_pool = 148;
     int pre_ctas_per_sm = 1;
@@ -1459,8 +1459,7 @@ void edgeconv_bf16_release(gnn_model& m) {
     for (auto& w : m.ws) { delete static_cast<Bf16Scratch*>(w.bf16_scratch); w.bf16_scratch = nullptr; }
 }
 
-// per-particle part of a block (u, v, shortcut): depends on x only, so the forward runs it on the workspace's auxiliary
-// stream next to the kNN of the same block
+// per-particle part of a block (u, v, shortcut): depends on x only, so the forward runs it beside the kNN of the same block
 // dep: DEP_* of gnn_internal.h (DEP_NONE = an ordinary launch); the tensor-core kernel can only be a primary
 bool pre_bf16_single_wave(const gnn_model& m, int block) { return static_cast<const Bf16BlockDev*>(m.bf16_blocks)[block].pre_wimg != nullptr; }
 
