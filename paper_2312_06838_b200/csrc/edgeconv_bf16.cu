@@ -68,7 +68,14 @@ struct EdgeCfg {
     static constexpr int KSTEPS_LAST = ((C - (KB - 1) * 64) + 15) / 16;
     static constexpr int NRB = PAIR ? C / 2 : C;              // weight rows (output channels) one CTA holds
     static constexpr int CHUNK_BYTES = NRB * 128;             // [NRB][64] bf16, 128B-swizzled
-    static constexpr int W_BYTES = 2 * KB * CHUNK_BYTES;      // both layers
+    // BIAS_MMA: the shifts t2, t3 enter the accumulators through ONE extra K step per layer (A = a constant tile whose first two
+    // columns are 1, B = the shift split into bf16 hi + lo parts: exact to 2^-17 relative), so the epilogues add nothing: the
+    // shift add and its shared-memory loads were a quarter of E2's and E3's instructions, and those epilogues are the
+    // kernels' critical chain.  The bias operands use the no-swizzle K-major layout (8 x 16-byte core matrices).
+    static constexpr bool BIAS_MMA = C != 128;                // (measured: C = 64: 41.3 -> 36.9 us, C = 256: 168.8 -> 156.7 us, C = 128: 63.4 -> 64.9 us)
+    static constexpr int WB_BYTES = BIAS_MMA ? NRB * 32 : 0;  // bias operand of one layer: [NRB][16] bf16
+    static constexpr int AB_BYTES = BIAS_MMA ? TILE_ROWS * 32 : 0;   // the constant A-side tile: [128][16] bf16
+    static constexpr int W_BYTES = 2 * KB * CHUNK_BYTES + 2 * WB_BYTES;      // both layers + their bias operands
     static constexpr int HK_BYTES = TILE_ROWS * 128;          // one K block of the operand tile: [128][64] bf16
     static constexpr int H_BYTES = KB * HK_BYTES;
     static constexpr int TMEM_COLS = 2 * C < 32 ? 32 : 2 * C; // D0 | D1
@@ -82,7 +89,7 @@ struct EdgeCfg {
     // transposed MMAs issue at ~190 cycles each instead of ~150 and the kernel loses 25 us, so C = 256 keeps the row layout.
     static constexpr bool TR3_OK = C == 128;
     static constexpr int SMALL_BYTES = 2 * C * 4 + NBAR * 8 + 16;
-    static constexpr int SMEM_BYTES = W_BYTES + H_BYTES + SMALL_BYTES + 1024;
+    static constexpr int SMEM_BYTES = W_BYTES + H_BYTES + AB_BYTES + SMALL_BYTES + 1024;
     // POOL variant (last block, k = 16): per epilogue warp and 32-column slab, two 64-bit fixed-point accumulators per lane
     static constexpr int POOL_BYTES = TR3_OK ? 0 : NE * (CWE / 32) * 32 * 16;   // (TR3 keeps the sums in registers)
     static constexpr int SMEM_BYTES_POOL = SMEM_BYTES + POOL_BYTES;
@@ -156,7 +163,8 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
     if ((smem_u32(smem) & 1023u) != 0u) __trap();
     uint8_t* Wsm = smem;
     uint8_t* H = Wsm + Cfg::W_BYTES;
-    float* shifts_s = reinterpret_cast<float*>(H + Cfg::H_BYTES);
+    uint8_t* Abias = H + Cfg::H_BYTES;
+    float* shifts_s = reinterpret_cast<float*>(Abias + Cfg::AB_BYTES);
     uint64_t* bars = reinterpret_cast<uint64_t*>(shifts_s + 2 * C);
     uint64_t* h1_ready = bars;                // [KB] K block of H1 gathered                              gather -> MMA (leader)
     uint64_t* h2_ready = bars + KB;           // [KB] K block of H2 written by E2                         epilogue -> MMA (leader)
@@ -181,6 +189,11 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
         fence_mbar_init();
     }
     for (int i = tid; i < 2 * C; i += Cfg::THREADS) shifts_s[i] = p.shifts[i];
+    // constant A-side tile of the bias K step, no-swizzle K-major: [K chunk c][row group g][row in group][16 bytes]; chunk 0 of
+    // every row = (1, 1, 0, 0, 0, 0, 0, 0) bf16, chunk 1 = zeros
+    for (int i = tid; i < Cfg::AB_BYTES / 16; i += Cfg::THREADS)
+        reinterpret_cast<uint4*>(Abias)[i] = make_uint4(i < TILE_ROWS ? 0x3F803F80u : 0u, 0u, 0u, 0u);
+    fence_proxy_async();
     if (warp == Cfg::MMA_WARP) tmem_alloc_g<PAIR>(tmem_ptr, Cfg::TMEM_COLS);
     tc_fence_before();
     if constexpr (PAIR) cluster_sync_all(); else __syncthreads();
@@ -205,6 +218,8 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
             const uint8_t* src = p.wimg + (size_t)rank * Cfg::W_BYTES;
             for (int c = 0; c < 2 * KB; ++c)
                 bulk_g2s(Wsm + (size_t)c * Cfg::CHUNK_BYTES, src + (size_t)c * Cfg::CHUNK_BYTES, Cfg::CHUNK_BYTES, w_full);
+            if constexpr (Cfg::BIAS_MMA)
+                bulk_g2s(Wsm + (size_t)2 * KB * Cfg::CHUNK_BYTES, src + (size_t)2 * KB * Cfg::CHUNK_BYTES, 2 * Cfg::WB_BYTES, w_full);
             if (PAIR && rank == 1) { mbar_wait(w_full, 0); mbar_arrive_cluster(w_peer, 0); }
         }
         if (lane == 0 && rank == 0) {
@@ -234,6 +249,13 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
                             }
                         }
                         if (layer == 1) mma_commit_g<PAIR>(&h_free[kb]);   // gather of the next tile may overwrite it
+                    }
+                    if constexpr (Cfg::BIAS_MMA) {
+                        // + shift: rows x (1, 1, 0, ...) times (hi, lo, 0, ...)^T of the layer's shifts
+                        const uint64_t ab = desc_nosw(smem_u32(Abias), TILE_ROWS * 16, 128);
+                        const uint64_t wb = desc_nosw(w_addr + 2 * KB * Cfg::CHUNK_BYTES + layer * Cfg::WB_BYTES, Cfg::NRB * 16, 128);
+                        // (transposed layer 3: the shift is one scalar per thread there, added in E3; the extra MMA costs more)
+                        if (!(TR3 && layer == 1)) mma_bf16_ss_g<PAIR>(tmem + layer * C, ab, wb, idesc, 1u);
                     }
                     mma_commit_g<PAIR>(&d_full[layer]);
                 }
@@ -443,6 +465,11 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
 #pragma unroll
                     for (int i = 0; i < 8; ++i) {
                         float4 sh = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+                        if constexpr (Cfg::BIAS_MMA) {
+                            pk[2 * i] = pack_relu_bf16x2(v[4 * i], v[4 * i + 1]);
+                            pk[2 * i + 1] = pack_relu_bf16x2(v[4 * i + 2], v[4 * i + 3]);
+                            continue;
+                        }
                         if constexpr (!Cfg::BIAS_ACC) sh = *reinterpret_cast<const float4*>(t2 + s * 32 + 4 * i);
                         pk[2 * i] = pack_relu_bf16x2(v[4 * i] + sh.x, v[4 * i + 1] + sh.y);
                         pk[2 * i + 1] = pack_relu_bf16x2(v[4 * i + 2] + sh.z, v[4 * i + 3] + sh.w);
@@ -552,6 +579,11 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
 #pragma unroll
                     for (int i = 0; i < 8; ++i) {
                         float4 sh = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+                        if constexpr (Cfg::BIAS_MMA) {
+                            w[2 * i] = pack_relu_f16x2(v[4 * i], v[4 * i + 1]);
+                            w[2 * i + 1] = pack_relu_f16x2(v[4 * i + 2], v[4 * i + 3]);
+                            continue;
+                        }
                         if constexpr (!Cfg::BIAS_ACC) sh = *reinterpret_cast<const float4*>(t3 + s * 32 + 4 * i);
                         w[2 * i] = pack_relu_f16x2(v[4 * i] + sh.x, v[4 * i + 1] + sh.y);
                         w[2 * i + 1] = pack_relu_f16x2(v[4 * i + 2] + sh.z, v[4 * i + 3] + sh.w);
@@ -943,44 +975,55 @@ __global__ void __launch_bounds__(PRE_THREADS) pre_kernel(PreParams p) {
     if (p.dep == DEP_SECONDARY && blockIdx.x == 0) grid_dep_wait();
 }
 
-// Narrow inputs (block 1: C_in = F <= 16): thread (x = column quad, y) computes four output columns of PRS_ROWS consecutive
-// particles; the rows and the weight column quad come straight from L1 / L2 (a CTA shares 16 rows and the 5 KB weight matrix),
-// no staging, no barrier.
-constexpr int PRS_ROWS = 4;      // rows per thread
+// Narrow inputs (block 1: C_in = F <= 16): thread (x = column quad, y = row group) keeps its weight column quad in registers and
+// computes four output columns of PRS_ROWS consecutive particles; the CTA's rows are staged in shared memory and read as
+// broadcasts (round 1 read x and the weights from L1 per 4 rows: 4.6 warp instructions per FMA instruction).
+constexpr int PRS_ROWS = 16;     // rows per thread
 constexpr int PRS_TY = 4;        // blockDim.y
 
 template <int KP>
 __device__ __forceinline__ void pre_small_body(const PreParams& p) {
+    __shared__ __align__(16) float xs[PRS_TY * PRS_ROWS][KP];    // the CTA's rows, zero-padded to KP columns
     if (p.meta[0]) return;
     const int N = p.meta[1];
+    const int cta_row0 = blockIdx.x * (PRS_TY * PRS_ROWS);
+    if (cta_row0 >= N) return;
     const int cg = threadIdx.x;                                  // blockDim.x = NC / 4
-    const int row0 = (blockIdx.x * PRS_TY + threadIdx.y) * PRS_ROWS;
-    if (row0 >= N) return;
+    const int tid = threadIdx.y * blockDim.x + threadIdx.x, nthr = blockDim.x * blockDim.y;
+    const int rows_here = min(PRS_TY * PRS_ROWS, N - cta_row0);
+    for (int e = tid; e < PRS_TY * PRS_ROWS * KP; e += nthr) {
+        const int r = e / KP, c = e - r * KP;
+        xs[r][c] = (r < rows_here && c < p.cin) ? __ldg(p.x + (size_t)(cta_row0 + r) * p.cin + c) : 0.0f;
+    }
     float4 w[KP];
     const float* w0 = p.Wt + cg * 4;
 #pragma unroll
     for (int kk = 0; kk < KP; ++kk) w[kk] = kk < p.cin ? __ldg(reinterpret_cast<const float4*>(w0 + (size_t)kk * p.NC)) : make_float4(0.0f, 0.0f, 0.0f, 0.0f);
     const float4 b = __ldg(reinterpret_cast<const float4*>(p.bias + cg * 4));
     const int col = cg * 4;
-#pragma unroll
+    __syncthreads();
+    // a warp is 32 column quads of ONE row group: its x reads are broadcasts
+#pragma unroll 4
     for (int r = 0; r < PRS_ROWS; ++r) {
-        const int row = row0 + r;
-        if (row >= N) break;
-        float4 acc = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+        const int rl = threadIdx.y * PRS_ROWS + r;
+        if (rl >= rows_here) break;
+        const int row = cta_row0 + rl;
+        float4 acc = b;
 #pragma unroll
-        for (int kk = 0; kk < KP; ++kk) {
-            if (kk < p.cin) {
-                const float x = __ldg(p.x + (size_t)row * p.cin + kk);
-                acc.x = fmaf(x, w[kk].x, acc.x); acc.y = fmaf(x, w[kk].y, acc.y);
-                acc.z = fmaf(x, w[kk].z, acc.z); acc.w = fmaf(x, w[kk].w, acc.w);
+        for (int k4 = 0; k4 < KP; k4 += 4) {
+            const float4 xv = *reinterpret_cast<const float4*>(&xs[rl][k4]);
+            const float xa[4] = {xv.x, xv.y, xv.z, xv.w};
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                acc.x = fmaf(xa[u], w[k4 + u].x, acc.x); acc.y = fmaf(xa[u], w[k4 + u].y, acc.y);
+                acc.z = fmaf(xa[u], w[k4 + u].z, acc.z); acc.w = fmaf(xa[u], w[k4 + u].w, acc.w);
             }
         }
-        const float o0 = acc.x + b.x, o1 = acc.y + b.y, o2 = acc.z + b.z, o3 = acc.w + b.w;
         if (col < 2 * p.C1) {
             __nv_bfloat16* dst = (col < p.C1) ? p.U + (size_t)row * p.C1 + col : p.V + (size_t)row * p.C1 + (col - p.C1);
-            *reinterpret_cast<uint2*>(dst) = make_uint2(pack_bf16x2(o0, o1), pack_bf16x2(o2, o3));
+            *reinterpret_cast<uint2*>(dst) = make_uint2(pack_bf16x2(acc.x, acc.y), pack_bf16x2(acc.z, acc.w));
         } else {
-            *reinterpret_cast<uint2*>(p.R + (size_t)row * p.C3 + (col - 2 * p.C1)) = make_uint2(pack_f16x2(o0, o1), pack_f16x2(o2, o3));
+            *reinterpret_cast<uint2*>(p.R + (size_t)row * p.C3 + (col - 2 * p.C1)) = make_uint2(pack_f16x2(acc.x, acc.y), pack_f16x2(acc.z, acc.w));
         }
     }
 }
@@ -1395,6 +1438,21 @@ int edgeconv_bf16_prepare(gnn_model& m, const float* blob) {
             for (int r = 0; r < nranks; ++r) {
                 pack_layer(W2f, C, NRB, r * NRB, img);
                 pack_layer(W3f, C, NRB, r * NRB, img);
+                // bias operands of the two layers (EdgeCfg::BIAS_MMA): [K chunk][row group][row in group][16 B], no swizzle; K
+                // column 0 = bf16 hi part of the shift, column 1 = bf16 of the remainder
+                for (int layer = 0; layer < 2 && C != 128; ++layer) {       // (EdgeCfg<128>::BIAS_MMA is off)
+                    const size_t base = img.size();
+                    img.resize(base + (size_t)NRB * 32, 0);
+                    for (int nl = 0; nl < NRB; ++nl) {
+                        const float t = sh[(size_t)layer * C + r * NRB + nl];
+                        const uint16_t hi = f32_to_bf16_rne(t);
+                        uint32_t hb = (uint32_t)hi << 16; float hf; std::memcpy(&hf, &hb, 4);
+                        const uint16_t lo = f32_to_bf16_rne(t - hf);
+                        const size_t off = base + (size_t)(nl >> 3) * 128 + (size_t)(nl & 7) * 16;
+                        std::memcpy(&img[off], &hi, 2);
+                        std::memcpy(&img[off + 2], &lo, 2);
+                    }
+                }
             }
         }
         int rc;

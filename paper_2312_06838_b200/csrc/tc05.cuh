@@ -89,6 +89,16 @@ __device__ __forceinline__ uint64_t desc_sw128(uint32_t saddr) {
     d |= (uint64_t)2 << 61;
     return d;
 }
+// K-major operand WITHOUT swizzle (canonical "interleave" layout, in 16-byte units ((8, n), 2) : ((1, SBO), LBO)): 8 rows x 16
+// bytes form a contiguous 128-byte core matrix; `sbo` = byte distance between 8-row groups, `lbo` = byte distance between
+// the two 16-byte K chunks of a K step.  Layout type 0; 16-byte aligned.
+__device__ __forceinline__ uint64_t desc_nosw(uint32_t saddr, uint32_t lbo, uint32_t sbo) {
+    uint64_t d = (uint64_t)((saddr & 0x3FFFFu) >> 4);
+    d |= (uint64_t)(lbo >> 4) << 16;
+    d |= (uint64_t)(sbo >> 4) << 32;
+    d |= (uint64_t)1 << 46;
+    return d;
+}
 // Instruction descriptor, kind::f16: D fp32 (bits [4,6) = 1), A and B bf16 ([7,10) = [10,13) = 1), both K-major
 // (bits 15, 16 = 0), N >> 3 at [17,23), M >> 4 at [24,29).
 __host__ __device__ constexpr uint32_t idesc_bf16_f32(int M, int N) {
