@@ -1259,6 +1259,193 @@ __global__ void __maxnreg__(80) pre_tc_kernel(PreTcParams p) {
     if (warp == PTC_MMA_WARP) tmem_dealloc(tmem, Cfg::TMEM_COLS);
 }
 
+// ---- the same GEMM for wide inputs (CIN = 256 -> 3 x 512: block 3 of the configs[4] wide variant) -------------------------------
+// A weight slice of the kernel above would be 256 KB there, so the 3C output columns are cut into slices of NS = 256 columns
+// (six for C = 512; a slice never straddles u / v / r), [NS][CIN] fp16 = 128 KB resident per CTA, and the operand tile is
+// another 64 KB: no room for a raw staging buffer, so the converter warps load x straight from global memory (eight 16-byte
+// loads in flight per thread), convert and store.  One accumulator per N half of the slice, as above.
+// Warps: 0-3 epilogue, 4-11 converters, 12 MMA issuer + TMEM owner.
+constexpr int PTB_EPI_WARPS = 4;
+constexpr int PTB_CVT_WARPS = 8;
+constexpr int PTB_MMA_WARP = PTB_EPI_WARPS + PTB_CVT_WARPS;
+constexpr int PTB_THREADS = 32 * (PTB_MMA_WARP + 1);
+
+template <int CIN, int C, int NS>
+struct PreBigCfg {
+    static constexpr int KBA = CIN / 64;
+    static constexpr int AK_BYTES = TILE_ROWS * 128;
+    static constexpr int A_BYTES = KBA * AK_BYTES;
+    static constexpr int WK_BYTES = NS * 128;                 // [NS][64] fp16 chunk
+    static constexpr int W_BYTES = KBA * WK_BYTES;            // one slice
+    static constexpr int NSL = 3 * C / NS;                    // slices
+    static constexpr int NH = NS / 2;
+    static constexpr int TMEM_COLS = NS;
+    static constexpr int NBAR = 8;
+    static constexpr int STAGE_BYTES = PTB_EPI_WARPS * 2048;
+    static constexpr int SMEM_BYTES = W_BYTES + A_BYTES + STAGE_BYTES + NS * 4 + NBAR * 8 + 16;
+};
+
+template <int CIN, int C, int NS>
+__global__ void __maxnreg__(80) pre_tc_big_kernel(PreTcParams p) {
+    using Cfg = PreBigCfg<CIN, C, NS>;
+    constexpr int KBA = Cfg::KBA, NH = Cfg::NH, NSL = Cfg::NSL;
+    extern __shared__ __align__(1024) uint8_t smem_raw[];
+    const int slice = blockIdx.x % NSL, gi = blockIdx.x / NSL, ng = gridDim.x / NSL;
+    uint8_t* smem = smem_raw;                                    // keeps the shared address space (see edge_kernel)
+    if ((smem_u32(smem) & 1023u) != 0u) __trap();
+    uint8_t* Wsm = smem;
+    uint8_t* A = Wsm + Cfg::W_BYTES;
+    uint8_t* stage = A + Cfg::A_BYTES;
+    float* bias_s = reinterpret_cast<float*>(stage + Cfg::STAGE_BYTES);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(bias_s + NS);
+    uint64_t* a_ready = bars;                 // converters -> MMA: operand tile written
+    uint64_t* a_free = bars + 1;              // MMA -> converters: the operand tile has been read
+    uint64_t* d_full = bars + 2;              // [2] accumulator of N half h complete
+    uint64_t* d_free = bars + 4;              // [2] ... drained
+    uint64_t* w_full = bars + 6;
+    uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(bars + Cfg::NBAR);
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    if (tid == 0) {
+        mbar_init(a_ready, PTB_CVT_WARPS);
+        mbar_init(a_free, 1);
+        for (int i = 0; i < 2; ++i) { mbar_init(&d_full[i], 1); mbar_init(&d_free[i], PTB_EPI_WARPS); }
+        mbar_init(w_full, 1);
+        fence_mbar_init();
+    }
+    for (int i = tid; i < NS; i += PTB_THREADS) bias_s[i] = p.bias[slice * NS + i];
+    if (warp == PTB_MMA_WARP) tmem_alloc(tmem_ptr, Cfg::TMEM_COLS);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = *tmem_ptr;
+    if (warp == PTB_MMA_WARP && lane == 0) {
+        mbar_arrive_expect_tx(w_full, Cfg::W_BYTES);
+        const uint8_t* src = p.wimg + (size_t)slice * Cfg::W_BYTES;
+        for (int c = 0; c < KBA; ++c)
+            bulk_g2s(Wsm + (size_t)c * Cfg::WK_BYTES, src + (size_t)c * Cfg::WK_BYTES, Cfg::WK_BYTES, w_full);
+    }
+    grid_dep_wait();                          // x and meta come from the kernels before this one
+    grid_dep_launch();
+    const int N = p.meta[0] ? 0 : p.meta[1];
+    const int n_tiles = min(p.n_tiles, (N + TILE_ROWS - 1) / TILE_ROWS);
+    const int T = gi < n_tiles ? (n_tiles - gi + ng - 1) / ng : 0;
+
+    if (warp == PTB_MMA_WARP) {
+        if (lane == 0) {
+            constexpr uint32_t idesc = idesc_f16_f32(128, NH);
+            const uint32_t a_addr = smem_u32(A), w_addr = smem_u32(Wsm);
+            mbar_wait(w_full, 0);
+            for (int t = 0; t < T; ++t) {
+                mbar_wait(a_ready, t & 1);
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    mbar_wait(&d_free[h], (t & 1) ^ 1);
+                    tc_fence_after();
+#pragma unroll
+                    for (int kb = 0; kb < KBA; ++kb)
+#pragma unroll
+                        for (int ks = 0; ks < 4; ++ks) {
+                            const uint64_t ad = desc_sw128(a_addr + kb * Cfg::AK_BYTES + ks * 32);
+                            const uint64_t bd = desc_sw128(w_addr + kb * Cfg::WK_BYTES + h * (NH * 128) + ks * 32);
+                            mma_bf16_ss(tmem + h * NH, ad, bd, idesc, (kb | ks) != 0);   // kind::f16; the descriptor says fp16
+                        }
+                    if (h == 1) mma_commit(a_free);
+                    mma_commit(&d_full[h]);
+                }
+            }
+        }
+    } else if (warp >= PTB_EPI_WARPS) {
+        // ===== converters: x rows from global memory -> fp16, 128B-swizzled K blocks; item = 8 columns of a row ===============
+        const int ct = tid - PTB_EPI_WARPS * 32;
+        constexpr int IPR = CIN / 8;                             // items per row
+        constexpr int NCT = PTB_CVT_WARPS * 32;
+        constexpr int ITEMS = TILE_ROWS * IPR / NCT;
+        constexpr int BATCH = 4;
+        for (int t = 0; t < T; ++t) {
+            const int r0 = (gi + t * ng) * TILE_ROWS;
+#pragma unroll 1
+            for (int i0 = 0; i0 < ITEMS; i0 += BATCH) {
+                float4 a[BATCH], b[BATCH];
+#pragma unroll
+                for (int u = 0; u < BATCH; ++u) {
+                    const int e = ct + (i0 + u) * NCT;
+                    const int r = e / IPR, c = e % IPR;
+                    a[u] = make_float4(0.0f, 0.0f, 0.0f, 0.0f); b[u] = a[u];
+                    if (r0 + r < N) {
+                        const float4* xp = reinterpret_cast<const float4*>(p.x + (size_t)(r0 + r) * CIN + 8 * c);
+                        a[u] = __ldg(xp); b[u] = __ldg(xp + 1);
+                    }
+                }
+                if (i0 == 0 && t > 0) mbar_wait(a_free, (t - 1) & 1);
+#pragma unroll
+                for (int u = 0; u < BATCH; ++u) {
+                    const int e = ct + (i0 + u) * NCT;
+                    const int r = e / IPR, c = e % IPR;
+                    const uint4 o = make_uint4(pack_f16x2(a[u].x, a[u].y), pack_f16x2(a[u].z, a[u].w), pack_f16x2(b[u].x, b[u].y), pack_f16x2(b[u].z, b[u].w));
+                    *reinterpret_cast<uint4*>(A + (c >> 3) * Cfg::AK_BYTES + r * 128 + (((c & 7) ^ (r & 7)) << 4)) = o;
+                }
+            }
+            fence_proxy_async();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(a_ready);
+        }
+    } else {
+        // ===== epilogue: thread = row = TMEM lane; columns [slice * NS, + NS) of [u | v | r] ===================================
+        const int q = warp;
+        const int gcol0 = slice * NS, which = gcol0 / C, ccol0 = gcol0 % C;
+        uint16_t* outp = reinterpret_cast<uint16_t*>(which == 0 ? (void*)p.U : (which == 1 ? (void*)p.V : (void*)p.R));
+        uint8_t* st = stage + warp * 2048;
+        for (int t = 0; t < T; ++t) {
+            const int tr0 = (gi + t * ng) * TILE_ROWS + 32 * q;
+#pragma unroll 1
+            for (int h = 0; h < 2; ++h) {
+                mbar_wait(&d_full[h], t & 1);
+                tc_fence_after();
+#pragma unroll 1
+                for (int s = 0; s < NH / 32; ++s) {
+                    const int col = h * NH + s * 32;
+                    float v[32];
+                    tmem_ld32(tmem + ((uint32_t)(32 * q) << 16) + col, v);
+                    tmem_ld_wait();
+                    if (s == NH / 32 - 1) {
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(&d_free[h]);
+                    }
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        const float4 b = *reinterpret_cast<const float4*>(bias_s + col + 4 * i);
+                        v[4 * i] += b.x; v[4 * i + 1] += b.y; v[4 * i + 2] += b.z; v[4 * i + 3] += b.w;
+                    }
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        uint4 o;
+                        if (which == 2)
+                            o = make_uint4(pack_f16x2(v[8 * i], v[8 * i + 1]), pack_f16x2(v[8 * i + 2], v[8 * i + 3]),
+                                           pack_f16x2(v[8 * i + 4], v[8 * i + 5]), pack_f16x2(v[8 * i + 6], v[8 * i + 7]));
+                        else
+                            o = make_uint4(pack_bf16x2(v[8 * i], v[8 * i + 1]), pack_bf16x2(v[8 * i + 2], v[8 * i + 3]),
+                                           pack_bf16x2(v[8 * i + 4], v[8 * i + 5]), pack_bf16x2(v[8 * i + 6], v[8 * i + 7]));
+                        *reinterpret_cast<uint4*>(st + lane * 64 + ((i ^ ((lane >> 1) & 3)) << 4)) = o;
+                    }
+                    __syncwarp();
+#pragma unroll
+                    for (int it = 0; it < 4; ++it) {
+                        const int r = it * 8 + (lane >> 2), c = lane & 3;
+                        const uint4 o = *reinterpret_cast<const uint4*>(st + r * 64 + ((c ^ ((r >> 1) & 3)) << 4));
+                        if (tr0 + r < N) *(reinterpret_cast<uint4*>(outp + (size_t)(tr0 + r) * C + ccol0 + col) + c) = o;
+                    }
+                    __syncwarp();
+                }
+            }
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == PTB_MMA_WARP) tmem_dealloc(tmem, Cfg::TMEM_COLS);
+}
+
 // ---- host side: weight packing and launch -----------------------------------------------------------------------------
 struct Bf16BlockDev {
     const uint8_t* wimg = nullptr;
@@ -1459,6 +1646,23 @@ int edgeconv_bf16_prepare(gnn_model& m, const float* blob) {
         if ((rc = upload(m, Wt, &b.pre_Wt)) != GNN_OK || (rc = upload(m, bias, &b.pre_bias)) != GNN_OK ||
             (rc = upload(m, img, &b.wimg)) != GNN_OK || (rc = upload(m, sh, &b.shifts)) != GNN_OK)
             return rc;
+        if (cin == 256 && C == 512) {
+            // pre_tc_big_kernel: six slices of 256 output columns, per slice and K block of 64: [256][64] fp16, 128B-swizzled
+            constexpr int NS = 256;
+            std::vector<uint8_t> pimg((size_t)3 * C * cin * 2, 0);
+            size_t base = 0;
+            for (int sl = 0; sl < 3 * C / NS; ++sl)
+                for (int kb = 0; kb < cin / 64; ++kb, base += (size_t)NS * 128)
+                    for (int nl = 0; nl < NS; ++nl)
+                        for (int kk = 0; kk < 64; ++kk) {
+                            const __half h = __float2half_rn(Wt[(size_t)(kb * 64 + kk) * b.NC + sl * NS + nl]);
+                            const size_t off = base + (size_t)nl * 128 + (size_t)(((kk >> 3) ^ (nl & 7)) << 4) + (kk & 7) * 2;
+                            std::memcpy(&pimg[off], &h, 2);
+                        }
+            if ((rc = upload(m, pimg, &b.pre_wimg)) != GNN_OK) return rc;
+            GNN_CUDA_TRY(cudaFuncSetAttribute(pre_tc_big_kernel<256, 512, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, PreBigCfg<256, 512, 256>::SMEM_BYTES));
+            b.pre_ctas_per_sm = 1;
+        }
         if ((cin == 64 && C == 128) || (cin == 128 && C == 256)) {
             // tensor-core pre kernel: per slice of C output columns (u, v, r) and K block of 64: [C][64] fp16 (RNE), 128B-swizzled
             std::vector<uint8_t> pimg((size_t)3 * C * cin * 2, 0);
@@ -1531,6 +1735,12 @@ int launch_pre_bf16(gnn_model& m, int block, const float* x, int N, Workspace& w
         PreTcParams tp;
         tp.x = x; tp.wimg = b.pre_wimg; tp.bias = b.pre_bias; tp.U = sc.U; tp.V = sc.V; tp.R = sc.R; tp.meta = w.meta;
         tp.n_tiles = (N + TILE_ROWS - 1) / TILE_ROWS;
+        if (b.C == 512) {
+            constexpr int NSL = PreBigCfg<256, 512, 256>::NSL;
+            const int gridb = NSL * std::min(tp.n_tiles, std::max(1, m.n_sms / NSL));
+            GNN_CUDA_TRY(launch_k(pre_tc_big_kernel<256, 512, 256>, dim3(gridb), dim3(PTB_THREADS), PreBigCfg<256, 512, 256>::SMEM_BYTES, s, pdl, tp));
+            return 1;
+        }
         const int grid = 3 * std::min(tp.n_tiles, std::max(1, m.n_sms * b.pre_ctas_per_sm / 3));
         if (b.C == 128) GNN_CUDA_TRY(launch_k(pre_tc_kernel<64, 128>, dim3(grid), dim3(PTC_THREADS), PreTcCfg<64, 128>::SMEM_BYTES, s, pdl, tp));
         else GNN_CUDA_TRY(launch_k(pre_tc_kernel<128, 256>, dim3(grid), dim3(PTC_THREADS), PreTcCfg<128, 256>::SMEM_BYTES, s, pdl, tp));

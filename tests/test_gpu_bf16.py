@@ -184,6 +184,20 @@ def test_sweep_wide_256_sampled():
     m.close()
 
 
+def test_sweep_wide_4096_sampled():
+    """configs[4] wide variant at B = 4096 (245 k particles: many tiles per CTA in every kernel, ragged tails); the oracle runs
+    the first 32 jets, compared inside the full batch; nested batch sizes give the same jets bit for bit."""
+    a, w, m = bf16_model("wide", 4096)
+    b = synth.make_sweep_batch(n_jets=4096)
+    lg = run_ragged(m, b)
+    assert m.status_check() == 0 and np.isfinite(lg).all()
+    h = b.head(32)
+    ref = oracle.forward(a, w, h.feats, h.coords, h.offsets)
+    check_logits(lg[:32], ref)
+    assert np.array_equal(run_ragged(m, b.head(16)), lg[:16])
+    m.close()
+
+
 def test_edge_case_set(pn):
     a, w, m = pn
     b = synth.make_edge_case_batch(a.in_features)
