@@ -9,7 +9,8 @@
 //   pre kernel   per particle: u_i, v_i (stored bf16) and the shortcut r_i = ss*(Ws x_i) + ts (fp32).
 //   edge_kernel  persistent; per tile of 128 edge rows (128/k particles x k neighbours), all on chip:
 //     build   H1[r] = bf16(relu(u_i + v_j))  gathered straight into the 128B-swizzled K-major operand tile in smem
-//     MMA2    D0 = H1 * W2'^T   (tcgen05.mma kind::f16, N = C, bf16 x bf16 -> fp32 in TMEM; W2' = s2*W2)
+//     MMA2    D0 = H1 * W2'^T + t2   (tcgen05.mma kind::f16, N = C, bf16 x bf16 -> fp32 in TMEM; W2' = s2*W2; the shift through
+//             one extra K step against a constant ones tile, EdgeCfg::BIAS_MMA)
 //     E2      H2 = bf16(relu(D0 + t2))  TMEM -> registers -> the same operand tile (H1 is dead by then)
 //     MMA3    D1 = H2 * W3'^T
 //     E3      relu(D1 + t3), mean over the k_eff valid neighbour rows of each particle by a halving butterfly of
@@ -95,9 +96,8 @@ struct EdgeCfg {
     static constexpr int SMEM_BYTES_POOL = SMEM_BYTES + POOL_BYTES;
     static constexpr int MIN_CTAS = C >= 256 ? 1 : (C >= 128 ? 2 : 4);
     static constexpr int NRANKS = PAIR ? 2 : 1;
-    // shift pre-loaded into the accumulators (tcgen05.st by the epilogue that drains them) or added in the epilogues: the
-    // re-arm costs ~0.9 k cycles on the epilogue warps' chain and delays d_free; measured slower for every C (10 % at C <= 128)
-    static constexpr bool BIAS_ACC = false;
+    // (pre-loading the shift into the accumulators with tcgen05.st by the epilogue that drains them was measured 10 % slower: the
+    // re-arm sits on the epilogue warps' chain and delays d_free; BIAS_MMA above has no such cost)
 };
 
 // y >= 0 (post-ReLU) -> unsigned 32.32 fixed point, EXACT for y < 2^32 whose ulp is >= 2^-32 (y >= 2^-8; below that the
@@ -240,7 +240,7 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
                         for (int ks = 0; ks < ksteps; ++ks) {
                             const uint64_t hd = desc_sw128(h_addr + kb * Cfg::HK_BYTES + ks * 32);
                             const uint64_t wd = desc_sw128(w_addr + (layer * KB + kb) * Cfg::CHUNK_BYTES + ks * 32);
-                            const uint32_t acc = Cfg::BIAS_ACC ? 1u : (uint32_t)((kb | ks) != 0);
+                            const uint32_t acc = (uint32_t)((kb | ks) != 0);
                             if (TR3 && layer == 1) {
                                 // D1[channel, edge]: weights are the M operand; pair mode: N = 256 = the 128 edge rows of each CTA
                                 mma_bf16_ss_g<PAIR>(tmem + C, wd, hd, idesc_tr, acc);
@@ -369,23 +369,8 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
             const int pt = p0 + (row >> logk);
             return (pt < N) ? __ldg(p.idx + (size_t)pt * k + (row & (k - 1))) : -1;
         };
-        // The accumulators are never zeroed: the epilogue that drains one writes the layer's shift back into it (tcgen05.st,
-        // one instruction per 32 columns), so every MMA accumulates and the epilogues need no bias add.
+        // an accumulator is handed back to the MMA thread as soon as this warp has read it
         auto reset_acc = [&](int layer) {
-            const float* sh = layer ? t3 : t2;
-            if constexpr (Cfg::BIAS_ACC) {
-#pragma unroll
-            for (int s = 0; s < SLABS; ++s) {
-                float w[32];
-#pragma unroll
-                for (int i = 0; i < 8; ++i) {
-                    const float4 f = *reinterpret_cast<const float4*>(sh + s * 32 + 4 * i);
-                    w[4 * i] = f.x; w[4 * i + 1] = f.y; w[4 * i + 2] = f.z; w[4 * i + 3] = f.w;
-                }
-                tmem_st32(tbase + layer * C + s * 32, w);
-            }
-            tmem_st_wait();
-            }
             tc_fence_before();
             arrive_leader(&d_free[layer]);
         };
@@ -470,7 +455,7 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
                             pk[2 * i + 1] = pack_relu_bf16x2(v[4 * i + 2], v[4 * i + 3]);
                             continue;
                         }
-                        if constexpr (!Cfg::BIAS_ACC) sh = *reinterpret_cast<const float4*>(t2 + s * 32 + 4 * i);
+                        sh = *reinterpret_cast<const float4*>(t2 + s * 32 + 4 * i);
                         pk[2 * i] = pack_relu_bf16x2(v[4 * i] + sh.x, v[4 * i + 1] + sh.y);
                         pk[2 * i + 1] = pack_relu_bf16x2(v[4 * i + 2] + sh.z, v[4 * i + 3] + sh.w);
                     }
@@ -584,7 +569,7 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
                             w[2 * i + 1] = pack_relu_f16x2(v[4 * i + 2], v[4 * i + 3]);
                             continue;
                         }
-                        if constexpr (!Cfg::BIAS_ACC) sh = *reinterpret_cast<const float4*>(t3 + s * 32 + 4 * i);
+                        sh = *reinterpret_cast<const float4*>(t3 + s * 32 + 4 * i);
                         w[2 * i] = pack_relu_f16x2(v[4 * i] + sh.x, v[4 * i + 1] + sh.y);
                         w[2 * i + 1] = pack_relu_f16x2(v[4 * i + 2] + sh.z, v[4 * i + 3] + sh.w);
                     }
