@@ -137,6 +137,15 @@ int gnn_softmax(const float* logits_dev, int32_t B, int32_t n_classes, float* pr
 int gnn_infer_host(gnn_model* m, int32_t slice, const float* feats_host, const float* coords_host,
                    const int32_t* offsets_host, int32_t B, int32_t N, float* logits_host, void* cuda_stream);
 
+/* The two halves of gnn_infer_host, for callers that keep several slices in flight: _begin enqueues the copies and the
+ * forward on `cuda_stream` and returns at once (host buffers must be pinned for the copies to be asynchronous, and must stay
+ * valid until _end); _end synchronises `cuda_stream`, after which logits_host is valid, and returns device-side errors.  With
+ * two slices on two streams the host -> device copy of one batch runs under the forward of the other (bench.py's e2e leg).
+ * One _begin per slice at a time. */
+int gnn_infer_host_begin(gnn_model* m, int32_t slice, const float* feats_host, const float* coords_host,
+                         const int32_t* offsets_host, int32_t B, int32_t N, float* logits_host, void* cuda_stream);
+int gnn_infer_host_end(gnn_model* m, int32_t slice, void* cuda_stream);
+
 const char* gnn_strerror(int status);
 /* number of kernels the library has launched on this model since gnn_create (bench.py's gpu_launches) */
 int64_t gnn_launch_count(const gnn_model* m);

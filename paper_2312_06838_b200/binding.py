@@ -69,6 +69,8 @@ def lib():
         L.gnn_infer_channel_first.argtypes = [vp, i32, f32p, f32p, f32p, i32, i32, i32, f32p, vp]
         L.gnn_softmax.argtypes = [f32p, i32, i32, f32p, vp]
         L.gnn_infer_host.argtypes = [vp, i32, vp, vp, vp, i32, i32, vp, vp]
+        L.gnn_infer_host_begin.argtypes = [vp, i32, vp, vp, vp, i32, i32, vp, vp]
+        L.gnn_infer_host_end.argtypes = [vp, i32, vp]
         L.gnn_profile_enable.argtypes = [vp, i32, i32]
         L.gnn_profile_read.argtypes = [vp, i32, i32, C.POINTER(C.c_float), C.POINTER(i32), C.POINTER(i32)]
         L.gnn_profile_stage_name.argtypes = [vp, i32, i32]; L.gnn_profile_stage_name.restype = C.c_char_p
@@ -201,6 +203,15 @@ class Model:
         self._check(lib().gnn_infer_host(self.h, slice, _hptr(feats), _hptr(coords), _hptr(offsets), B, N,
                                          _hptr(logits), _stream(stream)), "gnn_infer_host")
         return logits
+
+    def infer_host_begin(self, feats, coords, offsets, logits, stream=None, slice=0):
+        """gnn_infer_host_begin: enqueue copies + forward on `stream`; gnn_infer_host_end(slice) collects (pinned host tensors)."""
+        B, N = int(offsets.shape[0]) - 1, int(feats.shape[0])
+        self._check(lib().gnn_infer_host_begin(self.h, slice, _hptr(feats), _hptr(coords), _hptr(offsets), B, N,
+                                               _hptr(logits), _stream(stream)), "gnn_infer_host_begin")
+
+    def infer_host_end(self, stream=None, slice=0):
+        self._check(lib().gnn_infer_host_end(self.h, slice, _stream(stream)), "gnn_infer_host_end")
 
     def profile_enable(self, on=True, slice=0):
         self._check(lib().gnn_profile_enable(self.h, slice, 1 if on else 0), "gnn_profile_enable")

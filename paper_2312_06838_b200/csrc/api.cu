@@ -150,6 +150,8 @@ int alloc_workspace(gnn_model* m, Workspace& w) {
     if ((rc = dev_alloc(m, &w.pcounts, Bmax)) != GNN_OK) return rc;
     if ((rc = dev_alloc(m, &w.hlogits, Bmax * a.n_classes)) != GNN_OK) return rc;
     GNN_CUDA_TRY(cudaMemset(w.pool, 0, Bmax * (size_t)a.channels[a.n_blocks - 1][2] * sizeof(unsigned long long)));
+    GNN_CUDA_TRY(cudaMallocHost(reinterpret_cast<void**>(&w.h_status), sizeof(unsigned)));
+    *w.h_status = 0u;
     GNN_CUDA_TRY(cudaMemset(w.status, 0, sizeof(unsigned)));
     GNN_CUDA_TRY(cudaMemset(w.meta, 0, 4 * sizeof(int32_t)));
     return GNN_OK;
@@ -377,6 +379,7 @@ void gnn_destroy(gnn_model* m) {
     edgeconv_bf16_release(*m);
     for (auto& w : m->ws) {
         for (auto& g : w.graphs) if (g.exec) cudaGraphExecDestroy(g.exec);
+        if (w.h_status) cudaFreeHost(w.h_status);
         for (cudaEvent_t e : w.prof_events) cudaEventDestroy(e);
     }
     delete m;
@@ -453,16 +456,17 @@ int gnn_infer_padded(gnn_model* m, const float* feats_dev, const float* coords_d
     return gnn_infer_padded_slice(m, 0, feats_dev, coords_dev, mask_dev, B, P, logits_dev, cuda_stream);
 }
 
-int gnn_infer_host(gnn_model* m, int32_t slice, const float* feats_host, const float* coords_host,
-                   const int32_t* offsets_host, int32_t B, int32_t N, float* logits_host, void* cuda_stream) {
+int gnn_infer_host_begin(gnn_model* m, int32_t slice, const float* feats_host, const float* coords_host,
+                         const int32_t* offsets_host, int32_t B, int32_t N, float* logits_host, void* cuda_stream) {
     if (!m) return GNN_ERR_NULL;
     if (B < 0 || N < 0) return GNN_ERR_BAD_ARG;
     if (slice < 0 || slice >= (int)m->ws.size()) return GNN_ERR_BATCH_TOO_LARGE;
     if (B > m->arch.max_batch_jets || (int64_t)N > m->Nmax) return GNN_ERR_BATCH_TOO_LARGE;
+    Workspace& w = m->ws[slice];
+    w.host_pending = false;
     if (B == 0) return GNN_OK;
     if (!offsets_host || !logits_host || (N > 0 && (!feats_host || !coords_host))) return GNN_ERR_NULL;
     const gnn_arch& a = m->arch;
-    Workspace& w = m->ws[slice];
     cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
     if (N > 0) {
         GNN_CUDA_TRY(cudaMemcpyAsync(w.pfeats, feats_host, (size_t)N * a.in_features * sizeof(float), cudaMemcpyHostToDevice, s));
@@ -472,10 +476,21 @@ int gnn_infer_host(gnn_model* m, int32_t slice, const float* feats_host, const f
     int rc = forward(m, w, w.pfeats, w.pcoords, w.poffsets, nullptr, B, N, N, w.hlogits, s);
     if (rc != GNN_OK) return rc;
     GNN_CUDA_TRY(cudaMemcpyAsync(logits_host, w.hlogits, (size_t)B * a.n_classes * sizeof(float), cudaMemcpyDeviceToHost, s));
-    // the sticky status word rides the same stream: one synchronisation per call (gnn_status_check would add a second)
-    unsigned st = 0;
-    GNN_CUDA_TRY(cudaMemcpyAsync(&st, w.status, sizeof(unsigned), cudaMemcpyDeviceToHost, s));
+    // the sticky status word rides the same stream into pinned memory of the slice: gnn_infer_host_end needs one synchronisation
+    GNN_CUDA_TRY(cudaMemcpyAsync(w.h_status, w.status, sizeof(unsigned), cudaMemcpyDeviceToHost, s));
+    w.host_pending = true;
+    return GNN_OK;
+}
+
+int gnn_infer_host_end(gnn_model* m, int32_t slice, void* cuda_stream) {
+    if (!m) return GNN_ERR_NULL;
+    if (slice < 0 || slice >= (int)m->ws.size()) return GNN_ERR_BATCH_TOO_LARGE;
+    Workspace& w = m->ws[slice];
+    if (!w.host_pending) return GNN_OK;                          // nothing in flight (B = 0, or already collected)
+    w.host_pending = false;
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
     GNN_CUDA_TRY(cudaStreamSynchronize(s));
+    const unsigned st = *w.h_status;
     if (st) {
         GNN_CUDA_TRY(cudaMemsetAsync(w.status, 0, sizeof(unsigned), s));
         GNN_CUDA_TRY(cudaStreamSynchronize(s));
@@ -483,6 +498,12 @@ int gnn_infer_host(gnn_model* m, int32_t slice, const float* feats_host, const f
     if (st & GNN_DEV_BAD_OFFSETS) return GNN_ERR_BAD_OFFSETS;
     if (st & GNN_DEV_JET_TOO_LARGE) return GNN_ERR_JET_TOO_LARGE;
     return GNN_OK;
+}
+
+int gnn_infer_host(gnn_model* m, int32_t slice, const float* feats_host, const float* coords_host,
+                   const int32_t* offsets_host, int32_t B, int32_t N, float* logits_host, void* cuda_stream) {
+    const int rc = gnn_infer_host_begin(m, slice, feats_host, coords_host, offsets_host, B, N, logits_host, cuda_stream);
+    return rc != GNN_OK ? rc : gnn_infer_host_end(m, slice, cuda_stream);
 }
 
 int gnn_profile_enable(gnn_model* m, int32_t slice, int32_t on) {

@@ -55,6 +55,8 @@ struct Workspace {
     uint64_t graph_clock = 0;
     bool pool_self_cleaning = false;   // the head kernel of this model clears `pool` after reading it (else forward() does)
     float* hlogits = nullptr;      // [Bmax, n_classes] device staging of gnn_infer_host (inputs stage in pfeats/pcoords/poffsets)
+    unsigned* h_status = nullptr;  // pinned copy of the status word (gnn_infer_host_begin / _end)
+    bool host_pending = false;     // a gnn_infer_host_begin of this slice has not been collected yet
     // stage timing (gnn_profile_*): events of up to PROF_MAX_FORWARDS forwards, (n_stages + 1) per forward
     bool prof_on = false;
     int prof_stages = 0;                       // stages per forward (fixed for a model)

@@ -286,3 +286,34 @@ def test_forward_is_bitwise_repeatable_back_to_back(pn):
             assert torch.equal(out, first[i]), "forward %d (batch %d) differs from its first result" % (it, i)
     torch.cuda.synchronize()
     assert m.status_check() == 0
+
+
+def test_host_entry_pipelined_equals_blocking():
+    """gnn_infer_host_begin / _end with two slices in flight on two streams gives bitwise the logits of the blocking
+    gnn_infer_host and of the device-resident gnn_infer; device-side errors come back from _end."""
+    a = synth.ARCHS["particlenet"]
+    w = synth.make_weights(a)
+    m = make_model(a, w, precision=gnn.BF16, max_batch_jets=256, slices=2, max_particles=100)
+    bs = [synth.make_particlenet_batch(seed=700 + i, n_jets=64 + 32 * i) for i in range(4)]
+    hb = [tuple(torch.from_numpy(x).pin_memory() for x in (b.feats, b.coords, b.offsets)) for b in bs]
+    ref = [run_ragged(m, b).astype(np.float32) for b in bs]
+    outs = [torch.empty((b.n_jets, 2), dtype=torch.float32).pin_memory() for b in bs]
+    st = [torch.cuda.Stream(), torch.cuda.Stream()]
+    for i in range(4):
+        if i >= 2:
+            m.infer_host_end(stream=st[i & 1], slice=i & 1)
+        m.infer_host_begin(*hb[i], outs[i], stream=st[i & 1], slice=i & 1)
+    for sl in range(2):
+        m.infer_host_end(stream=st[sl], slice=sl)
+    for i in range(4):
+        assert np.array_equal(outs[i].numpy(), ref[i])
+        blocking = torch.empty_like(outs[i])
+        m.infer_host(*hb[i], blocking)
+        assert np.array_equal(blocking.numpy(), ref[i])
+    bad = hb[0][2].clone(); bad[3] = bad[5] + 1                 # offsets not monotone
+    m.infer_host_begin(hb[0][0], hb[0][1], bad.pin_memory(), outs[0], stream=st[0], slice=0)
+    with pytest.raises(gnn.GnnError) as e:
+        m.infer_host_end(stream=st[0], slice=0)
+    assert e.value.code == -6                                   # GNN_ERR_BAD_OFFSETS
+    m.infer_host_end(stream=st[0], slice=0)                     # nothing in flight: a no-op
+    m.close()
