@@ -92,10 +92,13 @@ struct EdgeCfg {
     static constexpr int SMALL_BYTES = 2 * C * 4 + NBAR * 8 + 16;
     static constexpr int SMEM_BYTES = W_BYTES + H_BYTES + AB_BYTES + SMALL_BYTES + 1024;
     // POOL variant (last block, k = 16): per epilogue warp and 32-column slab, two 64-bit fixed-point accumulators per lane
-    static constexpr int POOL_BYTES = TR3_OK ? 0 : NE * (CWE / 32) * 32 * 16;   // (TR3 keeps the sums in registers)
+    static constexpr int POOL_BYTES = TR3_OK ? 0 : NE * (CWE / 32) * 32 * 16;   // (TR3 keeps the sums in registers); per E3 worker NSE slabs
     static constexpr int SMEM_BYTES_POOL = SMEM_BYTES + POOL_BYTES;
     static constexpr int MIN_CTAS = C >= 256 ? 1 : (C >= 128 ? 2 : 4);
     static constexpr int NRANKS = PAIR ? 2 : 1;
+    // E3 shared between the epilogue warps and the gather warps (same number of each, row-layout E3): see E3Rows
+    static constexpr bool SPLIT_E3 = !TR3_OK && NG == NE && (CWE / 32) % 2 == 0;
+    static constexpr int NSE = SPLIT_E3 ? CWE / 64 : CWE / 32;     // slabs per E3 worker
     // (pre-loading the shift into the accumulators with tcgen05.st by the epilogue that drains them was measured 10 % slower: the
     // re-arm sits on the epilogue warps' chain and delays d_free; BIAS_MMA above has no such cost)
 };
@@ -123,6 +126,164 @@ struct EdgeParams {
     const float* shifts;         // [t2 | t3]
     int k, logk, TP, n_tiles;
     int chunk;                   // consecutive (pair) tiles a unit takes at a time
+};
+
+// Row-layout E3 of one warp: lane quadrant q (TMEM lanes = edge rows 32 q .. 32 q + 31 of the tile), NSE consecutive 32-column
+// slabs from column col0.  relu(D1) -> f16x2, sum over the k rows of a particle by a halving butterfly of warp shuffles (after
+// step s a lane keeps 8 >> s registers = partial sums over 2^(s+1) rows of 16 >> s columns), x k / k_eff (W3', t3 carry 1 / k),
+// + shortcut, ReLU, then either a coalesced fp32 store or (POOL) the exact fixed-point per-jet sums of step a7.  The worker is
+// run by the epilogue warps and, in the kernels where E3 is split (EdgeCfg::SPLIT_E3), by the gather warps for the other half
+// of the columns: E3 heads the per-tile chain E3 -> E2 -> MMA3 of the epilogue warps, and the gather warps are idle by then.
+template <int C, int LOGK, bool POOL, int NSE, bool BIAS_MMA>
+struct E3Rows {
+    const EdgeParams* p;
+    int N, k, logk, lane, row, col0, cb, nout;
+    unsigned gmask;
+    uint32_t tb;                     // TMEM address of (lane quadrant, D1 column col0)
+    const float* t3;                 // shifts of layer 3 from column col0 (unused with BIAS_MMA)
+    ulonglong2* acc_s;               // POOL: this lane's accumulators, slab s at acc_s[s * 32]
+    int idx_cur, jid_acc, jid_cur;
+
+    __device__ __forceinline__ int load_idx(int p0) const {
+        const int pt = p0 + (row >> logk);
+        return (pt < N) ? __ldg(p->idx + (size_t)pt * k + (row & (k - 1))) : -1;
+    }
+    __device__ __forceinline__ void init(const EdgeParams& pp, int N_, int k_, int logk_, int lane_, int q, int col0_, uint32_t tmem,
+                                         const float* shifts_s, ulonglong2* acc, int p0_first) {
+        p = &pp; N = N_; k = k_; logk = logk_; lane = lane_; row = 32 * q + lane_; col0 = col0_;
+        cb = 0;
+        for (int s = 0; s < logk; ++s) cb += ((lane >> s) & 1) * (16 >> s);
+        nout = 32 >> logk;
+        gmask = (k >= 32) ? 0xffffffffu : (((1u << k) - 1u) << (lane & ~(k - 1)));
+        tb = tmem + ((uint32_t)(32 * q) << 16) + C + col0;
+        t3 = shifts_s + C + col0;
+        acc_s = acc;
+        idx_cur = load_idx(p0_first);
+        jid_acc = -1; jid_cur = -1;
+        if constexpr (POOL) {
+#pragma unroll
+            for (int s = 0; s < NSE; ++s) acc_s[s * 32] = make_ulonglong2(0ull, 0ull);
+            const int pt0 = p0_first + (row >> logk);
+            jid_cur = pt0 < N ? __ldg(p->pjid + pt0) : -1;
+        }
+    }
+    __device__ __forceinline__ void pool_flush() {
+        if (jid_acc >= 0) {
+            unsigned long long* dst = p->pool + (size_t)jid_acc * C + col0 + cb;
+#pragma unroll
+            for (int s = 0; s < NSE; ++s) {
+                const ulonglong2 a = acc_s[s * 32];
+                atomicAdd(dst + s * 32, a.x);
+                atomicAdd(dst + s * 32 + 1, a.y);
+            }
+        }
+#pragma unroll
+        for (int s = 0; s < NSE; ++s) acc_s[s * 32] = make_ulonglong2(0ull, 0ull);
+    }
+    // tile at first particle p0 (the next one at p0_next, < 0: none); waits for the layer-3 accumulator (d_full1, parity ph)
+    __device__ __forceinline__ void tile(int p0, int p0_next, uint64_t* d_full1, uint32_t ph) {
+        const int pt = p0 + (row >> logk);
+        const size_t obase = (size_t)pt * C + col0 + cb;
+        const int idx_next = p0_next >= 0 ? load_idx(p0_next) : -1;
+        int jid_next = -1;
+        if constexpr (POOL) {
+            if (p0_next >= 0) { const int ptn = p0_next + (row >> logk); jid_next = ptn < N ? __ldg(p->pjid + ptn) : -1; }
+            if (jid_cur != jid_acc) { pool_flush(); jid_acc = jid_cur; }
+        }
+        uint32_t rr[NSE];                                    // shortcut values, packed fp16 until they are used
+        auto load_rr = [&]() {
+#pragma unroll
+            for (int s = 0; s < NSE; ++s) {
+                rr[s] = 0u;
+                if (pt < N) {
+                    if (nout == 2) rr[s] = __ldg(reinterpret_cast<const uint32_t*>(p->R + obase + s * 32));
+                    else if (nout == 1) rr[s] = (uint32_t)__ldg(reinterpret_cast<const uint16_t*>(p->R + obase + s * 32));
+                }
+            }
+        };
+        // C <= 64 runs at 64 registers (four CTAs per SM): loads in flight across the wait get spilled, and the spill store
+        // waits for them; there they are issued behind the wait (L2 hits: prefetched at the top of the tile)
+        if constexpr (C > 64) load_rr();
+        mbar_wait(d_full1, ph);
+        tc_fence_after();
+        if constexpr (C <= 64) load_rr();
+        const bool valid = idx_cur >= 0;
+        const unsigned vmask = __ballot_sync(0xffffffffu, valid);
+        const int cnt = __popc(vmask & gmask);
+        const float inv = cnt > 0 ? (float)k / (float)cnt : 0.0f;   // W3', t3 carry 1/k (host): the f16 row sum is the mean
+        float v[32];
+        tmem_ld32(tb, v);
+#pragma unroll
+        for (int s = 0; s < NSE; ++s) {
+            tmem_ld_wait();
+            uint32_t w[16];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                if constexpr (BIAS_MMA) {
+                    w[2 * i] = pack_relu_f16x2(v[4 * i], v[4 * i + 1]);
+                    w[2 * i + 1] = pack_relu_f16x2(v[4 * i + 2], v[4 * i + 3]);
+                } else {
+                    const float4 sh = *reinterpret_cast<const float4*>(t3 + s * 32 + 4 * i);
+                    w[2 * i] = pack_relu_f16x2(v[4 * i] + sh.x, v[4 * i + 1] + sh.y);
+                    w[2 * i + 1] = pack_relu_f16x2(v[4 * i + 2] + sh.z, v[4 * i + 3] + sh.w);
+                }
+            }
+            if (s + 1 < NSE) tmem_ld32(tb + (s + 1) * 32, v);        // in flight during this slab's butterfly
+            if (vmask != 0xffffffffu) {
+#pragma unroll
+                for (int i = 0; i < 16; ++i) w[i] = valid ? w[i] : 0u;
+            }
+#pragma unroll
+            for (int s2 = 0; s2 < 4; ++s2) {
+                if (s2 < logk) {
+                    const bool up = (lane >> s2) & 1;
+                    const int cntv = 8 >> s2;
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) {
+                        if (i < cntv) {
+                            const uint32_t keep = up ? w[i + cntv] : w[i];
+                            const uint32_t send = up ? w[i] : w[i + cntv];
+                            w[i] = add_f16x2(keep, __shfl_xor_sync(0xffffffffu, send, 1 << s2));
+                        }
+                    }
+                }
+            }
+            const size_t o = obase + s * 32;
+            if (logk == 5) {                                      // k = 32: one more step splits the last register's two columns
+                const float2 f = unpack_f16x2(w[0]);
+                const bool up = (lane >> 4) & 1;
+                const float sum = (up ? f.y : f.x) + __shfl_xor_sync(0xffffffffu, up ? f.x : f.y, 16);
+                if (pt < N) p->y[o] = fmaxf(fmaf(sum, inv, unpack_f16x2(rr[s]).x), 0.0f);
+            } else if (pt < N) {
+                if (nout == 2) {
+                    const float2 f = unpack_f16x2(w[0]), rs = unpack_f16x2(rr[s]);
+                    const float y0 = fmaxf(fmaf(f.x, inv, rs.x), 0.0f), y1 = fmaxf(fmaf(f.y, inv, rs.y), 0.0f);
+                    if constexpr (POOL) {
+                        ulonglong2 a = acc_s[s * 32];
+                        a.x += to_fixed_32_32(y0);
+                        a.y += to_fixed_32_32(y1);
+                        acc_s[s * 32] = a;
+                    } else {
+                        *reinterpret_cast<float2*>(p->y + o) = make_float2(y0, y1);
+                    }
+                } else {
+#pragma unroll
+                    for (int i = 0; i < 16; i += 2)
+                        if (2 * i < nout) {
+                            const float2 f0 = unpack_f16x2(w[i]), f1 = unpack_f16x2(w[i + 1]);
+                            const uint2 rh = __ldg(reinterpret_cast<const uint2*>(p->R + o + 2 * i));
+                            const float2 ra = unpack_f16x2(rh.x), rb = unpack_f16x2(rh.y);
+                            const float4 r4 = make_float4(ra.x, ra.y, rb.x, rb.y);
+                            *reinterpret_cast<float4*>(p->y + o + 2 * i) =
+                                make_float4(fmaxf(fmaf(f0.x, inv, r4.x), 0.0f), fmaxf(fmaf(f0.y, inv, r4.y), 0.0f),
+                                            fmaxf(fmaf(f1.x, inv, r4.z), 0.0f), fmaxf(fmaf(f1.y, inv, r4.w), 0.0f));
+                        }
+                }
+            }
+        }
+        idx_cur = idx_next;
+        if constexpr (POOL) jid_cur = jid_next;
+    }
 };
 
 // LOGK >= 0: k = 2^LOGK known at compile time (lets the gather keep one u chunk per particle in registers); -1: runtime
@@ -183,7 +344,9 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
             mbar_init(&h2_ready[i], 4 * (Cfg::KW > CWE ? Cfg::KW / CWE : 1) * Cfg::NRANKS);   // epilogue warps per K block
             mbar_init(&h_free[i], 1);
         }
-        for (int i = 0; i < 2; ++i) { mbar_init(&d_full[i], 1); mbar_init(&d_free[i], NE * Cfg::NRANKS); }
+        for (int i = 0; i < 2; ++i) mbar_init(&d_full[i], 1);
+        mbar_init(&d_free[0], NE * Cfg::NRANKS);
+        mbar_init(&d_free[1], (NE + (Cfg::SPLIT_E3 ? Cfg::NG : 0)) * Cfg::NRANKS);   // every warp that drains D1
         mbar_init(w_full, 1);
         mbar_init(w_peer, 1);
         fence_mbar_init();
@@ -209,6 +372,48 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
     auto arrive_leader = [&](uint64_t* bar) {
         __syncwarp();
         if (lane == 0) { if constexpr (PAIR) mbar_arrive_cluster(bar, 0); else mbar_arrive(bar); }
+    };
+
+    // ---- E2 of one epilogue warp: H2 = bf16(relu(D0)) for lane quadrant q_, CWE / 32 slabs of 32 columns from column c0; the TMEM
+    // load of slab s + 1 is in flight while slab s is converted and stored; a K block is announced when this warp's part of it
+    // is written.  (Sharing E2 with the gather warps like E3 was measured slower, 153 -> 167 us at C = 256: their loads of the
+    // next tile then start behind it, and the next layer-2 MMA waits for the gather.)
+    auto e2_run = [&](int q_, int c0, uint32_t ph) {
+        constexpr int NS2 = CWE / 32;
+        const int row_ = 32 * q_ + lane;
+        const uint32_t tb = tmem + ((uint32_t)(32 * q_) << 16) + c0;
+        mbar_wait(&d_full[0], ph);                               // implies every layer-2 read of H1 is done
+        tc_fence_after();
+        float v[32];
+        tmem_ld32(tb, v);
+#pragma unroll
+        for (int s = 0; s < NS2; ++s) {
+            tmem_ld_wait();
+            const int col = c0 + s * 32;
+            uint32_t pk[16];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                if constexpr (Cfg::BIAS_MMA) {
+                    pk[2 * i] = pack_relu_bf16x2(v[4 * i], v[4 * i + 1]);
+                    pk[2 * i + 1] = pack_relu_bf16x2(v[4 * i + 2], v[4 * i + 3]);
+                } else {
+                    const float4 sh = *reinterpret_cast<const float4*>(shifts_s + col + 4 * i);
+                    pk[2 * i] = pack_relu_bf16x2(v[4 * i] + sh.x, v[4 * i + 1] + sh.y);
+                    pk[2 * i + 1] = pack_relu_bf16x2(v[4 * i + 2] + sh.z, v[4 * i + 3] + sh.w);
+                }
+            }
+            if (s + 1 < NS2) tmem_ld32(tb + (s + 1) * 32, v);     // in flight while this slab is stored
+            uint8_t* dst = H + (col >> 6) * Cfg::HK_BYTES + row_ * 128;
+            const int c8 = (col & 63) >> 3;
+#pragma unroll
+            for (int c = 0; c < 4; ++c)
+                *reinterpret_cast<uint4*>(dst + (((c8 + c) ^ (row_ & 7)) << 4)) =
+                    make_uint4(pk[4 * c], pk[4 * c + 1], pk[4 * c + 2], pk[4 * c + 3]);
+            if (((col + 32) & 63) == 0 || s == NS2 - 1) {        // this warp's part of a K block is complete
+                fence_proxy_async();
+                arrive_leader(&h2_ready[col >> 6]);
+            }
+        }
     };
 
     if (warp == Cfg::MMA_WARP) {
@@ -290,6 +495,14 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
         };
         int idx_r[NI], idx_n[NI];
         load_idx2(tile_p0(0), idx_r);
+        // SPLIT_E3: this warp also runs E3 of the tile BEHIND the one it gathers (lane quadrant g & 3, second half of the columns
+        // of column group g >> 2); it hands D1 back like the epilogue warps do
+        E3Rows<C, LOGK, POOL, Cfg::NSE, Cfg::BIAS_MMA> e3;
+        if constexpr (Cfg::SPLIT_E3) {
+            e3.init(p, N, k, logk, lane, g & 3, (g >> 2) * CWE + Cfg::NSE * 32, tmem, shifts_s, pool_s + ((NE + g) * Cfg::NSE) * 32 + lane, tile_p0(0));
+            tc_fence_before();
+            arrive_leader(&d_free[1]);
+        }
         for (int t = 0; t < T; ++t) {
             const int p0 = tile_p0(t);
             // The U/V/R/x working set of a large batch exceeds L2, so the gathered rows come from HBM (~2300 cycles per
@@ -350,6 +563,17 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
             arrive_leader(&h1_ready[gk]);
 #pragma unroll
             for (int a = 0; a < NI; ++a) idx_r[a] = idx_n[a];
+            if constexpr (Cfg::SPLIT_E3) {
+                if (t >= 1) {
+                    e3.tile(tile_p0(t - 1), p0, &d_full[1], (uint32_t)((t - 1) & 1));
+                    tc_fence_before();
+                    arrive_leader(&d_free[1]);
+                }
+            }
+        }
+        if constexpr (Cfg::SPLIT_E3) {
+            e3.tile(tile_p0(T - 1), -1, &d_full[1], (uint32_t)((T - 1) & 1));
+            if constexpr (POOL) e3.pool_flush();
         }
     } else {
         // ===== epilogue warps: E2 (D0 -> H2) and E3 (D1 -> mean -> y) for lane quadrant q, columns [cg*CWE, +CWE) ==========
@@ -358,17 +582,9 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
         const int row = 32 * q + lane;                           // TMEM lane = edge row of the tile
         const int col0 = cg * CWE;
         constexpr int SLABS = CWE / 32;
-        const uint32_t tbase = tmem + ((uint32_t)(32 * q) << 16) + col0;
-        const float* t2 = shifts_s + col0;
-        const float* t3 = shifts_s + C + col0;
         int cb = 0;                                              // first of the 32 >> logk columns this lane ends up with
         for (int s = 0; s < logk; ++s) cb += ((lane >> s) & 1) * (16 >> s);
         const int nout = 32 >> logk;
-        const unsigned gmask = (k >= 32) ? 0xffffffffu : (((1u << k) - 1u) << (lane & ~(k - 1)));
-        auto load_idx = [&](int p0) {
-            const int pt = p0 + (row >> logk);
-            return (pt < N) ? __ldg(p.idx + (size_t)pt * k + (row & (k - 1))) : -1;
-        };
         // an accumulator is handed back to the MMA thread as soon as this warp has read it
         auto reset_acc = [&](int layer) {
             tc_fence_before();
@@ -376,29 +592,12 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
         };
         reset_acc(0);
         reset_acc(1);
-        int idx_cur = load_idx(tile_p0(0));
-        // POOL: this lane's accumulators (slab s -> columns col0 + 32 s + cb, + 1) of the jet `jid_acc` it is walking
-        ulonglong2* acc_s = pool_s + ((warp % NE) * SLABS) * 32 + lane;
-        int jid_acc = -1, jid_cur = -1;
-        auto pool_flush = [&]() {
-            if (jid_acc >= 0) {
-                unsigned long long* dst = p.pool + (size_t)jid_acc * C + col0 + cb;
-#pragma unroll
-                for (int s = 0; s < SLABS; ++s) {
-                    const ulonglong2 a = acc_s[s * 32];
-                    atomicAdd(dst + s * 32, a.x);
-                    atomicAdd(dst + s * 32 + 1, a.y);
-                }
-            }
-#pragma unroll
-            for (int s = 0; s < SLABS; ++s) acc_s[s * 32] = make_ulonglong2(0ull, 0ull);
-        };
-        if constexpr (POOL && !TR3) {
-#pragma unroll
-            for (int s = 0; s < SLABS; ++s) acc_s[s * 32] = make_ulonglong2(0ull, 0ull);
-            const int pt0 = tile_p0(0) + (row >> logk);
-            jid_cur = pt0 < N ? __ldg(p.pjid + pt0) : -1;
-        }
+        // row-layout E3: this warp's worker (with SPLIT_E3 the first half of the warp's columns; the gather warp of the same lane
+        // quadrant and column group runs the second half); POOL accumulators: worker slot (warp % NE), NSE slabs each
+        constexpr int NSE = Cfg::NSE;
+        E3Rows<C, LOGK, POOL, NSE, Cfg::BIAS_MMA> e3;
+        if constexpr (!TR3) e3.init(p, N, k, logk, lane, q, col0, tmem, shifts_s, pool_s + ((warp % NE) * NSE) * 32 + lane, tile_p0(0));
+        int jid_acc = -1;                                        // (TR3 + POOL)
         // ---- TR3 state: lane l < NP describes particle l of the (pair) tile: packed row (-1: none), valid-neighbour mask,
         // k / k_eff, jet.  Pair tile w covers the 16 consecutive particles of tiles 2w and 2w + 1.
         constexpr int NP = PAIR ? 16 : 8;                        // particles of a (pair) tile, k = 16
@@ -436,42 +635,7 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
 #pragma unroll
                 for (int s = 0; s < SLABS; ++s) asm volatile("prefetch.global.L2 [%0];" ::"l"(p.R + obase + s * 32));
             }
-            // ---- E2: H2 = bf16(relu(D0)); the TMEM load of slab s+1 is in flight while slab s is converted ---------------
-            mbar_wait(&d_full[0], ph);                           // implies every layer-2 read of H1 is done
-            tc_fence_after();
-            {
-                float v[32];
-                tmem_ld32(tbase, v);
-#pragma unroll
-                for (int s = 0; s < SLABS; ++s) {
-                    tmem_ld_wait();
-                    const int col = col0 + s * 32;
-                    uint32_t pk[16];
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        float4 sh = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-                        if constexpr (Cfg::BIAS_MMA) {
-                            pk[2 * i] = pack_relu_bf16x2(v[4 * i], v[4 * i + 1]);
-                            pk[2 * i + 1] = pack_relu_bf16x2(v[4 * i + 2], v[4 * i + 3]);
-                            continue;
-                        }
-                        sh = *reinterpret_cast<const float4*>(t2 + s * 32 + 4 * i);
-                        pk[2 * i] = pack_relu_bf16x2(v[4 * i] + sh.x, v[4 * i + 1] + sh.y);
-                        pk[2 * i + 1] = pack_relu_bf16x2(v[4 * i + 2] + sh.z, v[4 * i + 3] + sh.w);
-                    }
-                    if (s + 1 < SLABS) tmem_ld32(tbase + (s + 1) * 32, v);     // in flight while this slab is stored
-                    uint8_t* dst = H + (col >> 6) * Cfg::HK_BYTES + row * 128;
-                    const int c8 = (col & 63) >> 3;
-#pragma unroll
-                    for (int c = 0; c < 4; ++c)
-                        *reinterpret_cast<uint4*>(dst + (((c8 + c) ^ (row & 7)) << 4)) =
-                            make_uint4(pk[4 * c], pk[4 * c + 1], pk[4 * c + 2], pk[4 * c + 3]);
-                    if (((col + 32) & 63) == 0 || s == SLABS - 1) {      // this warp's part of a K block is complete
-                        fence_proxy_async();
-                        arrive_leader(&h2_ready[col >> 6]);
-                    }
-                }
-            }
+            e2_run(q, col0, ph);
             if (t + 1 < T) reset_acc(0);
             // ---- E3: mean over the valid neighbours of relu(D1), + shortcut, ReLU.  The row reduction runs on packed f16x2
             // (two columns per register): a halving butterfly over the k rows of a particle, fp32 again for the mean ------------
@@ -527,115 +691,13 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
                 if (t + 1 < T) reset_acc(1);
                 m_pt = n_pt; m_mask = n_mask; m_inv = n_inv; m_jid = n_jid;
             } else {
-            const int idx_next = (t + 1 < T) ? load_idx(tile_p0(t + 1)) : -1;
-            int jid_next = -1;
-            if constexpr (POOL) {
-                if (t + 1 < T) { const int ptn = tile_p0(t + 1) + (row >> logk); jid_next = ptn < N ? __ldg(p.pjid + ptn) : -1; }
-                if (jid_cur != jid_acc) { pool_flush(); jid_acc = jid_cur; }
-            }
-            uint32_t rr[SLABS];                                  // shortcut values, packed fp16 until they are used
-            auto load_rr = [&]() {
-#pragma unroll
-                for (int s = 0; s < SLABS; ++s) {
-                    rr[s] = 0u;
-                    if (pt < N) {
-                        if (nout == 2) rr[s] = __ldg(reinterpret_cast<const uint32_t*>(p.R + obase + s * 32));
-                        else if (nout == 1) rr[s] = (uint32_t)__ldg(reinterpret_cast<const uint16_t*>(p.R + obase + s * 32));
-                    }
-                }
-            };
-            // C <= 64 runs at 64 registers (four CTAs per SM): loads in flight across the wait get spilled, and the spill store
-            // waits for them; there they are issued behind the wait (L2 hits: prefetched at the top of the tile)
-            if constexpr (C > 64) load_rr();
-            mbar_wait(&d_full[1], ph);
-            tc_fence_after();
-            if constexpr (C <= 64) load_rr();
-            {
-                const bool valid = idx_cur >= 0;
-                const unsigned vmask = __ballot_sync(0xffffffffu, valid);
-                const int cnt = __popc(vmask & gmask);
-                const float inv = cnt > 0 ? (float)k / (float)cnt : 0.0f;   // W3', t3 carry 1/k (host): the f16 row sum is the mean
-                float v[32];
-                tmem_ld32(tbase + C, v);
-#pragma unroll
-                for (int s = 0; s < SLABS; ++s) {
-                    tmem_ld_wait();
-                    uint32_t w[16];
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        float4 sh = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-                        if constexpr (Cfg::BIAS_MMA) {
-                            w[2 * i] = pack_relu_f16x2(v[4 * i], v[4 * i + 1]);
-                            w[2 * i + 1] = pack_relu_f16x2(v[4 * i + 2], v[4 * i + 3]);
-                            continue;
-                        }
-                        sh = *reinterpret_cast<const float4*>(t3 + s * 32 + 4 * i);
-                        w[2 * i] = pack_relu_f16x2(v[4 * i] + sh.x, v[4 * i + 1] + sh.y);
-                        w[2 * i + 1] = pack_relu_f16x2(v[4 * i + 2] + sh.z, v[4 * i + 3] + sh.w);
-                    }
-                    if (s + 1 < SLABS) tmem_ld32(tbase + C + (s + 1) * 32, v);  // in flight during this slab's butterfly
-                    if (vmask != 0xffffffffu) {
-#pragma unroll
-                        for (int i = 0; i < 16; ++i) w[i] = valid ? w[i] : 0u;
-                    }
-                    // after step s2 a lane keeps 8 >> s2 registers = partial sums over 2^(s2+1) rows of 16 >> s2 columns
-#pragma unroll
-                    for (int s2 = 0; s2 < 4; ++s2) {
-                        if (s2 < logk) {
-                            const bool up = (lane >> s2) & 1;
-                            const int cntv = 8 >> s2;
-#pragma unroll
-                            for (int i = 0; i < 8; ++i) {
-                                if (i < cntv) {
-                                    const uint32_t keep = up ? w[i + cntv] : w[i];
-                                    const uint32_t send = up ? w[i] : w[i + cntv];
-                                    w[i] = add_f16x2(keep, __shfl_xor_sync(0xffffffffu, send, 1 << s2));
-                                }
-                            }
-                        }
-                    }
-                    const size_t o = obase + s * 32;
-                    if (logk == 5) {                              // k = 32: one more step splits the last register's two columns
-                        const float2 f = unpack_f16x2(w[0]);
-                        const bool up = (lane >> 4) & 1;
-                        const float sum = (up ? f.y : f.x) + __shfl_xor_sync(0xffffffffu, up ? f.x : f.y, 16);
-                        if (pt < N) p.y[o] = fmaxf(fmaf(sum, inv, unpack_f16x2(rr[s]).x), 0.0f);
-                    } else if (pt < N) {
-                        if (nout == 2) {
-                            const float2 f = unpack_f16x2(w[0]), rs = unpack_f16x2(rr[s]);
-                            const float y0 = fmaxf(fmaf(f.x, inv, rs.x), 0.0f), y1 = fmaxf(fmaf(f.y, inv, rs.y), 0.0f);
-                            if constexpr (POOL) {
-                                ulonglong2 a = acc_s[s * 32];
-                                a.x += to_fixed_32_32(y0);
-                                a.y += to_fixed_32_32(y1);
-                                acc_s[s * 32] = a;
-                            } else {
-                                *reinterpret_cast<float2*>(p.y + o) = make_float2(y0, y1);
-                            }
-                        } else {
-#pragma unroll
-                            for (int i = 0; i < 16; i += 2)
-                                if (2 * i < nout) {
-                                    const float2 f0 = unpack_f16x2(w[i]), f1 = unpack_f16x2(w[i + 1]);
-                                    const uint2 rh = __ldg(reinterpret_cast<const uint2*>(p.R + o + 2 * i));
-                                    const float2 ra = unpack_f16x2(rh.x), rb = unpack_f16x2(rh.y);
-                                    const float4 r4 = make_float4(ra.x, ra.y, rb.x, rb.y);
-                                    *reinterpret_cast<float4*>(p.y + o + 2 * i) =
-                                        make_float4(fmaxf(fmaf(f0.x, inv, r4.x), 0.0f), fmaxf(fmaf(f0.y, inv, r4.y), 0.0f),
-                                                    fmaxf(fmaf(f1.x, inv, r4.z), 0.0f), fmaxf(fmaf(f1.y, inv, r4.w), 0.0f));
-                                }
-                        }
-                    }
-                }
-            }
-            if (t + 1 < T) reset_acc(1);
-            idx_cur = idx_next;
-            if constexpr (POOL) jid_cur = jid_next;
+                e3.tile(p0, t + 1 < T ? tile_p0(t + 1) : -1, &d_full[1], ph);
+                if (t + 1 < T) reset_acc(1);
             }
         }
         if constexpr (POOL) {
             if constexpr (TR3) { if (jid_acc >= 0) atomicAdd(p.pool + (size_t)jid_acc * C + ((PAIR ? 128 * (int)rank : 0) + 32 * q + lane), pacc); }
-            else pool_flush();
+            else e3.pool_flush();
         }
     }
     tc_fence_before();
