@@ -317,3 +317,50 @@ def test_host_entry_pipelined_equals_blocking():
     assert e.value.code == -6                                   # GNN_ERR_BAD_OFFSETS
     m.infer_host_end(stream=st[0], slice=0)                     # nothing in flight: a no-op
     m.close()
+
+
+def test_forward_in_a_callers_cuda_graph_and_graph_replay(pn):
+    """include/gnn.h: the forward is enqueued on the caller's stream alone, so it can be captured into a CUDA graph of the
+    caller's; and gnn_infer replays a graph of its own when a call's arguments repeat.  Both must read the CURRENT contents of
+    the input buffers: the same buffers refilled with other jets (same B and N) give those jets' logits, bitwise equal to a
+    first-time call on fresh buffers."""
+    _, _, m = pn
+    b1 = synth.make_particlenet_batch(seed=901, n_jets=48)
+    # a second batch with the same multiplicities (hence the same B, N and offsets) but other particles
+    b2 = synth.make_particlenet_batch(seed=902, n_jets=400)
+    order = np.argsort(b2.counts(), kind="stable")
+    picked, pool = [], list(order)
+    for n in b1.counts():
+        j = next((j for j in pool if b2.counts()[j] == n), None)
+        if j is None:
+            pytest.skip("no jet of matching multiplicity in the donor batch")
+        pool.remove(j); picked.append(int(j))
+    b2 = b2.select(picked)
+    assert np.array_equal(b2.offsets, b1.offsets)
+    ref1, ref2 = run_ragged(m, b1), run_ragged(m, b2)              # fresh buffers each: never a replay
+    f, c, o = dev(b1.feats), dev(b1.coords), dev(b1.offsets)
+    out = torch.empty((b1.n_jets, 2), dtype=torch.float32, device="cuda")
+    for _ in range(3):                                             # third call: the library's own graph replay
+        m.infer(f, c, o, logits=out)
+    torch.cuda.synchronize()
+    assert np.array_equal(out.cpu().numpy().astype(np.float64), ref1)
+    f.copy_(dev(b2.feats)); c.copy_(dev(b2.coords))
+    m.infer(f, c, o, logits=out)                                   # replayed graph, new contents
+    torch.cuda.synchronize()
+    assert np.array_equal(out.cpu().numpy().astype(np.float64), ref2)
+    # the caller's own capture
+    g = torch.cuda.CUDAGraph()
+    out2 = torch.empty_like(out)
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        m.infer(f, c, o, logits=out2, stream=side)                 # warm (nothing lazy inside the capture)
+        side.synchronize()
+        with torch.cuda.graph(g, stream=side):
+            m.infer(f, c, o, logits=out2, stream=side)
+    torch.cuda.current_stream().wait_stream(side)
+    f.copy_(dev(b1.feats)); c.copy_(dev(b1.coords))
+    g.replay()
+    torch.cuda.synchronize()
+    assert np.array_equal(out2.cpu().numpy().astype(np.float64), ref1)
+    assert m.status_check() == 0
