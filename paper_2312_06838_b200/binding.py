@@ -295,6 +295,12 @@ class Batcher:
         rc = lib().gnn_batcher_wait(self.h, ticket, timeout_us, C.byref(q), C.byref(c))
         return int(rc), q.value, c.value
 
+    def wait_ex(self, ticket, timeout_us=-1):
+        """gnn_batcher_wait_ex -> (status, {queue_us, compute_us, transfer_us, inference_us})"""
+        t = (C.c_double * 4)()
+        rc = lib().gnn_batcher_wait_ex(self.h, ticket, timeout_us, C.cast(t, C.c_void_p))
+        return int(rc), dict(zip(("queue_us", "compute_us", "transfer_us", "inference_us"), list(t)))
+
     def stats(self):
         a, b, c, d = C.c_uint64(0), C.c_uint64(0), C.c_uint64(0), C.c_double(0)
         lib().gnn_batcher_stats(self.h, C.byref(a), C.byref(b), C.byref(c), C.byref(d))

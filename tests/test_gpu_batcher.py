@@ -91,3 +91,27 @@ def test_deadline_and_host_validation(served):
     rc, _, _ = bt.wait(bt.submit(r.feats, r.coords, r.offsets)[0], timeout_us=0)
     assert rc in (0, -9)
     bt.close()                                                             # drains the pending ticket
+
+
+def test_request_time_split_and_load_generator(served):
+    """gnn_batcher_wait_ex: the device-side parts (host <-> device copies, forward; CUDA events on the instance's stream) lie
+    inside the host-clock compute time; gnn_loadgen_run: closed-loop native clients, every request of the pool answered, the
+    reported split consistent (queue / network / inference per request)."""
+    a, w, m = served
+    bt = gnn.Batcher(m, max_batch_jets=256, max_queue_delay_us=500, n_instances=2)
+    r = synth.make_client_pool(3, n_requests=1)[0]
+    t, out = bt.submit(r.feats, r.coords, r.offsets)
+    rc, tm = bt.wait_ex(t)
+    assert rc == 0 and np.array_equal(out.astype(np.float64), run_ragged(m, r))
+    assert tm["transfer_us"] > 0 and tm["inference_us"] > 0
+    assert tm["transfer_us"] + tm["inference_us"] <= tm["compute_us"] * 1.05 + 20
+    assert 400 <= tm["queue_us"] < 50000                                   # one lonely request waits out the queue delay
+    big = synth.make_particlenet_batch(seed=77, n_jets=512)
+    rfj = np.arange(0, 513, 16, dtype=np.int32)
+    res = bt.loadgen(big.feats, big.coords, big.offsets, rfj, n_clients=8, warmup_ms=50, run_ms=300)
+    assert res["n_requests"] > 50 and res["n_jets"] == 16 * res["n_requests"]
+    assert res["p50_us"] <= res["p90_us"] <= res["p99_us"]
+    assert abs(res["queue_us_mean"] + res["compute_us_mean"] - res["mean_us"]) < 0.25 * res["mean_us"] + 50
+    assert 0 < res["transfer_us_mean"] + res["inference_us_mean"] <= res["compute_us_mean"] * 1.05 + 20
+    assert 16 <= res["mean_batch_jets"] <= 256
+    bt.close()
