@@ -190,11 +190,11 @@ knn_group_coords_kernel(const float* __restrict__ space, int D, const int32_t* _
 }
 
 // ---- feature spaces: Gram matrix on the tensor cores -------------------------------------------------------------------------
-// warps 0-3: thread = row = TMEM lane (selection); warps 4-7 help with the load, the means and the centring pass; warp 4 owns
+// four warps: thread = row = TMEM lane; warp 0 owns
 // the TMEM allocation and its lane 0 issues the MMAs
-constexpr int KG_THREADS = 256;
-constexpr int KG_MMA_WARP = 4;
-constexpr int KG_BATCH = 2;                // items a thread has in flight (registers: three CTAs per SM, beside the pre kernel)
+constexpr int KG_THREADS = 128;
+constexpr int KG_MMA_WARP = 0;
+constexpr int KG_BATCH = 4;                // items a thread has in flight (one or two round trips per tile)
 
 template <int D>
 struct KnnGroupCfg {
@@ -204,8 +204,10 @@ struct KnnGroupCfg {
     static constexpr int SMEM_BYTES = X_BYTES + KG_ROWS * 4 + KG_ROWS * 4 + (int)sizeof(GroupInfo) + 2 * 8 + 16 + 64;
 };
 
+// 128 threads (thread = row): a CTA is small enough in registers for several to sit on an SM BESIDE the pre kernel's CTA, so the
+// groups of a batch run in one or two waves while the two kernels of a block run side by side
 template <int D, int K>
-__global__ void __launch_bounds__(KG_THREADS, 3)
+__global__ void __launch_bounds__(KG_THREADS)
 knn_group_gram_kernel(const float* __restrict__ space, const int32_t* __restrict__ jet_start, const int32_t* __restrict__ jet_n,
                       const int32_t* __restrict__ meta, const int2* __restrict__ groups, int32_t* __restrict__ idx_out,
                       int32_t* __restrict__ pjid, int k, int local_out, int dep) {
