@@ -180,6 +180,31 @@ int gnn_debug_edgeconv_pool(gnn_model* m, const float* x_dev, const int32_t* idx
 int gnn_debug_pool_head(gnn_model* m, const float* x_dev, const int32_t* offsets_dev, int32_t B, int32_t N,
                         float* logits_dev, void* cuda_stream);
 
+/* ---- exact kNN without a model and without any allocation --------------------------------------------------------------
+ * For callers that are not allowed to allocate device memory: a plugin whose host application owns the device heap and hands
+ * out fixed buffers, a real-time loop that must never wait on the allocator's device-wide lock, a process whose GPU memory
+ * was fully budgeted before this library was loaded.  Those callers cannot call gnn_create either (it allocates the weights
+ * and a workspace), so this entry needs no gnn_model: it is the exact kNN step alone ("k=16 nearest
+ * neighbors"; same kernels, same fp32 arithmetic and (d, j) order as gnn_debug_knn on a GNN_FP32_VALIDATION model, so the
+ * two return identical indices).  The kernels' intermediate data (ragged descriptors, particle -> jet map, per-jet distance
+ * matrix) goes to a fixed array compiled into libgnn.so: about 4.1 MiB on every GPU that loads the library, held until the
+ * process exits.  The call itself never calls cudaMalloc / cudaFree or any routine that does.
+ *   space_dev [N, D] fp32 row-major (1 <= D <= 1024), offsets_dev int32 [B + 1] CSR, idx_dev int32 [N, k] (written:
+ *   jet-local indices in (d, j) order, -1 behind the k_eff = min(k, n - 1) valid ones); all three are the caller's
+ *   buffers on the CURRENT device (cudaSetDevice before the call on multi-GPU hosts).  Asynchronous on cuda_stream.
+ * Limits: B <= 1024 jets and N <= 8192 particles per call, max_particles <= GNN_MAX_PARTICLES; anything larger is
+ *   refused with GNN_ERR_BATCH_TOO_LARGE (and a line on stderr) before anything is enqueued -- split the batch.
+ * First call on a device: looks up the array's device address (one cudaGetSymbolAddress, remembered per device).  Make that
+ *   first call outside any stream capture.
+ * Sharing: every call on a device uses the same array, and it keeps the previous call's contents (the call clears the few
+ *   words that must start at zero).  Two calls whose kernels can overlap on the GPU -- different streams, or several host
+ *   threads -- race on it and return garbage: keep all calls on one stream, or order them with events.
+ * Offsets are checked on the device only for memory safety: with an invalid CSR (offsets[0] != 0, not monotone, offsets[B]
+ *   != N) idx_dev is left untouched, and a jet with more than max_particles particles gets rows of -1; no status is
+ *   reported (validate offsets on the host, where this caller has them). */
+int gnn_knn_noalloc(const float* space_dev, int32_t D, const int32_t* offsets_dev, int32_t B, int32_t N,
+                    int32_t max_particles, int32_t k, int32_t* idx_dev, void* cuda_stream);
+
 /* ---- host dynamic batcher ("dynamic batching", L268 preferred batch 1024, L271 instance group) -- */
 typedef struct {
     int32_t max_batch_jets;        /* coalesce up to this many jets per launch (<= arch.max_batch_jets); 1024 (L268) */

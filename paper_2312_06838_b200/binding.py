@@ -77,6 +77,7 @@ def lib():
         L.gnn_strerror.argtypes = [C.c_int]; L.gnn_strerror.restype = C.c_char_p
         L.gnn_launch_count.argtypes = [vp]; L.gnn_launch_count.restype = C.c_int64
         L.gnn_debug_knn.argtypes = [vp, f32p, i32, i32p, i32, i32, i32, i32p, vp]
+        L.gnn_knn_noalloc.argtypes = [f32p, i32, i32p, i32, i32, i32, i32, i32p, vp]
         L.gnn_debug_edgeconv.argtypes = [vp, i32, f32p, i32p, i32p, i32, i32, f32p, vp]
         L.gnn_debug_pool_head.argtypes = [vp, f32p, i32p, i32, i32, f32p, vp]
         L.gnn_debug_edgeconv_pool.argtypes = [vp, f32p, i32p, i32p, i32, i32, f32p, vp]
@@ -140,6 +141,21 @@ def _stream(stream):
     import torch
     s = stream if stream is not None else torch.cuda.current_stream()
     return C.c_void_p(s.cuda_stream)
+
+
+def knn_noalloc(space, offsets, k, max_particles=128, idx=None, stream=None):
+    """gnn_knn_noalloc: exact kNN with no gnn_model and no device allocation inside the library (its scratch is a fixed
+    array inside libgnn.so; at most 1024 jets / 8192 particles per call; calls must not overlap on the GPU).  Pass `idx`
+    ([N, k] int32, device) to keep this wrapper from allocating too; torch tensors on the current device."""
+    import torch
+    N, D = space.shape
+    if idx is None:
+        idx = torch.full((N, k), -7, dtype=torch.int32, device=space.device)
+    rc = lib().gnn_knn_noalloc(_ptr(space), D, _ptr(offsets), offsets.numel() - 1, N, max_particles, k, _ptr(idx),
+                               _stream(stream))
+    if rc != 0:
+        raise GnnError(rc, "gnn_knn_noalloc")
+    return idx
 
 
 class Model:

@@ -18,6 +18,7 @@
 //   block 1) skip the matrix: the selection computes d(i, j) on the fly with the same arithmetic.
 #include "gnn_internal.h"
 #include <cfloat>
+#include <mutex>
 
 namespace {
 
@@ -382,4 +383,80 @@ int launch_globalize_idx(const int32_t* idx_local, int k, int B, const Workspace
 int knn_configure() {
     return cudaFuncSetAttribute(knn_dist_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024) == cudaSuccess
                ? GNN_OK : GNN_ERR_CUDA;
+}
+
+// ---- gnn_knn_noalloc: the exact kNN above for callers that may not allocate device memory ----------------------------------
+// Who this is for: code that runs where a cudaMalloc is forbidden or fails by construction -- a plugin inside a host
+// application that hands the plugin fixed buffers and owns the device heap itself, a latency-critical loop that has promised
+// its scheduler never to take the allocator's device-wide lock, a process whose memory budget was carved up before this
+// library was loaded.  Such a caller cannot even call gnn_create (which allocates weights and a workspace), so this entry
+// takes no gnn_model.  Everything the two kernels need besides the caller's input and output -- the sanitised ragged
+// descriptors, the particle -> jet map and the per-jet distance matrix -- lives in ONE array that is part of the library's
+// image: the driver sets it aside on every GPU that loads libgnn.so and keeps it until the process exits (about 4.1 MiB).
+//
+// `knn_noalloc_scratch` below is that array.  In host code its name is only a handle the runtime knows the array by, NOT a
+// device address (a kernel given `knn_noalloc_scratch` from the host would fault, or scribble on host memory on systems where
+// the GPU can reach it).  The address a kernel may use comes from cudaGetSymbolAddress, asked for once per device with that
+// device current, in knn_noalloc_base().
+constexpr int NOALLOC_MAX_JETS = 1024;          // largest B of one call
+constexpr int NOALLOC_MAX_ROWS = 8192;          // largest N of one call (particles of the whole batch)
+constexpr int NOALLOC_MAX_DEVICES = 64;
+// layout (byte offsets, every part 256-byte aligned):  [0, 256) status word + meta[4]  |  jet_start [MAX_JETS] int32  |
+// jet_n [MAX_JETS] int32  |  pjet [MAX_ROWS] int2  |  dm [MAX_ROWS][GNN_MAX_PARTICLES] fp32
+constexpr size_t NOALLOC_OFF_START = 256;
+constexpr size_t NOALLOC_OFF_N = NOALLOC_OFF_START + sizeof(int32_t) * NOALLOC_MAX_JETS;
+constexpr size_t NOALLOC_OFF_PJET = NOALLOC_OFF_N + sizeof(int32_t) * NOALLOC_MAX_JETS;
+constexpr size_t NOALLOC_OFF_DM = NOALLOC_OFF_PJET + sizeof(int2) * NOALLOC_MAX_ROWS;
+constexpr size_t NOALLOC_BYTES = NOALLOC_OFF_DM + sizeof(float) * NOALLOC_MAX_ROWS * GNN_MAX_PARTICLES;
+static_assert(NOALLOC_OFF_N % 256 == 0 && NOALLOC_OFF_PJET % 256 == 0 && NOALLOC_OFF_DM % 256 == 0, "scratch parts stay 256-byte aligned");
+static __device__ __align__(256) unsigned char knn_noalloc_scratch[NOALLOC_BYTES];
+
+// device address of the scratch array on the CURRENT device (looked up on the first call per device, then remembered)
+static int knn_noalloc_base(unsigned char** out) {
+    static std::mutex mu;
+    static unsigned char* base[NOALLOC_MAX_DEVICES] = {};
+    int device = -1;
+    GNN_CUDA_TRY(cudaGetDevice(&device));
+    if (device < 0 || device >= NOALLOC_MAX_DEVICES) return GNN_ERR_BAD_ARG;
+    std::lock_guard<std::mutex> lock(mu);
+    if (base[device] == nullptr) {
+        unsigned char* p = nullptr;
+        GNN_CUDA_TRY(cudaGetSymbolAddress((void**)&p, knn_noalloc_scratch));
+        if (p == nullptr) return GNN_ERR_CUDA;
+        base[device] = p;
+    }
+    *out = base[device];
+    return GNN_OK;
+}
+
+extern "C" int gnn_knn_noalloc(const float* space_dev, int32_t D, const int32_t* offsets_dev, int32_t B, int32_t N,
+                               int32_t max_particles, int32_t k, int32_t* idx_dev, void* cuda_stream) {
+    if (B < 0 || N < 0 || D < 1 || D > 1024 || k < 1 || k > GNN_MAX_K || max_particles < 1 || max_particles > GNN_MAX_PARTICLES)
+        return GNN_ERR_BAD_ARG;
+    if (B > NOALLOC_MAX_JETS || N > NOALLOC_MAX_ROWS) {
+        std::fprintf(stderr, "libgnn: gnn_knn_noalloc: B = %d, N = %d exceed the built-in scratch (at most %d jets and %d particles "
+                     "per call); split the batch or use gnn_debug_knn on a gnn_model\n", B, N, NOALLOC_MAX_JETS, NOALLOC_MAX_ROWS);
+        return GNN_ERR_BATCH_TOO_LARGE;
+    }
+    if (B == 0) return GNN_OK;
+    if (!offsets_dev || !idx_dev || (N > 0 && !space_dev)) return GNN_ERR_NULL;
+    unsigned char* base = nullptr;
+    int rc = knn_noalloc_base(&base);
+    if (rc != GNN_OK) return rc;
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    Workspace w;                                // a view of the static array: nothing here is allocated or freed
+    w.status = reinterpret_cast<unsigned*>(base);
+    w.meta = reinterpret_cast<int32_t*>(base + 16);
+    w.jet_start = reinterpret_cast<int32_t*>(base + NOALLOC_OFF_START);
+    w.jet_n = reinterpret_cast<int32_t*>(base + NOALLOC_OFF_N);
+    w.pjet = reinterpret_cast<int2*>(base + NOALLOC_OFF_PJET);
+    w.dm = reinterpret_cast<float*>(base + NOALLOC_OFF_DM);
+    w.groups = nullptr;                         // no group schedule: the exact path does not use one
+    // The array still holds whatever the previous call left.  Only the status word and meta[] are read before they are
+    // written (the status word is OR-ed into), so those 256 bytes are cleared on the stream; the descriptors, the map and the
+    // distances are written for every row of this batch before the selection reads them.
+    GNN_CUDA_TRY(cudaMemsetAsync(base, 0, 256, s));
+    if ((rc = launch_ingest(offsets_dev, nullptr, B, N, N, max_particles, w, s)) < 0) return rc;
+    if ((rc = launch_knn(space_dev, D, k, B, max_particles, w, idx_dev, /*local_out=*/1, /*gram=*/0, s, DEP_NONE)) < 0) return rc;
+    return cudaGetLastError() == cudaSuccess ? GNN_OK : GNN_ERR_CUDA;
 }
