@@ -196,7 +196,13 @@ int forward(gnn_model* m, Workspace& w, const float* feats, const float* coords,
     // bf16 mode: the last block adds its output straight into the per-jet channel sums (step a7 inside E3 of step a6).  The
     // sums are zero between forwards: the head kernel that reads them clears them (head_split_kernel), else they are cleared here.
     static const bool no_fuse = std::getenv("GNN_NO_POOL_FUSE") != nullptr;     // developer knob: A/B of the pooling epilogue
-    const bool fuse_pool = bf16 && !no_fuse && edgeconv_bf16_can_pool(*m, a.n_blocks - 1);
+    // The pooling epilogue finds a particle's jet in w.pjid, and only the grouped kNN kernels write that map: the epilogue is
+    // used only if some block of THIS forward takes the grouped path (otherwise -- coord_dims > 4 with no 64 / 128 / 256-wide
+    // feature space, or max_particles beyond a tile -- the last block stores its output and pool_head_kernel pools it).
+    bool pjid_written = false;
+    for (int l = 0; l < a.n_blocks; ++l)
+        pjid_written = pjid_written || knn_group_supported(l == 0 ? a.coord_dims : block_in(a, l), a.max_particles);
+    const bool fuse_pool = bf16 && !no_fuse && pjid_written && edgeconv_bf16_can_pool(*m, a.n_blocks - 1);
     if (fuse_pool && !w.pool_self_cleaning &&
         cudaMemsetAsync(w.pool, 0, (size_t)B * a.channels[a.n_blocks - 1][2] * sizeof(unsigned long long), s) != cudaSuccess)
         return GNN_ERR_CUDA;
@@ -208,8 +214,10 @@ int forward(gnn_model* m, Workspace& w, const float* feats, const float* coords,
             // One stream, programmatic dependent launches.  u, v and the shortcut of a block depend on x only, as does its kNN,
             // so the two kernels run SIDE BY SIDE as a primary / secondary pair (gnn_internal.h, DEP_*); the primary is the one
             // whose CTAs are all resident at once: the tensor-core pre kernel (blocks >= 2), else the grouped kNN kernel.  The
-            // primary's prologue (weights, TMEM) runs under the tail of the kernel before it.  edge_l is a normal launch: it
-            // starts when the secondary, hence the pair, has completed.
+            // primary's prologue (weights, TMEM) runs under the tail of the kernel before it.  edge_l is itself launched as a
+            // dependent of the secondary (launch_edge_t passes the attribute): its prologue may start while the secondary
+            // drains, and its grid_dep_wait returns when the secondary -- whose CTA 0 waits for the primary -- has completed,
+            // i.e. when the pair has.
             int rc_pre, rc_knn;
             if (N_upper == 0 || !knn_group_supported(D, a.max_particles)) {          // no pair: ordinary launches
                 if ((rc_pre = launch_pre_bf16(*m, l, x, N_upper, w, s, DEP_NONE)) < 0) return rc_pre;

@@ -300,6 +300,7 @@ __device__ __forceinline__ void edge_body(const EdgeParams& p) {
     constexpr bool PAIR = Cfg::PAIR;
     constexpr int KB = Cfg::KB, NE = Cfg::NE, CWE = Cfg::CWE;
     extern __shared__ __align__(1024) uint8_t smem_raw[];
+    // meta[] is the ingest kernel's, at least two kernels back: readable before grid_dep_wait (gnn_internal.h, PDL notes)
     if (p.meta[0]) return;                                       // grid-uniform
     const int N = p.meta[1];
     const int n_tiles = min(p.n_tiles, (N + p.TP - 1) / p.TP);

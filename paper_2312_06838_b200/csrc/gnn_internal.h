@@ -132,7 +132,12 @@ int edgeconv_f32_configure();
 //   DEP_SECONDARY  launched as a dependent of the primary; does NOT wait before reading its inputs -- a secondary CTA exists
 //                  only after every primary CTA has passed its wait, i.e. the inputs of both are complete -- but its CTA 0
 //                  waits for the primary before it exits, so that the pair is complete when the secondary is: the next
-//                  kernel, a normal launch, then starts after both.
+//                  kernel (the edge kernel, also launched with the attribute) passes its own grid_dep_wait after both.
+// What a kernel may read BEFORE its grid_dep_wait: anything written two or more kernels back.  A dependent CTA exists only
+// once every CTA of its predecessor has released its dependents, and the predecessors here release only after their own
+// wait (primary) or exist only after the primary's wait (secondary); so everything before the pair -- the ingest kernel's
+// meta[] and jet descriptors in particular -- is complete and visible to any CTA of any later kernel from its first
+// instruction.  The edge kernels read meta[0..1] that early for this reason.
 enum { DEP_NONE = 0, DEP_PRIMARY = 1, DEP_SECONDARY = 2 };
 #ifdef __CUDACC__
 __device__ __forceinline__ void grid_dep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }

@@ -346,6 +346,9 @@ head_split_kernel(const unsigned long long* pooled, const int32_t* __restrict__ 
     __shared__ float s_inv[HS_JETS];                                 // 1 / n (0 for empty, offending or absent jets)
     __shared__ float cl_share[HS_MAX_SPLIT * HS_JETS * HS_MAX_CLASSES];   // rank 0: [rank][jet][class]
     const unsigned rank = tc_cluster_rank(), n_rank = gridDim.y;
+    // Distributed shared memory may only be touched once every CTA of the cluster has started.  Arrive now, wait just before
+    // the remote stores below: by then the other CTAs have long arrived, so the wait costs nothing.
+    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
     const int b0 = blockIdx.x * HS_JETS, o0 = blockIdx.y * HS_OUT;
     const int nj = min(HS_JETS, B - b0);
     const int tid = threadIdx.x, oq = tid % (HS_OUT / 4), ks = tid / (HS_OUT / 4);
@@ -425,6 +428,7 @@ head_split_kernel(const unsigned long long* pooled, const int32_t* __restrict__ 
         __syncthreads();                                            // zT and part are rewritten by the next pass
     }
     // final layer, this CTA's HS_OUT terms: one warp per jet (all classes), then into the first CTA's shared memory
+    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");   // pairs with the arrive at kernel entry: rank 0 exists
     float* dst = tc_map_shared_rank(cl_share, 0) + rank * (HS_JETS * HS_MAX_CLASSES);
     for (int jb = wid; jb < HS_JETS; jb += HS_THREADS / 32) {
         const float ha = hT[jb * HS_OUT + ln], hb = hT[jb * HS_OUT + 32 + ln];

@@ -364,3 +364,27 @@ def test_forward_in_a_callers_cuda_graph_and_graph_replay(pn):
     torch.cuda.synchronize()
     assert np.array_equal(out2.cpu().numpy().astype(np.float64), ref1)
     assert m.status_check() == 0
+
+
+def test_no_grouped_knn_anywhere_still_pools_correctly():
+    """An architecture none of whose kNN spaces has a grouped kernel (5 coordinates; the later block's space is 32 wide), with
+    k = 16 and C_last = 64, so the last edge kernel COULD pool in its epilogue.  That epilogue reads the particle -> jet map
+    only the grouped kNN kernels write; the forward must notice that nobody wrote it and pool the stored block output instead
+    (before the fix it scattered the sums through uninitialised jet ids).  Run twice: a second forward must not depend on
+    what the first left behind."""
+    a = synth.Arch(in_features=6, k=16, channels=((32, 32, 32), (64, 64, 64)), fc_hidden=(64,), coord_dims=5, max_particles=128)
+    w = synth.make_weights(a)
+    m = make_model(a, w, precision=gnn.BF16, max_batch_jets=64)
+    rng = np.random.default_rng(515)
+    counts = [1, 2, 17, 40, 100, 5, 16, 0, 61, 40, 33, 128, 3, 40]
+    off = np.zeros(len(counts) + 1, np.int32); off[1:] = np.cumsum(counts)
+    feats = rng.normal(0, 1, (off[-1], a.in_features)).astype(np.float32)
+    coords = rng.normal(0, 0.3, (off[-1], a.coord_dims)).astype(np.float32)
+    ref = oracle.forward(a, w, feats, coords, off)
+    f, c, o = dev(feats), dev(coords), dev(off)
+    for _ in range(2):
+        lg = m.infer(f, c, o)
+        torch.cuda.synchronize()
+        assert m.status_check() == 0
+        check_logits(lg.cpu().numpy().astype(np.float64), ref)
+    m.close()
