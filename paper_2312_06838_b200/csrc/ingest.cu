@@ -214,7 +214,9 @@ int launch_compact_padded(const float* feats, const float* coords, const float* 
 
 // ---- class probabilities (PAPER.md L262 ends the network in "two nodes"; the served model's FP32 output, L270, is read as
 // softmax scores by the analyses): row-wise softmax of [B, n_classes] logits in fp32, max subtracted first; NaN rows stay NaN
-__global__ void softmax_kernel(const float* __restrict__ logits, int B, int n_classes, float* __restrict__ probs) {
+// logits and probs may be the SAME buffer (gnn.h: "may alias"; gnn_infer_channel_first runs it in place), so neither pointer is
+// __restrict__: a thread owns its row, reads z[c] before it writes probs[c], and never reads an element it has written
+__global__ void softmax_kernel(const float* logits, int B, int n_classes, float* probs) {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= B) return;
     const float* z = logits + (size_t)b * n_classes;
