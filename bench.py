@@ -160,12 +160,13 @@ def cpu_baseline(arch, weights, batch, target_s=12.0):
     n = int(max(32, min(batch.n_jets, n0 / t0 * target_s)))
     n, t = time_oracle(arch, weights, batch, n)
     # the same oracle on ONE thread beside the all-cores figure, on a smaller sample (about a quarter of the time)
-    n1 = int(max(8, min(n, n / t / max(1, oracle.max_threads()) * target_s / 4)))
+    cores = oracle.max_threads()                    # read before the one-thread call (the OpenMP thread count is sticky)
+    n1 = int(max(8, min(n, n / t / max(1, cores) * target_s / 4)))
     sub = batch.head(n1)
     t1 = time.perf_counter()
     oracle.forward(arch, weights, sub.feats, sub.coords, sub.offsets, nthreads=1)
     t1 = time.perf_counter() - t1
-    return {"value": n / t, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle",
+    return {"value": n / t, "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": "first %d jets of batch 0 (%d particles), one oracle.forward call, %.1f s" %
                       (n, int(batch.offsets[n]), t),
             "one_thread": {"value": n1 / t1, "sample": "first %d jets, nthreads=1, %.1f s" % (n1, t1)}}

@@ -266,7 +266,7 @@ typedef struct gnn_bdt gnn_bdt;
 int gnn_bdt_create(const int32_t* feature_host, const float* threshold_host, const float* leaf_host, int32_t n_trees,
                    int32_t depth, int32_t n_features, int device, gnn_bdt** out);
 void gnn_bdt_destroy(gnn_bdt* b);
-/* x_dev [N, n_features] fp32 row-major -> out_dev [N, 2]; asynchronous on cuda_stream */
+/* x_dev [N, n_features] fp32 row-major -> out_dev [N, 2] (8-byte aligned, else GNN_ERR_BAD_ARG); asynchronous on cuda_stream */
 int gnn_bdt_infer(gnn_bdt* b, const float* x_dev, int64_t N, float* out_dev, void* cuda_stream);
 /* the same from / to HOST buffers (pinned memory makes the copies asynchronous); blocking; device staging owned by `b` grows
  * to the largest N seen */

@@ -32,6 +32,7 @@ struct gnn_bdt {
 namespace {
 
 constexpr int BDT_THREADS = 256;
+constexpr int BDT_MAX_SMEM = 200 * 1024;   // largest forest + staging a CTA may ask for (one CTA per SM then)
 
 __global__ void __launch_bounds__(BDT_THREADS)
 bdt_kernel(const uint2* __restrict__ nodes, const float* __restrict__ leaves, int n_trees, int depth, int F,
@@ -79,7 +80,7 @@ int gnn_bdt_create(const int32_t* feature_host, const float* threshold_host, con
     if (n_trees < 1 || n_trees > 4096 || depth < 1 || depth > 12 || n_features < 1 || n_features > 1024) return GNN_ERR_BAD_ARCH;
     const size_t n_int = ((size_t)1 << depth) - 1, n_leaf = (size_t)1 << depth;
     const size_t smem = (size_t)n_trees * (n_int * sizeof(uint2) + n_leaf * sizeof(float)) + (size_t)BDT_THREADS * (n_features + 1) * sizeof(float);
-    if (smem > 200 * 1024) return GNN_ERR_BAD_ARCH;              // the forest must fit one SM's shared memory
+    if (smem > (size_t)BDT_MAX_SMEM) return GNN_ERR_BAD_ARCH;              // the forest must fit one SM's shared memory
     for (size_t i = 0; i < (size_t)n_trees * n_int; ++i)
         if (feature_host[i] < 0 || feature_host[i] >= n_features) return GNN_ERR_BAD_ARG;
     int ndev = 0;
@@ -103,7 +104,9 @@ int gnn_bdt_create(const int32_t* feature_host, const float* threshold_host, con
               cudaMalloc(&b->leaves, (size_t)n_trees * n_leaf * sizeof(float)) == cudaSuccess &&
               cudaMemcpy(b->nodes, nd.data(), nd.size() * sizeof(uint2), cudaMemcpyHostToDevice) == cudaSuccess &&
               cudaMemcpy(b->leaves, leaf_host, (size_t)n_trees * n_leaf * sizeof(float), cudaMemcpyHostToDevice) == cudaSuccess &&
-              cudaFuncSetAttribute(bdt_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess;
+              // the attribute belongs to the kernel on this device, not to this forest: always the 200 KB ceiling checked
+              // above, so that creating a smaller forest later never lowers the cap under an earlier, larger one
+              cudaFuncSetAttribute(bdt_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, BDT_MAX_SMEM) == cudaSuccess;
     if (!ok) { gnn_bdt_destroy(b); return GNN_ERR_CUDA; }
     *out = b;
     return GNN_OK;
@@ -125,6 +128,7 @@ int gnn_bdt_infer(gnn_bdt* b, const float* x_dev, int64_t N, float* out_dev, voi
     if (N < 0) return GNN_ERR_BAD_ARG;
     if (N == 0) return GNN_OK;
     if (!x_dev || !out_dev) return GNN_ERR_NULL;
+    if ((reinterpret_cast<uintptr_t>(out_dev) & 7u) != 0) return GNN_ERR_BAD_ARG;   // rows are stored as float2
     const long long tiles = (N + BDT_THREADS - 1) / BDT_THREADS;
     const int per_sm = std::max(1, (int)((220 * 1024) / b->smem));
     const int grid = (int)std::min<long long>(tiles, (long long)b->n_sms * per_sm);

@@ -39,3 +39,23 @@ def test_bdt_argument_checks():
     m = gnn.Bdt(f, t, l, 5)
     assert m.infer(torch.empty((0, 5), device="cuda")).shape == (0, 2)
     m.close()
+
+
+def test_a_later_smaller_forest_does_not_break_an_earlier_larger_one():
+    """The dynamic-shared-memory cap is an attribute of the kernel on the device, not of one forest: creating a small forest
+    after a large one must leave the large one launchable (the cap is always raised to the 200 KB ceiling)."""
+    fb, tb, lb = synth.make_bdt(seed=71, n_trees=100, depth=6, n_features=20)        # ~ 130 KB of shared memory
+    fs, ts, ls = synth.make_bdt(seed=72, n_trees=3, depth=2, n_features=4)           # a few KB
+    x = synth.make_bdt_events(3000, 20, seed=73)
+    big = gnn.Bdt(fb, tb, lb, 20)
+    small = gnn.Bdt(fs, ts, ls, 4)
+    xs = synth.make_bdt_events(100, 4, seed=74)
+    assert np.abs(small.infer(torch.from_numpy(xs).cuda()).cpu().numpy() - obdt.predict(fs, ts, ls, xs)).max() < 2e-6
+    out = big.infer(torch.from_numpy(x).cuda())
+    torch.cuda.synchronize()
+    assert np.abs(out.cpu().numpy().astype(np.float64) - obdt.predict(fb, tb, lb, x)).max() < 2e-6
+    # rows are stored as float2: an output pointer that is not 8-byte aligned is refused, not written through
+    buf = torch.empty(2 * 3000 + 1, dtype=torch.float32, device="cuda")
+    with pytest.raises(gnn.GnnError):
+        big.infer(torch.from_numpy(x).cuda(), out=buf[1:].view(3000, 2))
+    big.close(); small.close()
