@@ -6,7 +6,8 @@ complete binary trees of one depth, internal node i tests x[feature[i]] < thresh
 
 The walk is written level by level over all events at once with numpy indexing; nothing else is vectorised or reordered.
 Pins (tests/test_oracle_bdt.py): a pure-Python per-event walk, the hand-worked forest of tests/golden/bdt_worked_example.txt,
-depth-1 stumps as a closed form, forests whose thresholds send every event to one known leaf."""
+depth-1 stumps as a closed form, forests whose thresholds send every event to one known leaf; predict(): the golden file's
+decimal-arithmetic probabilities, scipy.special.expit, margin 0 and +-40 (column order and sign)."""
 import numpy as np
 
 

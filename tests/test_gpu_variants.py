@@ -9,7 +9,7 @@ import torch
 import oracle
 import synth
 import paper_2312_06838_b200 as gnn
-from gpu_util import dev, make_model
+from gpu_util import dev, make_model, staged_fp32
 
 pytestmark = pytest.mark.gpu
 
@@ -29,8 +29,16 @@ def test_paper_f5_channel_first_softmax(precision, tol):
     torch.cuda.synchronize()
     assert m.status_check() == 0
     err = np.abs(lg - ref).max(1)
+    ok = np.ones(b.n_jets, bool)
     if precision == gnn.FP32_VALIDATION:
-        assert (err < tol).mean() >= 0.99                                # near-tie jets: see test_gpu_fp32 (R21)
+        # R21 to the letter (as test_gpu_fp32): a jet may miss the bar only if it holds a point inside the oracle's 1e-5
+        # near-tie band whose GPU neighbour set actually differs; the staged run on the same jets (ragged form) finds them
+        staged, _, report, excluded = staged_fp32(m, a, w, b)
+        assert all(bad == 0 for bad, _ in report), report
+        assert np.array_equal(lg, staged)                                # the channel-first entry == the staged ragged run
+        assert excluded.sum() <= 3
+        ok = ~excluded
+        assert (err[ok] < tol).all()
     else:
         assert err.max() < tol and (lg.argmax(1) == ref.argmax(1)).mean() >= 0.999
     pr = m.infer_channel_first(dev(pts), dev(fts), dev(msk), softmax=True).cpu().numpy().astype(np.float64)
@@ -38,7 +46,6 @@ def test_paper_f5_channel_first_softmax(precision, tol):
     # the device softmax of the device logits is the oracle's softmax of the same logits to fp32 rounding ...
     assert np.abs(pr - oracle.softmax(lg)).max() < 1e-6
     # ... and of the oracle's logits to the logit tolerance (|dp| <= |dz| / 2 for two classes)
-    ok = err < tol
     assert np.abs(pr - oracle.softmax(ref))[ok].max() < tol
     m.close()
 

@@ -24,8 +24,26 @@ def test_worked_example():
     want = _rows(d["margin"], np.float64)[0]
     m = bdt.margins(f, t, l, x)
     assert np.abs(m - want).max() < 1e-6            # leaves are fp32 roundings of the decimals
+    # the logistic output and its column order, pinned to the golden file's decimal-arithmetic values and to scipy's expit
+    # (the leaves are fp32 roundings of the decimals, so the margins differ from the decimals by ~1e-8)
+    from scipy.special import expit
     p = bdt.predict(f, t, l, x)
-    assert np.abs(p[:, 1] - 1 / (1 + np.exp(-m))).max() < 1e-15 and np.abs(p.sum(1) - 1).max() < 1e-15
+    prob = _rows(d["prob"], np.float64)[0]
+    assert p.shape == (5, 2)
+    assert np.abs(p[:, 1] - prob).max() < 1e-7 and np.abs(p[:, 0] - (1.0 - prob)).max() < 1e-7
+    assert np.abs(p[:, 1] - expit(m)).max() < 1e-15 and np.abs(p[:, 0] - expit(-m)).max() < 1e-15
+    assert (p[:, 1] > 0.5).tolist() == [True, False, True, True, False]        # positive margin -> second column wins
+
+
+def test_logistic_special_cases():
+    """margin 0 -> (0.5, 0.5) exactly; a large positive margin puts all the mass on the SECOND column, a large negative one on
+    the first (a swapped column order or a wrong sign in the exponent fails here)"""
+    f = np.zeros((1, 1), np.int32); t = np.zeros((1, 1), np.float32)
+    x = np.array([[-1.0], [1.0]], np.float32)                                   # first event goes left, second right
+    p = bdt.predict(f, t, np.array([[0.0, 0.0]], np.float32), x)
+    assert np.array_equal(p, np.full((2, 2), 0.5))
+    p = bdt.predict(f, t, np.array([[40.0, -40.0]], np.float32), x)
+    assert p[0, 1] > 1 - 1e-15 and p[0, 0] < 1e-15 and p[1, 0] > 1 - 1e-15 and p[1, 1] < 1e-15
 
 
 def walk(feature, threshold, leaf, x):
