@@ -1,6 +1,10 @@
 """Builds libgnn.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).
 
     python -m paper_2312_06838_b200.build [--force]
+
+The shipped library reads no environment variable at run time.  Developer builds: extra nvcc flags come from the build-time
+variable GNN_NVCC_DEFS, e.g. GNN_NVCC_DEFS="-DGNN_DEV_KNOBS" compiles in the A/B switches GNN_NO_POOL_FUSE, GNN_NO_GRAPHS,
+GNN_NO_PDL and GNN_EDGE_CHUNK (csrc/api.cu, csrc/edgeconv_bf16.cu), "-DEDGE_CWE_256=64" changes an epilogue tile shape.
 """
 import os
 import subprocess

@@ -195,7 +195,11 @@ int forward(gnn_model* m, Workspace& w, const float* feats, const float* coords,
     const bool bf16 = a.precision == GNN_BF16;
     // bf16 mode: the last block adds its output straight into the per-jet channel sums (step a7 inside E3 of step a6).  The
     // sums are zero between forwards: the head kernel that reads them clears them (head_split_kernel), else they are cleared here.
-    static const bool no_fuse = std::getenv("GNN_NO_POOL_FUSE") != nullptr;     // developer knob: A/B of the pooling epilogue
+#ifdef GNN_DEV_KNOBS                              // developer builds only (build.py: GNN_NVCC_DEFS=-DGNN_DEV_KNOBS): A/B of the pooling epilogue
+    static const bool no_fuse = std::getenv("GNN_NO_POOL_FUSE") != nullptr;
+#else
+    constexpr bool no_fuse = false;               // the shipped library's launch plan does not depend on the environment
+#endif
     // The pooling epilogue finds a particle's jet in w.pjid, and only the grouped kNN kernels write that map: the epilogue is
     // used only if some block of THIS forward takes the grouped path (otherwise -- coord_dims > 4 with no 64 / 128 / 256-wide
     // feature space, or max_particles beyond a tile -- the last block stores its output and pool_head_kernel pools it).
@@ -263,7 +267,11 @@ int forward(gnn_model* m, Workspace& w, const float* feats, const float* coords,
 // captured (the forward is then simply recorded into the caller's graph: one stream, no host synchronisation).
 int forward_cached(gnn_model* m, Workspace& w, const float* feats, const float* coords, const int32_t* offsets, int B, int N,
                    float* logits, cudaStream_t s) {
-    static const bool no_graphs = std::getenv("GNN_NO_GRAPHS") != nullptr;      // developer knob
+#ifdef GNN_DEV_KNOBS
+    static const bool no_graphs = std::getenv("GNN_NO_GRAPHS") != nullptr;
+#else
+    constexpr bool no_graphs = false;
+#endif
     cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
     if (no_graphs || w.prof_on || cudaStreamIsCapturing(s, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone)
         return forward(m, w, feats, coords, offsets, nullptr, B, N, N, logits, s);
@@ -323,8 +331,12 @@ int forward_cached(gnn_model* m, Workspace& w, const float* feats, const float* 
 }  // namespace
 
 bool gnn_pdl_enabled() {
+#ifdef GNN_DEV_KNOBS
     static const bool on = std::getenv("GNN_NO_PDL") == nullptr;
     return on;
+#else
+    return true;
+#endif
 }
 
 extern "C" {

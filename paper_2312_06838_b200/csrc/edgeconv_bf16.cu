@@ -1590,7 +1590,7 @@ int launch_edge_t(const EdgeParams& p_in, int grid_cap, cudaStream_t s) {
     EdgeParams p = p_in;
     const int n_work = Cfg::PAIR ? (p.n_tiles + 1) / 2 : p.n_tiles;
     const int n_units = Cfg::PAIR ? std::min(n_work, grid_cap / 2) : std::min(n_work, grid_cap);
-    // tiles a unit takes at a time (GNN_EDGE_CHUNK overrides, developer knob).  Measured on configs[1]: without the pooling
+    // tiles a unit takes at a time (GNN_EDGE_CHUNK overrides in -DGNN_DEV_KNOBS builds).  Measured on configs[1]: without the pooling
     // epilogue tile-by-tile round-robin is best (39 / 72 us for C = 64 / 128 against 42 / 72 us with one contiguous range per
     // unit); the pooling epilogue wants ONE contiguous range per unit -- a jet's partial sums then stay on chip across
     // its tiles (161 us against 176 us round-robin, where every tile flushes 2048 atomics)
@@ -1831,7 +1831,11 @@ int launch_edge_bf16(gnn_model& m, int block, const int32_t* idx, int N, float* 
     while ((1 << ep.logk) < k) ++ep.logk;
     ep.TP = TILE_ROWS / k;
     ep.n_tiles = (N + ep.TP - 1) / ep.TP;
+#ifdef GNN_DEV_KNOBS
     static const int chunk_env = [] { const char* e = std::getenv("GNN_EDGE_CHUNK"); return e ? std::atoi(e) : 0; }();
+#else
+    constexpr int chunk_env = 0;
+#endif
     ep.chunk = chunk_env;                                       // <= 0: chosen per kernel in launch_edge_t
     int rc;
     switch (b.C) {

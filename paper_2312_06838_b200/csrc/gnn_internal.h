@@ -143,7 +143,7 @@ enum { DEP_NONE = 0, DEP_PRIMARY = 1, DEP_SECONDARY = 2 };
 __device__ __forceinline__ void grid_dep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void grid_dep_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 
-bool gnn_pdl_enabled();       // false with GNN_NO_PDL in the environment (developer knob: A/B of the overlap)
+bool gnn_pdl_enabled();       // always true; -DGNN_DEV_KNOBS builds turn it off with GNN_NO_PDL in the environment (A/B of the overlap)
 
 template <typename... KArgs, typename... Args>
 cudaError_t launch_k(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s, bool pdl, Args&&... args) {

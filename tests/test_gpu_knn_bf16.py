@@ -1,5 +1,5 @@
 """-m gpu parity tests of the PRODUCTION kNN path (GNN_BF16 mode): the grouped kernels of csrc/knn_group.cu -- several jets
-per 128-row tile, Gram distances in tf32 on the tensor cores for the feature spaces (D = 64 / 128 / 256), exact direct
+per 128-row tile, Gram distances on fp16 operands (fp32 accumulate) on the tensor cores for the feature spaces (D = 64 / 128 / 256), exact direct
 differences for the coordinates, 32-bit selection keys (d to 16 mantissa bits | j) -- against the fp64 oracle's kNN,
 through gnn_debug_knn on a GNN_BF16 model (which runs exactly what that model's forward runs).
 
