@@ -56,7 +56,10 @@ typedef enum {
     GNN_BF16 = 1              /* edge-MLP GEMMs as bf16 x bf16 -> fp32 tcgen05 MMAs; per-particle GEMM of blocks >= 2, kNN Gram
                                  matrices of blocks >= 2 and the stored shortcut in fp16 (10 mantissa bits; saturating at 65504:
                                  activations must stay below that); neighbour selection on 32-bit keys in every block; E3 row
-                                 sum in f16x2; accumulators, block outputs, pool, head fp32 (R19, R28) */
+                                 sum in f16x2; accumulators, block outputs, pool, head fp32 (R19, R28).
+                                 Non-finite or blown-up activations are NOT propagated in this mode: each ReLU is an fmax
+                                 (NaN -> 0), fp16 operands and the fixed-point pooled sums saturate, so such a jet gets finite
+                                 logits and no status bit; GNN_FP32_VALIDATION propagates NaN / Inf to the logits */
 } gnn_precision;
 
 /* Architecture.  Constraints checked by gnn_create: 1 <= n_blocks <= GNN_MAX_BLOCKS;
