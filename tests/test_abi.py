@@ -79,3 +79,23 @@ def test_product_does_not_import_the_oracle():
     osrc = open(os.path.join(ROOT, "oracle", "__init__.py")).read() + open(os.path.join(ROOT, "oracle", "oracle.c")).read()
     assert not re.search(r"^\s*(import|from)\s+paper_2312_06838_b200", osrc, flags=re.M)
     assert "gnn.h\"" not in osrc
+
+
+def test_noalloc_entry_allocates_nothing_and_its_scratch_is_the_documented_size():
+    """gnn_knn_noalloc is the entry for callers that may not allocate device memory: its source (and the helper that looks up the
+    scratch address) must not name an allocating call, the scratch must be a file-scope static __device__ array aligned to 256
+    bytes, and its size must be what gnn.h and the README tell those callers (about 4.1 MiB, 1024 jets / 8192 particles)."""
+    src = open(os.path.join(ROOT, "paper_2312_06838_b200", "csrc", "knn.cu")).read()
+    tail = src[src.index("constexpr int NOALLOC_MAX_JETS"):]
+    code = re.sub(r"//[^\n]*", "", tail)                                 # comments may (and do) name cudaMalloc
+    for banned in ("cudaMalloc", "cudaFree", "cudaHostAlloc", "cudaMallocAsync", "new ", "std::vector"):
+        assert banned not in code, banned
+    assert "cudaGetSymbolAddress" in code and "static __device__ __align__(256) unsigned char knn_noalloc_scratch" in code
+    jets = int(re.search(r"NOALLOC_MAX_JETS = (\d+)", tail).group(1))
+    rows = int(re.search(r"NOALLOC_MAX_ROWS = (\d+)", tail).group(1))
+    assert (jets, rows) == (1024, 8192)
+    size = 256 + 2 * 4 * jets + 8 * rows + 4 * rows * 128                # status/meta | jet_start | jet_n | pjet | dm
+    assert size == 4268288 and abs(size / 2 ** 20 - 4.1) < 0.05
+    hdr = open(os.path.join(ROOT, "include", "gnn.h")).read()
+    assert "B <= 1024 jets and N <= 8192 particles" in hdr and "4.1 MiB" in hdr
+    assert "4.1 MiB" in open(os.path.join(ROOT, "README.md")).read()
